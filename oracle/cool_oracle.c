@@ -1,0 +1,549 @@
+/*
+ * cool_oracle.c — ORACLE (test infrastructure, NOT the product).
+ *
+ * Plain, slow, fp64 CPU statement of the per-cell two-temperature cooling step of
+ * arXiv 2505.08855 (reference text: PAPER.md).  Only tests/, __graft_entry__.smoke()
+ * and bench.py's cpu_baseline / --impl reference legs may call it.  It shares no code,
+ * header, table or constant generator with paper_2505_08855_b200/ (the CUDA product).
+ *
+ * Part A  analytic physics, §II eqs 1-15 (L57-L147)
+ * Part B  the table-interpolated, limited, sub-stepped update (PAPER.md L122-L124,
+ *         L181, L185, L197; readings C-1..C-17 of SURVEY.md §8(c) / DESIGN.md)
+ *
+ * Pins (tests/test_oracle_*.py): closed-form brems scaling, incomplete-gamma closed
+ * form of the synchrotron integral, scipy.special.kve for the Bessel functions,
+ * residual of eq 5, limits of eqs 7 and 11, node-exact / linear-exact interpolation,
+ * conservation / positivity / no-crossing of the update, brute force on tiny tables.
+ * Nothing here is "parity unpinned".
+ *
+ * Everything is double precision; no blocking, fusion or reordering beyond what the
+ * equations state.
+ */
+#include <math.h>
+#include <stddef.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+/* ---- CODATA-2018 constants, cgs ------------------------------------------------ */
+#define ORC_C      2.99792458e10      /* cm/s  */
+#define ORC_KB     1.380649e-16       /* erg/K */
+#define ORC_ME     9.1093837015e-28   /* g     */
+#define ORC_MP     1.67262192369e-24  /* g     */
+#define ORC_QE     4.80320471257e-10  /* esu   */
+#define ORC_HPL    6.62607015e-27     /* erg s */
+#define ORC_SIGT   6.6524587321e-25   /* cm^2  */
+#define ORC_SIGSB  5.670374419e-5     /* erg cm^-2 s^-1 K^-4 */
+#define ORC_GMSUN  1.32712440018e26   /* cm^3/s^2 */
+#define ORC_PI     3.14159265358979323846
+
+/* Unit system of the caller (SURVEY §8 conventions; PAPER.md L220 M = 10 Msun,
+ * Table I L287-L296 rho_scale, L207 gamma = 5/3, a = 0.9375). */
+typedef struct {
+    double rho_scale_cgs;        /* g cm^-3 per code density unit              */
+    double mbh_msun;             /* black-hole mass                            */
+    double gamma_e, gamma_i;     /* adiabatic indices                          */
+    double ln_lambda;            /* Coulomb logarithm, C-4: 20                 */
+    double ion_theta_mass_ratio; /* C-3: theta_i(eq 15) = Theta_i / this       */
+    double hth_cm;               /* C-6: fixed H_th for 3-D tables             */
+    double r_ref_rg, spin;       /* C-6: radius/spin for H_th in 4-D tables    */
+} orc_units;
+
+static double orc_rg(const orc_units *u) { return ORC_GMSUN * u->mbh_msun / (ORC_C * ORC_C); }
+static double orc_tg(const orc_units *u) { return orc_rg(u) / ORC_C; }
+/* erg cm^-3 s^-1  ->  code energy density per code time */
+static double orc_rate_conv(const orc_units *u) { return orc_tg(u) / (u->rho_scale_cgs * ORC_C * ORC_C); }
+
+double orc_ne_cgs(const orc_units *u, double rho) { return rho * u->rho_scale_cgs / ORC_MP; }   /* C-14 */
+double orc_bfield_gauss(const orc_units *u, double bsq)                                         /* L173 */
+{
+    return sqrt(4.0 * ORC_PI * bsq * u->rho_scale_cgs * ORC_C * ORC_C);
+}
+
+/* ================================================================================
+ * Part A.1  Bremsstrahlung, eqs 1-2.
+ * ============================================================================== */
+double orc_brems_cgs(double ne, double th)
+{
+    double fee, fei;
+    if (th < 1.0) {
+        fee = pow(th, 1.5) * (1.0 + 1.1 * th + th * th - 1.25 * pow(th, 2.5));
+        fei = 4.0 * sqrt(2.0 * th / (ORC_PI * ORC_PI * ORC_PI)) * (1.0 + 1.781 * pow(th, 1.34));
+    } else {
+        fee = 1.34 * th * (log(1.123 * th) + 1.28);
+        fei = 9.0 * th / (2.0 * ORC_PI) * (log(1.123 * th + 0.48) + 1.5);
+    }
+    return 2.56e-22 * ne * ne * fee + 1.48e-22 * ne * ne * fei;
+}
+
+/* ================================================================================
+ * Modified Bessel functions of the second kind, exponentially scaled:
+ *   Khat_nu(x) = e^x K_nu(x) = int_0^inf exp(-x (cosh t - 1)) cosh(nu t) dt
+ * (textbook integral representation).  Trapezoid rule, which
+ * converges geometrically for this analytic, doubly-exponentially decaying
+ * integrand.  The upper limit is where the exponent reaches -80.
+ * ============================================================================== */
+double orc_bessel_k_scaled(double nu, double x)
+{
+    /* cosh t - 1 = 2 sinh^2(t/2) is used so that large x (tiny t) keeps full precision */
+    const int N = 256;
+    const double tmax = 2.0 * asinh(sqrt(40.0 / x));   /* x (cosh tmax - 1) = 80 */
+    const double h = tmax / N;
+    double s = 0.5; /* f(0)/2 = 1/2 */
+    for (int k = 1; k <= N; ++k) {
+        double t = k * h;
+        double sh = sinh(0.5 * t);
+        s += exp(-2.0 * x * sh * sh) * cosh(nu * t);
+    }
+    return s * h;
+}
+/* K2 from the recurrence K_{n+1} = K_{n-1} + (2n/x) K_n (holds for the scaled form). */
+double orc_bessel_k2_scaled(double x)
+{
+    return orc_bessel_k_scaled(0.0, x) + (2.0 / x) * orc_bessel_k_scaled(1.0, x);
+}
+
+/* ================================================================================
+ * Part A.2  Synchrotron, eqs 3-6.
+ * ============================================================================== */
+/* ln I'(x) at x = e^u, eq 4 (L76). */
+static double orc_ln_iprime(double u)
+{
+    return log(4.0505) - u / 6.0 + log(1.0 + 0.4 * exp(-0.25 * u) + 0.5316 * exp(-0.5 * u))
+           - 1.8899 * exp(u / 3.0);
+}
+double orc_iprime(double x) { return exp(orc_ln_iprime(log(x))); }
+
+/* K2(1/theta_e), with the paper's low-temperature substitution 2 theta_e^2 for
+ * T_e <= 1e8 K (L87, reading C-12: literal threshold). */
+double orc_k2_tilde(double th)
+{
+    double te = th * ORC_ME * ORC_C * ORC_C / ORC_KB;
+    if (te > 1.0e8) {
+        double x = 1.0 / th;
+        return orc_bessel_k2_scaled(x) * exp(-x);
+    }
+    return 2.0 * th * th;
+}
+
+/* nu = s * x_M  (inverse of x_M = 4 pi m_e c nu / (3 e B theta_e^2), L74). */
+static double orc_synch_s(double B, double th)
+{
+    return 3.0 * ORC_QE * B * th * th / (4.0 * ORC_PI * ORC_ME * ORC_C);
+}
+
+/* x_c = x_M(nu_c): root of eq 5 (L80), H eps_s(nu_c) = 2 pi nu_c^2 k_B T_e / c^2,
+ * i.e. I'(x)/x = s theta_e m_e K2tilde / (2*4.43e-30 H n_e).  Bisection in u = ln x
+ * (reading C-11: "numerical integration" = numerical root finding).  The left side
+ * decreases monotonically from +inf to 0, so the root is unique. */
+double orc_synch_xc(double H, double B, double ne, double th)
+{
+    double s = orc_synch_s(B, th);
+    double lnR = log(s) + log(th) + log(ORC_ME) + log(orc_k2_tilde(th)) - log(2.0 * 4.43e-30 * H * ne);
+    double a = -1200.0, b = 90.0; /* ln x bracket */
+    for (int it = 0; it < 200; ++it) {
+        double m = 0.5 * (a + b);
+        double g = orc_ln_iprime(m) - m - lnR;
+        if (g > 0.0) a = m; else b = m;
+    }
+    return exp(0.5 * (a + b));
+}
+
+/* 16-point Gauss-Legendre nodes by Newton iteration on P_16 (textbook). */
+static void orc_gauss_legendre16(double *xn, double *wn)
+{
+    const int n = 16;
+    for (int i = 0; i < n; ++i) {
+        double z = cos(ORC_PI * (i + 0.75) / (n + 0.5)), pp = 1.0;
+        for (int it = 0; it < 100; ++it) {
+            double p1 = 1.0, p2 = 0.0;
+            for (int j = 1; j <= n; ++j) {
+                double p3 = p2; p2 = p1;
+                p1 = ((2.0 * j - 1.0) * z * p2 - (j - 1.0) * p3) / j;
+            }
+            pp = n * (z * p1 - p2) / (z * z - 1.0);
+            double dz = p1 / pp;
+            z -= dz;
+            if (fabs(dz) < 1e-16) break;
+        }
+        xn[i] = z;
+        wn[i] = 2.0 / ((1.0 - z * z) * pp * pp);
+    }
+}
+
+/* J(x_c) = int_{x_c}^inf x I'(x) dx, composite Gauss-Legendre in u = ln x
+ * (integrand x^2 I'(x) du).  Upper limit where exp(-1.8899 x^{1/3}) has fallen by
+ * e^-80 from its value at x_c. */
+double orc_synch_J(double xc)
+{
+    double xn[16], wn[16];
+    orc_gauss_legendre16(xn, wn);
+    double uc = log(xc);
+    double tc = 1.8899 * cbrt(xc);
+    double umax = 3.0 * log((tc + 80.0) / 1.8899);
+    if (umax <= uc) return 0.0;
+    int npanel = (int)ceil((umax - uc) / 0.5);
+    double hw = (umax - uc) / npanel;
+    double sum = 0.0;
+    for (int p = 0; p < npanel; ++p) {
+        double c = uc + (p + 0.5) * hw;
+        for (int i = 0; i < 16; ++i) {
+            double u = c + 0.5 * hw * xn[i];
+            sum += wn[i] * exp(2.0 * u + orc_ln_iprime(u));
+        }
+    }
+    return sum * 0.5 * hw;
+}
+
+/* Q_syn of eq 6 (L84): Rayleigh-Jeans part below nu_c (prefactor 2piR^2/(2H piR^2) = 1/H)
+ * plus optically thin part above nu_c.  Returns erg cm^-3 s^-1; *nu_c_out = nu_c [Hz]. */
+double orc_synch_cgs(double H, double B, double ne, double th, double *nu_c_out)
+{
+    double s = orc_synch_s(B, th);
+    double xc = orc_synch_xc(H, B, ne, th);
+    double nuc = s * xc;
+    double te = th * ORC_ME * ORC_C * ORC_C / ORC_KB;
+    double rj = 2.0 * ORC_PI * ORC_KB * te * nuc * nuc * nuc / (3.0 * ORC_C * ORC_C * H);
+    double thin = 4.43e-30 * 4.0 * ORC_PI * ne * s * s * orc_synch_J(xc) / orc_k2_tilde(th);
+    if (nu_c_out) *nu_c_out = nuc;
+    return rj + thin;
+}
+
+/* ================================================================================
+ * Part A.3  Inverse-Compton enhancement, eqs 7-9.
+ * Reading C-1: exponent -1 - ln P / ln A (series sum); the printed "1 - lnP/lnA"
+ * is available with printed_exponent != 0 for comparison only.
+ * ============================================================================== */
+double orc_compton_eta_ex(double nu_c, double ne, double H, double th, int printed_exponent)
+{
+    double x = ORC_HPL * nu_c / (ORC_ME * ORC_C * ORC_C);    /* E_init / m_e c^2 */
+    if (!(x < 3.0 * th)) return 1.0;                         /* L99: soft photons only */
+    double tau = 2.0 * ne * ORC_SIGT * H;
+    double P = -expm1(-tau);
+    if (!(P > 0.0)) return 1.0;
+    double Am1 = 4.0 * th + 16.0 * th * th;
+    double A = 1.0 + Am1;
+    double lnA = log1p(Am1);
+    double PA = P * A;
+    if (fabs(1.0 - PA) < 1e-8)
+        return 1.0 + P * Am1 * log(3.0 * th / x) / lnA;
+    double expo = (printed_exponent ? 1.0 : -1.0) - log(P) / lnA;
+    return 1.0 + P * Am1 / (1.0 - PA) * (1.0 - pow(x / (3.0 * th), expo));
+}
+double orc_compton_eta(double nu_c, double ne, double H, double th)
+{
+    return orc_compton_eta_ex(nu_c, ne, H, th, 0);
+}
+
+/* ================================================================================
+ * Part A.4  Totals, eqs 10-12 (reading C-2: sigma = Stefan-
+ * Boltzmann, tau_obs = tau_abs).
+ * ============================================================================== */
+double orc_bridge_cgs(double H, double ne, double th, double qthin)
+{
+    double te = th * ORC_ME * ORC_C * ORC_C / ORC_KB;
+    double bb = 4.0 * ORC_SIGSB * te * te * te * te;
+    double tau_sca = 2.0 * ne * ORC_SIGT * H;
+    double tau_abs = H * qthin / bb;
+    return (bb / H) / (1.5 * (tau_abs + tau_sca) + sqrt(3.0) + 1.0 / tau_abs);
+}
+/* out[0]=Q_brem, out[1]=Q_syn, out[2]=eta, out[3]=Q_thin, out[4]=Q_total, out[5]=nu_c */
+void orc_cooling_cgs(double H, double B, double ne, double th, double *out)
+{
+    double nuc;
+    double qbr = orc_brems_cgs(ne, th);
+    double qsy = orc_synch_cgs(H, B, ne, th, &nuc);
+    double eta = orc_compton_eta(nuc, ne, H, th);
+    double qthin = qbr + eta * qsy;
+    out[0] = qbr; out[1] = qsy; out[2] = eta; out[3] = qthin;
+    out[4] = orc_bridge_cgs(H, ne, th, qthin);
+    out[5] = nuc;
+}
+
+/* ================================================================================
+ * Part A.5  Scale height, eqs 13-14 (code units c = 1, lengths
+ * r_g).  P_s = rho Theta_s m_e/m_p (Theta_i defined with m_e, L147 / C-3),
+ * u_s = P_s/(gamma_s - 1); rho h = rho + u + P; gamma P -> gamma_e P_e + gamma_i P_i
+ * (equal to eq 14 when gamma_e = gamma_i).  rho cancels.
+ * ============================================================================== */
+double orc_omega_k(double r_rg, double spin) { return 1.0 / (pow(r_rg, 1.5) + spin); }
+double orc_hth_cm(const orc_units *u, double th_e, double th_i, double r_rg)
+{
+    double mr = ORC_ME / ORC_MP;
+    double pe = th_e * mr, pi = th_i * mr;
+    double cs2 = (u->gamma_e * pe + u->gamma_i * pi) /
+                 (1.0 + pe / (u->gamma_e - 1.0) + pi / (u->gamma_i - 1.0) + pe + pi);
+    return orc_rg(u) * sqrt(cs2) / orc_omega_k(r_rg, u->spin);
+}
+
+/* ================================================================================
+ * Part A.6  Coulomb exchange, eq 15.  With scaled Bessel
+ * functions the exponentials cancel identically because 1/theta_m = 1/theta_e +
+ * 1/theta_i.  C(theta_e, theta_i) is the Bessel bracket / [K2 K2].
+ * ============================================================================== */
+double orc_coulomb_C(double th_e, double th_i)
+{
+    double xe = 1.0 / th_e, xi = 1.0 / th_i, xm = xe + xi;
+    double s = th_e + th_i;
+    double num = (2.0 * s * s + 1.0) / s * orc_bessel_k_scaled(1.0, xm) + 2.0 * orc_bessel_k_scaled(0.0, xm);
+    return num / (orc_bessel_k2_scaled(xe) * orc_bessel_k2_scaled(xi));
+}
+/* erg cm^-3 s^-1 per unit rho_code^2 (Theta_i - Theta_e) C :
+ * (3/2)(m_e/m_p) lnLambda c sigma_T m_e c^2 (rho_scale/m_p)^2 ; k_B(T_i-T_e) = m_e c^2 (Theta_i-Theta_e). */
+double orc_coulomb_pref_cgs(const orc_units *u)
+{
+    double n1 = u->rho_scale_cgs / ORC_MP;
+    return 1.5 * (ORC_ME / ORC_MP) * u->ln_lambda * ORC_C * ORC_SIGT * ORC_ME * ORC_C * ORC_C * n1 * n1;
+}
+/* Q_cc in code units; > 0 heats the electrons. */
+double orc_coulomb_code(const orc_units *u, double rho, double th_e, double th_i)
+{
+    double C = orc_coulomb_C(th_e, th_i / u->ion_theta_mass_ratio);
+    return orc_coulomb_pref_cgs(u) * orc_rate_conv(u) * rho * rho * (th_i - th_e) * C;
+}
+
+/* ================================================================================
+ * Table nodes (what a cooling table stores; reading C-5: log10 of the code-unit
+ * rate, eta stored as log10 eta).
+ * ============================================================================== */
+/* 3-D table (log rho, log Theta_e, log bsq) at fixed H = hth_cm: log10 Lambda_code. */
+double orc_node_total_log10(const orc_units *u, double rho, double th_e, double bsq)
+{
+    double out[6];
+    orc_cooling_cgs(u->hth_cm, orc_bfield_gauss(u, bsq), orc_ne_cgs(u, rho), th_e, out);
+    return log10(out[4] * orc_rate_conv(u));
+}
+/* 4-D process tables (log rho, log Theta_e, log bsq, log Theta_i), H from eqs 13-14
+ * at r_ref: out = {log10 Qbrem_code, log10 Qsyn_code, log10 eta}. */
+void orc_node_proc_log10(const orc_units *u, double rho, double th_e, double bsq, double th_i, double *out3)
+{
+    double out[6];
+    double H = orc_hth_cm(u, th_e, th_i, u->r_ref_rg);
+    orc_cooling_cgs(H, orc_bfield_gauss(u, bsq), orc_ne_cgs(u, rho), th_e, out);
+    out3[0] = log10(out[0] * orc_rate_conv(u));
+    out3[1] = log10(out[1] * orc_rate_conv(u));
+    out3[2] = log10(out[2]);
+}
+
+/* Combine per-process code-unit rates into Q_total (code units), eqs 10-12, with the
+ * cell's own H (eqs 13-14 at r_ref).  frac3 (optional) = shares of Q_thin:
+ * brems, synchrotron, Compton-added. */
+double orc_combine_code(const orc_units *u, double rho, double th_e, double th_i,
+                        double qbr, double qsy, double eta, double *frac3)
+{
+    double conv = orc_rate_conv(u);
+    double H = orc_hth_cm(u, th_e, th_i, u->r_ref_rg);
+    double qthin = qbr + eta * qsy;
+    if (frac3) { frac3[0] = qbr / qthin; frac3[1] = qsy / qthin; frac3[2] = (eta - 1.0) * qsy / qthin; }
+    return orc_bridge_cgs(H, orc_ne_cgs(u, rho), th_e, qthin / conv) * conv;
+}
+
+/* ================================================================================
+ * Part B  the step.
+ * ============================================================================== */
+enum { ORC_AX_LOG_RHO = 0, ORC_AX_LOG_THETA_E = 1, ORC_AX_LOG_BSQ = 2, ORC_AX_LOG_THETA_I = 3 };
+
+typedef struct {
+    int ndim;               /* 3 or 4 (any 1..4 works)                              */
+    int axis[4];            /* which primitive each table axis is the log10 of      */
+    int n[4];               /* nodes per axis                                       */
+    double lo[4], hi[4];    /* log10 bounds, node-centred                           */
+    int nproc;              /* 1: total Lambda; 3: brems, synch, eta                */
+    const float *data[3];   /* row-major, axis[ndim-1] fastest, log10 values        */
+    const float *coul;      /* optional log10 C over (log Theta_i, log Theta_e)     */
+    int nc[2];
+    double clo[2], chi[2];
+} orc_table;
+
+/* B1: coordinate -> (i, w) with edge clamping (C-7).  Returns 1 if clamped. */
+static int orc_locate(double x, double lo, double hi, int n, int *i, double *w)
+{
+    double delta = (hi - lo) / (n - 1);
+    double t = (x - lo) / delta;
+    int clamped = 0;
+    if (t < 0.0) { t = 0.0; clamped = 1; }
+    if (t > (double)(n - 1)) { t = (double)(n - 1); clamped = 1; }
+    int ii = (int)floor(t);
+    if (ii > n - 2) ii = n - 2;
+    *i = ii; *w = t - ii;
+    return clamped;
+}
+
+/* B2: multilinear interpolation, y = sum over the 2^ndim corners of prod(w) * T. */
+double orc_interp(int ndim, const int *n, const double *lo, const double *hi,
+                  const float *T, const double *x, int *clamped)
+{
+    int i[4]; double w[4]; int cl = 0;
+    for (int k = 0; k < ndim; ++k) {
+        if (isnan(x[k])) { if (clamped) *clamped = 0; return NAN; }
+        cl |= orc_locate(x[k], lo[k], hi[k], n[k], &i[k], &w[k]);
+    }
+    if (clamped) *clamped = cl;
+    double y = 0.0;
+    for (int c = 0; c < (1 << ndim); ++c) {
+        double pw = 1.0; size_t off = 0;
+        for (int k = 0; k < ndim; ++k) {
+            int bit = (c >> k) & 1;
+            pw *= bit ? w[k] : (1.0 - w[k]);
+            off = off * (size_t)n[k] + (size_t)(i[k] + bit);
+        }
+        y += pw * (double)T[off];
+    }
+    return y;
+}
+
+/* One cell, nsub sub-steps (reading C-10).  rate_mode 0: table, 1: analytic Part A.
+ * coulomb_mode 0: off, 1: coefficient table, 2: analytic eq 15.
+ * diag7: lum_total, lum_brems, lum_synch, lum_compton, limited, floored, clamped. */
+static void orc_step_cell(const orc_table *tab, const orc_units *un,
+                          double rho, double bsq, double *the_io, double *thi_io,
+                          double r, double vol, double dt, int nsub, double f_limit, double h_floor,
+                          int rate_mode, int coulomb_mode,
+                          double *lam0, double *qcc0, double *diag7)
+{
+    const double mr = ORC_ME / ORC_MP;
+    const double ge1 = un->gamma_e - 1.0, gi1 = un->gamma_i - 1.0;
+    const double h = dt / nsub;
+    double the = *the_io, thi = *thi_io;
+    double de_sum[4] = {0, 0, 0, 0};
+    int limited = 0, floored = 0, clamped = 0;
+
+    for (int s = 0; s < nsub; ++s) {
+        /* B1/B2: rate lookup */
+        double prim[4];
+        prim[ORC_AX_LOG_RHO] = rho; prim[ORC_AX_LOG_THETA_E] = the;
+        prim[ORC_AX_LOG_BSQ] = bsq; prim[ORC_AX_LOG_THETA_I] = thi;
+        double lam, frac[3] = {0, 0, 0};
+        if (rate_mode == 0) {
+            double x[4]; int cl = 0;
+            for (int k = 0; k < tab->ndim; ++k) {       /* C-7: non-positive -> lower edge */
+                double q = prim[tab->axis[k]];
+                x[k] = (q > 0.0) ? log10(q) : -INFINITY;
+            }
+            if (tab->nproc == 1) {
+                lam = pow(10.0, orc_interp(tab->ndim, tab->n, tab->lo, tab->hi, tab->data[0], x, &cl));
+            } else {
+                double q[3];
+                for (int p = 0; p < 3; ++p)
+                    q[p] = pow(10.0, orc_interp(tab->ndim, tab->n, tab->lo, tab->hi, tab->data[p], x, &cl));
+                lam = orc_combine_code(un, rho, the, thi, q[0], q[1], q[2], frac);
+            }
+            clamped |= cl;
+        } else {
+            double out[6];
+            double H = (tab->ndim == 4) ? orc_hth_cm(un, the, thi, un->r_ref_rg) : un->hth_cm;
+            orc_cooling_cgs(H, orc_bfield_gauss(un, bsq), orc_ne_cgs(un, rho), the, out);
+            lam = out[4] * orc_rate_conv(un);
+            frac[0] = out[0] / out[3]; frac[1] = out[1] / out[3]; frac[2] = (out[2] - 1.0) * out[1] / out[3];
+        }
+        /* B3: temperature floor, eq 19 (L195), reading C-13 */
+        if (h_floor > 0.0 && r > 0.0) {
+            double tfloor = 0.5 * ORC_PI * pow(h_floor * orc_omega_k(r, un->spin) * r, 2.0);
+            if ((the + thi) * mr < tfloor) { lam = 0.0; floored = 1; }
+        }
+        /* B4: Coulomb */
+        double qcc = 0.0;
+        if (coulomb_mode == 1) {
+            double xc[2] = { thi > 0.0 ? log10(thi) : -INFINITY, the > 0.0 ? log10(the) : -INFINITY };
+            double C = pow(10.0, orc_interp(2, tab->nc, tab->clo, tab->chi, tab->coul, xc, NULL));
+            qcc = orc_coulomb_pref_cgs(un) * orc_rate_conv(un) * rho * rho * (thi - the) * C;
+        } else if (coulomb_mode == 2) {
+            qcc = (thi == the) ? 0.0 : orc_coulomb_code(un, rho, the, thi);
+        }
+        if (s == 0) { if (lam0) *lam0 = lam; if (qcc0) *qcc0 = qcc; }
+        /* B5: limited explicit update (L185; readings C-8, C-9) */
+        double ue = rho * the * mr / ge1, ui = rho * thi * mr / gi1;
+        double de = lam * h;
+        if (de > f_limit * ue) { de = f_limit * ue; limited = 1; }
+        double xeq = (ui * gi1 - ue * ge1) / (ge1 + gi1);   /* transfer that equalises Theta */
+        double x = fabs(qcc) * h;
+        double udonor = (qcc > 0.0) ? ui : ue;
+        if (x > f_limit * udonor) x = f_limit * udonor;
+        if (x > fabs(xeq)) x = fabs(xeq);
+        if (qcc < 0.0) x = -x;
+        if (qcc == 0.0) x = 0.0;
+        ue = ue - de + x;
+        ui = ui - x;
+        the = ue * ge1 / (mr * rho);
+        thi = ui * gi1 / (mr * rho);
+        de_sum[0] += de;
+        de_sum[1] += de * frac[0]; de_sum[2] += de * frac[1]; de_sum[3] += de * frac[2];
+    }
+    *the_io = the; *thi_io = thi;
+    /* B6: luminosity diagnostic, eq 22 (L222) restricted to the applied loss */
+    for (int k = 0; k < 4; ++k) diag7[k] = de_sum[k] * vol / dt;
+    diag7[4] = limited; diag7[5] = floored; diag7[6] = clamped;
+}
+
+/* Whole field.  r, vol, lam0, qcc0 may be NULL.  diag7 is the sum over cells. */
+void orc_step(const orc_table *tab, const orc_units *un, long long ncell,
+              const double *rho, const double *bsq, const double *the_in, const double *thi_in,
+              const double *r, const double *vol,
+              double dt, int nsub, double f_limit, double h_floor, int rate_mode, int coulomb_mode,
+              double *the_out, double *thi_out, double *lam0, double *qcc0, double *diag7, int nthreads)
+{
+    double acc[7] = {0, 0, 0, 0, 0, 0, 0};
+    if (nthreads < 1) nthreads = 1;
+#pragma omp parallel num_threads(nthreads)
+    {
+        double loc[7] = {0, 0, 0, 0, 0, 0, 0};
+#pragma omp for schedule(static)
+        for (long long c = 0; c < ncell; ++c) {
+            double the = the_in[c], thi = thi_in[c], d7[7];
+            if (isnan(rho[c]) || isnan(bsq[c]) || isnan(the) || isnan(thi)) {
+                the_out[c] = NAN; thi_out[c] = NAN;
+                if (lam0) lam0[c] = NAN;
+                if (qcc0) qcc0[c] = NAN;
+                continue;
+            }
+            if (!(rho[c] > 0.0)) {          /* no matter to cool: pass through */
+                the_out[c] = the; thi_out[c] = thi;
+                if (lam0) lam0[c] = 0.0;
+                if (qcc0) qcc0[c] = 0.0;
+                continue;
+            }
+            orc_step_cell(tab, un, rho[c], bsq[c], &the, &thi, r ? r[c] : 0.0, vol ? vol[c] : 1.0,
+                          dt, nsub, f_limit, h_floor, rate_mode, coulomb_mode,
+                          lam0 ? &lam0[c] : NULL, qcc0 ? &qcc0[c] : NULL, d7);
+            the_out[c] = the; thi_out[c] = thi;
+            for (int k = 0; k < 7; ++k) loc[k] += d7[k];
+        }
+#pragma omp critical
+        for (int k = 0; k < 7; ++k) acc[k] += loc[k];
+    }
+    if (diag7) memcpy(diag7, acc, sizeof acc);
+}
+
+/* Fill tables node by node from Part A (used by tests to check the product's builder
+ * and to build tiny brute-force tables).  Node coordinate = lo + i*(hi-lo)/(n-1). */
+void orc_fill_total3(const orc_units *un, const int *n, const double *lo, const double *hi, float *out, int nthreads)
+{
+    long long tot = (long long)n[0] * n[1] * n[2];
+#pragma omp parallel for schedule(dynamic, 64) num_threads(nthreads > 0 ? nthreads : 1)
+    for (long long t = 0; t < tot; ++t) {
+        int k = (int)(t % n[2]), j = (int)((t / n[2]) % n[1]), i = (int)(t / ((long long)n[1] * n[2]));
+        double rho = pow(10.0, lo[0] + i * (hi[0] - lo[0]) / (n[0] - 1));
+        double the = pow(10.0, lo[1] + j * (hi[1] - lo[1]) / (n[1] - 1));
+        double bsq = pow(10.0, lo[2] + k * (hi[2] - lo[2]) / (n[2] - 1));
+        out[t] = (float)orc_node_total_log10(un, rho, the, bsq);
+    }
+}
+void orc_fill_coulomb2(const orc_units *un, const int *nc, const double *clo, const double *chi, float *out)
+{
+    for (int a = 0; a < nc[0]; ++a)
+        for (int b = 0; b < nc[1]; ++b) {
+            double thi = pow(10.0, clo[0] + a * (chi[0] - clo[0]) / (nc[0] - 1));
+            double the = pow(10.0, clo[1] + b * (chi[1] - clo[1]) / (nc[1] - 1));
+            out[(size_t)a * nc[1] + b] = (float)log10(orc_coulomb_C(the, thi / un->ion_theta_mass_ratio));
+        }
+}
+int orc_max_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}

@@ -1,0 +1,296 @@
+"""Pins for oracle Part B (interpolation + limited, sub-stepped update; PAPER.md L122-L124,
+L181, L185, L197 and readings C-5..C-17): node-exactness, linear-exactness, a library
+interpolator, brute force on tiny tables, conservation / positivity / limits of the update.
+CPU only."""
+import itertools
+import math
+
+import numpy as np
+import pytest
+from scipy.interpolate import RegularGridInterpolator
+
+ME, MP = 9.1093837015e-28, 1.67262192369e-24
+MR = ME / MP
+AX3 = [0, 1, 2]            # (log rho, log Theta_e, log bsq)
+AX4 = [0, 1, 2, 3]         # (..., log Theta_i)
+
+
+def _rand_table(rng, n):
+    return rng.uniform(-30.0, -2.0, size=n).astype(np.float32)
+
+
+# ---------------------------------------------------------------- interpolation (B1, B2)
+@pytest.mark.parametrize("n", [(5, 4, 6), (3, 3, 3, 3), (7, 2, 5, 4)])
+def test_interp_exact_at_nodes_and_vs_scipy(oracle, n):
+    rng = np.random.default_rng(1)
+    nd = len(n)
+    lo = [-6.0, -3.0, -8.0, -3.0][:nd]
+    hi = [0.0, 1.5, 0.0, 1.5][:nd]
+    T = _rand_table(rng, n)
+    axes = [np.linspace(lo[k], hi[k], n[k]) for k in range(nd)]
+    for idx in itertools.islice(itertools.product(*[range(m) for m in n]), 0, None, 7):
+        y, cl = oracle.interp(n, lo, hi, T, [axes[k][idx[k]] for k in range(nd)])
+        assert y == pytest.approx(float(T[idx]), abs=1e-12) and not cl
+    rgi = RegularGridInterpolator(axes, T.astype(np.float64), method="linear")
+    pts = np.stack([rng.uniform(lo[k], hi[k], 400) for k in range(nd)], axis=1)
+    ref = rgi(pts)
+    for p, r in zip(pts, ref):
+        y, cl = oracle.interp(n, lo, hi, T, list(p))
+        assert y == pytest.approx(r, abs=1e-11) and not cl
+        corners = T  # interpolant bounded by table extrema (weights in [0,1], sum 1)
+        assert corners.min() - 1e-9 <= y <= corners.max() + 1e-9
+
+
+def test_interp_linear_functions_exact(oracle):
+    n, lo, hi = (9, 7, 5, 6), [-6.0, -3.0, -8.0, -3.0], [0.0, 1.5, 0.0, 1.5]
+    axes = np.meshgrid(*[np.linspace(lo[k], hi[k], n[k]) for k in range(4)], indexing="ij")
+    coef = [2.0, 0.5, -0.25, 1.0]
+    # choose coefficients/nodes so that node values are exactly representable in fp32
+    T = (4.0 + sum(c * np.round(a * 8) / 8 for c, a in zip(coef, axes))).astype(np.float32)
+    rng = np.random.default_rng(2)
+    lin = lambda x: 4.0 + sum(c * xi for c, xi in zip(coef, x))
+    # node coordinates were rounded to multiples of 1/8 only if they already are: use exact grid
+    n2, lo2, hi2 = (7, 5, 9, 4), [-6.0, -3.0, -8.0, -1.5], [0.0, 1.0, 0.0, 1.5]
+    axes2 = np.meshgrid(*[np.linspace(lo2[k], hi2[k], n2[k]) for k in range(4)], indexing="ij")
+    T2 = (4.0 + sum(c * a for c, a in zip(coef, axes2))).astype(np.float32)   # steps of 1, 1, 1, 1: exact
+    for _ in range(300):
+        x = [rng.uniform(lo2[k], hi2[k]) for k in range(4)]
+        y, _cl = oracle.interp(n2, lo2, hi2, T2, x)
+        assert y == pytest.approx(lin(x), abs=1e-12)
+
+
+def test_interp_clamps_to_edge(oracle):
+    rng = np.random.default_rng(3)
+    n, lo, hi = (4, 5, 3), [-6.0, -3.0, -8.0], [0.0, 1.5, 0.0]
+    T = _rand_table(rng, n)
+    inside, _ = oracle.interp(n, lo, hi, T, [-6.0, 0.3, -8.0])
+    out, cl = oracle.interp(n, lo, hi, T, [-9.5, 0.3, -20.0])
+    assert cl and out == inside
+    inside, _ = oracle.interp(n, lo, hi, T, [0.0, 1.5, -2.0])
+    out, cl = oracle.interp(n, lo, hi, T, [0.7, 1e3, -2.0])
+    assert cl and out == inside
+    out, cl = oracle.interp(n, lo, hi, T, [-math.inf, 0.3, -8.0])          # non-positive primitive
+    assert cl and out == oracle.interp(n, lo, hi, T, [-6.0, 0.3, -8.0])[0]
+    assert math.isnan(oracle.interp(n, lo, hi, T, [math.nan, 0.3, -8.0])[0])
+
+
+def test_interp_brute_force_formula(oracle):
+    """y = sum_corners prod(w) T written out directly on a 3^3 and a 3^4 table."""
+    rng = np.random.default_rng(4)
+    for n in ((3, 3, 3), (3, 3, 3, 3)):
+        nd = len(n)
+        lo, hi = [0.0] * nd, [2.0] * nd       # node spacing 1: t = x
+        T = _rand_table(rng, n)
+        for _ in range(200):
+            x = rng.uniform(0, 2, nd)
+            i = np.minimum(np.floor(x).astype(int), 1)
+            w = x - i
+            ref = 0.0
+            for c in itertools.product((0, 1), repeat=nd):
+                pw = np.prod([w[k] if c[k] else 1 - w[k] for k in range(nd)])
+                ref += pw * float(T[tuple(i + np.array(c))])
+            assert oracle.interp(n, lo, hi, T, list(x))[0] == pytest.approx(ref, abs=1e-12)
+
+
+# ---------------------------------------------------------------- the update (B3-B6)
+def _const_table(oracle, log_lambda, coul_logC=None, ndim=3):
+    n = [3] * ndim
+    lo = [-6.0, -3.0, -8.0, -3.0][:ndim]
+    hi = [0.0, 1.5, 0.0, 1.5][:ndim]
+    data = [np.full(n, log_lambda, dtype=np.float32)]
+    if coul_logC is None:
+        return oracle.Table(AX4[:ndim], n, lo, hi, data)
+    return oracle.Table(AX4[:ndim], n, lo, hi, data, coul=np.full((3, 3), coul_logC, np.float32),
+                        clo=[-3.0, -3.0], chi=[1.5, 1.5])
+
+
+def _cells(n, seed=5):
+    rng = np.random.default_rng(seed)
+    return (10 ** rng.uniform(-6, 0, n), 10 ** rng.uniform(-8, 0, n),
+            10 ** rng.uniform(-3, 1.5, n), 10 ** rng.uniform(-3, 1.5, n))
+
+
+def _u(rho, th, gam=5 / 3):
+    return rho * th * MR / (gam - 1)
+
+
+def test_update_conservation_positivity_diag(oracle):
+    un = oracle.Units()
+    rho, bsq, the, thi = _cells(2000)
+    vol = np.random.default_rng(6).uniform(0.5, 2.0, rho.size)
+    tab = _const_table(oracle, -9.0, coul_logC=0.0)
+    for nsub in (1, 4):
+        dt = 5.0
+        o = oracle.step(tab, un, rho, bsq, the, thi, dt, nsub=nsub, vol=vol, want_rates=True)
+        ue, ui = _u(rho, the), _u(rho, thi)
+        ue2, ui2 = _u(rho, o["theta_e"]), _u(rho, o["theta_i"])
+        assert (ue2 > 0).all() and (ui2 > 0).all()
+        # total energy changes only by the radiated part; the diagnostic is its volume integral
+        lost = (ue + ui) - (ue2 + ui2)
+        assert (lost >= -1e-14 * (ue + ui)).all()
+        assert o["diag"]["lum_total"] == pytest.approx(float((lost * vol).sum() / dt), rel=1e-10)
+        assert 0 < o["diag"]["n_limited"] < rho.size
+        assert o["diag"]["n_floored"] == 0
+        if nsub == 1:
+            assert o["diag"]["n_clamped"] == 0      # inputs are inside the table range
+        assert o["lam0"] == pytest.approx(1e-9, rel=1e-12)
+
+
+def test_update_strong_cooling_limit(oracle):
+    """Lambda -> inf, Coulomb off: u_e' = 0.7^nsub u_e (30 % limiter, L185), ions untouched."""
+    un = oracle.Units()
+    rho, bsq, the, thi = _cells(300)
+    tab = _const_table(oracle, 30.0)
+    for nsub in (1, 2, 4):
+        o = oracle.step(tab, un, rho, bsq, the, thi, 1e-3, nsub=nsub, coulomb_mode=oracle.COULOMB_OFF)
+        assert o["theta_e"] == pytest.approx(the * 0.7 ** nsub, rel=1e-13)
+        assert o["theta_i"] == pytest.approx(thi, rel=1e-15)
+        assert o["diag"]["n_limited"] == rho.size
+    o = oracle.step(tab, un, rho, bsq, the, thi, 1e-3, nsub=1, f_limit=0.1, coulomb_mode=oracle.COULOMB_OFF)
+    assert o["theta_e"] == pytest.approx(the * 0.9, rel=1e-13)
+
+
+def test_update_constant_rate_independent_of_nsub(oracle):
+    un = oracle.Units()
+    rho, bsq, the, thi = _cells(300)
+    tab = _const_table(oracle, -16.0)
+    a = oracle.step(tab, un, rho, bsq, the, thi, 1e-3, nsub=1, coulomb_mode=oracle.COULOMB_OFF)
+    b = oracle.step(tab, un, rho, bsq, the, thi, 1e-3, nsub=4, coulomb_mode=oracle.COULOMB_OFF)
+    assert a["diag"]["n_limited"] == 0
+    assert a["theta_e"] == pytest.approx(b["theta_e"], rel=1e-13)
+    # du_e = -Lambda dt exactly
+    assert _u(rho, the) - _u(rho, a["theta_e"]) == pytest.approx(1e-16 * 1e-3, rel=1e-6)
+
+
+def test_update_small_dt_derivative(oracle):
+    """dt -> 0: (u' - u)/dt -> -Lambda + Q_cc for electrons, -Q_cc for ions."""
+    un = oracle.Units()
+    rho, bsq, the, thi = _cells(200)
+    tab = _const_table(oracle, -14.0, coul_logC=-0.3)
+    dt = 1e-6
+    o = oracle.step(tab, un, rho, bsq, the, thi, dt, want_rates=True)
+    pref = oracle.coulomb_pref_cgs(un) * 4.925491e-5 / (3e-7 * 2.99792458e10 ** 2)
+    qcc = pref * rho ** 2 * (thi - the) * 10 ** -0.3
+    assert o["qcc0"] == pytest.approx(qcc, rel=2e-6)
+    assert o["lam0"] == pytest.approx(1e-14, rel=1e-12)
+    ue, ui = _u(rho, the), _u(rho, thi)
+    due = (_u(rho, o["theta_e"]) - ue) / dt
+    dui = (_u(rho, o["theta_i"]) - ui) / dt
+    ok = (np.abs(qcc) * dt < 1e-3 * np.minimum(ue, ui)) & (1e-14 * dt < 1e-3 * ue)   # limiter idle
+    assert ok.sum() > 50
+    # an unlimited explicit step is exactly linear in dt: only rounding of u remains
+    assert (np.abs(due - (-1e-14 + qcc)) <= 1e-6 * (1e-14 + np.abs(qcc)) + 8e-16 * ue / dt)[ok].all()
+    assert (np.abs(dui + qcc) <= 1e-6 * np.abs(qcc) + 8e-16 * ui / dt)[ok].all()
+    # and the rates are visible above the rounding noise for a good share of the cells
+    assert ((1e-14 + np.abs(qcc)) > 1e3 * 8e-16 * ue / dt)[ok].sum() > 20
+
+
+def test_coulomb_alone_no_crossing_and_zero_at_equality(oracle):
+    un = oracle.Units()
+    rho, bsq, the, thi = _cells(500)
+    tab = _const_table(oracle, -300.0, coul_logC=6.0)          # no radiation, violent exchange
+    o = oracle.step(tab, un, rho, bsq, the, thi, 1e3, nsub=8)
+    s0 = np.sign(thi - the)
+    d1 = o["theta_i"] - o["theta_e"]
+    d1[np.abs(d1) < 1e-14 * o["theta_i"]] = 0.0               # equalised up to rounding
+    s1 = np.sign(d1)
+    assert ((s1 == s0) | (s1 == 0)).all()                      # temperatures never cross
+    assert (np.abs(o["theta_i"] - o["theta_e"]) <= np.abs(thi - the) * (1 + 1e-12)).all()
+    # total energy conserved by the exchange
+    assert _u(rho, o["theta_e"]) + _u(rho, o["theta_i"]) == pytest.approx(_u(rho, the) + _u(rho, thi), rel=1e-12)
+    # after many strong sub-steps a good fraction has equalised exactly
+    assert (np.abs(o["theta_i"] / o["theta_e"] - 1) < 1e-12).mean() > 0.3
+    # exact zero exchange at T_e = T_i (north_star pin)
+    o = oracle.step(tab, un, rho, bsq, the, the.copy(), 1e3, nsub=3)
+    assert (o["theta_e"] == o["theta_i"]).all()
+    assert o["theta_e"] == pytest.approx(the, rel=1e-15)
+    # analytic Coulomb too
+    tab2 = _const_table(oracle, -300.0)
+    o = oracle.step(tab2, un, rho[:20], bsq[:20], the[:20], the[:20].copy(), 1e3, coulomb_mode=oracle.COULOMB_ANALYTIC)
+    assert (o["theta_e"] == o["theta_i"]).all() and o["theta_e"] == pytest.approx(the[:20], rel=1e-15)
+
+
+def test_equalising_transfer_unequal_gammas(oracle):
+    un = oracle.Units(gamma_e=4.0 / 3.0, gamma_i=5.0 / 3.0)
+    rho, bsq, the, thi = _cells(200)
+    tab = _const_table(oracle, -300.0, coul_logC=12.0)
+    o = oracle.step(tab, un, rho, bsq, the, thi, 1e6, nsub=40, f_limit=0.45)
+    assert o["theta_e"] == pytest.approx(o["theta_i"], rel=1e-9)   # converge to common Theta
+    etot0 = _u(rho, the, 4 / 3) + _u(rho, thi, 5 / 3)
+    etot1 = _u(rho, o["theta_e"], 4 / 3) + _u(rho, o["theta_i"], 5 / 3)
+    assert etot1 == pytest.approx(etot0, rel=1e-12)
+
+
+def test_floor_switches_cooling_off(oracle):
+    """eq 19 (L195): T_gas = p/rho below (pi/2)(h_floor Omega_K r)^2 => no cooling."""
+    un = oracle.Units()
+    n = 400
+    rho, bsq, _, _ = _cells(n)
+    r = np.full(n, 20.0)
+    tfloor = 0.5 * math.pi * (0.1 * 20.0 / (20.0 ** 1.5 + 0.9375)) ** 2
+    th_tot = tfloor / MR * np.linspace(0.5, 1.5, n)               # straddles the floor
+    the, thi = 0.25 * th_tot, 0.75 * th_tot
+    tab = _const_table(oracle, -6.0)
+    o = oracle.step(tab, un, rho, bsq, the, thi, 1e-2, h_floor=0.1, r=r, coulomb_mode=oracle.COULOMB_OFF)
+    below = (the + thi) * MR < tfloor
+    assert below.sum() > 100 and (~below).sum() > 100
+    assert o["theta_e"][below] == pytest.approx(the[below], rel=1e-15)
+    assert (o["theta_e"][~below] < the[~below]).all()
+    assert o["diag"]["n_floored"] == int(below.sum())
+    o2 = oracle.step(tab, un, rho, bsq, the, thi, 1e-2, h_floor=0.0, r=r, coulomb_mode=oracle.COULOMB_OFF)
+    assert (o2["theta_e"] < the).all()
+
+
+def test_passthrough_and_nan(oracle):
+    un = oracle.Units()
+    tab = _const_table(oracle, -6.0, coul_logC=0.0)
+    rho = np.array([0.0, -1.0, 1e-3, np.nan, 1e-3])
+    bsq = np.array([1e-4, 1e-4, 0.0, 1e-4, 1e-4])
+    the = np.array([0.5, 0.5, 0.5, 0.5, np.nan])
+    thi = np.array([2.0, 2.0, 2.0, 2.0, 2.0])
+    o = oracle.step(tab, un, rho, bsq, the, thi, 1e-3)
+    assert o["theta_e"][0] == 0.5 and o["theta_i"][1] == 2.0           # rho <= 0: unchanged
+    assert np.isfinite(o["theta_e"][2]) and o["theta_e"][2] != 0.5     # bsq = 0 clamps to lower edge
+    assert np.isnan(o["theta_e"][3]) and np.isnan(o["theta_e"][4])     # NaN in, NaN out, that cell only
+    assert o["diag"]["n_clamped"] == 1
+
+
+def test_table_step_reproduces_analytic_at_nodes(oracle):
+    """Exact reproduction at table nodes (north_star pin) + brute force on a tiny grid:
+    cells that sit exactly on nodes of an oracle-filled table give the analytic step."""
+    un = oracle.Units()
+    n, lo, hi = [4, 5, 4], [-5.0, -2.0, -6.0], [-2.0, 1.0, -3.0]      # node spacing 1, 0.75, 1 dex
+    T = oracle.fill_total3(un, n, lo, hi, nthreads=4)
+    tab = oracle.Table(AX3, n, lo, hi, [T])
+    g = np.meshgrid(*[np.linspace(lo[k], hi[k], n[k]) for k in range(3)], indexing="ij")
+    rho, the, bsq = (10 ** a.ravel() for a in g)
+    thi = 3.0 * the
+    a = oracle.step(tab, un, rho, bsq, the, thi, 1e-3, coulomb_mode=oracle.COULOMB_OFF, want_rates=True)
+    b = oracle.step(tab, un, rho, bsq, the, thi, 1e-3, coulomb_mode=oracle.COULOMB_OFF, want_rates=True,
+                    rate_mode=oracle.RATE_ANALYTIC)
+    assert a["lam0"] == pytest.approx(b["lam0"], rel=3e-6)        # fp32 rounding of log10 Lambda (|y|<~40)
+    assert a["theta_e"] == pytest.approx(b["theta_e"], rel=1e-6)
+    # and the stored node is the fp32 rounding of the analytic value
+    k = 37
+    idx = np.unravel_index(k, n)
+    assert float(T[idx]) == np.float32(oracle.node_total_log10(un, rho[k], the[k], bsq[k]))
+
+
+def test_process_tables_and_luminosity_split(oracle):
+    """nproc = 3 (config 5): per-process tables recombined by eqs 10-12 with the cell's H;
+    luminosity shares add up to the total."""
+    un = oracle.Units()
+    n, lo, hi = [3, 4, 3, 3], [-4.0, -1.5, -5.0, -1.0], [-2.0, 1.5, -3.0, 1.0]
+    g = np.meshgrid(*[np.linspace(lo[k], hi[k], n[k]) for k in range(4)], indexing="ij")
+    nodes = np.stack([10 ** a.ravel() for a in g], axis=1)
+    vals = np.array([oracle.node_proc_log10(un, *row) for row in nodes], dtype=np.float32)
+    data = [vals[:, p].reshape(n) for p in range(3)]
+    tab = oracle.Table(AX4, n, lo, hi, data)
+    rho, the, bsq, thi = nodes.T
+    a = oracle.step(tab, un, rho, bsq, the, thi, 1e-2, coulomb_mode=oracle.COULOMB_OFF, want_rates=True)
+    b = oracle.step(tab, un, rho, bsq, the, thi, 1e-2, coulomb_mode=oracle.COULOMB_OFF, want_rates=True,
+                    rate_mode=oracle.RATE_ANALYTIC)
+    assert a["lam0"] == pytest.approx(b["lam0"], rel=1e-5)
+    d = a["diag"]
+    assert d["lum_brems"] + d["lum_synch"] + d["lum_compton"] == pytest.approx(d["lum_total"], rel=1e-12)
+    assert d["lum_brems"] > 0 and d["lum_synch"] > 0 and d["lum_compton"] >= 0
