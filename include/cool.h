@@ -1,0 +1,171 @@
+/*
+ * cool.h — C ABI of the B200-native per-cell two-temperature radiative cooling step of
+ * arXiv 2505.08855.  The library is libcool_b200.so; every compute step runs in
+ * hand-written sm_100a CUDA kernels.  There is no CPU fallback: every entry point that
+ * touches a device returns COOL_ECUDA when no usable CUDA device exists.
+ *
+ * What the step computes (per cell: "The cooling function utilizes the
+ * values of H_th, B, n_e and T_e obtained from the simulation to find the appropriate
+ * interpolated cooling rate from a precomputed table"; L185: the explicit limiter;
+ * L197: the temperature floor; L140-L147: Coulomb exchange):
+ *
+ *   repeat nsub times with h = dt/nsub:
+ *     x_k   = log10(primitive of table axis k)            (L122-L124: log-spaced axes)
+ *     t_k   = clamp((x_k - lo_k)/Delta_k, 0, n_k - 1)      (edge clamp, texture-clamp semantics)
+ *     y     = multilinear interpolation of the stored log10 values;  rate = 10^y
+ *     nproc = 1: Lambda = rate.   nproc = 3: Q_thin = Q_brem + eta Q_syn (eq 10) and
+ *             Lambda = Q_total of eqs 11-12 (L110-L116) with the cell's H_th (eqs 13-14)
+ *     floor : Lambda = 0 when p_gas/rho < (pi/2)(h_floor Omega_K r)^2      (eq 19)
+ *     Q_cc  : eq 15 (L142-L144), from a coefficient table or analytically
+ *     dE    = min(Lambda h, f_limit u_e)                                   (L185)
+ *     x     = sign(Q_cc) min(|Q_cc| h, f_limit u_donor, equalising transfer)
+ *     u_e  += x - dE ;  u_i -= x ;  Theta_s = u_s (gamma_s - 1)(m_p/m_e)/rho
+ *   luminosity diagnostic  L = sum dE vol / dt                             (eq 22)
+ *
+ * Conventions: Theta_s = k_B T_s/(m_e c^2) for BOTH species (L63, L147); rho in units of
+ * units.rho_scale_cgs; bsq = b^2 with (4 pi)^-1/2 absorbed (L173); times in r_g/c of
+ * units.mbh_msun; u_s = rho Theta_s (m_e/m_p)/(gamma_s - 1).  dt is fluid-frame time.
+ *
+ * All functions return cool_status (0 = COOL_OK), never abort and never print.  After a
+ * failure cool_last_error() holds a thread-local message.
+ */
+#ifndef COOL_H
+#define COOL_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum { COOL_OK = 0, COOL_EINVAL = 1, COOL_ENOMEM = 2, COOL_ECUDA = 3, COOL_EUNSUPPORTED = 4 } cool_status;
+typedef enum { COOL_F32 = 0, COOL_F64 = 1 } cool_dtype;
+typedef enum { COOL_AX_LOG_RHO = 0, COOL_AX_LOG_THETA_E = 1, COOL_AX_LOG_BSQ = 2, COOL_AX_LOG_THETA_I = 3 } cool_axis;
+
+/* Kernel variants (north_star (c)).  All give the same result within the fp tolerance except
+ * COOL_V_TEX_HWFILTER, whose hardware filter uses 8-bit fixed-point weights (reported, not
+ * gated), and COOL_V_ANALYTIC, which ignores the table values and evaluates eqs 1-12. */
+typedef enum {
+    COOL_V_AUTO = 0,         /* library picks: SMEM if the table fits, else GLOBAL          */
+    COOL_V_TEX_POINT = 1,    /* cudaTextureObject point fetches + software weights          */
+    COOL_V_TEX_HWFILTER = 2, /* hardware-filtered texture (linear filter mode)              */
+    COOL_V_SMEM = 3,         /* table staged in shared memory (<= ~200 KB)                  */
+    COOL_V_GLOBAL = 4,       /* L2-resident global-memory gathers through the read-only path */
+    COOL_V_ANALYTIC = 5      /* eqs 1-12 evaluated per cell, no table                       */
+} cool_variant;
+
+typedef enum { COOL_COULOMB_AUTO = 0, /* coefficient table if the cool_table has one, else analytic */
+               COOL_COULOMB_OFF = 1, COOL_COULOMB_TABLE = 2, COOL_COULOMB_ANALYTIC = 3 } cool_coulomb_mode;
+
+/* Unit system and fixed parameters of the physics (Table I). */
+typedef struct {
+    double rho_scale_cgs;        /* g cm^-3 per code density unit (Table I)                      */
+    double mbh_msun;             /* black-hole mass in solar masses (L220: 10)                   */
+    double gamma_e, gamma_i;     /* adiabatic indices (L207: 5/3)                                */
+    double ln_lambda;            /* Coulomb logarithm (L147: 20)                                 */
+    double ion_theta_mass_ratio; /* theta_i used inside eq 15 = Theta_i / this; 1 = as printed   */
+    double hth_cm;               /* H_th [cm] for tables without a Theta_i axis                  */
+    double r_ref_rg, spin;       /* radius [r_g] and spin for H_th = c_s/Omega_K (eqs 13-14)     */
+} cool_units;
+
+/* A cooling table as data.  Two shapes are supported:
+ *   ndim = 3, nproc = 1 : axes are a permutation of {LOG_RHO, LOG_THETA_E, LOG_BSQ};
+ *                         host_data[0] = log10 Lambda_code (total rate at H_th = units.hth_cm)
+ *   ndim = 4, nproc = 3 : axes are a permutation of all four; host_data[0..2] =
+ *                         log10 Q_brem_code, log10 Q_syn_code, log10 eta_compton; H_th from
+ *                         eqs 13-14 at r_ref with the cell's Theta_e + Theta_i
+ * nproc = 0 (no data) is allowed: only COOL_V_ANALYTIC can then be applied.
+ * Arrays are row-major with axis[ndim-1] fastest, n[0]*...*n[ndim-1] floats each, node k of
+ * axis a at log10-coordinate lo[a] + k (hi[a]-lo[a])/(n[a]-1); n[a] >= 2, hi[a] > lo[a].
+ * host_coulomb (optional, may be NULL) = log10 C(Theta_i, Theta_e), nc[0] x nc[1] floats,
+ * Theta_e fastest, where Q_cc = pref rho^2 (Theta_i - Theta_e) C (eq 15). */
+typedef struct {
+    int ndim;
+    int axis[4];                 /* cool_axis values */
+    int n[4];
+    double lo[4], hi[4];
+    int nproc;
+    const float *host_data[3];   /* HOST pointers; copied by cool_table_create */
+    const float *host_coulomb;   /* HOST pointer or NULL */
+    int nc[2];
+    double clo[2], chi[2];
+    cool_units units;
+} cool_table_desc;
+
+/* One batch of cells, structure of arrays, ncell contiguous elements of `dtype` each.
+ * cool_apply: DEVICE pointers.  cool_apply_host: HOST pointers (pinned memory makes the
+ * copies asynchronous).  theta_*_out may alias theta_*_in.  The caller owns all of them;
+ * the library never frees or keeps them.  16-byte alignment enables 128-bit accesses;
+ * other alignments are accepted and take a scalar path. */
+typedef struct {
+    long long ncell;
+    cool_dtype dtype;
+    const void *rho, *bsq;                     /* read-only */
+    const void *theta_e_in, *theta_i_in;       /* read-only unless aliased by the outputs */
+    void *theta_e_out, *theta_i_out;
+    const void *r;                             /* optional radius [r_g] per cell; NULL: no floor */
+    const void *vol;                           /* optional sqrt(-g) dV weights; NULL: 1 */
+} cool_cells;
+
+typedef struct {
+    double dt;                   /* fluid-frame time step [r_g/c], > 0 */
+    int nsub;                    /* >= 1 equal sub-steps */
+    double f_limit;              /* 0 < f_limit < 0.5; the paper uses 0.3 (L185) */
+    double h_floor;              /* (H/R)_floor of eq 19; 0 = off; needs cells.r */
+    cool_variant variant;
+    cool_coulomb_mode coulomb;
+} cool_params;
+
+/* Diagnostics of one call (sums over the cells of the call; overwritten, not accumulated).
+ * lum_* = sum dE vol/dt, split by the shares of Q_thin (brems, synch, Compton-added) when
+ * nproc = 3, zero otherwise.  n_* count cells in which the event happened in any sub-step. */
+typedef struct {
+    double lum_total, lum_brems, lum_synch, lum_compton;
+    long long n_limited, n_floored, n_clamped;
+} cool_diag;
+
+typedef struct cool_table cool_table;      /* opaque */
+
+/* Host table builder (north_star (a)): tabulates eqs 1-12 (and eq 15's coefficient C when
+ * out_coulomb != NULL) on the grid that `shape` describes (its host_data / host_coulomb
+ * pointers are ignored).  out[p] must hold prod(n) floats for p < nproc; out_coulomb
+ * nc[0]*nc[1] floats.  Runs on `nthreads` host threads (<= 0: all available).  Host only;
+ * needs no GPU.  Errors: COOL_EINVAL for a malformed shape. */
+cool_status cool_table_build_host(const cool_table_desc *shape, float *const out[3], float *out_coulomb, int nthreads);
+
+/* Uploads a table to `device` and prepares every device representation (linear arrays,
+ * cudaArray + texture objects, the shared-memory image).  Host arrays are copied; the
+ * caller may free them on return.  *out is owned by the library until cool_table_destroy.
+ * Errors: COOL_EINVAL (shape, NULL, non-finite values), COOL_ENOMEM, COOL_ECUDA. */
+cool_status cool_table_create(const cool_table_desc *desc, int device, cool_table **out);
+
+/* One cooling + Coulomb update of all cells, asynchronous on `cuda_stream` (a cudaStream_t;
+ * NULL = the default stream).  Does not synchronise.  Safe to call concurrently on different
+ * streams with the same table.  d_diag: DEVICE pointer to one cool_diag, or NULL.
+ * Per-cell numerical trouble is not an error: non-positive bsq/Theta clamp to the lower
+ * table edge, rho <= 0 leaves the cell unchanged, NaN inputs give NaN outputs for that
+ * cell only.  Errors: COOL_EINVAL (NULL/negative sizes/params out of range),
+ * COOL_EUNSUPPORTED (variant impossible for this table, e.g. SMEM with a table that does not
+ * fit; COOL_V_AUTO never fails this way), COOL_ECUDA. */
+cool_status cool_apply(const cool_table *table, const cool_cells *cells, const cool_params *params,
+                       cool_diag *d_diag, void *cuda_stream);
+
+/* Same update for HOST arrays: the library stages chunks through device memory it owns,
+ * overlapping host->device copies, kernels and device->host copies on internal streams, and
+ * returns after the outputs (and *h_diag, if not NULL) are complete in host memory. */
+cool_status cool_apply_host(const cool_table *table, const cool_cells *host_cells, const cool_params *params,
+                            cool_diag *h_diag);
+
+/* Which variant COOL_V_AUTO resolves to for this table (always a concrete variant). */
+cool_variant cool_table_auto_variant(const cool_table *table);
+
+/* Number of kernel launches the last cool_apply / cool_apply_host on this thread issued. */
+int cool_last_launch_count(void);
+
+cool_status cool_table_destroy(cool_table *table);
+
+const char *cool_last_error(void);         /* thread-local, never NULL */
+const char *cool_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* COOL_H */

@@ -1,0 +1,374 @@
+// cool_api.cu — the C ABI of include/cool.h: table objects, argument checking, launches,
+// the host-buffer (end-to-end) path.  No compute happens here.
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "cool_internal.h"
+
+namespace cool {
+
+static thread_local char g_err[512] = "";
+static thread_local int g_launches = 0;
+
+void set_error(const char *fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof g_err, fmt, ap);
+    va_end(ap);
+}
+
+#define CUDA_TRY(call, what)                                                            \
+    do {                                                                                \
+        cudaError_t e_ = (call);                                                        \
+        if (e_ != cudaSuccess) {                                                        \
+            set_error("%s: %s", what, cudaGetErrorString(e_));                          \
+            return e_ == cudaErrorMemoryAllocation ? COOL_ENOMEM : COOL_ECUDA;          \
+        }                                                                               \
+    } while (0)
+
+static int canon_slot(int axis_kind)
+{
+    switch (axis_kind) {
+        case COOL_AX_LOG_RHO: return CAX_RHO;
+        case COOL_AX_LOG_THETA_E: return CAX_THE;
+        case COOL_AX_LOG_THETA_I: return CAX_THI;
+        default: return CAX_BSQ;
+    }
+}
+
+static AxisCoef make_axis(int n, double lo, double hi)
+{
+    AxisCoef a{};
+    const double L10 = 3.321928094887362;
+    const double delta = (hi - lo) / (n - 1);
+    a.n = n;
+    a.lo10 = lo; a.inv10 = 1.0 / delta;
+    const double lo2 = lo * L10, inv2 = 1.0 / (delta * L10);
+    const double e0 = floor(lo2);
+    a.e0 = (float)e0; a.invf = (float)inv2;
+    a.cf = (float)(-(lo2 - e0) * inv2);
+    return a;
+}
+
+static void free_table(cool_table *t)
+{
+    if (!t) return;
+    cudaSetDevice(t->device);
+    if (t->dev.tex_pt) cudaDestroyTextureObject(t->dev.tex_pt);
+    if (t->dev.tex_lin) cudaDestroyTextureObject(t->dev.tex_lin);
+    if (t->arr) cudaFreeArray(t->arr);
+    if (t->d_lin) cudaFree(t->d_lin);
+    if (t->d_coul) cudaFree(t->d_coul);
+    for (auto &kv : t->diag_ws) { cudaFree(kv.second.partials); cudaFree(kv.second.ticket); }
+    for (auto &s : t->stages) {
+        for (void *b : s.buf) if (b) cudaFree(b);
+        if (s.d_diag) cudaFree(s.d_diag);
+        if (s.s) cudaStreamDestroy(s.s);
+    }
+    if (t->h_diag_pinned) cudaFreeHost(t->h_diag_pinned);
+    delete t;
+}
+
+static cool_status get_diag_ws(const cool_table *t, cudaStream_t st, DiagWorkspace *out)
+{
+    std::lock_guard<std::mutex> lk(t->mu);
+    auto it = t->diag_ws.find(st);
+    if (it == t->diag_ws.end()) {
+        DiagWorkspace w;
+        w.capacity_blocks = t->sm_count * 32;
+        CUDA_TRY(cudaMalloc(&w.partials, sizeof(double) * 8 * (size_t)w.capacity_blocks), "cudaMalloc(diag partials)");
+        CUDA_TRY(cudaMalloc(&w.ticket, sizeof(unsigned)), "cudaMalloc(diag ticket)");
+        CUDA_TRY(cudaMemset(w.ticket, 0, sizeof(unsigned)), "cudaMemset(diag ticket)");
+        it = t->diag_ws.emplace(st, w).first;
+    }
+    *out = it->second;
+    return COOL_OK;
+}
+
+static cool_status check_args(const cool_table *t, const cool_cells *c, const cool_params *p, cool_variant *v, int *coul)
+{
+    if (!t || !c || !p) { set_error("NULL table, cells or params"); return COOL_EINVAL; }
+    if (c->ncell < 0) { set_error("ncell < 0"); return COOL_EINVAL; }
+    if (c->dtype != COOL_F32 && c->dtype != COOL_F64) { set_error("unknown dtype"); return COOL_EINVAL; }
+    if (c->ncell > 0 && (!c->rho || !c->bsq || !c->theta_e_in || !c->theta_i_in || !c->theta_e_out || !c->theta_i_out)) {
+        set_error("NULL cell array"); return COOL_EINVAL;
+    }
+    if (!(p->dt > 0.0) || !std::isfinite(p->dt)) { set_error("dt must be finite and > 0"); return COOL_EINVAL; }
+    if (p->nsub < 1 || p->nsub > 1024) { set_error("nsub must be in [1, 1024]"); return COOL_EINVAL; }
+    if (!(p->f_limit > 0.0 && p->f_limit < 0.5)) { set_error("f_limit must be in (0, 0.5)"); return COOL_EINVAL; }
+    if (!(p->h_floor >= 0.0)) { set_error("h_floor must be >= 0"); return COOL_EINVAL; }
+    cool_variant vv = p->variant;
+    if (vv == COOL_V_AUTO) vv = cool_table_auto_variant(t);
+    if (vv < COOL_V_TEX_POINT || vv > COOL_V_ANALYTIC) { set_error("unknown variant"); return COOL_EINVAL; }
+    std::string why;
+    if (!variant_supported(t, vv, c->dtype, &why)) { set_error("variant unsupported: %s", why.c_str()); return COOL_EUNSUPPORTED; }
+    if ((vv == COOL_V_TEX_POINT || vv == COOL_V_TEX_HWFILTER) && !t->dev.tex_pt) { set_error("variant unsupported: table too large for a 3-D texture"); return COOL_EUNSUPPORTED; }
+    int cm;
+    switch (p->coulomb) {
+        case COOL_COULOMB_AUTO: cm = t->dev.coul ? 1 : 2; break;
+        case COOL_COULOMB_OFF: cm = 0; break;
+        case COOL_COULOMB_TABLE:
+            if (!t->dev.coul) { set_error("COOL_COULOMB_TABLE but the table has no Coulomb coefficient table"); return COOL_EINVAL; }
+            cm = 1; break;
+        case COOL_COULOMB_ANALYTIC: cm = 2; break;
+        default: set_error("unknown coulomb mode"); return COOL_EINVAL;
+    }
+    *v = vv; *coul = cm;
+    return COOL_OK;
+}
+
+}  // namespace cool
+
+using namespace cool;
+
+extern "C" const char *cool_last_error(void) { return g_err; }
+extern "C" const char *cool_version(void) { return "cool_b200 0.1 (sm_100a)"; }
+extern "C" int cool_last_launch_count(void) { return g_launches; }
+
+extern "C" cool_variant cool_table_auto_variant(const cool_table *t)
+{
+    if (!t || t->dev.mode == 0) return COOL_V_ANALYTIC;
+    if ((size_t)t->dev.table_bytes + 1024 <= (size_t)t->max_smem_optin) return COOL_V_SMEM;
+    return COOL_V_GLOBAL;
+}
+
+extern "C" cool_status cool_table_create(const cool_table_desc *desc, int device, cool_table **out)
+{
+    if (!out) { set_error("cool_table_create: out is NULL"); return COOL_EINVAL; }
+    *out = nullptr;
+    std::string why;
+    if (!desc_valid(desc, desc && desc->host_coulomb != nullptr, &why)) { set_error("cool_table_create: %s", why.c_str()); return COOL_EINVAL; }
+    for (int p = 0; p < desc->nproc; ++p)
+        if (!desc->host_data[p]) { set_error("cool_table_create: host_data[%d] is NULL", p); return COOL_EINVAL; }
+    int ndev = 0;
+    CUDA_TRY(cudaGetDeviceCount(&ndev), "cudaGetDeviceCount");
+    if (device < 0 || device >= ndev) { set_error("cool_table_create: device %d of %d", device, ndev); return COOL_ECUDA; }
+    CUDA_TRY(cudaSetDevice(device), "cudaSetDevice");
+
+    cool_table *t = new (std::nothrow) cool_table();
+    if (!t) { set_error("out of host memory"); return COOL_ENOMEM; }
+    t->device = device;
+    t->desc = *desc;
+    t->desc.host_data[0] = t->desc.host_data[1] = t->desc.host_data[2] = nullptr;
+    t->desc.host_coulomb = nullptr;
+    cudaDeviceProp prop;
+    cudaError_t pe = cudaGetDeviceProperties(&prop, device);
+    if (pe != cudaSuccess) { set_error("cudaGetDeviceProperties: %s", cudaGetErrorString(pe)); free_table(t); return COOL_ECUDA; }
+    t->sm_count = prop.multiProcessorCount;
+    t->max_smem_optin = (int)prop.sharedMemPerBlockOptin;
+
+    // unit constants
+    DevConst &K = t->cst;
+    K.units = to_units(desc->units);
+    K.der = coolphys::derive(K.units);
+    K.mr = coolphys::kMR; K.ge1 = K.units.gamma_e - 1.0; K.gi1 = K.units.gamma_i - 1.0;
+    K.coul_k = K.der.coul_pref_code / K.mr;
+    const double t1 = coolphys::kTHETA_TO_K;
+    K.bb_k = 4.0 * coolphys::kSIGSB * t1 * t1 * t1 * t1 * K.der.rate_conv;
+    K.tausca_k = 2.0 * coolphys::kSIGT * K.der.ne_per_rho;
+    K.log2_ue_k = log2(K.mr / K.ge1);
+
+    DevTable &D = t->dev;
+    auto fail = [&](cool_status s) { free_table(t); return s; };
+    const int nd = desc->ndim;
+    D.mode = desc->nproc == 0 ? 0 : nd;
+    int ncan[4] = {1, 1, 1, 1};
+    for (int k = 0; k < nd; ++k) {
+        const int slot = canon_slot(desc->axis[k]);
+        D.ax[slot] = make_axis(desc->n[k], desc->lo[k], desc->hi[k]);
+        ncan[slot] = desc->n[k];
+    }
+    if (nd == 3) D.ax[CAX_THI] = make_axis(2, 0.0, 1.0);
+    D.s_thi = ncan[CAX_BSQ];
+    D.s_the = ncan[CAX_THI] * D.s_thi;
+    D.s_rho = ncan[CAX_THE] * D.s_the;
+
+    if (desc->nproc > 0) {
+        const long long total = (long long)ncan[0] * ncan[1] * ncan[2] * ncan[3];
+        const int chan = (nd == 3) ? 1 : 4;
+        const size_t bytes = ((size_t)total * chan * sizeof(float) + 15) & ~(size_t)15;
+        if (bytes > 0xffffffffull) { set_error("table too large"); return fail(COOL_EINVAL); }
+        std::vector<float> canon;
+        try { canon.assign(bytes / sizeof(float), 0.f); } catch (...) { set_error("out of host memory"); return fail(COOL_ENOMEM); }
+        long long sstride[4];
+        { long long s = 1; for (int k = nd - 1; k >= 0; --k) { sstride[k] = s; s *= desc->n[k]; } }
+        long long cstride_of_src[4];          // canonical stride (in nodes) for source axis k
+        for (int k = 0; k < nd; ++k) {
+            const int slot = canon_slot(desc->axis[k]);
+            cstride_of_src[k] = slot == CAX_RHO ? D.s_rho : slot == CAX_THE ? D.s_the : slot == CAX_THI ? D.s_thi : 1;
+        }
+        int idx[4] = {0, 0, 0, 0};
+        for (long long f = 0; f < total; ++f) {
+            long long coff = 0;
+            for (int k = 0; k < nd; ++k) coff += idx[k] * cstride_of_src[k];
+            for (int p = 0; p < desc->nproc; ++p) {
+                const float v = desc->host_data[p][f];
+                if (!std::isfinite(v)) { set_error("cool_table_create: non-finite value in host_data[%d]", p); return fail(COOL_EINVAL); }
+                canon[(size_t)coff * chan + p] = v;
+            }
+            for (int k = nd - 1; k >= 0; --k) { if (++idx[k] < desc->n[k]) break; idx[k] = 0; }
+        }
+        (void)sstride;
+        cudaError_t e = cudaMalloc(&t->d_lin, bytes);
+        if (e != cudaSuccess) { set_error("cudaMalloc(table): %s", cudaGetErrorString(e)); return fail(e == cudaErrorMemoryAllocation ? COOL_ENOMEM : COOL_ECUDA); }
+        e = cudaMemcpy(t->d_lin, canon.data(), bytes, cudaMemcpyHostToDevice);
+        if (e != cudaSuccess) { set_error("cudaMemcpy(table): %s", cudaGetErrorString(e)); return fail(COOL_ECUDA); }
+        D.table_bytes = (unsigned)bytes;
+        if (nd == 3) D.lin1 = t->d_lin; else D.lin4 = (const float4 *)t->d_lin;
+
+        // cudaArray + texture objects (x = bsq, y = theta_e | theta_i, z = rho | rho*n_the + i_the)
+        const size_t ex = ncan[CAX_BSQ];
+        const size_t ey = nd == 3 ? ncan[CAX_THE] : ncan[CAX_THI];
+        const size_t ez = nd == 3 ? ncan[CAX_RHO] : (size_t)ncan[CAX_RHO] * ncan[CAX_THE];
+        if (ex <= 16384 && ey <= 16384 && ez <= 16384) {
+            cudaChannelFormatDesc cd = nd == 3 ? cudaCreateChannelDesc<float>() : cudaCreateChannelDesc<float4>();
+            e = cudaMalloc3DArray(&t->arr, &cd, make_cudaExtent(ex, ey, ez));
+            if (e == cudaSuccess) {
+                cudaMemcpy3DParms cp{};
+                cp.srcPtr = make_cudaPitchedPtr(canon.data(), ex * chan * sizeof(float), ex, ey);
+                cp.dstArray = t->arr;
+                cp.extent = make_cudaExtent(ex, ey, ez);
+                cp.kind = cudaMemcpyHostToDevice;
+                e = cudaMemcpy3D(&cp);
+            }
+            if (e == cudaSuccess) {
+                cudaResourceDesc rd{};
+                rd.resType = cudaResourceTypeArray; rd.res.array.array = t->arr;
+                cudaTextureDesc td{};
+                td.addressMode[0] = td.addressMode[1] = td.addressMode[2] = cudaAddressModeClamp;
+                td.readMode = cudaReadModeElementType; td.normalizedCoords = 0;
+                td.filterMode = cudaFilterModePoint;
+                e = cudaCreateTextureObject(&D.tex_pt, &rd, &td, nullptr);
+                if (e == cudaSuccess) { td.filterMode = cudaFilterModeLinear; e = cudaCreateTextureObject(&D.tex_lin, &rd, &td, nullptr); }
+            }
+            if (e != cudaSuccess) { set_error("texture setup: %s", cudaGetErrorString(e)); return fail(e == cudaErrorMemoryAllocation ? COOL_ENOMEM : COOL_ECUDA); }
+        }
+    }
+    if (desc->host_coulomb) {
+        const size_t n = (size_t)desc->nc[0] * desc->nc[1];
+        for (size_t k = 0; k < n; ++k)
+            if (!std::isfinite(desc->host_coulomb[k])) { set_error("cool_table_create: non-finite value in host_coulomb"); return fail(COOL_EINVAL); }
+        cudaError_t e = cudaMalloc(&t->d_coul, n * sizeof(float));
+        if (e == cudaSuccess) e = cudaMemcpy(t->d_coul, desc->host_coulomb, n * sizeof(float), cudaMemcpyHostToDevice);
+        if (e != cudaSuccess) { set_error("Coulomb table upload: %s", cudaGetErrorString(e)); return fail(e == cudaErrorMemoryAllocation ? COOL_ENOMEM : COOL_ECUDA); }
+        D.coul = t->d_coul;
+        D.cax[0] = make_axis(desc->nc[0], desc->clo[0], desc->chi[0]);
+        D.cax[1] = make_axis(desc->nc[1], desc->clo[1], desc->chi[1]);
+    }
+    *out = t;
+    return COOL_OK;
+}
+
+extern "C" cool_status cool_table_destroy(cool_table *t)
+{
+    if (!t) return COOL_OK;
+    free_table(t);
+    return COOL_OK;
+}
+
+extern "C" cool_status cool_apply(const cool_table *t, const cool_cells *c, const cool_params *p, cool_diag *d_diag, void *stream)
+{
+    g_launches = 0;
+    cool_variant v; int coul;
+    cool_status s = check_args(t, c, p, &v, &coul);
+    if (s != COOL_OK) return s;
+    CUDA_TRY(cudaSetDevice(t->device), "cudaSetDevice");
+    cudaStream_t st = (cudaStream_t)stream;
+    LaunchArgs a{};
+    a.ncell = c->ncell; a.rho = c->rho; a.bsq = c->bsq; a.the_in = c->theta_e_in; a.thi_in = c->theta_i_in;
+    a.r = c->r; a.vol = c->vol; a.the_out = c->theta_e_out; a.thi_out = c->theta_i_out;
+    a.dt = p->dt; a.nsub = p->nsub; a.f_limit = p->f_limit; a.h_floor = p->h_floor; a.coulomb = coul;
+    a.want_diag = d_diag != nullptr; a.d_diag = d_diag;
+    if (d_diag) {
+        DiagWorkspace w;
+        s = get_diag_ws(t, st, &w);
+        if (s != COOL_OK) return s;
+        a.partials = w.partials; a.ticket = w.ticket;
+    }
+    if (c->ncell == 0) {
+        if (d_diag) CUDA_TRY(cudaMemsetAsync(d_diag, 0, sizeof(cool_diag), st), "cudaMemsetAsync(diag)");
+        return COOL_OK;
+    }
+    return launch_step(t, v, c->dtype, a, st, &g_launches);
+}
+
+extern "C" cool_status cool_apply_host(const cool_table *t, const cool_cells *c, const cool_params *p, cool_diag *h_diag)
+{
+    g_launches = 0;
+    cool_variant v; int coul;
+    cool_status s = check_args(t, c, p, &v, &coul);
+    if (s != COOL_OK) return s;
+    CUDA_TRY(cudaSetDevice(t->device), "cudaSetDevice");
+    if (h_diag) memset(h_diag, 0, sizeof *h_diag);
+    if (c->ncell == 0) return COOL_OK;
+
+    std::lock_guard<std::mutex> lk_host(t->host_mu);
+    const size_t es = c->dtype == COOL_F32 ? 4 : 8;
+    const int NST = 3;
+    size_t chunk = (size_t)1 << 22;                               // cells per staged chunk
+    if ((size_t)c->ncell < chunk) chunk = ((size_t)c->ncell + 3) & ~(size_t)3;
+    const size_t need_bytes = chunk * es;
+    if (t->stages.empty()) {
+        t->stages.resize(NST);
+        for (auto &sg : t->stages) {
+            CUDA_TRY(cudaStreamCreateWithFlags(&sg.s, cudaStreamNonBlocking), "cudaStreamCreate");
+            CUDA_TRY(cudaMalloc(&sg.d_diag, sizeof(cool_diag)), "cudaMalloc(stage diag)");
+        }
+    }
+    if (t->stage_bytes < need_bytes) {
+        for (auto &sg : t->stages)
+            for (void *&b : sg.buf) {
+                if (b) { cudaFree(b); b = nullptr; }
+                CUDA_TRY(cudaMalloc(&b, need_bytes), "cudaMalloc(stage buffer)");
+            }
+        t->stage_bytes = need_bytes;
+    }
+    const size_t nchunks = ((size_t)c->ncell + chunk - 1) / chunk;
+    if (h_diag && t->h_diag_cap < nchunks) {
+        if (t->h_diag_pinned) cudaFreeHost(t->h_diag_pinned);
+        t->h_diag_pinned = nullptr; t->h_diag_cap = 0;
+        CUDA_TRY(cudaMallocHost(&t->h_diag_pinned, nchunks * sizeof(cool_diag)), "cudaMallocHost(diag)");
+        t->h_diag_cap = nchunks;
+    }
+    const void *src[6] = {c->rho, c->bsq, c->theta_e_in, c->theta_i_in, c->r, c->vol};
+    int nl = 0;
+    for (size_t k = 0; k < nchunks; ++k) {
+        auto &sg = t->stages[k % NST];
+        const size_t off = k * chunk;
+        const size_t n = std::min(chunk, (size_t)c->ncell - off);
+        for (int j = 0; j < 6; ++j)
+            if (src[j]) CUDA_TRY(cudaMemcpyAsync(sg.buf[j], (const char *)src[j] + off * es, n * es, cudaMemcpyHostToDevice, sg.s), "cudaMemcpyAsync(H2D)");
+        LaunchArgs a{};
+        a.ncell = (long long)n; a.rho = sg.buf[0]; a.bsq = sg.buf[1]; a.the_in = sg.buf[2]; a.thi_in = sg.buf[3];
+        a.r = c->r ? sg.buf[4] : nullptr; a.vol = c->vol ? sg.buf[5] : nullptr;
+        a.the_out = sg.buf[6]; a.thi_out = sg.buf[7];
+        a.dt = p->dt; a.nsub = p->nsub; a.f_limit = p->f_limit; a.h_floor = p->h_floor; a.coulomb = coul;
+        a.want_diag = h_diag != nullptr; a.d_diag = h_diag ? sg.d_diag : nullptr;
+        if (h_diag) {
+            DiagWorkspace w;
+            s = get_diag_ws(t, sg.s, &w);
+            if (s != COOL_OK) return s;
+            a.partials = w.partials; a.ticket = w.ticket;
+        }
+        s = launch_step(t, v, c->dtype, a, sg.s, &nl);
+        if (s != COOL_OK) return s;
+        CUDA_TRY(cudaMemcpyAsync((char *)c->theta_e_out + off * es, sg.buf[6], n * es, cudaMemcpyDeviceToHost, sg.s), "cudaMemcpyAsync(D2H)");
+        CUDA_TRY(cudaMemcpyAsync((char *)c->theta_i_out + off * es, sg.buf[7], n * es, cudaMemcpyDeviceToHost, sg.s), "cudaMemcpyAsync(D2H)");
+        if (h_diag) CUDA_TRY(cudaMemcpyAsync(&t->h_diag_pinned[k], sg.d_diag, sizeof(cool_diag), cudaMemcpyDeviceToHost, sg.s), "cudaMemcpyAsync(diag)");
+    }
+    for (auto &sg : t->stages) CUDA_TRY(cudaStreamSynchronize(sg.s), "cudaStreamSynchronize");
+    g_launches = nl;
+    if (h_diag)
+        for (size_t k = 0; k < nchunks; ++k) {
+            const cool_diag &d = t->h_diag_pinned[k];
+            h_diag->lum_total += d.lum_total; h_diag->lum_brems += d.lum_brems; h_diag->lum_synch += d.lum_synch;
+            h_diag->lum_compton += d.lum_compton; h_diag->n_limited += d.n_limited; h_diag->n_floored += d.n_floored;
+            h_diag->n_clamped += d.n_clamped;
+        }
+    return COOL_OK;
+}

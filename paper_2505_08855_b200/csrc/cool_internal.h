@@ -1,0 +1,99 @@
+// cool_internal.h — private declarations shared by the translation units of libcool_b200.so.
+#pragma once
+#include <cuda_runtime.h>
+#include <map>
+#include <mutex>
+#include <string>
+#include <vector>
+
+#include "../../include/cool.h"
+#include "cool_physics.cuh"
+
+namespace cool {
+
+// Canonical device axis order (the library re-lays the caller's table out at create time):
+//   MODE 3 (ndim 3, nproc 1):  [rho][theta_e][bsq]            bsq fastest, float texels
+//   MODE 4 (ndim 4, nproc 3):  [rho][theta_e][theta_i][bsq]   bsq fastest, float4 texels
+//                              {log10 Qbrem, log10 Qsyn, log10 eta, 0}
+// bsq is fastest because in GRMHD fields plasma-beta varies cell to cell far more than rho or
+// Theta do along a grid line, so the scattered index stays inside one contiguous table row.
+enum { CAX_RHO = 0, CAX_THE = 1, CAX_THI = 2, CAX_BSQ = 3 };   // canonical slots (THI unused in MODE 3)
+
+struct AxisCoef {          // node-index coordinate t of a primitive q along one table axis
+    int n;
+    // fp64 path
+    double lo10, inv10;    // t = (log10 q - lo10) * inv10
+    // fp32 path: log2 q = e + lm (e integer, lm in [0,1)):  t = (e - e0)*invf + (lm*invf + cf)
+    float e0, invf, cf;
+};
+
+struct DevTable {
+    int mode;                      // 3 or 4; 0 = no data (analytic only)
+    AxisCoef ax[4];                // indexed by CAX_*
+    int s_rho, s_the, s_thi;       // strides in texels (bsq stride = 1)
+    const float *lin1;             // MODE 3 linear copy
+    const float4 *lin4;            // MODE 4 linear copy
+    cudaTextureObject_t tex_pt, tex_lin;   // 3-D array: x = bsq, y = theta_e (MODE 3) / theta_i (MODE 4),
+                                           // z = rho (MODE 3) / rho*n_the + i_the (MODE 4, the paper's flattening)
+    unsigned table_bytes;          // bytes of the linear copy (for the smem variant)
+    // Coulomb coefficient table log10 C [theta_i][theta_e]
+    const float *coul;
+    AxisCoef cax[2];               // 0: theta_i, 1: theta_e
+};
+
+// Unit-dependent constants, precomputed on the host in fp64 (and rounded copies for fp32).
+struct DevConst {
+    coolphys::Units units;
+    coolphys::Derived der;
+    double mr, ge1, gi1;           // m_e/m_p, gamma_e - 1, gamma_i - 1
+    double coul_k;                 // dTheta_e/dt from Coulomb = coul_k * rho * C * (Th_i - Th_e) * ge1
+    // MODE 4 combine (eqs 10-14) in code units
+    double bb_k;                   // (4 sigma_SB T^4 conv) = bb_k * Theta_e^4
+    double tausca_k;               // tau_sca = tausca_k * rho * H_cm
+    double log2_ue_k;              // log2(u_e) = log2 rho + log2 Theta_e + this
+};
+
+struct LaunchArgs {
+    long long ncell;
+    const void *rho, *bsq, *the_in, *thi_in, *r, *vol;
+    void *the_out, *thi_out;
+    double dt; int nsub; double f_limit, h_floor;
+    int coulomb;                   // 0 off, 1 table, 2 analytic
+    int want_diag;
+    double *partials;              // [grid][8]
+    unsigned *ticket;
+    cool_diag *d_diag;
+};
+
+struct DiagWorkspace { double *partials = nullptr; unsigned *ticket = nullptr; int capacity_blocks = 0; };
+
+}  // namespace cool
+
+struct cool_table {
+    int device = 0;
+    cool_table_desc desc{};        // host_data pointers nulled
+    cool::DevTable dev{};
+    cool::DevConst cst{};
+    float *d_lin = nullptr;        // owns lin1 / lin4
+    float *d_coul = nullptr;
+    cudaArray_t arr = nullptr;
+    int sm_count = 148;
+    int max_smem_optin = 0;
+    bool persist_l2 = false;
+    mutable std::mutex mu, host_mu;
+    mutable std::map<cudaStream_t, cool::DiagWorkspace> diag_ws;     // per-stream, so concurrent streams never share
+    // host-path staging (cool_apply_host), created lazily, used under mu
+    struct HostStage { cudaStream_t s = nullptr; void *buf[8] = {}; cool_diag *d_diag = nullptr; };
+    mutable std::vector<HostStage> stages;
+    mutable size_t stage_bytes = 0;         // per staging buffer
+    mutable cool_diag *h_diag_pinned = nullptr;
+    mutable size_t h_diag_cap = 0;
+};
+
+namespace cool {
+void set_error(const char *fmt, ...);
+bool desc_valid(const cool_table_desc *d, bool need_coulomb_shape, std::string *why);
+coolphys::Units to_units(const cool_units &u);
+cool_status launch_step(const cool_table *t, cool_variant v, cool_dtype dt, const LaunchArgs &a, cudaStream_t s, int *nlaunch);
+bool variant_supported(const cool_table *t, cool_variant v, cool_dtype dt, std::string *why);
+}
