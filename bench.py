@@ -1,0 +1,335 @@
+#!/usr/bin/env python
+"""bench.py — throughput of the cooling step (BASELINE.json metric: Gcell-updates/s and achieved
+HBM GB/s on one B200).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c5|c5u|c2|c3|c4-<n>|s512]
+                    [--variant auto|global|smem|tex_point|tex_hwfilter|analytic] [--impl ours|reference]
+
+A "step" is one cool_apply over the whole batch (every row of SURVEY.md §8(a): load, coordinates,
+table retrieval, process combination, Coulomb exchange, limiter, sub-steps, store, luminosity).
+Default workload c5 = BASELINE.json configs[4]: 512^3 cells fp32, three 48^4 process tables,
+Coulomb coefficient table 48^2, 4 sub-steps, luminosity diagnostic, on the MAD-like field of
+configs[2] resampled to 512^3 (north_star: "measured on synthetic MAD-like cell fields").
+Prints ONE JSON line on rank 0.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_2505_08855_b200 import synth  # noqa: E402  (numpy only)
+
+METRIC = "Gcell-updates/s of the cooling step"
+UNIT = "Gcell-updates/s"
+SPEC_HBM_GBS = 8000.0                     # BASELINE.json: "vs 8 TB/s"
+FALLBACK_HBM_GBS = 6650.0                 # B200_PROFILING.md fallback
+
+
+# ------------------------------------------------------------------------------------------------
+# workloads
+# ------------------------------------------------------------------------------------------------
+def workload_spec(name: str):
+    """-> dict(label, table n, nc, nsub, dt, field recipe, diag, vol)."""
+    if name == "c5":
+        return dict(label="configs[4]: 512^3 fp32 MAD-like field, 3x48^4 tables + 48^2 Coulomb, nsub=4, luminosity",
+                    n=[48, 48, 48, 48], nc=[48, 48], nsub=4, dt=1e-3, field=("mad", 512, 512, 512), diag=True, vol=True)
+    if name == "c5u":
+        return dict(label="configs[4] with log-uniform (worst-locality) cells: 512^3 fp32, 3x48^4 tables, nsub=4, luminosity",
+                    n=[48, 48, 48, 48], nc=[48, 48], nsub=4, dt=1e-3, field=("logu", 512 ** 3, 5, 0.0), diag=True, vol=False)
+    if name == "c2":
+        return dict(label="configs[1]: 256^3 fp32 log-uniform with 1% outliers, table 128^3, single update",
+                    n=[128, 128, 128], nc=[64, 64], nsub=1, dt=1e-3, field=("logu", 256 ** 3, 2, 0.01), diag=False, vol=False)
+    if name == "c3":
+        return dict(label="configs[2]: MAD-like 288x192x144 fp32, table 128^3, floor on, single update",
+                    n=[128, 128, 128], nc=[64, 64], nsub=1, dt=1e-3, field=("mad", 288, 192, 144), diag=True, vol=True, floor=0.1)
+    if name.startswith("c4-"):
+        m = int(name[3:])
+        return dict(label=f"configs[3]: 2^26 fp32 log-uniform cells, table {m}^3, single update",
+                    n=[m, m, m], nc=[64, 64], nsub=1, dt=1e-3, field=("logu", 1 << 26, 4, 0.0), diag=False, vol=False)
+    if name == "s512":
+        return dict(label="512^3 fp32 MAD-like field, single update, table 128^3 + 64^2 Coulomb (3-D step of configs[2] at 512^3)",
+                    n=[128, 128, 128], nc=[64, 64], nsub=1, dt=1e-3, field=("mad", 512, 512, 512), diag=False, vol=False)
+    raise SystemExit(f"unknown workload {name}")
+
+
+def make_fields(spec, rank=0):
+    f = spec["field"]
+    if f[0] == "mad":
+        return synth.mad_like_cells(f[1], f[2], f[3], dtype=np.float32, config=3 + 16 * rank)
+    return synth.log_uniform_cells(f[1], dtype=np.float32, config=f[2] + 16 * rank, outlier_frac=f[3])
+
+
+def table_ranges(n):
+    rng = {0: synth.LOG_RHO, 1: synth.LOG_THETA, 2: synth.LOG_BSQ, 3: synth.LOG_THETA}
+    nd = len(n)
+    return list(range(nd)), [rng[a][0] for a in range(nd)], [rng[a][1] for a in range(nd)]
+
+
+def bytes_per_cell(spec):
+    return 24 + (4 if spec.get("vol") else 0) + (4 if spec.get("floor") else 0)
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as fh:
+            return float(json.load(fh)["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs (measured copy bandwidth)"
+    return FALLBACK_HBM_GBS, "fallback 6.65 TB/s of B200_PROFILING.md (MEASURED_PEAKS.json absent)"
+
+
+# ------------------------------------------------------------------------------------------------
+# oracle legs (cpu_baseline and --impl reference): the only places bench.py touches oracle/
+# ------------------------------------------------------------------------------------------------
+def oracle_leg(spec, desc, data, coul, fields, sample_cells, steps=1):
+    import oracle as O
+    O.build()
+    nd = desc.ndim
+    otab = O.Table([desc.axis[k] for k in range(nd)], [desc.n[k] for k in range(nd)], [desc.lo[k] for k in range(nd)],
+                   [desc.hi[k] for k in range(nd)], data, coul=coul, clo=[desc.clo[0], desc.clo[1]], chi=[desc.chi[0], desc.chi[1]])
+    u = desc.units
+    un = O.Units(u.rho_scale_cgs, u.mbh_msun, u.gamma_e, u.gamma_i, u.ln_lambda, u.ion_theta_mass_ratio, u.hth_cm, u.r_ref_rg, u.spin)
+    ncell = fields["rho"].size
+    m = min(sample_cells, ncell)
+    lo = (ncell - m) // 2                     # contiguous sample from the middle of the field
+    sl = slice(lo, lo + m)
+    cores = O.max_threads()
+    times = []
+    for _ in range(steps):
+        t0 = time.perf_counter()
+        O.step(otab, un, fields["rho"][sl], fields["bsq"][sl], fields["theta_e"][sl], fields["theta_i"][sl], spec["dt"],
+               nsub=spec["nsub"], h_floor=spec.get("floor", 0.0), r=fields["r"][sl] if spec.get("floor") else None,
+               vol=fields["vol"][sl] if spec.get("vol") else None, nthreads=cores)
+        times.append(time.perf_counter() - t0)
+    return m, cores, times
+
+
+# ------------------------------------------------------------------------------------------------
+def clocks_monitor_start(gpu_index):
+    f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+    q = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
+        "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+    try:
+        p = subprocess.Popen(["nvidia-smi", f"--id={gpu_index}", f"--query-gpu={q}", "--format=csv,noheader,nounits", "-lms", "100"],
+                             stdout=f, stderr=subprocess.DEVNULL)
+    except OSError:
+        return None, f.name
+    return p, f.name
+
+
+def clocks_monitor_stop(p, path):
+    out = dict(sm_mhz=None, sm_max_mhz=None, reasons=[], samples=0)
+    if p is not None:
+        p.terminate()
+        try:
+            p.wait(timeout=5)
+        except Exception:
+            p.kill()
+    try:
+        rows = [r.strip().split(",") for r in open(path) if r.strip()]
+        sm = [float(r[0]) for r in rows if len(r) >= 7]
+        if sm:
+            out["sm_mhz"] = float(np.median(sm)); out["sm_max_mhz"] = float(rows[0][1]); out["samples"] = len(sm)
+            names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+            for k, nm in enumerate(names):
+                if any(r[3 + k].strip().lower().startswith("active") for r in rows if len(r) >= 7):
+                    out["reasons"].append(nm)
+    except Exception:
+        pass
+    finally:
+        try:
+            os.unlink(path)
+        except OSError:
+            pass
+    return out
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="c5")
+    ap.add_argument("--variant", default="auto")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-sample", type=int, default=1 << 24)
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = 3                                       # timing rule: W >= 3
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    spec = workload_spec(args.workload)
+    axis, lo, hi = table_ranges(spec["n"])
+
+    # ---------------- reference arm: the oracle on host cores, rank 0 only ----------------------
+    if args.impl == "reference":
+        if rank != 0:
+            return 0
+        from paper_2505_08855_b200 import api
+        desc = api.make_desc(axis, spec["n"], lo, hi, 1 if len(spec["n"]) == 3 else 3, nc=spec["nc"],
+                             clo=[synth.LOG_THETA[0]] * 2, chi=[synth.LOG_THETA[1]] * 2)
+        data, coul = api.cool_table_build_host(desc, want_coulomb=True)      # host builder: tables are data
+        small = dict(spec); f = spec["field"]
+        if f[0] == "mad":
+            small["field"] = ("mad", f[1], f[2], max(1, (1 << 22) // (f[1] * f[2])))   # a phi-slab of the same field
+        else:
+            small["field"] = ("logu", min(f[1], 1 << 22), f[2], f[3])
+        fields = make_fields(small)
+        sample = min(fields["rho"].size, 1 << 22)
+        for _ in range(min(args.warmup, 1)):
+            oracle_leg(spec, desc, data, coul, fields, sample, 1)
+        m, cores, times = oracle_leg(spec, desc, data, coul, fields, sample, args.steps)
+        tot = float(np.sum(times))
+        val = m * args.steps / tot / 1e9
+        line = dict(metric=METRIC, value=val, unit=UNIT, n_gpus=args.gpus, steps=args.steps, warmup=args.warmup,
+                    ms_per_step=1e3 * tot / args.steps, higher_is_better=True, scaling="weak", vs_baseline=None,
+                    dtype="f64", data="synthetic", impl="reference",
+                    config=dict(workload=args.workload, description=spec["label"], cells_per_step=m,
+                                note="oracle (oracle/cool_oracle.c, gcc -O2, OpenMP) on a bounded contiguous sample of the workload"),
+                    cpu_baseline=dict(value=val, unit=UNIT, cores=cores, kind="oracle", sample=f"{m} contiguous cells of the workload per step"),
+                    e2e=dict(value=val, unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0), gpu_launches=0)
+        print(json.dumps(line))
+        return 0
+
+    # ---------------- our arm ---------------------------------------------------------------------
+    import torch
+    from paper_2505_08855_b200 import api
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    desc = api.make_desc(axis, spec["n"], lo, hi, 1 if len(spec["n"]) == 3 else 3, nc=spec["nc"],
+                         clo=[synth.LOG_THETA[0]] * 2, chi=[synth.LOG_THETA[1]] * 2)
+    data, coul = api.cool_table_build_host(desc, want_coulomb=True)
+    table = api.cool_table_create(desc, data, coul, device=local_rank)
+    variant = api.VARIANTS[args.variant]
+    resolved = table.auto_variant() if variant == api.COOL_V_AUTO else variant
+
+    fields = make_fields(spec, rank)          # weak scaling: every rank owns a full batch (cells are independent)
+    ncell = fields["rho"].size
+    keys = ["rho", "bsq", "theta_e", "theta_i"] + (["vol"] if spec.get("vol") else []) + (["r"] if spec.get("floor") else [])
+    host = {k: torch.from_numpy(fields[k]).pin_memory() for k in keys}
+    d = {k: host[k].to(dev, non_blocking=True) for k in keys}
+    the_o = torch.empty(ncell, dtype=torch.float32, device=dev)
+    thi_o = torch.empty(ncell, dtype=torch.float32, device=dev)
+    d_diag = torch.zeros(api.DIAG_BYTES, dtype=torch.uint8, device=dev) if spec["diag"] else None
+    params = api.make_params(spec["dt"], spec["nsub"], 0.3, spec.get("floor", 0.0), variant, api.COOL_COULOMB_TABLE)
+    stream = torch.cuda.current_stream().cuda_stream
+
+    def step():
+        api.cool_apply(table, ncell, api.COOL_F32, d["rho"], d["bsq"], d["theta_e"], d["theta_i"], the_o, thi_o, params,
+                       r=d.get("r"), vol=d.get("vol"), d_diag=d_diag, stream=stream)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        step()
+    launches_per_step = api.cool_last_launch_count()
+    barrier()
+    mon, mon_path = clocks_monitor_start(local_rank) if rank == 0 else (None, None)
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+    barrier()
+    ev[0].record()
+    for k in range(args.steps):
+        step()
+        ev[k + 1].record()
+    barrier()
+    clocks = clocks_monitor_stop(mon, mon_path) if rank == 0 else None
+    per_step_ms = np.array([ev[k].elapsed_time(ev[k + 1]) for k in range(args.steps)])
+    total_ms = float(ev[0].elapsed_time(ev[-1]))
+    if world > 1:
+        t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    value = ncell * world * args.steps / (total_ms * 1e-3) / 1e9
+    diag_out = None
+    if d_diag is not None:
+        dd = api.cool_diag.from_buffer_copy(d_diag.cpu().numpy().tobytes()).as_dict()
+        if world > 1:                           # the only cross-rank datum: 4 luminosity sums
+            t = torch.tensor([dd["lum_total"], dd["lum_brems"], dd["lum_synch"], dd["lum_compton"]], dtype=torch.float64, device=dev)
+            dist.all_reduce(t)
+            dd["lum_total"], dd["lum_brems"], dd["lum_synch"], dd["lum_compton"] = [float(x) for x in t.tolist()]
+        diag_out = dd
+
+    # ---- end to end: host buffers, copies inside the timed region (rank-local, max over ranks) ----
+    e2e = None
+    if not args.no_e2e:
+        ho_e = torch.empty(ncell, dtype=torch.float32).pin_memory()
+        ho_i = torch.empty(ncell, dtype=torch.float32).pin_memory()
+        e2e_steps = max(1, min(args.steps, 3))
+
+        def hstep():
+            return api.cool_apply_host(table, ncell, api.COOL_F32, host["rho"], host["bsq"], host["theta_e"], host["theta_i"],
+                                       ho_e, ho_i, params, r=host.get("r"), vol=host.get("vol"), want_diag=spec["diag"])
+        hstep()
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(e2e_steps):
+            hstep()
+        barrier()
+        dt_e2e = time.perf_counter() - t0
+        if world > 1:
+            t = torch.tensor([dt_e2e], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            dt_e2e = float(t.item())
+        e2e = dict(value=ncell * world * e2e_steps / dt_e2e / 1e9, unit=UNIT,
+                   h2d_bytes_per_step=int(sum(host[k].numel() * 4 for k in keys)),
+                   d2h_bytes_per_step=int(2 * ncell * 4 + (api.DIAG_BYTES if spec["diag"] else 0)),
+                   steps=e2e_steps, api="cool_apply_host (C ABI, pinned host buffers, chunked copy/compute overlap)")
+        same = bool(torch.equal(ho_e, the_o.cpu()) and torch.equal(ho_i, thi_o.cpu()))
+        e2e["matches_device_path"] = same
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return 0
+
+    peak, peak_src = peaks()
+    bpc = bytes_per_cell(spec)
+    kern_ms = float(np.mean(per_step_ms))                     # one kernel per step: step time == kernel time
+    achieved = bpc * ncell / (kern_ms * 1e-3) / 1e9
+    line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=args.warmup,
+                ms_per_step=total_ms / args.steps, higher_is_better=True, scaling="weak", vs_baseline=None,
+                dtype="f32", data="synthetic",
+                config=dict(workload=args.workload, description=spec["label"], cells_per_gpu=ncell, nsub=spec["nsub"],
+                            variant=api.VARIANT_NAMES[resolved], l2="inputs (%.2f GB per step) larger than L2" % (bpc * ncell / 1e9),
+                            cell_substeps_per_s=value * spec["nsub"] * 1e9),
+                hbm_gbs=achieved * world, frac_of_8TBs=achieved / SPEC_HBM_GBS,
+                clocks=clocks, e2e=e2e, gpu_launches=launches_per_step * args.steps,
+                roofline=dict(bound="hbm", achieved=achieved, peak=peak, unit="GB/s", frac=achieved / peak, traffic=None,
+                              kernel="cool_step_kernel<float,%d,%s>" % (len(spec["n"]), api.VARIANT_NAMES[resolved]),
+                              bytes_per_cell=bpc, peak_source=peak_src,
+                              ms_per_launch_median=float(np.median(per_step_ms)), ms_per_launch_best=float(per_step_ms.min())),
+                diag=diag_out)
+    if not args.no_cpu_baseline:
+        m, cores, times = oracle_leg(spec, desc, data, coul, fields, args.cpu_sample, 1)
+        line["cpu_baseline"] = dict(value=m / times[0] / 1e9, unit=UNIT, cores=cores, kind="oracle",
+                                    sample=f"{m} contiguous cells from the middle of the workload, one pass, {times[0]:.1f} s")
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -1,0 +1,330 @@
+"""Parity of the CUDA path (through the C ABI) against the oracle, element by element, on the
+same seeded inputs.  Tolerances (north_star): relative error on the updated energies <= 1e-5
+for the fp32 software-interpolation variants, <= 1e-12 for fp64.  The hardware-filtered texture
+variant is reported, not gated (8-bit fixed-point filter weights).  All tests need a GPU."""
+import numpy as np
+import pytest
+
+import common as cm
+from paper_2505_08855_b200 import api, synth
+
+pytestmark = pytest.mark.gpu
+
+TOL = {np.float32: 1e-5, np.float64: 1e-12}
+SOFT = [api.COOL_V_GLOBAL, api.COOL_V_TEX_POINT, api.COOL_V_SMEM]
+
+
+@pytest.fixture(scope="module")
+def tab3(oracle):
+    """config 1: table 64^3 + 64^2 Coulomb coefficients (1 MiB: spans many tiles, too big for smem)."""
+    desc, data, coul = cm.build_tables([64, 64, 64], nc=[64, 64])
+    t = api.cool_table_create(desc, data, coul)
+    yield t, cm.oracle_table(oracle, desc, data, coul), cm.oracle_units(oracle, desc)
+    t.destroy()
+
+
+@pytest.fixture(scope="module")
+def tab3_small(oracle):
+    """32^3 = 128 KiB: fits shared memory (AUTO -> SMEM)."""
+    desc, data, coul = cm.build_tables([32, 32, 32], nc=[32, 32])
+    t = api.cool_table_create(desc, data, coul)
+    yield t, cm.oracle_table(oracle, desc, data, coul), cm.oracle_units(oracle, desc)
+    t.destroy()
+
+
+@pytest.fixture(scope="module")
+def tab4(oracle):
+    """config-5 shape at reduced size: ragged 4-D process tables + Coulomb table."""
+    desc, data, coul = cm.build_tables([12, 10, 14, 11], nc=[24, 20])
+    t = api.cool_table_create(desc, data, coul)
+    yield t, cm.oracle_table(oracle, desc, data, coul), cm.oracle_units(oracle, desc)
+    t.destroy()
+
+
+@pytest.fixture(scope="module")
+def tab4_tiny(oracle):
+    """6^4 float4 texels = 20 KiB: the 4-D table in shared memory."""
+    desc, data, coul = cm.build_tables([6, 7, 5, 6], nc=[16, 16])
+    t = api.cool_table_create(desc, data, coul)
+    yield t, cm.oracle_table(oracle, desc, data, coul), cm.oracle_units(oracle, desc)
+    t.destroy()
+
+
+def _check(got, ref, fields, dtype, label):
+    tol = TOL[dtype]
+    ee = cm.rel_err(got["theta_e"], ref["theta_e"]).max()
+    ei = cm.rel_err(got["theta_i"], ref["theta_i"]).max()
+    assert ee <= tol and ei <= tol, f"{label}: rel err e={ee:.3e} i={ei:.3e} > {tol}"
+    # anti-vacuity: the update must actually change a good share of the cells
+    ce, nact = cm.change_err(got["theta_e"], ref["theta_e"], fields["theta_e"].astype(np.float64))
+    return ee, ei, ce, nact
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+@pytest.mark.parametrize("dt,nsub", [(1e-3, 1), (10.0, 4)])
+def test_config1_all_software_variants(oracle, tab3, dtype, dt, nsub):
+    """configs[0]: 32^3 cells (+3 ragged tail), log-uniform, table 64^3."""
+    table, otab, un = tab3
+    f = synth.log_uniform_cells(32 ** 3 + 3, dtype=dtype, config=1)
+    ref = cm.oracle_step(oracle, otab, un, f, dt, nsub=nsub)
+    for v in (api.COOL_V_GLOBAL, api.COOL_V_TEX_POINT):
+        got = cm.gpu_step(table, f, dtype, dt, nsub=nsub, variant=v)
+        ee, ei, ce, nact = _check(got, ref, f, dtype, api.VARIANT_NAMES[v])
+        assert nact > 5000                                     # not a vacuous comparison
+        assert ce < (2e-3 if dtype == np.float32 else 1e-9)    # error of the change itself on active cells
+        d, r = got["diag"], ref["diag"]
+        assert d["lum_total"] == pytest.approx(r["lum_total"], rel=1e-6 if dtype == np.float32 else 1e-10)
+        assert abs(d["n_limited"] - r["n_limited"]) <= (3 if dtype == np.float32 else 0)
+        assert abs(d["n_clamped"] - r["n_clamped"]) <= (3 if dtype == np.float32 else 0)
+        assert got["launches"] == 1
+    with pytest.raises(api.CoolError) as ei_:
+        cm.gpu_step(table, f, dtype, dt, nsub=nsub, variant=api.COOL_V_SMEM)
+    assert ei_.value.status == api.COOL_EUNSUPPORTED          # 1 MiB does not fit; AUTO must still work
+    got = cm.gpu_step(table, f, dtype, dt, nsub=nsub, variant=api.COOL_V_AUTO)
+    _check(got, ref, f, dtype, "auto")
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+def test_smem_variant_and_auto(oracle, tab3_small, dtype):
+    table, otab, un = tab3_small
+    assert table.auto_variant() == api.COOL_V_SMEM
+    f = synth.log_uniform_cells(50001, dtype=dtype, config=1, outlier_frac=0.01)
+    ref = cm.oracle_step(oracle, otab, un, f, 0.5, nsub=2)
+    base = None
+    for v in SOFT + [api.COOL_V_AUTO]:
+        got = cm.gpu_step(table, f, dtype, 0.5, nsub=2, variant=v)
+        _check(got, ref, f, dtype, api.VARIANT_NAMES[v])
+        assert got["diag"]["n_clamped"] == pytest.approx(ref["diag"]["n_clamped"], abs=3)
+        assert ref["diag"]["n_clamped"] > 300                  # outliers really exercise the clamp
+        if base is None:
+            base = got
+        else:                                                  # software variants agree bit for bit
+            assert np.array_equal(base["theta_e"], got["theta_e"]) and np.array_equal(base["theta_i"], got["theta_i"])
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+@pytest.mark.parametrize("dt,nsub", [(1e-3, 1), (3.0, 4)])
+def test_config5_shape_process_tables(oracle, tab4, dtype, dt, nsub):
+    """4-D brems/synch/eta tables, eqs 10-14 combination, Coulomb table, sub-steps, luminosity split."""
+    table, otab, un = tab4
+    f = synth.log_uniform_cells(40007, dtype=dtype, config=5, outlier_frac=0.01)
+    f["vol"] = np.random.default_rng(7).uniform(0.5, 2.0, f["rho"].size).astype(dtype)
+    ref = cm.oracle_step(oracle, otab, un, f, dt, nsub=nsub, use_vol=True)
+    for v in (api.COOL_V_GLOBAL, api.COOL_V_TEX_POINT):
+        got = cm.gpu_step(table, f, dtype, dt, nsub=nsub, variant=v, use_vol=True)
+        _check(got, ref, f, dtype, api.VARIANT_NAMES[v])
+        rt = 2e-6 if dtype == np.float32 else 1e-10
+        for k in ("lum_total", "lum_brems", "lum_synch", "lum_compton"):
+            assert got["diag"][k] == pytest.approx(ref["diag"][k], rel=rt), k
+        s = got["diag"]
+        assert s["lum_brems"] + s["lum_synch"] + s["lum_compton"] == pytest.approx(s["lum_total"], rel=1e-6)
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+def test_4d_table_in_shared_memory(oracle, tab4_tiny, dtype):
+    table, otab, un = tab4_tiny
+    assert table.auto_variant() == api.COOL_V_SMEM
+    f = synth.log_uniform_cells(30011, dtype=dtype, config=5)
+    ref = cm.oracle_step(oracle, otab, un, f, 0.3, nsub=3)
+    for v in SOFT:
+        got = cm.gpu_step(table, f, dtype, 0.3, nsub=3, variant=v)
+        _check(got, ref, f, dtype, api.VARIANT_NAMES[v])
+
+
+@pytest.mark.parametrize("which", ["tab3", "tab4"])
+def test_hw_filtered_texture_is_reported_not_gated(oracle, request, which):
+    """COOL_V_TEX_HWFILTER: the texture unit interpolates with 8 fractional weight bits, so the
+    error is ~1e-3..1e-2; we bound it loosely and print it (north_star: 'reported with its
+    measured error')."""
+    table, otab, un = request.getfixturevalue(which)
+    f = synth.log_uniform_cells(32768, dtype=np.float32, config=1)
+    ref = cm.oracle_step(oracle, otab, un, f, 1e-3)
+    got = cm.gpu_step(table, f, np.float32, 1e-3, variant=api.COOL_V_TEX_HWFILTER)
+    err = cm.rel_err(got["theta_e"], ref["theta_e"])
+    print(f"\nhw-filter {which}: max rel err {err.max():.3e}, median {np.median(err):.3e}")
+    assert 1e-5 < err.max() < 5e-2
+    assert cm.rel_err(got["theta_i"], ref["theta_i"]).max() < 5e-2
+
+
+@pytest.mark.parametrize("dtype,tol", [(np.float64, 1e-9), (np.float32, 2e-7)])
+@pytest.mark.parametrize("which", ["tab3", "tab4"])
+def test_analytic_variant_vs_part_a(oracle, request, which, dtype, tol):
+    """COOL_V_ANALYTIC evaluates eqs 1-12 and eq 15 per cell (no table): oracle Part A."""
+    table, otab, un = request.getfixturevalue(which)
+    f = synth.log_uniform_cells(4099, dtype=dtype, config=1)
+    ref = cm.oracle_step(oracle, otab, un, f, 1.0, nsub=2, rate_mode=oracle.RATE_ANALYTIC, coulomb_mode=oracle.COULOMB_ANALYTIC)
+    got = cm.gpu_step(table, f, dtype, 1.0, nsub=2, variant=api.COOL_V_ANALYTIC, coulomb=api.COOL_COULOMB_ANALYTIC)
+    assert cm.rel_err(got["theta_e"], ref["theta_e"]).max() <= tol
+    assert cm.rel_err(got["theta_i"], ref["theta_i"]).max() <= tol
+    assert got["diag"]["lum_total"] == pytest.approx(ref["diag"]["lum_total"], rel=1e-8)
+
+
+def test_analytic_without_table_data(oracle):
+    desc = api.make_desc([0, 1, 2], [4, 4, 4], cm.LO3, cm.HI3, 0)
+    table = api.cool_table_create(desc, [])
+    assert table.auto_variant() == api.COOL_V_ANALYTIC
+    f = synth.log_uniform_cells(1000, dtype=np.float64, config=1)
+    otab = oracle.Table([0, 1, 2], [2, 2, 2], cm.LO3, cm.HI3, [np.zeros((2, 2, 2), np.float32)])
+    ref = cm.oracle_step(oracle, otab, oracle.Units(), f, 0.1, rate_mode=oracle.RATE_ANALYTIC, coulomb_mode=oracle.COULOMB_ANALYTIC)
+    got = cm.gpu_step(table, f, np.float64, 0.1)
+    assert cm.rel_err(got["theta_e"], ref["theta_e"]).max() <= 1e-9
+    with pytest.raises(api.CoolError) as e:
+        cm.gpu_step(table, f, np.float64, 0.1, variant=api.COOL_V_GLOBAL)
+    assert e.value.status == api.COOL_EUNSUPPORTED
+    table.destroy()
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+def test_coulomb_modes(oracle, tab3, dtype):
+    table, otab, un = tab3
+    f = synth.log_uniform_cells(3001, dtype=dtype, config=1)
+    for cmode, omode in ((api.COOL_COULOMB_OFF, oracle.COULOMB_OFF), (api.COOL_COULOMB_TABLE, oracle.COULOMB_TABLE),
+                         (api.COOL_COULOMB_ANALYTIC, oracle.COULOMB_ANALYTIC)):
+        ref = cm.oracle_step(oracle, otab, un, f, 5.0, nsub=2, coulomb_mode=omode)
+        got = cm.gpu_step(table, f, dtype, 5.0, nsub=2, variant=api.COOL_V_GLOBAL, coulomb=cmode)
+        _check(got, ref, f, dtype, f"coulomb mode {cmode}")
+    # exact zero exchange at T_e = T_i: the ions are untouched, bit for bit (north_star pin)
+    g = dict(f); g["theta_i"] = f["theta_e"].copy()
+    got = cm.gpu_step(table, g, dtype, 3.0, nsub=1, variant=api.COOL_V_GLOBAL)
+    assert np.array_equal(got["theta_i"], g["theta_i"].astype(np.float64))
+    assert (got["theta_e"] <= g["theta_e"]).all() and (got["theta_e"] < g["theta_e"]).any()
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+def test_config3_mad_field_floor_vol_sweep(oracle, dtype):
+    """configs[2] at reduced resolution: MAD-like torus, floor on (needs r), volume-weighted
+    luminosity, density normalisation swept over the four accretion rates (table rebuilt per rho_scale).
+    The recipe's gas temperature sits 1.37x above the h_floor = 0.1 floor at every radius, so the test
+    uses h_floor = 0.117 to put the 5 % noise astride the floor and exercise both branches."""
+    f = synth.mad_like_cells(36, 24, 20, dtype=dtype)
+    for mdot in (1e-6, 1e-4, 1e-2, 0.3):
+        rs = synth.rho_scale_for_mdot(mdot)
+        desc, data, coul = cm.build_tables([24, 24, 24], nc=[24, 24], units_kw=dict(rho_scale_cgs=rs))
+        table = api.cool_table_create(desc, data, coul)
+        otab, un = cm.oracle_table(oracle, desc, data, coul), cm.oracle_units(oracle, desc)
+        ref = cm.oracle_step(oracle, otab, un, f, 50.0, nsub=2, h_floor=0.117, use_r=True, use_vol=True)
+        for v in (api.COOL_V_GLOBAL, api.COOL_V_SMEM):
+            got = cm.gpu_step(table, f, dtype, 50.0, nsub=2, h_floor=0.117, variant=v, use_r=True, use_vol=True)
+            _check(got, ref, f, dtype, f"mdot={mdot} {api.VARIANT_NAMES[v]}")
+            assert got["diag"]["n_floored"] == pytest.approx(ref["diag"]["n_floored"], abs=3)
+            assert got["diag"]["lum_total"] == pytest.approx(ref["diag"]["lum_total"], rel=2e-6 if dtype == np.float32 else 1e-10)
+        assert ref["diag"]["n_floored"] > 100 and ref["diag"]["n_clamped"] > 100
+        table.destroy()
+
+
+def test_permuted_axes_table(oracle):
+    """The caller's axis order is arbitrary; the library re-lays the table out."""
+    desc, data, coul = cm.build_tables([9, 11, 10, 8], nc=[16, 16], axis=[3, 2, 0, 1])
+    table = api.cool_table_create(desc, data, coul)
+    otab, un = cm.oracle_table(oracle, desc, data, coul), cm.oracle_units(oracle, desc)
+    f = synth.log_uniform_cells(20000, dtype=np.float64, config=5)
+    ref = cm.oracle_step(oracle, otab, un, f, 0.2, nsub=2)
+    for v in SOFT:
+        got = cm.gpu_step(table, f, np.float64, 0.2, nsub=2, variant=v)
+        _check(got, ref, f, np.float64, "permuted")
+    table.destroy()
+    desc, data, coul = cm.build_tables([13, 17, 15], nc=[16, 16], axis=[2, 0, 1])
+    table = api.cool_table_create(desc, data, coul)
+    otab = cm.oracle_table(oracle, desc, data, coul)
+    ref = cm.oracle_step(oracle, otab, un, f, 0.2)
+    got = cm.gpu_step(table, f, np.float64, 0.2, variant=api.COOL_V_GLOBAL)
+    _check(got, ref, f, np.float64, "permuted3")
+    table.destroy()
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+def test_edge_cases(oracle, tab3, dtype):
+    table, otab, un = tab3
+    # empty batch
+    e = {k: np.zeros(0, dtype) for k in ("rho", "bsq", "theta_e", "theta_i")}
+    got = cm.gpu_step(table, e, dtype, 1e-3)
+    assert got["theta_e"].size == 0 and got["diag"]["lum_total"] == 0.0 and got["launches"] == 0
+    # ragged sizes around the vector width, misaligned pointers, in-place update
+    for n in (1, 2, 3, 5, 1023, 4097):
+        f = synth.log_uniform_cells(n, dtype=dtype, config=1)
+        ref = cm.oracle_step(oracle, otab, un, f, 0.7, nsub=2)
+        for off, inplace in ((0, False), (1, False), (0, True), (3, True)):
+            got = cm.gpu_step(table, f, dtype, 0.7, nsub=2, variant=api.COOL_V_GLOBAL, offset=off, inplace=inplace)
+            _check(got, ref, f, dtype, f"n={n} off={off} inplace={inplace}")
+    # degenerate cells: rho <= 0 passes through, non-positive bsq / Theta clamp, NaN stays local
+    f = synth.log_uniform_cells(64, dtype=dtype, config=1)
+    f["rho"][0] = 0.0; f["rho"][1] = -1.0; f["bsq"][2] = 0.0; f["theta_i"][3] = 0.0
+    f["rho"][4] = np.nan; f["theta_e"][5] = np.nan; f["bsq"][6] = np.nan; f["theta_i"][7] = np.nan
+    f["rho"][8] = 1e30; f["theta_e"][9] = 1e-30; f["bsq"][10] = 1e30
+    ref = cm.oracle_step(oracle, otab, un, f, 1e-3)
+    got = cm.gpu_step(table, f, dtype, 1e-3, variant=api.COOL_V_GLOBAL)
+    assert np.isnan(got["theta_e"][4:8]).all() and np.isnan(got["theta_i"][4:8]).all()
+    assert got["theta_e"][0] == f["theta_e"][0] and got["theta_i"][1] == f["theta_i"][1]
+    _check(got, ref, f, dtype, "degenerate")
+    assert np.isfinite(got["theta_e"][8:]).all()
+
+
+def test_update_invariants_on_gpu(oracle, tab3):
+    """Properties that hold at any size: positivity, energy only leaves through radiation, the
+    diagnostic equals the energy drop, the 30 % limiter bounds the change per sub-step."""
+    table, otab, un = tab3
+    f = synth.log_uniform_cells(200000, dtype=np.float64, config=2)
+    f["vol"] = np.random.default_rng(3).uniform(0.5, 2.0, f["rho"].size)
+    got = cm.gpu_step(table, f, np.float64, 20.0, nsub=3, use_vol=True)
+    mr = 9.1093837015e-28 / 1.67262192369e-24
+    u0 = f["rho"] * (f["theta_e"] + f["theta_i"]) * mr * 1.5
+    u1 = f["rho"] * (got["theta_e"] + got["theta_i"]) * mr * 1.5
+    assert (got["theta_e"] > 0).all() and (got["theta_i"] > 0).all()
+    assert (u1 <= u0 * (1 + 1e-14)).all()
+    assert got["diag"]["lum_total"] == pytest.approx(((u0 - u1) * f["vol"]).sum() / 20.0, rel=1e-10)
+    assert (got["theta_e"] >= f["theta_e"] * 0.4 ** 3 * (1 - 1e-12)).all()
+
+
+def test_diag_is_bit_reproducible(tab3):
+    table, _, _ = tab3
+    f = synth.log_uniform_cells(300000, dtype=np.float32, config=2)
+    a = cm.gpu_step(table, f, np.float32, 1.0, nsub=2)
+    b = cm.gpu_step(table, f, np.float32, 1.0, nsub=2)
+    assert a["diag"] == b["diag"] and np.array_equal(a["theta_e"], b["theta_e"])
+
+
+def test_host_buffer_path_matches_device_path(oracle, tab4):
+    """cool_apply_host (the e2e path of bench.py): chunked, overlapped copies; same bits."""
+    import torch
+    table, otab, un = tab4
+    n = (1 << 22) * 2 + 12345                                  # three staged chunks, ragged tail
+    f = synth.log_uniform_cells(n, dtype=np.float32, config=5)
+    dev = cm.gpu_step(table, f, np.float32, 0.5, nsub=2)
+    pin = {k: torch.from_numpy(f[k]).pin_memory() for k in ("rho", "bsq", "theta_e", "theta_i")}
+    oe = torch.empty(n, dtype=torch.float32).pin_memory(); oi = torch.empty(n, dtype=torch.float32).pin_memory()
+    d = api.cool_apply_host(table, n, api.COOL_F32, pin["rho"], pin["bsq"], pin["theta_e"], pin["theta_i"], oe, oi,
+                            api.make_params(0.5, 2), want_diag=True)
+    assert np.array_equal(oe.numpy().astype(np.float64), dev["theta_e"]) and np.array_equal(oi.numpy().astype(np.float64), dev["theta_i"])
+    assert d["lum_total"] == pytest.approx(dev["diag"]["lum_total"], rel=1e-12)
+    assert d["n_limited"] == dev["diag"]["n_limited"] and api.cool_last_launch_count() == 3
+    # pageable numpy buffers work too
+    oe2 = np.empty(n, np.float32); oi2 = np.empty(n, np.float32)
+    api.cool_apply_host(table, n, api.COOL_F32, f["rho"], f["bsq"], f["theta_e"], f["theta_i"], oe2, oi2, api.make_params(0.5, 2))
+    assert np.array_equal(oe2, oe.numpy())
+    # sampled cells against the oracle
+    idx = np.random.default_rng(1).choice(n, 5000, replace=False)
+    sub = {k: f[k][idx] for k in ("rho", "bsq", "theta_e", "theta_i")}
+    ref = cm.oracle_step(oracle, otab, un, sub, 0.5, nsub=2)
+    assert cm.rel_err(oe.numpy()[idx], ref["theta_e"]).max() <= 1e-5
+
+
+def test_bad_arguments(tab3):
+    import torch
+    table, _, _ = tab3
+    f = synth.log_uniform_cells(16, dtype=np.float32, config=1)
+    for kw in (dict(dt=0.0), dict(dt=float("nan")), dict(nsub=0), dict(f_limit=0.5), dict(f_limit=0.0), dict(h_floor=-1.0)):
+        args = dict(dt=1e-3, nsub=1, f_limit=0.3, h_floor=0.0); args.update(kw)
+        with pytest.raises(api.CoolError) as e:
+            cm.gpu_step(table, f, np.float32, args["dt"], nsub=args["nsub"], f_limit=args["f_limit"], h_floor=args["h_floor"])
+        assert e.value.status == api.COOL_EINVAL
+    x = torch.zeros(16, device="cuda")
+    with pytest.raises(api.CoolError) as e:
+        api.cool_apply(table, 16, api.COOL_F32, x, x, x, None, x, x, api.make_params(1e-3))
+    assert e.value.status == api.COOL_EINVAL
+    with pytest.raises(api.CoolError):
+        api.cool_apply(table, -1, api.COOL_F32, x, x, x, x, x, x, api.make_params(1e-3))
+    bad = api.make_desc([0, 1, 2], [4, 4, 4], cm.LO3, cm.HI3, 1)
+    data = [np.full((4, 4, 4), np.inf, np.float32)]
+    with pytest.raises(api.CoolError) as e:
+        api.cool_table_create(bad, data)
+    assert e.value.status == api.COOL_EINVAL
