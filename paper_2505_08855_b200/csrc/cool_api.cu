@@ -52,6 +52,8 @@ static AxisCoef make_axis(int n, double lo, double hi)
     const double e0 = floor(lo2);
     a.e0 = (float)e0; a.invf = (float)inv2;
     a.cf = (float)(-(lo2 - e0) * inv2);
+    a.nm1f = (float)(n - 1);
+    a.tmaxf = nextafterf(a.nm1f, 0.f);
     return a;
 }
 
@@ -259,6 +261,10 @@ extern "C" cool_status cool_table_create(const cool_table_desc *desc, int device
         D.coul = t->d_coul;
         D.cax[0] = make_axis(desc->nc[0], desc->clo[0], desc->chi[0]);
         D.cax[1] = make_axis(desc->nc[1], desc->clo[1], desc->chi[1]);
+        D.coul_bytes = (int)(n * sizeof(float));
+        auto same = [](const AxisCoef &x, const AxisCoef &y) { return x.n == y.n && x.lo10 == y.lo10 && x.inv10 == y.inv10; };
+        D.coul_share_the = D.mode != 0 && same(D.cax[1], D.ax[CAX_THE]);
+        D.coul_share_thi = D.mode == 4 && same(D.cax[0], D.ax[CAX_THI]);
     }
     *out = t;
     return COOL_OK;

@@ -25,6 +25,7 @@ struct AxisCoef {          // node-index coordinate t of a primitive q along one
     double lo10, inv10;    // t = (log10 q - lo10) * inv10
     // fp32 path: log2 q = e + lm (e integer, lm in [0,1)):  t = (e - e0)*invf + (lm*invf + cf)
     float e0, invf, cf;
+    float nm1f, tmaxf;     // n-1 (clamp flag) and the largest float below n-1 (keeps floor(t) <= n-2)
 };
 
 struct DevTable {
@@ -39,6 +40,8 @@ struct DevTable {
     // Coulomb coefficient table log10 C [theta_i][theta_e]
     const float *coul;
     AxisCoef cax[2];               // 0: theta_i, 1: theta_e
+    int coul_bytes;                // size of the Coulomb table (staged in shared memory when small)
+    int coul_share_the, coul_share_thi;   // Coulomb axis identical to the table's Theta_e / Theta_i axis
 };
 
 // Unit-dependent constants, precomputed on the host in fp64 (and rounded copies for fp32).
