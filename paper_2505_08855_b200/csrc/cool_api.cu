@@ -54,7 +54,35 @@ static AxisCoef make_axis(int n, double lo, double hi)
     a.cf = (float)(-(lo2 - e0) * inv2);
     a.nm1f = (float)(n - 1);
     a.tmaxf = nextafterf(a.nm1f, 0.f);
+    a.ke = (float)(8388608.0 + 127.0 + e0);
+    a.d2f = (float)(delta * L10);
     return a;
+}
+
+// 3-D cudaArray + point / linear texture objects over a canonical host array (x = bsq fastest)
+static cudaError_t make_textures(const float *host, int chan, size_t ex, size_t ey, size_t ez, cudaArray_t *arr,
+                                 cudaTextureObject_t *pt, cudaTextureObject_t *lin)
+{
+    cudaChannelFormatDesc cd = chan == 1 ? cudaCreateChannelDesc<float>() : cudaCreateChannelDesc<float4>();
+    cudaError_t e = cudaMalloc3DArray(arr, &cd, make_cudaExtent(ex, ey, ez));
+    if (e != cudaSuccess) return e;
+    cudaMemcpy3DParms cp{};
+    cp.srcPtr = make_cudaPitchedPtr((void *)host, ex * chan * sizeof(float), ex, ey);
+    cp.dstArray = *arr;
+    cp.extent = make_cudaExtent(ex, ey, ez);
+    cp.kind = cudaMemcpyHostToDevice;
+    e = cudaMemcpy3D(&cp);
+    if (e != cudaSuccess) return e;
+    cudaResourceDesc rd{};
+    rd.resType = cudaResourceTypeArray; rd.res.array.array = *arr;
+    cudaTextureDesc td{};
+    td.addressMode[0] = td.addressMode[1] = td.addressMode[2] = cudaAddressModeClamp;
+    td.readMode = cudaReadModeElementType; td.normalizedCoords = 0;
+    td.filterMode = cudaFilterModePoint;
+    e = cudaCreateTextureObject(pt, &rd, &td, nullptr);
+    if (e != cudaSuccess) return e;
+    td.filterMode = cudaFilterModeLinear;
+    return cudaCreateTextureObject(lin, &rd, &td, nullptr);
 }
 
 static void free_table(cool_table *t)
@@ -63,9 +91,14 @@ static void free_table(cool_table *t)
     cudaSetDevice(t->device);
     if (t->dev.tex_pt) cudaDestroyTextureObject(t->dev.tex_pt);
     if (t->dev.tex_lin) cudaDestroyTextureObject(t->dev.tex_lin);
+    if (t->dev.ftex_pt) cudaDestroyTextureObject(t->dev.ftex_pt);
+    if (t->dev.ftex_lin) cudaDestroyTextureObject(t->dev.ftex_lin);
     if (t->arr) cudaFreeArray(t->arr);
+    if (t->arr32) cudaFreeArray(t->arr32);
     if (t->d_lin) cudaFree(t->d_lin);
+    if (t->d_f32) cudaFree(t->d_f32);
     if (t->d_coul) cudaFree(t->d_coul);
+    if (t->d_fcoul) cudaFree(t->d_fcoul);
     for (auto &kv : t->diag_ws) { cudaFree(kv.second.partials); cudaFree(kv.second.ticket); }
     for (auto &s : t->stages) {
         for (void *b : s.buf) if (b) cudaFree(b);
@@ -135,7 +168,7 @@ extern "C" int cool_last_launch_count(void) { return g_launches; }
 extern "C" cool_variant cool_table_auto_variant(const cool_table *t)
 {
     if (!t || t->dev.mode == 0) return COOL_V_ANALYTIC;
-    if ((size_t)t->dev.table_bytes + 1024 <= (size_t)t->max_smem_optin) return COOL_V_SMEM;
+    if (variant_supported(t, COOL_V_SMEM, COOL_F32, nullptr)) return COOL_V_SMEM;
     return COOL_V_GLOBAL;
 }
 
@@ -223,31 +256,46 @@ extern "C" cool_status cool_table_create(const cool_table_desc *desc, int device
         D.table_bytes = (unsigned)bytes;
         if (nd == 3) D.lin1 = t->d_lin; else D.lin4 = (const float4 *)t->d_lin;
 
+        // fp32-path copy: log2 of the rate per unit electron energy at the node (see cool_internal.h)
+        auto same = [](const AxisCoef &x, const AxisCoef &y) { return x.n == y.n && x.lo10 == y.lo10 && x.inv10 == y.inv10; };
+        AxisCoef c0{}, c1{};
+        if (desc->host_coulomb) { c0 = make_axis(desc->nc[0], desc->clo[0], desc->chi[0]); c1 = make_axis(desc->nc[1], desc->clo[1], desc->chi[1]); }
+        D.f4_has_coul = nd == 4 && desc->host_coulomb && same(c0, D.ax[CAX_THI]) && same(c1, D.ax[CAX_THE]);
+        std::vector<float> canon32;
+        try { canon32.assign(bytes / sizeof(float), 0.f); } catch (...) { set_error("out of host memory"); return fail(COOL_ENOMEM); }
+        {
+            const double L10 = 3.321928094887362, lue = log2(K.mr / K.ge1);
+            const AxisCoef &ar = D.ax[CAX_RHO], &ae = D.ax[CAX_THE];
+            const int nr = ncan[CAX_RHO], ne = ncan[CAX_THE], ni = ncan[CAX_THI], nb = ncan[CAX_BSQ];
+            for (int ir = 0; ir < nr; ++ir)
+                for (int ie = 0; ie < ne; ++ie) {
+                    // log2(u_e / (rho Theta_e)) + log2 rho_node + log2 Theta_e_node
+                    const double sub = lue + L10 * ((ar.lo10 + ir / ar.inv10) + (ae.lo10 + ie / ae.inv10));
+                    for (int ii = 0; ii < ni; ++ii)
+                        for (int ib = 0; ib < nb; ++ib) {
+                            const size_t o = ((((size_t)ir * ne + ie) * ni + ii) * nb + ib) * chan;
+                            if (nd == 3) canon32[o] = (float)(L10 * (double)canon[o] - sub);
+                            else {
+                                canon32[o + 0] = (float)(L10 * (double)canon[o + 0] - sub);
+                                canon32[o + 1] = (float)(L10 * (double)canon[o + 1] - sub);
+                                canon32[o + 2] = (float)(L10 * (double)canon[o + 2]);
+                                canon32[o + 3] = D.f4_has_coul ? (float)(L10 * (double)desc->host_coulomb[(size_t)ii * desc->nc[1] + ie]) : 0.f;
+                            }
+                        }
+                }
+        }
+        e = cudaMalloc(&t->d_f32, bytes);
+        if (e == cudaSuccess) e = cudaMemcpy(t->d_f32, canon32.data(), bytes, cudaMemcpyHostToDevice);
+        if (e != cudaSuccess) { set_error("fp32 table upload: %s", cudaGetErrorString(e)); return fail(e == cudaErrorMemoryAllocation ? COOL_ENOMEM : COOL_ECUDA); }
+        if (nd == 3) D.f1 = t->d_f32; else D.f4 = (const float4 *)t->d_f32;
+
         // cudaArray + texture objects (x = bsq, y = theta_e | theta_i, z = rho | rho*n_the + i_the)
         const size_t ex = ncan[CAX_BSQ];
         const size_t ey = nd == 3 ? ncan[CAX_THE] : ncan[CAX_THI];
         const size_t ez = nd == 3 ? ncan[CAX_RHO] : (size_t)ncan[CAX_RHO] * ncan[CAX_THE];
         if (ex <= 16384 && ey <= 16384 && ez <= 16384) {
-            cudaChannelFormatDesc cd = nd == 3 ? cudaCreateChannelDesc<float>() : cudaCreateChannelDesc<float4>();
-            e = cudaMalloc3DArray(&t->arr, &cd, make_cudaExtent(ex, ey, ez));
-            if (e == cudaSuccess) {
-                cudaMemcpy3DParms cp{};
-                cp.srcPtr = make_cudaPitchedPtr(canon.data(), ex * chan * sizeof(float), ex, ey);
-                cp.dstArray = t->arr;
-                cp.extent = make_cudaExtent(ex, ey, ez);
-                cp.kind = cudaMemcpyHostToDevice;
-                e = cudaMemcpy3D(&cp);
-            }
-            if (e == cudaSuccess) {
-                cudaResourceDesc rd{};
-                rd.resType = cudaResourceTypeArray; rd.res.array.array = t->arr;
-                cudaTextureDesc td{};
-                td.addressMode[0] = td.addressMode[1] = td.addressMode[2] = cudaAddressModeClamp;
-                td.readMode = cudaReadModeElementType; td.normalizedCoords = 0;
-                td.filterMode = cudaFilterModePoint;
-                e = cudaCreateTextureObject(&D.tex_pt, &rd, &td, nullptr);
-                if (e == cudaSuccess) { td.filterMode = cudaFilterModeLinear; e = cudaCreateTextureObject(&D.tex_lin, &rd, &td, nullptr); }
-            }
+            e = make_textures(canon.data(), chan, ex, ey, ez, &t->arr, &D.tex_pt, &D.tex_lin);
+            if (e == cudaSuccess) e = make_textures(canon32.data(), chan, ex, ey, ez, &t->arr32, &D.ftex_pt, &D.ftex_lin);
             if (e != cudaSuccess) { set_error("texture setup: %s", cudaGetErrorString(e)); return fail(e == cudaErrorMemoryAllocation ? COOL_ENOMEM : COOL_ECUDA); }
         }
     }
@@ -259,6 +307,14 @@ extern "C" cool_status cool_table_create(const cool_table_desc *desc, int device
         if (e == cudaSuccess) e = cudaMemcpy(t->d_coul, desc->host_coulomb, n * sizeof(float), cudaMemcpyHostToDevice);
         if (e != cudaSuccess) { set_error("Coulomb table upload: %s", cudaGetErrorString(e)); return fail(e == cudaErrorMemoryAllocation ? COOL_ENOMEM : COOL_ECUDA); }
         D.coul = t->d_coul;
+        {   // fp32 path: log2 C
+            std::vector<float> c2(n);
+            for (size_t k = 0; k < n; ++k) c2[k] = (float)(3.321928094887362 * (double)desc->host_coulomb[k]);
+            e = cudaMalloc(&t->d_fcoul, n * sizeof(float));
+            if (e == cudaSuccess) e = cudaMemcpy(t->d_fcoul, c2.data(), n * sizeof(float), cudaMemcpyHostToDevice);
+            if (e != cudaSuccess) { set_error("Coulomb table upload: %s", cudaGetErrorString(e)); return fail(e == cudaErrorMemoryAllocation ? COOL_ENOMEM : COOL_ECUDA); }
+            D.fcoul = t->d_fcoul;
+        }
         D.cax[0] = make_axis(desc->nc[0], desc->clo[0], desc->chi[0]);
         D.cax[1] = make_axis(desc->nc[1], desc->clo[1], desc->chi[1]);
         D.coul_bytes = (int)(n * sizeof(float));

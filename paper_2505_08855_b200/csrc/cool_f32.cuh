@@ -1,0 +1,660 @@
+// cool_f32.cuh — the fp32 kernels of the cooling step (include/cool.h), written for sm_100a.
+//
+// Structure of one launch (persistent CTAs, one tile = THREADS*4 consecutive cells):
+//   * cell tiles (rho, bsq, Theta_e, Theta_i [, vol, r]) are staged into shared memory by 1-D TMA
+//     bulk copies (cp.async.bulk + mbarrier), double buffered, so HBM latency never sits on a
+//     warp's scoreboard; outputs leave as 128-bit streaming stores;
+//   * the table is read through one of four lookup policies (L1/L2-resident global gathers,
+//     shared-memory image, point texture, hardware-filtered texture);
+//   * the luminosity diagnostic is reduced warp -> block -> fixed-order last-block pass.
+// The step is a gather plus scalar arithmetic: no tensor cores.  On B200 it
+// is bound by instruction issue and the L1 data pipe, not by HBM, so the arithmetic is written to
+// minimise instructions:
+//   * the table nodes are stored as T' = log2(rate / u_e at the node) (cool_internal.h), so that
+//     Lambda h / u_e = 2^(interp(T') + log2 h + clamp correction): no large-number cancellation, no
+//     compensated products;
+//   * log2 of a primitive is (exponent, log2 mantissa) folded straight into the node coordinate;
+//   * floor() is a round-down add of 1.5*2^23 whose mantissa bits are the node index, and the
+//     bias is folded into the address constant (no F2I/I2F, no masking);
+//   * MODE 4: the (rho, bsq) contraction of the 16 corners is loop invariant over sub-steps, so a
+//     bilinear patch in (w_e, w_i) is cached per visited (i_e, i_i) table cell — 3 FMAs per channel
+//     per sub-step — and the Coulomb coefficient rides in the 4th texel channel;
+//   * a sub-step that leaves both temperatures bit-identical repeats itself: exact early exit.
+#pragma once
+#include "cool_kernels.cuh"
+
+namespace cool {
+
+// Per-launch constants of the fp32 path (host fp64 -> rounded once).
+struct F32Const {
+    float k0;                         // log2(h)
+    float f_limit, mr, eq_frac, gi1_over_ge1, coul_kh, cap1e, cap1i;
+    float ae, ai, be, bi;             // c_s^2 = (ae Th_e + ai Th_i)/(1 + be Th_e + bi Th_i)           (eq 14)
+    float inv_kB;                     // tau_abs = r_thin * inv_kB rho c_s / Theta_e^3                  (eq 12 in ratio form)
+    float ksca;                       // tau_sca = ksca rho c_s
+    float hfloor2, spin;              // floor: (pi/2) h_floor^2 (Omega_K r)^2                          (eq 19)
+    double lum_k;                     // lum = sum(dTheta_rad rho vol) * lum_k
+    double ion_ratio;                 // theta_i of eq 15 = Theta_i / ion_ratio (analytic Coulomb only)
+    int nsub, coulomb, has_r, has_vol, use_tma, coul_smem, nf;
+    unsigned stage_bytes, coul_off, table_off;     // dynamic shared memory layout
+};
+
+// ------------------------------------------------------------------------------------------
+// mbarrier / TMA 1-D bulk copy
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned bar, unsigned count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned bar, unsigned bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void tma_load_1d(unsigned dst, const void *src, unsigned bytes, unsigned bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity)
+{
+    asm volatile("{\n\t.reg .pred p;\n"
+                 "COOL_WAIT:\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t@p bra COOL_DONE;\n\tbra COOL_WAIT;\n"
+                 "COOL_DONE:\n\t}" ::"r"(bar), "r"(parity) : "memory");
+}
+__device__ __forceinline__ float lg2_approx(float x)
+{
+    float y;
+    asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+__device__ __forceinline__ float ex2_approx(float x)
+{
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+__device__ __forceinline__ float rcp_approx(float x)
+{
+    float y;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+// opaque register copy of a constant: lets ptxas fold (b & m) | c into one LOP3 (one immediate per LOP3)
+__device__ __forceinline__ int opaque_const(int c)
+{
+    int r;
+    asm("mov.b32 %0, %1;" : "=r"(r) : "r"(c));
+    return r;
+}
+__device__ __forceinline__ int and_or(int a, int andmask, int orbits)          // (a & andmask) | orbits
+{
+    int r;
+    asm("lop3.b32 %0, %1, %2, %3, 0xEA;" : "=r"(r) : "r"(a), "r"(andmask), "r"(orbits));
+    return r;
+}
+// address of element `off` (>= 0) of a float / float4 array: unsigned offset -> one IMAD.WIDE.U32
+__device__ __forceinline__ const float *elem_addr(const float *base, int off) { return base + (unsigned)off; }
+__device__ __forceinline__ const float4 *elem_addr(const float4 *base, int off) { return base + (unsigned)off; }
+__device__ __forceinline__ float rsqrt_approx(float x)
+{
+    float y;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+// ------------------------------------------------------------------------------------------
+// Node coordinate of a primitive along one table axis.
+//   tf : t_clamped + 1.5*2^23 rounded down; its bit pattern is 0x4B400000 + floor(t)
+//   fi : floor(t) as a float,  w = t_clamped - floor(t) in [0,1)
+//   d  : t_clamped - t (0 inside the table): the clamp correction of the T' form is d * d2f
+// ------------------------------------------------------------------------------------------
+constexpr float kMagic = 12582912.0f;              // 1.5 * 2^23
+constexpr unsigned kMagicBits = 0x4B400000u;
+struct Loc32 { float tf, fi, w, d; };
+template <bool DIAG>
+__device__ __forceinline__ Loc32 locate32(const AxisCoef &a, float q, int &clamped, int one_bits)
+{
+    // non-positive (and negative-NaN) -> bits 0 -> exponent -127: below every table (lower-edge clamp)
+    const int b = max(__float_as_int(q), 0);
+    const float u = __int_as_float((b >> 23) | 0x4B000000);                     // 2^23 + biased exponent, exact
+    const float lm = lg2_approx(__int_as_float(and_or(b, 0x007fffff, one_bits)));   // MUFU.LG2 on [1,2): abs err 2^-22
+    const float t = fmaf(u - a.ke, a.invf, fmaf(lm, a.invf, a.cf));
+    if constexpr (DIAG) clamped |= (t < 0.f) | (t > a.nm1f);
+    const float tc = fminf(fmaxf(t, 0.f), a.tmaxf);
+    Loc32 L;
+    L.tf = __fadd_rd(tc, kMagic);
+    L.fi = L.tf - kMagic;
+    L.w = tc - L.fi;
+    L.d = tc - t;
+    return L;
+}
+__device__ __forceinline__ int loc_bits(const Loc32 &l) { return __float_as_int(l.tf); }
+__device__ __forceinline__ float lerp(float w, float a, float b) { return fmaf(w, b - a, a); }
+
+// ------------------------------------------------------------------------------------------
+// Lookup policies over the T' tables.
+// ------------------------------------------------------------------------------------------
+struct F32Global {
+    static constexpr bool kHw = false, kSmem = false;
+    const float *p1; const float4 *p4; int sr, se, si, c3, c4;
+    __device__ F32Global(const DevTable &T, const void *) : p1(T.f1), p4(T.f4), sr(T.s_rho), se(T.s_the), si(T.s_thi)
+    {
+        c3 = (int)(0u - kMagicBits * (unsigned)(sr + se + 1));            // removes the bias of the three index words
+        c4 = (int)(0u - kMagicBits * (unsigned)(sr + se + si + 1));
+    }
+    // c[cr*4 + ce*2 + cb]
+    __device__ __forceinline__ void corners3(const Loc32 &r, const Loc32 &e, const Loc32 &b, float (&c)[8]) const
+    {
+        const int off = loc_bits(r) * sr + (loc_bits(e) * se + (loc_bits(b) + c3));
+        const float *p = elem_addr(p1, off), *q = elem_addr(p1, off + se), *u = elem_addr(p1, off + sr), *v = elem_addr(p1, off + sr + se);
+        c[0] = __ldg(p); c[1] = __ldg(p + 1); c[2] = __ldg(q); c[3] = __ldg(q + 1);
+        c[4] = __ldg(u); c[5] = __ldg(u + 1); c[6] = __ldg(v); c[7] = __ldg(v + 1);
+    }
+    // the 16 texels around (r, e, ii, b): q[ce][ci][cr*2 + cb]
+    __device__ __forceinline__ void corners4(const Loc32 &r, const Loc32 &e, const Loc32 &ii, const Loc32 &b, float4 (&q)[2][2][4]) const
+    {
+        const int off = loc_bits(r) * sr + (loc_bits(e) * se + (loc_bits(ii) * si + (loc_bits(b) + c4)));
+#pragma unroll
+        for (int ce = 0; ce < 2; ++ce)
+#pragma unroll
+            for (int ci = 0; ci < 2; ++ci) {
+                const int o = off + (ce ? se : 0) + (ci ? si : 0);
+                const float4 *a = elem_addr(p4, o), *u = elem_addr(p4, o + sr);
+                q[ce][ci][0] = __ldg(a); q[ce][ci][1] = __ldg(a + 1); q[ce][ci][2] = __ldg(u); q[ce][ci][3] = __ldg(u + 1);
+            }
+    }
+};
+struct F32Smem {
+    static constexpr bool kHw = false, kSmem = true;
+    const float *p1; const float4 *p4; int sr, se, si, c3, c4;
+    __device__ F32Smem(const DevTable &T, const void *img) : p1((const float *)img), p4((const float4 *)img), sr(T.s_rho), se(T.s_the), si(T.s_thi)
+    {
+        c3 = (int)(0u - kMagicBits * (unsigned)(sr + se + 1));
+        c4 = (int)(0u - kMagicBits * (unsigned)(sr + se + si + 1));
+    }
+    __device__ __forceinline__ void corners3(const Loc32 &r, const Loc32 &e, const Loc32 &b, float (&c)[8]) const
+    {
+        const int off = loc_bits(r) * sr + (loc_bits(e) * se + (loc_bits(b) + c3));
+        const float *p = p1 + off, *q = p + se, *u = p + sr, *v = u + se;
+        c[0] = p[0]; c[1] = p[1]; c[2] = q[0]; c[3] = q[1]; c[4] = u[0]; c[5] = u[1]; c[6] = v[0]; c[7] = v[1];
+    }
+    __device__ __forceinline__ void corners4(const Loc32 &r, const Loc32 &e, const Loc32 &ii, const Loc32 &b, float4 (&q)[2][2][4]) const
+    {
+        const int off = loc_bits(r) * sr + (loc_bits(e) * se + (loc_bits(ii) * si + (loc_bits(b) + c4)));
+        const float4 *p = p4 + off;
+#pragma unroll
+        for (int ce = 0; ce < 2; ++ce)
+#pragma unroll
+            for (int ci = 0; ci < 2; ++ci) {
+                const float4 *a = p + (ce ? se : 0) + (ci ? si : 0), *u = a + sr;
+                q[ce][ci][0] = a[0]; q[ce][ci][1] = a[1]; q[ce][ci][2] = u[0]; q[ce][ci][3] = u[1];
+            }
+    }
+};
+struct F32TexPoint {
+    static constexpr bool kHw = false, kSmem = false;
+    cudaTextureObject_t tex; float nef;
+    __device__ F32TexPoint(const DevTable &T, const void *) : tex(T.ftex_pt), nef((float)T.ax[CAX_THE].n) {}
+    // float node indices (Loc32::fi) avoid int->float conversions; texel centres are at +0.5
+    __device__ __forceinline__ void corners3(const Loc32 &r, const Loc32 &e, const Loc32 &b, float (&c)[8]) const
+    {
+        const float x = b.fi + 0.5f, y = e.fi + 0.5f, z = r.fi + 0.5f;
+        c[0] = tex3D<float>(tex, x, y, z); c[1] = tex3D<float>(tex, x + 1.f, y, z);
+        c[2] = tex3D<float>(tex, x, y + 1.f, z); c[3] = tex3D<float>(tex, x + 1.f, y + 1.f, z);
+        c[4] = tex3D<float>(tex, x, y, z + 1.f); c[5] = tex3D<float>(tex, x + 1.f, y, z + 1.f);
+        c[6] = tex3D<float>(tex, x, y + 1.f, z + 1.f); c[7] = tex3D<float>(tex, x + 1.f, y + 1.f, z + 1.f);
+    }
+    // the paper's flattening (L155-L159): z = i_rho * n_the + i_the
+    __device__ __forceinline__ void corners4(const Loc32 &r, const Loc32 &e, const Loc32 &ii, const Loc32 &b, float4 (&q)[2][2][4]) const
+    {
+        const float x = b.fi + 0.5f;
+#pragma unroll
+        for (int ce = 0; ce < 2; ++ce)
+#pragma unroll
+            for (int ci = 0; ci < 2; ++ci) {
+                const float y = ii.fi + (float)ci + 0.5f, z = fmaf(r.fi, nef, e.fi + (float)ce + 0.5f);
+                q[ce][ci][0] = tex3D<float4>(tex, x, y, z); q[ce][ci][1] = tex3D<float4>(tex, x + 1.f, y, z);
+                q[ce][ci][2] = tex3D<float4>(tex, x, y, z + nef); q[ce][ci][3] = tex3D<float4>(tex, x + 1.f, y, z + nef);
+            }
+    }
+};
+struct F32TexHw {
+    static constexpr bool kHw = true, kSmem = false;
+    cudaTextureObject_t tex; float nef;
+    __device__ F32TexHw(const DevTable &T, const void *) : tex(T.ftex_lin), nef((float)T.ax[CAX_THE].n) {}
+    // MODE 3: one trilinear fetch.  MODE 4: hardware bilinear on (bsq, theta_i) at the four
+    // (rho, theta_e) slices; the flattened dimension is interpolated manually (the paper's scheme).
+    __device__ __forceinline__ float hw3(const Loc32 &r, const Loc32 &e, const Loc32 &b) const
+    {
+        return tex3D<float>(tex, (b.fi + b.w) + 0.5f, (e.fi + e.w) + 0.5f, (r.fi + r.w) + 0.5f);
+    }
+    __device__ __forceinline__ float4 hw4(const Loc32 &r, const Loc32 &e, const Loc32 &ii, const Loc32 &b) const
+    {
+        const float x = (b.fi + b.w) + 0.5f, y = (ii.fi + ii.w) + 0.5f, z = fmaf(r.fi, nef, e.fi + 0.5f);
+        const float4 v00 = tex3D<float4>(tex, x, y, z), v01 = tex3D<float4>(tex, x, y, z + 1.f);
+        const float4 v10 = tex3D<float4>(tex, x, y, z + nef), v11 = tex3D<float4>(tex, x, y, z + nef + 1.f);
+        float4 o;
+        o.x = lerp(r.w, lerp(e.w, v00.x, v01.x), lerp(e.w, v10.x, v11.x));
+        o.y = lerp(r.w, lerp(e.w, v00.y, v01.y), lerp(e.w, v10.y, v11.y));
+        o.z = lerp(r.w, lerp(e.w, v00.z, v01.z), lerp(e.w, v10.z, v11.z));
+        o.w = lerp(r.w, lerp(e.w, v00.w, v01.w), lerp(e.w, v10.w, v11.w));
+        return o;
+    }
+    __device__ __forceinline__ void corners3(const Loc32 &, const Loc32 &, const Loc32 &, float (&)[8]) const {}
+    __device__ __forceinline__ void corners4(const Loc32 &, const Loc32 &, const Loc32 &, const Loc32 &, float4 (&)[2][2][4]) const {}
+};
+
+// ------------------------------------------------------------------------------------------
+// MODE 3: trilinear interpolation of T' (contract bsq, then Theta_e, then rho)
+// ------------------------------------------------------------------------------------------
+template <class Fetch>
+__device__ __forceinline__ float interp3_f32(const Fetch &F, const Loc32 &r, const Loc32 &e, const Loc32 &b)
+{
+    if constexpr (Fetch::kHw) {
+        return F.hw3(r, e, b);
+    } else {
+        float c[8];
+        F.corners3(r, e, b, c);
+        const float a00 = lerp(b.w, c[0], c[1]), a01 = lerp(b.w, c[2], c[3]);
+        const float a10 = lerp(b.w, c[4], c[5]), a11 = lerp(b.w, c[6], c[7]);
+        return lerp(r.w, lerp(e.w, a00, a01), lerp(e.w, a10, a11));
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// MODE 4: bilinear patch in (w_e, w_i) of the four channels over one (i_e, i_i) table cell:
+//   y_k = c[k][0] + c[k][1] w_e + c[k][2] w_i + c[k][3] w_e w_i     (rho, bsq already contracted)
+// ------------------------------------------------------------------------------------------
+struct Patch4 { float c[4][4]; int ke, ki; };
+template <class Fetch>
+__device__ __forceinline__ void build_patch(const Fetch &F, const Loc32 &r, const Loc32 &b, const Loc32 &e, const Loc32 &ii, Patch4 &P)
+{
+    P.ke = loc_bits(e); P.ki = loc_bits(ii);
+    float4 q[2][2][4];
+    F.corners4(r, e, ii, b, q);
+    float v[2][2][4];
+#pragma unroll
+    for (int ce = 0; ce < 2; ++ce)
+#pragma unroll
+        for (int ci = 0; ci < 2; ++ci) {
+            const float4 *t = q[ce][ci];
+            v[ce][ci][0] = lerp(r.w, lerp(b.w, t[0].x, t[1].x), lerp(b.w, t[2].x, t[3].x));
+            v[ce][ci][1] = lerp(r.w, lerp(b.w, t[0].y, t[1].y), lerp(b.w, t[2].y, t[3].y));
+            v[ce][ci][2] = lerp(r.w, lerp(b.w, t[0].z, t[1].z), lerp(b.w, t[2].z, t[3].z));
+            v[ce][ci][3] = t[0].w;                       // log2 C depends on (i_e, i_i) only
+        }
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        P.c[k][0] = v[0][0][k];
+        P.c[k][1] = v[1][0][k] - v[0][0][k];
+        P.c[k][2] = v[0][1][k] - v[0][0][k];
+        P.c[k][3] = (v[1][1][k] - v[1][0][k]) - P.c[k][2];
+    }
+}
+__device__ __forceinline__ float patch_eval(const Patch4 &P, int k, float we, float wi)
+{
+    return fmaf(we, fmaf(wi, P.c[k][3], P.c[k][1]), fmaf(wi, P.c[k][2], P.c[k][0]));
+}
+
+// Coulomb coefficient C = 2^(bilinear log2 C).  SMEM: `cs` is a shared-memory window address
+// (LDS, no generic loads); otherwise the table is read from global memory.
+__device__ __forceinline__ float lds_f32(unsigned addr)
+{
+    float v;
+    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(addr));
+    return v;
+}
+template <bool SMEM>
+__device__ __forceinline__ float coulomb_C32(int n1, const float *cg, unsigned cs, const Loc32 &a, const Loc32 &b)
+{
+    const int off = loc_bits(a) * n1 + (loc_bits(b) + (int)(0u - kMagicBits * (unsigned)(n1 + 1)));
+    float c00, c01, c10, c11;
+    if constexpr (SMEM) {
+        const unsigned p = cs + 4u * (unsigned)off, q = p + 4u * (unsigned)n1;
+        c00 = lds_f32(p); c01 = lds_f32(p + 4); c10 = lds_f32(q); c11 = lds_f32(q + 4);
+    } else {
+        const float *p = elem_addr(cg, off), *q = elem_addr(cg, off + n1);
+        c00 = __ldg(p); c01 = __ldg(p + 1); c10 = __ldg(q); c11 = __ldg(q + 1);
+    }
+    return ex2_approx(lerp(a.w, lerp(b.w, c00, c01), lerp(b.w, c10, c11)));
+}
+
+struct Ctx32 { const DevTable &T; const F32Const &S; unsigned coul_s; };      // coul_s: shared-memory address of the staged log2 C table
+
+// ------------------------------------------------------------------------------------------
+// NV cells of one thread through all sub-steps, straight-line (no per-cell branches except the
+// MODE-4 patch rebuild), so the compiler interleaves them for ILP.
+//   CM: 1 = Coulomb from the coefficient table (fast path), 0 = runtime S.coulomb (off / table / analytic)
+// ------------------------------------------------------------------------------------------
+template <int MODE, class Fetch, bool DIAG, int CM, bool NSUB1, int NV>
+__device__ __forceinline__ void step_cells_f32(const Ctx32 &X, const Fetch &F, const float *rho, const float *bsq, float *the, float *thi,
+                                               const float *rr, const float *vol, DiagAcc &acc)
+{
+    const DevTable &T = X.T; const F32Const &S = X.S;
+    const int coulomb = (CM == 1) ? 1 : S.coulomb;
+    const int one_bits = opaque_const(0x3f800000);
+    const bool use_floor = S.hfloor2 > 0.f;                 // warp-uniform
+    bool bad[NV]; float fb_e[NV], fb_i[NV];
+    Loc32 lr[NV], lb[NV];
+    float kcell[NV], coul_kr[NV], tfloor[NV], lsum[NV][4];
+    int clamped[NV], limited[NV], floored[NV];
+    Patch4 P[(MODE == 4 && !Fetch::kHw) ? NV : 1];
+#pragma unroll
+    for (int j = 0; j < NV; ++j) {
+        // rho <= 0: pass through; any NaN: NaN out (that cell only) — resolved by one select per output
+        const float chk = (rho[j] + bsq[j]) + (the[j] + thi[j]);
+        const float z = __fsub_rn(chk, chk);                      // 0, or NaN when any input is NaN (or the sum overflows)
+        bad[j] = !(rho[j] > 0.f) || z != 0.f;
+        fb_e[j] = the[j] + z; fb_i[j] = thi[j] + z;
+        clamped[j] = limited[j] = floored[j] = 0;
+        lr[j] = locate32<DIAG>(T.ax[CAX_RHO], rho[j], clamped[j], one_bits);
+        lb[j] = locate32<DIAG>(T.ax[CAX_BSQ], bsq[j], clamped[j], one_bits);
+        tfloor[j] = 0.f;
+        kcell[j] = fmaf(lr[j].d, T.ax[CAX_RHO].d2f, S.k0);     // log2 h + clamp correction of the rho axis
+        coul_kr[j] = S.coul_kh * rho[j];
+        lsum[j][0] = lsum[j][1] = lsum[j][2] = lsum[j][3] = 0.f;
+        if (MODE == 4 && !Fetch::kHw) { P[j].ke = 0; P[j].ki = 0; }
+    }
+    if (use_floor) {
+#pragma unroll
+        for (int j = 0; j < NV; ++j)
+            if (rr[j] > 0.f) {
+                const float ok = __fdividef(rr[j], fmaf(rr[j], sqrtf(rr[j]), S.spin));     // Omega_K r
+                tfloor[j] = S.hfloor2 * ok * ok;
+            }
+    }
+
+    const int nsub = NSUB1 ? 1 : S.nsub;
+    for (int s = 0; s < nsub; ++s) {
+        bool changed = false;
+        float drad_last[NV], fr[NV][3];
+#pragma unroll
+        for (int j = 0; j < NV; ++j) {
+            const Loc32 le = locate32<DIAG>(T.ax[CAX_THE], the[j], clamped[j], one_bits);
+            const float kk = fmaf(le.d, T.ax[CAX_THE].d2f, kcell[j]);
+            float rrad, yc = 0.f;
+            fr[j][0] = fr[j][1] = fr[j][2] = 0.f;
+            Loc32 li{0.f, 0.f, 0.f, 0.f};
+            if constexpr (MODE == 3) {
+                rrad = ex2_approx(interp3_f32(F, lr[j], le, lb[j]) + kk);
+            } else {
+                li = locate32<DIAG>(T.ax[CAX_THI], thi[j], clamped[j], one_bits);
+                float y0, y1, y2;
+                if constexpr (Fetch::kHw) {
+                    const float4 v = F.hw4(lr[j], le, li, lb[j]);
+                    y0 = v.x; y1 = v.y; y2 = v.z; yc = v.w;
+                } else {
+                    if (loc_bits(le) != P[j].ke || loc_bits(li) != P[j].ki) build_patch(F, lr[j], lb[j], le, li, P[j]);
+                    y0 = patch_eval(P[j], 0, le.w, li.w); y1 = patch_eval(P[j], 1, le.w, li.w);
+                    y2 = patch_eval(P[j], 2, le.w, li.w); yc = patch_eval(P[j], 3, le.w, li.w);
+                }
+                const float rbr = ex2_approx(fminf(y0 + kk, 100.f));
+                const float esy = y1 + kk;
+                const float rsy = ex2_approx(fminf(esy + y2, 100.f));                              // eta * Q_syn
+                const float rthin = rbr + rsy;                                                     // eq 10
+                // eqs 13-14 and 11-12 in ratio form: tau_abs = r_thin inv_kB rho c_s / Theta_e^3
+                const float num = fmaf(S.ae, the[j], S.ai * thi[j]), den = fmaf(S.be, the[j], fmaf(S.bi, thi[j], 1.f));
+                const float rcs = rho[j] * (num * rsqrt_approx(num * den));                       // rho c_s
+                const float th3 = fmaxf(the[j] * the[j] * the[j], 1e-30f);
+                const float tau_abs = rthin * (S.inv_kB * rcs) * rcp_approx(th3);                 // eq 12
+                const float tau_sca = S.ksca * rcs;
+                rrad = rthin * rcp_approx(fmaf(tau_abs, fmaf(1.5f, tau_abs + tau_sca, 1.7320508f), 1.f));   // eq 11
+                if constexpr (DIAG) {
+                    const float inv = rcp_approx(fmaxf(rthin, 1e-37f));
+                    const float rs0 = ex2_approx(fminf(esy, 100.f));                               // Q_syn alone
+                    fr[j][0] = rbr * inv; fr[j][1] = rs0 * inv; fr[j][2] = (rsy - rs0) * inv;
+                }
+            }
+            if (use_floor) {
+                if ((the[j] + thi[j]) * S.mr < tfloor[j]) { rrad = 0.f; floored[j] = 1; }
+            }
+            if constexpr (DIAG) limited[j] |= (rrad > S.f_limit);
+            rrad = fminf(rrad, S.f_limit);
+            // Coulomb exchange (eq 15), capped by f_limit of the donor and by the equalising transfer
+            float dthe = 0.f;
+            const float D = thi[j] - the[j];
+            if (coulomb != 0) {
+                float C;
+                if (coulomb == 1) {
+                    if (MODE == 4 && T.f4_has_coul) {
+                        C = ex2_approx(yc);
+                    } else {
+                        int dummy = 0;
+                        Loc32 ca, cb;                                   // Coulomb-table coordinates of Theta_i, Theta_e
+                        if (MODE == 4 && T.coul_share_thi) ca = li; else ca = locate32<false>(T.cax[0], thi[j], dummy, one_bits);
+                        if (T.coul_share_the) cb = le; else cb = locate32<false>(T.cax[1], the[j], dummy, one_bits);
+                        // CM = 1 is only launched with the table staged in shared memory
+                        C = (CM == 1) ? coulomb_C32<true>(T.cax[1].n, T.fcoul, X.coul_s, ca, cb) : coulomb_C32<false>(T.cax[1].n, T.fcoul, 0u, ca, cb);
+                    }
+                } else {
+                    C = (D != 0.f && !bad[j]) ? (float)coolphys::coulomb_C((double)the[j], (double)thi[j] / S.ion_ratio) : 0.f;
+                }
+                const float raw = coul_kr[j] * C * fabsf(D);
+                const float cap1 = (D > 0.f) ? S.cap1i * thi[j] : S.cap1e * the[j];
+                const float mag = fminf(raw, fminf(cap1, fabsf(D) * S.eq_frac));
+                dthe = copysignf(mag, D);
+            }
+            // explicit _rn intrinsics: never contracted, so every instantiation rounds identically
+            const float drad = __fmul_rn(rrad, the[j]);
+            const float the_n = __fadd_rn(__fsub_rn(the[j], drad), dthe);
+            const float thi_n = __fmaf_rn(-dthe, S.gi1_over_ge1, thi[j]);
+            if constexpr (DIAG) {
+                drad_last[j] = drad;
+                lsum[j][0] += drad; lsum[j][1] = fmaf(drad, fr[j][0], lsum[j][1]);
+                lsum[j][2] = fmaf(drad, fr[j][1], lsum[j][2]); lsum[j][3] = fmaf(drad, fr[j][2], lsum[j][3]);
+            }
+            if constexpr (!NSUB1) changed |= (the_n != the[j]) | (thi_n != thi[j]);
+            the[j] = the_n; thi[j] = thi_n;
+        }
+        if constexpr (!NSUB1) {
+            // exact early exit: a sub-step that leaves every temperature bit-identical repeats itself
+            if (!changed) {
+                if constexpr (DIAG) {
+                    const float rem = (float)(nsub - 1 - s);
+#pragma unroll
+                    for (int j = 0; j < NV; ++j) {
+                        lsum[j][0] = fmaf(rem, drad_last[j], lsum[j][0]);
+#pragma unroll
+                        for (int k = 0; k < 3; ++k) lsum[j][k + 1] = fmaf(rem, drad_last[j] * fr[j][k], lsum[j][k + 1]);
+                    }
+                }
+                break;
+            }
+        }
+    }
+#pragma unroll
+    for (int j = 0; j < NV; ++j) {
+        if (bad[j]) { the[j] = fb_e[j]; thi[j] = fb_i[j]; }
+        if constexpr (DIAG) {
+            if (!bad[j]) {
+                const float wgt = rho[j] * vol[j];
+#pragma unroll
+                for (int k = 0; k < 4; ++k) acc.lum[k] += (double)(lsum[j][k] * wgt);
+                acc.lim += limited[j]; acc.flo += floored[j]; acc.cla += clamped[j];
+            }
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// The kernel.  Dynamic shared memory: [2 mbarriers | 2 stages x nf arrays x TILE floats |
+// Coulomb table (when small) | table image (SMEM variant)].
+// ------------------------------------------------------------------------------------------
+constexpr int kF32CellsPerThread = 4;
+constexpr unsigned kF32BarBytes = 16;
+
+template <int MODE, class Fetch, bool DIAG, int CM, bool NSUB1, int THREADS, int MINB>
+__global__ void __launch_bounds__(THREADS, MINB)
+cool_f32_kernel(const DevTable T, const F32Const S, const CellPtrs C, double *partials, unsigned *ticket, cool_diag *d_diag)
+{
+    constexpr int TILE = THREADS * kF32CellsPerThread;
+    constexpr int G = (MODE == 4) ? 1 : kF32CellsPerThread;      // cells advanced together (MODE 4: the patch is 16 registers per cell)
+    extern __shared__ __align__(128) unsigned char smem_f32[];
+    const unsigned bar0 = smem_u32(smem_f32), bar1 = bar0 + 8;
+    float *stages = (float *)(smem_f32 + kF32BarBytes);
+    const unsigned stage_u32 = smem_u32(stages);
+    const int tid = threadIdx.x;
+
+    if (CM == 1 && S.coul_smem) {
+        float *s_coul = (float *)(smem_f32 + S.coul_off);
+        for (int k = tid; k < (T.coul_bytes >> 2); k += THREADS) s_coul[k] = __ldg(T.fcoul + k);
+    }
+    if constexpr (Fetch::kSmem) {
+        const float4 *src = MODE == 3 ? (const float4 *)T.f1 : T.f4;
+        float4 *dst = (float4 *)(smem_f32 + S.table_off);
+        const unsigned n16 = T.table_bytes >> 4;                  // table_bytes is padded to 16 B at create time
+        for (unsigned k = tid; k < n16; k += THREADS) dst[k] = __ldg(src + k);
+    }
+    const Fetch F(T, smem_f32 + S.table_off);
+    const Ctx32 X{T, S, smem_u32(smem_f32 + S.coul_off)};
+
+    const long long ncell = C.ncell;
+    const long long ntiles = (ncell + TILE - 1) / TILE;
+    const void *src[6] = {C.rho, C.bsq, C.the_in, C.thi_in, C.vol, C.r};     // staged in this order; vol / r only when present
+    const int nf = S.nf;
+    const unsigned arr_bytes = TILE * 4u;
+
+    // one elected thread arms the stage's mbarrier and issues the bulk copies of one full tile
+    auto issue = [&](long long tile, int s) {
+        const unsigned bar = s ? bar1 : bar0;
+        const unsigned dst = stage_u32 + (unsigned)s * S.stage_bytes;
+        const size_t goff = (size_t)tile * TILE * 4u;
+        mbar_expect_tx(bar, arr_bytes * (unsigned)nf);
+        int k = 0;
+#pragma unroll
+        for (int a = 0; a < 6; ++a) {
+            if (a == 4 && !S.has_vol) continue;
+            if (a == 5 && !S.has_r) continue;
+            tma_load_1d(dst + (unsigned)k * arr_bytes, (const char *)src[a] + goff, arr_bytes, bar);
+            ++k;
+        }
+    };
+    auto is_tma_tile = [&](long long tile) { return S.use_tma && tile < ntiles && (tile + 1) * TILE <= ncell; };
+
+    if (tid == 0) {
+        mbar_init(bar0, 1); mbar_init(bar1, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        if (is_tma_tile(blockIdx.x)) issue(blockIdx.x, 0);
+        if (is_tma_tile((long long)blockIdx.x + gridDim.x)) issue((long long)blockIdx.x + gridDim.x, 1);
+    }
+    __syncthreads();
+
+    DiagAcc acc;
+    int it = 0;
+    for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x, ++it) {
+        const int s = it & 1;
+        float *st = (float *)((unsigned char *)stages + (size_t)s * S.stage_bytes);
+        const long long c0 = tile * TILE;
+        const bool full = (tile + 1) * TILE <= ncell;
+        if (S.use_tma && full) {
+            mbar_wait(s ? bar1 : bar0, (unsigned)(it >> 1) & 1u);
+        } else {
+            // ragged last tile, or arrays that are not 16-byte aligned: cooperative plain loads (zero fill past the end)
+            int k = 0;
+#pragma unroll
+            for (int a = 0; a < 6; ++a) {
+                if (a == 4 && !S.has_vol) continue;
+                if (a == 5 && !S.has_r) continue;
+                const float *g = (const float *)src[a] + c0;
+                for (int i = tid; i < TILE; i += THREADS) st[k * TILE + i] = (c0 + i < ncell) ? __ldg(g + i) : 0.f;
+                ++k;
+            }
+            __syncthreads();
+        }
+        const float4 *s4 = (const float4 *)st;
+        float4 rho = s4[tid], bsq = s4[THREADS + tid], the = s4[2 * THREADS + tid], thi = s4[3 * THREADS + tid];
+        float4 vv = make_float4(1.f, 1.f, 1.f, 1.f), rr = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (S.has_vol) vv = s4[4 * THREADS + tid];
+        if (S.has_r) rr = s4[(S.has_vol ? 5 : 4) * THREADS + tid];
+        __syncthreads();                                        // every thread holds its cells: the stage is free
+        if (tid == 0) {
+            const long long nxt = tile + 2ll * gridDim.x;
+            if (is_tma_tile(nxt)) {
+                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                issue(nxt, s);
+            }
+        }
+#pragma unroll
+        for (int j = 0; j < kF32CellsPerThread; j += G)
+            step_cells_f32<MODE, Fetch, DIAG, CM, NSUB1, G>(X, F, &rho.x + j, &bsq.x + j, &the.x + j, &thi.x + j, &rr.x + j, &vv.x + j, acc);
+        const long long c = c0 + (long long)tid * kF32CellsPerThread;
+        if (full && S.use_tma) {
+            st_stream((float4 *)C.the_out + (c >> 2), the);
+            st_stream((float4 *)C.thi_out + (c >> 2), thi);
+        } else {
+#pragma unroll
+            for (int j = 0; j < kF32CellsPerThread; ++j)
+                if (c + j < ncell) { ((float *)C.the_out)[c + j] = (&the.x)[j]; ((float *)C.thi_out)[c + j] = (&thi.x)[j]; }
+        }
+    }
+    if constexpr (DIAG) reduce_diag(acc, S.lum_k, partials, ticket, d_diag);
+}
+
+// ------------------------------------------------------------------------------------------
+// Host side
+// ------------------------------------------------------------------------------------------
+struct LaunchCtx32 { const cool_table *t; F32Const S; const LaunchArgs *a; cudaStream_t st; };
+
+// fills the shared-memory layout fields of S for a launch with THREADS threads; returns the total
+inline size_t f32_smem_layout(F32Const &S, int threads, bool table_in_smem, const cool_table *t)
+{
+    const size_t tile_bytes = (size_t)threads * kF32CellsPerThread * 4u;
+    S.stage_bytes = (unsigned)(tile_bytes * S.nf);
+    size_t off = kF32BarBytes + 2 * (size_t)S.stage_bytes;
+    S.coul_off = (unsigned)off;
+    if (S.coul_smem) off += ((size_t)t->dev.coul_bytes + 15) & ~(size_t)15;
+    S.table_off = (unsigned)off;
+    if (table_in_smem) off += t->dev.table_bytes;
+    return off;
+}
+
+template <int MODE, class Fetch, bool DIAG, int CM, bool NSUB1, int THREADS, int MINB>
+static cudaError_t launch_f32_one(const LaunchCtx32 &L)
+{
+    F32Const S = L.S;
+    const size_t smem = f32_smem_layout(S, THREADS, Fetch::kSmem, L.t);
+    auto kern = cool_f32_kernel<MODE, Fetch, DIAG, CM, NSUB1, THREADS, MINB>;
+    static int occ_cache = -1; static size_t occ_smem = ~(size_t)0;
+    if (smem > 48 * 1024) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+    }
+    if (occ_cache < 0 || occ_smem != smem) {
+        int occ = 0;
+        cudaError_t eo = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, THREADS, smem);
+        if (eo != cudaSuccess) return eo;
+        occ_cache = occ < 1 ? 1 : occ; occ_smem = smem;
+    }
+    const LaunchArgs &a = *L.a;
+    constexpr long long TILE = (long long)THREADS * kF32CellsPerThread;
+    const long long ntiles = (a.ncell + TILE - 1) / TILE;
+    const long long cap = (long long)L.t->sm_count * occ_cache;
+    const int grid = (int)(ntiles < cap ? (ntiles < 1 ? 1 : ntiles) : cap);
+    CellPtrs C{a.rho, a.bsq, a.the_in, a.thi_in, a.r, a.vol, a.the_out, a.thi_out, a.ncell};
+    kern<<<grid, THREADS, smem, L.st>>>(L.t->dev, S, C, a.partials, a.ticket, a.d_diag);
+    return cudaGetLastError();
+}
+
+constexpr int kF32SmemThreads = 384;
+
+// dispatch over the four table variants for fixed <MODE, DIAG, CM, NSUB1>
+template <int MODE, bool DIAG, int CM, bool NSUB1>
+static cudaError_t launch_f32_by_variant(const LaunchCtx32 &L, cool_variant v)
+{
+    constexpr int MB = 2;
+    switch (v) {
+        case COOL_V_GLOBAL: return launch_f32_one<MODE, F32Global, DIAG, CM, NSUB1, 256, MB>(L);
+        case COOL_V_TEX_POINT: return launch_f32_one<MODE, F32TexPoint, DIAG, CM, NSUB1, 256, MB>(L);
+        case COOL_V_TEX_HWFILTER: return launch_f32_one<MODE, F32TexHw, DIAG, CM, NSUB1, 256, MB>(L);
+        case COOL_V_SMEM: return launch_f32_one<MODE, F32Smem, DIAG, CM, NSUB1, kF32SmemThreads, 1>(L);
+        default: return cudaErrorInvalidValue;
+    }
+}
+
+// one function per translation unit of instantiations (cool_inst_f32_*.cu)
+cudaError_t launch_f32_m3(const LaunchCtx32 &L, cool_variant v, bool diag, int cm, bool nsub1);
+cudaError_t launch_f32_m4(const LaunchCtx32 &L, cool_variant v, bool diag, int cm);
+
+}  // namespace cool

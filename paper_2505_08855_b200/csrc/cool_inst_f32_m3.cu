@@ -1,9 +1,14 @@
-// fp32 cells, MODE 3 tables: {diag off/on} x {Coulomb generic / table fast path} x 4 lookup variants
-#include "cool_kernels.cuh"
+// fp32 cells, MODE 3 tables: {diag off/on} x {Coulomb generic / table fast path} x {nsub loop / single update} x 4 lookup variants
+#include "cool_f32.cuh"
 namespace cool {
-cudaError_t launch_f32_m3(const LaunchCtx &L, cool_variant v, bool diag, int cm)
+template <bool DIAG, int CM>
+static cudaError_t go(const LaunchCtx32 &L, cool_variant v, bool nsub1)
 {
-    if (diag) return cm ? launch_by_variant<float, 3, true, 1>(L, v) : launch_by_variant<float, 3, true, 0>(L, v);
-    return cm ? launch_by_variant<float, 3, false, 1>(L, v) : launch_by_variant<float, 3, false, 0>(L, v);
+    return nsub1 ? launch_f32_by_variant<3, DIAG, CM, true>(L, v) : launch_f32_by_variant<3, DIAG, CM, false>(L, v);
+}
+cudaError_t launch_f32_m3(const LaunchCtx32 &L, cool_variant v, bool diag, int cm, bool nsub1)
+{
+    if (diag) return cm ? go<true, 1>(L, v, nsub1) : go<true, 0>(L, v, nsub1);
+    return cm ? go<false, 1>(L, v, nsub1) : go<false, 0>(L, v, nsub1);
 }
 }  // namespace cool

@@ -1,9 +1,9 @@
 // fp32 cells, MODE 4 tables: {diag off/on} x {Coulomb generic / table fast path} x 4 lookup variants
-#include "cool_kernels.cuh"
+#include "cool_f32.cuh"
 namespace cool {
-cudaError_t launch_f32_m4(const LaunchCtx &L, cool_variant v, bool diag, int cm)
+cudaError_t launch_f32_m4(const LaunchCtx32 &L, cool_variant v, bool diag, int cm)
 {
-    if (diag) return cm ? launch_by_variant<float, 4, true, 1>(L, v) : launch_by_variant<float, 4, true, 0>(L, v);
-    return cm ? launch_by_variant<float, 4, false, 1>(L, v) : launch_by_variant<float, 4, false, 0>(L, v);
+    if (diag) return cm ? launch_f32_by_variant<4, true, 1, false>(L, v) : launch_f32_by_variant<4, true, 0, false>(L, v);
+    return cm ? launch_f32_by_variant<4, false, 1, false>(L, v) : launch_f32_by_variant<4, false, 0, false>(L, v);
 }
 }  // namespace cool

@@ -26,6 +26,8 @@ struct AxisCoef {          // node-index coordinate t of a primitive q along one
     // fp32 path: log2 q = e + lm (e integer, lm in [0,1)):  t = (e - e0)*invf + (lm*invf + cf)
     float e0, invf, cf;
     float nm1f, tmaxf;     // n-1 (clamp flag) and the largest float below n-1 (keeps floor(t) <= n-2)
+    float ke;              // 2^23 + 127 + e0: (2^23 + biased exponent) - ke = e - e0, exactly
+    float d2f;             // node spacing in log2 units (clamp correction of the fp32 path)
 };
 
 struct DevTable {
@@ -37,6 +39,15 @@ struct DevTable {
     cudaTextureObject_t tex_pt, tex_lin;   // 3-D array: x = bsq, y = theta_e (MODE 3) / theta_i (MODE 4),
                                            // z = rho (MODE 3) / rho*n_the + i_the (MODE 4, the paper's flattening)
     unsigned table_bytes;          // bytes of the linear copy (for the smem variant)
+    // fp32 path: the same nodes re-expressed as log2 of the rate per unit electron energy,
+    //   MODE 3: f1 = log2(Lambda ge1 / (mr rho_node Theta_e_node))
+    //   MODE 4: f4 = {log2(Q_brem ge1/(mr rho Theta_e)), log2(Q_syn ge1/(mr rho Theta_e)), log2 eta, log2 C or 0}
+    // so that Lambda h / u_e = 2^(interp + log2 h) without cancelling large fp32 numbers.
+    const float *f1;
+    const float4 *f4;
+    cudaTextureObject_t ftex_pt, ftex_lin;
+    const float *fcoul;            // log2 C [theta_i][theta_e]
+    int f4_has_coul;               // MODE 4: f4.w = log2 C (Coulomb axes identical to the table's Theta axes)
     // Coulomb coefficient table log10 C [theta_i][theta_e]
     const float *coul;
     AxisCoef cax[2];               // 0: theta_i, 1: theta_e
@@ -78,8 +89,9 @@ struct cool_table {
     cool::DevTable dev{};
     cool::DevConst cst{};
     float *d_lin = nullptr;        // owns lin1 / lin4
-    float *d_coul = nullptr;
-    cudaArray_t arr = nullptr;
+    float *d_f32 = nullptr;        // owns f1 / f4
+    float *d_coul = nullptr, *d_fcoul = nullptr;
+    cudaArray_t arr = nullptr, arr32 = nullptr;
     int sm_count = 148;
     int max_smem_optin = 0;
     bool persist_l2 = false;

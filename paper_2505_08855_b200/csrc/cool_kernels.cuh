@@ -1,4 +1,6 @@
-// cool_kernels.cuh — hand-written sm_100a kernels of the per-cell cooling step (include/cool.h).
+// cool_kernels.cuh — hand-written sm_100a kernels of the per-cell cooling step (include/cool.h):
+// the fp64 table variants and the analytic variant (either cell dtype), plus what the fp32 kernels
+// of cool_f32.cuh share with them (streaming I/O, diagnostics reduction).
 //
 // One kernel template, instantiated per (cell dtype) x (table shape) x (lookup variant) x flags:
 //   * cells stream as SoA with 128-bit L1-bypassing loads/stores, 16 B per thread per array;
@@ -6,11 +8,8 @@
 //     texture, hardware-filtered texture) or not at all (analytic);
 //   * the luminosity diagnostic is reduced warp -> block -> fixed-order last-block pass, so it is
 //     bit-reproducible for a given launch shape.
-// The step is a gather plus scalar arithmetic: no tensor cores.  On B200
-// the fp32 path is bound by instruction issue (~133 thread-instructions per cell at the HBM
-// roofline), so the fp32 code below is written to minimise instructions: no int<->float
-// conversions, floor() by a round-down add, compile-time flags for diagnostics and Coulomb mode,
-// table patches cached across sub-steps, exact early exit once a cell stops changing.
+// The fp64 path mirrors the definition step by step (tolerance 1e-12); it is the correctness
+// path of configs[0], not the throughput path.
 #pragma once
 #include "cool_internal.h"
 
@@ -25,15 +24,7 @@ struct StepConst {
     double ae, ai, be, bi;         // c_s^2 = (ae Th_e + ai Th_i)/(1 + be Th_e + bi Th_i)      (eq 14)
     double hfloor2, spin;          // floor: (pi/2) h_floor^2 (Omega_K r)^2                     (eq 19)
     double lum_k;                  // lum = sum(dTheta_rad rho vol) * lum_k,  lum_k = mr/(ge1 dt)
-    // fp32 path
-    float L10h, L10l;              // log2(10) = L10h + L10l
-    float ksm;                     // log2(h) - log2(mr/ge1): fraction-sized constant of the rate exponent
-    float f_limitf, mrf, eq_fracf, ge1_over_gi1, gi1_over_ge1, coul_khf, cap1e, cap1i;
-    float aef, aif, bef, bif;
-    float inv_kB;                  // 1 / ( bb_k h ge1 / (h_per_cs mr) ): 1/r_B = inv_kB rho c_s / Theta_e^3
-    float kscaf;                   // tau_sca = kscaf * rho * c_s
-    float hfloor2f, spinf;
-    int nsub, coulomb, has_r, has_vol, aligned, coul_smem;
+    int nsub, coulomb, has_r, has_vol, aligned;
 };
 
 // ------------------------------------------------------------------------------------------
@@ -324,269 +315,6 @@ __device__ __noinline__ void step_cell_analytic(const DevTable &T, const DevCons
     }
 }
 
-// ==========================================================================================
-// fp32 path.  log2 of every primitive is kept as (integer exponent e, fraction lm = log2 mantissa)
-// so that node coordinates and the exponent of the rate are formed without cancelling large
-// fp32 numbers; the rate is applied as the dimensionless ratio rrad = Lambda h / u_e.
-// NV cells of one thread advance together through straight-line code (no per-cell branches), so
-// the compiler interleaves them for ILP and loads each launch constant once per NV cells.
-// ==========================================================================================
-struct Spl { float e, lm; };
-__device__ __forceinline__ Spl split_log2(float q)
-{
-    // non-positive (and NaN) -> bits of 0 -> exponent -127: below every table (lower-edge clamp)
-    const int b = __float_as_int(fmaxf(q, 0.f));
-    Spl r;
-    r.e = __int_as_float((b >> 23) | 0x4B000000) - 8388735.0f;           // exponent field - 127, no I2F
-    r.lm = __log2f(__int_as_float((b & 0x007fffff) | 0x3f800000));       // MUFU.LG2 on [1,2): abs err 2^-22
-    return r;
-}
-struct Loc32 { int i; float w, fi; };
-template <bool DIAG>
-__device__ __forceinline__ Loc32 locate32(const AxisCoef &a, const Spl &q, int &clamped)
-{
-    Loc32 L;
-    float t = fmaf(q.e - a.e0, a.invf, fmaf(q.lm, a.invf, a.cf));
-    if constexpr (DIAG) clamped |= (t < 0.f) | (t > a.nm1f);
-    t = fminf(fmaxf(t, 0.f), a.tmaxf);
-    // floor without F2I/I2F: adding 1.5*2^23 with round-down leaves floor(t) in the low mantissa bits
-    const float tf = __fadd_rd(t, 12582912.0f);
-    L.i = __float_as_int(tf) & 0x003fffff;
-    L.fi = tf - 12582912.0f;
-    L.w = t - L.fi;
-    return L;
-}
-
-// (base, delta) form: y = base + delta with base an exact table value and |delta| small
-template <class Fetch>
-__device__ __forceinline__ void interp3_f32(const Fetch &F, const Loc32 &r, const Loc32 &e, const Loc32 &b, float &base, float &delta)
-{
-    if constexpr (Fetch::kHw) {
-        base = 0.f;
-        delta = F.hw3(r.fi + r.w, e.fi + e.w, b.fi + b.w);
-    } else {
-        float c[8];                      // [cr][ce][cb]
-        F.corners3(r, e, b, c);
-        base = c[0];
-        const float d010 = c[2] - c[0], d100 = c[4] - c[0], d110 = c[6] - c[0];
-        const float a00 = b.w * (c[1] - c[0]);
-        const float a01 = fmaf(b.w, c[3] - c[2], d010);
-        const float a10 = fmaf(b.w, c[5] - c[4], d100);
-        const float a11 = fmaf(b.w, c[7] - c[6], d110);
-        const float b0 = fmaf(e.w, a01 - a00, a00), b1 = fmaf(e.w, a11 - a10, a10);
-        delta = fmaf(r.w, b1 - b0, b0);
-    }
-}
-
-// MODE 4: the (rho, bsq) interpolation is loop-invariant over sub-steps, so it is done once per
-// visited (i_the, i_thi) cell of the table: patch[ce][ci][channel] relative to base[channel].
-struct Patch4 { float base[3]; float p[2][2][3]; int ie, ii; };
-template <class Fetch>
-__device__ __forceinline__ void build_patch(const Fetch &F, const Loc32 &r, const Loc32 &b, const Loc32 &e, const Loc32 &ii, Patch4 &P)
-{
-    P.ie = e.i; P.ii = ii.i;
-#pragma unroll
-    for (int ce = 0; ce < 2; ++ce)
-#pragma unroll
-        for (int ci = 0; ci < 2; ++ci) {
-            float4 q[4];                 // [cr][cb] at (ie+ce, ii+ci)
-            F.quad4(r, e, ii, b, ce, ci, q);
-            if (ce == 0 && ci == 0) { P.base[0] = q[0].x; P.base[1] = q[0].y; P.base[2] = q[0].z; }
-            const float *a = &q[0].x, *bb = &q[1].x, *c = &q[2].x, *d = &q[3].x;
-#pragma unroll
-            for (int k = 0; k < 3; ++k) {
-                const float x0 = fmaf(b.w, bb[k] - a[k], a[k] - P.base[k]);
-                const float x1 = fmaf(b.w, d[k] - c[k], c[k] - P.base[k]);
-                P.p[ce][ci][k] = fmaf(r.w, x1 - x0, x0);
-            }
-        }
-}
-__device__ __forceinline__ float patch_eval(const Patch4 &P, int k, float we, float wi)
-{
-    const float a0 = fmaf(wi, P.p[0][1][k] - P.p[0][0][k], P.p[0][0][k]);
-    const float a1 = fmaf(wi, P.p[1][1][k] - P.p[1][0][k], P.p[1][0][k]);
-    return fmaf(we, a1 - a0, a0);
-}
-template <class Fetch>
-__device__ __forceinline__ void interp4_hw_f32(const Fetch &F, const Loc32 &r, const Loc32 &e, const Loc32 &ii, const Loc32 &b,
-                                               float base[3], float delta[3])
-{
-    const float ti = ii.fi + ii.w, tb = b.fi + b.w;
-    const float4 v00 = F.hw4(r.fi, e.fi, ti, tb), v01 = F.hw4(r.fi, e.fi + 1.f, ti, tb);
-    const float4 v10 = F.hw4(r.fi + 1.f, e.fi, ti, tb), v11 = F.hw4(r.fi + 1.f, e.fi + 1.f, ti, tb);
-    const float *p00 = &v00.x, *p01 = &v01.x, *p10 = &v10.x, *p11 = &v11.x;
-#pragma unroll
-    for (int k = 0; k < 3; ++k) {
-        base[k] = p00[k];
-        const float a0 = e.w * (p01[k] - p00[k]);
-        const float a1 = fmaf(e.w, p11[k] - p10[k], p10[k] - p00[k]);
-        delta[k] = fmaf(r.w, a1 - a0, a0);
-    }
-}
-
-// Coulomb coefficient C = 10^(bilinear log10 C); cs points to shared or global memory
-__device__ __forceinline__ float coulomb_C32(int n1, const float *cs, const Loc32 &a, const Loc32 &b)
-{
-    const float *p = cs + (a.i * n1 + b.i);
-    const float c00 = p[0], c01 = p[1], c10 = p[n1], c11 = p[n1 + 1];
-    const float y0 = fmaf(b.w, c01 - c00, c00), y1 = fmaf(b.w, c11 - c10, c10);
-    return exp2f(3.3219280948873623f * fmaf(a.w, y1 - y0, y0));
-}
-
-struct Ctx32 { const DevTable &T; const DevConst &K; const StepConst &S; const float *coul; };
-
-// CM: 1 = Coulomb from the coefficient table (fast path), 0 = runtime S.coulomb (off / table / analytic)
-template <int MODE, class Fetch, bool DIAG, int CM, int NV>
-__device__ __forceinline__ void step_cells_f32(const Ctx32 &X, const Fetch &F, const float *rho, const float *bsq, float *the, float *thi,
-                                               const float *rr, const float *vol, DiagAcc &acc)
-{
-    const DevTable &T = X.T; const StepConst &S = X.S;
-    const int coulomb = (CM == 1) ? 1 : S.coulomb;
-    bool bad[NV]; float the0[NV], thi0[NV], nanv[NV];
-    Spl l_r[NV]; Loc32 lr[NV], lb[NV];
-    float kr[NV], coul_kr[NV], tfloor[NV], lsum[NV][4];
-    int clamped[NV], limited[NV], floored[NV];
-    Patch4 P[MODE == 4 && !Fetch::kHw ? NV : 1];
-#pragma unroll
-    for (int j = 0; j < NV; ++j) {
-        // rho <= 0: pass through; any NaN: NaN out (that cell only) — resolved by selects at the end
-        const float chk = (rho[j] + bsq[j]) + (the[j] + thi[j]);
-        bad[j] = !(rho[j] > 0.f) || chk != chk;
-        nanv[j] = chk;
-        the0[j] = the[j]; thi0[j] = thi[j];
-        clamped[j] = limited[j] = floored[j] = 0;
-        l_r[j] = split_log2(rho[j]);
-        const Spl l_b = split_log2(bsq[j]);
-        lr[j] = locate32<DIAG>(T.ax[CAX_RHO], l_r[j], clamped[j]);
-        lb[j] = locate32<DIAG>(T.ax[CAX_BSQ], l_b, clamped[j]);
-        tfloor[j] = 0.f;
-        if (S.hfloor2f > 0.f && rr[j] > 0.f) {
-            const float ok = __fdividef(rr[j], fmaf(rr[j], sqrtf(rr[j]), S.spinf));       // Omega_K r
-            tfloor[j] = S.hfloor2f * ok * ok;
-        }
-        kr[j] = S.ksm - l_r[j].lm;         // loop-invariant fraction part of the rate exponent
-        coul_kr[j] = S.coul_khf * rho[j];
-        lsum[j][0] = lsum[j][1] = lsum[j][2] = lsum[j][3] = 0.f;
-        if (MODE == 4 && !Fetch::kHw) { P[j].ie = -1; P[j].ii = -1; }
-    }
-
-    for (int s = 0; s < S.nsub; ++s) {
-        bool changed = false;
-        float drad_last[NV], fr[NV][3];
-#pragma unroll
-        for (int j = 0; j < NV; ++j) {
-            const Spl l_e = split_log2(the[j]);
-            const Loc32 le = locate32<DIAG>(T.ax[CAX_THE], l_e, clamped[j]);
-            // exponent (log2) of 10^y h/u_e = big + small;  big = exact sum of the large terms
-            const float esum = l_r[j].e + l_e.e;
-            const float ksmall = kr[j] - l_e.lm;
-            auto rate_exp = [&](float base, float delta) {
-                const float Pm = __fmul_rn(base, S.L10h);      // rounded product; the next line recovers its error exactly
-                const float small = fmaf(delta, S.L10h, fmaf(base, S.L10l, fmaf(base, S.L10h, -Pm))) + ksmall;
-                return (Pm - esum) + small;
-            };
-            float rrad;
-            fr[j][0] = fr[j][1] = fr[j][2] = 0.f;
-            Spl l_i{0.f, 0.f}; Loc32 li{0, 0.f, 0.f};
-            if constexpr (MODE == 3) {
-                float base, delta;
-                interp3_f32(F, lr[j], le, lb[j], base, delta);
-                rrad = exp2f(rate_exp(base, delta));
-                if (coulomb == 1) l_i = split_log2(thi[j]);
-            } else {
-                l_i = split_log2(thi[j]);
-                li = locate32<DIAG>(T.ax[CAX_THI], l_i, clamped[j]);
-                float y[3], bs[3];
-                if constexpr (Fetch::kHw) {
-                    interp4_hw_f32(F, lr[j], le, li, lb[j], bs, y);
-                } else {
-                    if (le.i != P[j].ie || li.i != P[j].ii) build_patch(F, lr[j], lb[j], le, li, P[j]);
-#pragma unroll
-                    for (int k = 0; k < 3; ++k) { bs[k] = P[j].base[k]; y[k] = patch_eval(P[j], k, le.w, li.w); }
-                }
-                const float zeta = S.L10h * (bs[2] + y[2]);
-                const float rbr = exp2f(fminf(rate_exp(bs[0], y[0]), 100.f));
-                const float rsy = exp2f(fminf(rate_exp(bs[1], y[1]) + zeta, 100.f));            // eta * Q_syn
-                const float rthin = rbr + rsy;                                                    // eq 10
-                // eqs 13-14 and 11-12 in ratio form: 1/r_B = inv_kB rho c_s / Theta_e^3
-                const float cs2 = __fdividef(fmaf(S.aef, the[j], S.aif * thi[j]), fmaf(S.bef, the[j], fmaf(S.bif, thi[j], 1.f)));
-                const float rcs = rho[j] * sqrtf(cs2);
-                const float tau_abs = rthin * __fdividef(S.inv_kB * rcs, fmaxf(the[j] * the[j] * the[j], 1e-30f));   // eq 12
-                const float tau_sca = S.kscaf * rcs;
-                rrad = __fdividef(rthin, fmaf(tau_abs, fmaf(1.5f, tau_abs + tau_sca, 1.7320508f), 1.f));   // eq 11
-                if constexpr (DIAG) {
-                    const float inv = __fdividef(1.f, rthin);
-                    fr[j][0] = rbr * inv;
-                    fr[j][1] = rsy * exp2f(-zeta) * inv;
-                    fr[j][2] = rsy * inv - fr[j][1];
-                }
-            }
-            if (tfloor[j] > 0.f && (the[j] + thi[j]) * S.mrf < tfloor[j]) { rrad = 0.f; floored[j] = 1; }
-            if constexpr (DIAG) limited[j] |= (rrad > S.f_limitf);
-            rrad = fminf(rrad, S.f_limitf);
-            // Coulomb exchange (eq 15), capped by f_limit of the donor and by the equalising transfer
-            float dthe = 0.f;
-            const float D = thi[j] - the[j];
-            if (coulomb != 0) {
-                float C;
-                if (coulomb == 1) {
-                    int dummy = 0;
-                    Loc32 ca, cb;                                   // Coulomb-table coordinates of Theta_i, Theta_e
-                    if (MODE == 4 && T.coul_share_thi) ca = li; else ca = locate32<false>(T.cax[0], l_i, dummy);
-                    if (T.coul_share_the) cb = le; else cb = locate32<false>(T.cax[1], l_e, dummy);
-                    C = coulomb_C32(T.cax[1].n, X.coul, ca, cb);
-                } else {
-                    C = (D != 0.f && !bad[j]) ? (float)coolphys::coulomb_C((double)the[j], (double)thi[j] / X.K.units.ion_theta_mass_ratio) : 0.f;
-                }
-                const float raw = coul_kr[j] * C * fabsf(D);
-                const float cap1 = (D > 0.f) ? S.cap1i * thi[j] : S.cap1e * the[j];
-                const float mag = fminf(raw, fminf(cap1, fabsf(D) * S.eq_fracf));
-                dthe = copysignf(mag, D);
-            }
-            // explicit _rn intrinsics: never contracted, so every instantiation rounds identically
-            const float drad = __fmul_rn(rrad, the[j]);
-            const float the_n = __fadd_rn(__fsub_rn(the[j], drad), dthe);
-            const float thi_n = __fmaf_rn(-dthe, S.gi1_over_ge1, thi[j]);
-            if constexpr (DIAG) {
-                drad_last[j] = drad;
-                lsum[j][0] += drad; lsum[j][1] = fmaf(drad, fr[j][0], lsum[j][1]);
-                lsum[j][2] = fmaf(drad, fr[j][1], lsum[j][2]); lsum[j][3] = fmaf(drad, fr[j][2], lsum[j][3]);
-            }
-            changed |= (the_n != the[j]) | (thi_n != thi[j]);
-            the[j] = the_n; thi[j] = thi_n;
-        }
-        // exact early exit: a sub-step that leaves every temperature bit-identical repeats itself
-        if (!changed) {
-            if constexpr (DIAG) {
-                const float rem = (float)(S.nsub - 1 - s);
-#pragma unroll
-                for (int j = 0; j < NV; ++j) {
-                    lsum[j][0] = fmaf(rem, drad_last[j], lsum[j][0]);
-#pragma unroll
-                    for (int k = 0; k < 3; ++k) lsum[j][k + 1] = fmaf(rem, drad_last[j] * fr[j][k], lsum[j][k + 1]);
-                }
-            }
-            break;
-        }
-    }
-#pragma unroll
-    for (int j = 0; j < NV; ++j) {
-        if (bad[j]) {
-            const bool isn = nanv[j] != nanv[j];
-            the[j] = isn ? __int_as_float(0x7fc00000) : the0[j];
-            thi[j] = isn ? __int_as_float(0x7fc00000) : thi0[j];
-        }
-        if constexpr (DIAG) {
-            if (!bad[j]) {
-                const float wgt = rho[j] * vol[j];
-#pragma unroll
-                for (int k = 0; k < 4; ++k) acc.lum[k] += (double)(lsum[j][k] * wgt);
-                acc.lim += limited[j]; acc.flo += floored[j]; acc.cla += clamped[j];
-            }
-        }
-    }
-}
-
 // ------------------------------------------------------------------------------------------
 // Diagnostics reduction: warp shuffle -> block smem -> per-block partials -> the last block to
 // finish sums the partials in a fixed order (bit-reproducible for a given grid).
@@ -659,15 +387,10 @@ __device__ __forceinline__ void do_cells(const DevTable &T, const DevConst &K, c
             step_cell_analytic<MODE, DIAG>(T, K, S, (double)rho[j], (double)bsq[j], te, ti, (double)r[j], (double)vol[j], acc);
             the[j] = (Real)te; thi[j] = (Real)ti;
         }
-    } else if constexpr (sizeof(Real) == 8) {
+    } else {
+        static_assert(sizeof(Real) == 8, "fp32 table variants live in cool_f32.cuh");
 #pragma unroll
         for (int j = 0; j < NV; ++j) step_cell_f64<MODE, Fetch, DIAG>(T, K, S, F, rho[j], bsq[j], the[j], thi[j], r[j], vol[j], acc);
-    } else {
-        const Ctx32 X{T, K, S, coul};
-        constexpr int G = (MODE == 4) ? 1 : NV;       // cells advanced together (MODE 4: patch cache = 17 registers per cell)
-#pragma unroll
-        for (int j = 0; j < NV; j += G)
-            step_cells_f32<MODE, Fetch, DIAG, CM, G>(X, F, rho + j, bsq + j, the + j, thi + j, r + j, vol + j, acc);
     }
 }
 
@@ -681,14 +404,7 @@ cool_step_kernel(const DevTable T, const DevConst K, const StepConst S, const Ce
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const Fetch F(T, smem_raw);
     const float *coul = T.coul;
-    if constexpr (sizeof(Real) == 4 && !ANALYTIC) {
-        if (S.coul_smem) {
-            float *s_coul = (float *)(smem_raw + (Fetch::kSmem ? T.table_bytes : 0));
-            for (int k = threadIdx.x; k < (T.coul_bytes >> 2); k += THREADS) s_coul[k] = __ldg(T.coul + k);
-            coul = s_coul;
-        }
-    }
-    if (Fetch::kSmem || (sizeof(Real) == 4 && !ANALYTIC)) __syncthreads();
+    if (Fetch::kSmem) __syncthreads();
     using V = typename VecT<Real>::type;
     constexpr int N = VecT<Real>::N;
     DiagAcc acc;
@@ -726,7 +442,6 @@ struct LaunchCtx { const cool_table *t; const StepConst *S; const LaunchArgs *a;
 template <class Real, int MODE, class Fetch, bool ANALYTIC, bool DIAG, int CM, int THREADS, int MINB>
 static cudaError_t launch_one(const LaunchCtx &L, size_t smem)
 {
-    if (sizeof(Real) == 4 && !ANALYTIC && L.S->coul_smem) smem += (size_t)L.t->dev.coul_bytes;
     auto kern = cool_step_kernel<Real, MODE, Fetch, ANALYTIC, DIAG, CM, THREADS, MINB>;
     static int occ_cache = -1; static size_t occ_smem = ~(size_t)0;
     if (smem > 48 * 1024) {
@@ -751,8 +466,6 @@ static cudaError_t launch_one(const LaunchCtx &L, size_t smem)
 }
 
 // one function per translation unit of instantiations (cool_inst_*.cu)
-cudaError_t launch_f32_m3(const LaunchCtx &L, cool_variant v, bool diag, int cm);
-cudaError_t launch_f32_m4(const LaunchCtx &L, cool_variant v, bool diag, int cm);
 cudaError_t launch_f64(const LaunchCtx &L, int mode, cool_variant v, bool diag);
 cudaError_t launch_analytic(const LaunchCtx &L, int mode, cool_dtype dt, bool diag);
 

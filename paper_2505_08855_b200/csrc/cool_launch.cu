@@ -1,5 +1,5 @@
 // cool_launch.cu — per-launch constants and dispatch to the kernel instantiations.
-#include "cool_kernels.cuh"
+#include "cool_f32.cuh"
 
 namespace cool {
 
@@ -16,22 +16,37 @@ static StepConst make_step_const(const cool_table *t, cool_dtype dt, const Launc
     S.hfloor2 = (a.h_floor > 0.0 && a.r) ? 0.5 * coolphys::kPI * a.h_floor * a.h_floor : 0.0;
     S.spin = K.units.spin;
     S.lum_k = K.mr / (K.ge1 * a.dt);
-    const double L10 = 3.321928094887362;
-    S.L10h = (float)L10; S.L10l = (float)(L10 - (double)S.L10h);
-    S.ksm = (float)(log2(S.h) - K.log2_ue_k);
-    S.f_limitf = (float)a.f_limit; S.mrf = (float)K.mr; S.eq_fracf = (float)S.eq_frac;
-    S.ge1_over_gi1 = (float)(K.ge1 / K.gi1); S.gi1_over_ge1 = (float)(K.gi1 / K.ge1);
-    S.coul_khf = (float)S.coul_kh;
-    S.cap1e = (float)a.f_limit; S.cap1i = (float)(a.f_limit * K.ge1 / K.gi1);
-    S.aef = (float)S.ae; S.aif = (float)S.ai; S.bef = (float)S.be; S.bif = (float)S.bi;
-    S.inv_kB = (float)(K.der.h_per_cs * K.mr / (K.bb_k * S.h * K.ge1));
-    S.kscaf = (float)(K.tausca_k * K.der.h_per_cs);
-    S.hfloor2f = (float)S.hfloor2; S.spinf = (float)S.spin;
     S.nsub = a.nsub; S.coulomb = a.coulomb;
     S.has_r = a.r != nullptr; S.has_vol = a.vol != nullptr;
     auto ok = [&](const void *p) { return p == nullptr || ((size_t)p % 16) == 0; };
     S.aligned = ok(a.rho) && ok(a.bsq) && ok(a.the_in) && ok(a.thi_in) && ok(a.the_out) && ok(a.thi_out) && ok(a.r) && ok(a.vol);
-    S.coul_smem = dt == COOL_F32 && a.coulomb == 1 && t->dev.coul && t->dev.coul_bytes <= kCoulSmemMax;
+    return S;
+}
+
+static F32Const make_f32_const(const cool_table *t, const LaunchArgs &a)
+{
+    const DevConst &K = t->cst;
+    F32Const S{};
+    const double h = a.dt / a.nsub;
+    S.k0 = (float)log2(h);
+    S.f_limit = (float)a.f_limit; S.mr = (float)K.mr; S.eq_frac = (float)(K.ge1 / (K.ge1 + K.gi1));
+    S.gi1_over_ge1 = (float)(K.gi1 / K.ge1);
+    S.coul_kh = (float)(K.coul_k * h * K.ge1);
+    S.cap1e = (float)a.f_limit; S.cap1i = (float)(a.f_limit * K.ge1 / K.gi1);
+    S.ae = (float)(K.units.gamma_e * K.mr); S.ai = (float)(K.units.gamma_i * K.mr);
+    S.be = (float)(K.mr * K.units.gamma_e / K.ge1); S.bi = (float)(K.mr * K.units.gamma_i / K.gi1);
+    S.inv_kB = (float)(K.der.h_per_cs * K.mr / (K.bb_k * h * K.ge1));
+    S.ksca = (float)(K.tausca_k * K.der.h_per_cs);
+    S.hfloor2 = (float)((a.h_floor > 0.0 && a.r) ? 0.5 * coolphys::kPI * a.h_floor * a.h_floor : 0.0);
+    S.spin = (float)K.units.spin;
+    S.lum_k = K.mr / (K.ge1 * a.dt);
+    S.ion_ratio = K.units.ion_theta_mass_ratio;
+    S.nsub = a.nsub; S.coulomb = a.coulomb;
+    S.has_r = a.r != nullptr; S.has_vol = a.vol != nullptr;
+    S.nf = 4 + S.has_r + S.has_vol;
+    auto ok = [&](const void *p) { return p == nullptr || ((size_t)p % 16) == 0; };
+    S.use_tma = ok(a.rho) && ok(a.bsq) && ok(a.the_in) && ok(a.thi_in) && ok(a.the_out) && ok(a.thi_out) && ok(a.r) && ok(a.vol);
+    S.coul_smem = a.coulomb == 1 && t->dev.fcoul && t->dev.coul_bytes <= kCoulSmemMax && !(t->dev.mode == 4 && t->dev.f4_has_coul);
     return S;
 }
 
@@ -39,7 +54,8 @@ bool variant_supported(const cool_table *t, cool_variant v, cool_dtype, std::str
 {
     if (v == COOL_V_ANALYTIC) return true;
     if (t->dev.mode == 0) { if (why) *why = "table has no data (nproc = 0): only COOL_V_ANALYTIC applies"; return false; }
-    if (v == COOL_V_SMEM && (size_t)t->dev.table_bytes + kCoulSmemMax + 8192 > (size_t)t->max_smem_optin) {
+    // SMEM variant: table image + two 6-array cell stages of the 512-thread kernel + Coulomb table + barriers
+    if (v == COOL_V_SMEM && (size_t)t->dev.table_bytes + kCoulSmemMax + 2 * 6 * (size_t)kF32SmemThreads * kF32CellsPerThread * 4 + 1024 > (size_t)t->max_smem_optin) {
         if (why) *why = "table does not fit in shared memory"; return false;
     }
     return true;
@@ -55,8 +71,10 @@ cool_status launch_step(const cool_table *t, cool_variant v, cool_dtype dt, cons
     if (v == COOL_V_ANALYTIC) e = launch_analytic(L, mode, dt, diag);
     else if (dt == COOL_F64) e = launch_f64(L, mode, v, diag);
     else {
-        const int cm = (a.coulomb == 1) ? 1 : 0;          // fast path: Coulomb from the coefficient table
-        e = (mode == 3) ? launch_f32_m3(L, v, diag, cm) : launch_f32_m4(L, v, diag, cm);
+        const LaunchCtx32 L32{t, make_f32_const(t, a), &a, st};
+        // fast path: Coulomb from the coefficient table staged in shared memory (or riding in the 4-D texels)
+        const int cm = (a.coulomb == 1 && (L32.S.coul_smem || (mode == 4 && t->dev.f4_has_coul))) ? 1 : 0;
+        e = (mode == 3) ? launch_f32_m3(L32, v, diag, cm, a.nsub == 1) : launch_f32_m4(L32, v, diag, cm);
     }
     if (e != cudaSuccess) { set_error("kernel launch failed: %s", cudaGetErrorString(e)); return COOL_ECUDA; }
     if (nlaunch) *nlaunch += 1;
