@@ -41,7 +41,8 @@ def _compile(src: str, verbose: bool) -> str:
     src_p = os.path.join(CSRC, src)
     if os.path.exists(obj) and os.path.getmtime(obj) > max(hdr_t, os.path.getmtime(src_p), os.path.getmtime(os.path.abspath(__file__))):
         return obj
-    cmd = [_nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-c", src_p, "-o", obj]
+    extra = os.environ.get("COOL_NVCC_EXTRA", "").split()          # e.g. -DCOOL_SOMETHING=1 for experiments
+    cmd = [_nvcc()] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-c", src_p, "-o", obj]
     r = subprocess.run(cmd, capture_output=True, text=True)
     if verbose or r.returncode != 0:
         sys.stderr.write(r.stdout + r.stderr)

@@ -4,6 +4,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 
@@ -56,6 +57,7 @@ static AxisCoef make_axis(int n, double lo, double hi)
     a.tmaxf = nextafterf(a.nm1f, 0.f);
     a.ke = (float)(8388608.0 + 127.0 + e0);
     a.d2f = (float)(delta * L10);
+    a.c2f = (float)(-lo2 * inv2);
     return a;
 }
 
@@ -99,6 +101,8 @@ static void free_table(cool_table *t)
     if (t->d_f32) cudaFree(t->d_f32);
     if (t->d_coul) cudaFree(t->d_coul);
     if (t->d_fcoul) cudaFree(t->d_fcoul);
+    if (t->d_fcoulq) cudaFree(t->d_fcoulq);
+    if (t->d_q3) cudaFree(t->d_q3);
     for (auto &kv : t->diag_ws) { cudaFree(kv.second.partials); cudaFree(kv.second.ticket); }
     for (auto &s : t->stages) {
         for (void *b : s.buf) if (b) cudaFree(b);
@@ -289,6 +293,33 @@ extern "C" cool_status cool_table_create(const cool_table_desc *desc, int device
         if (e != cudaSuccess) { set_error("fp32 table upload: %s", cudaGetErrorString(e)); return fail(e == cudaErrorMemoryAllocation ? COOL_ENOMEM : COOL_ECUDA); }
         if (nd == 3) D.f1 = t->d_f32; else D.f4 = (const float4 *)t->d_f32;
 
+        // MODE 3 quad layout (4x the bytes): one float4 holds the four (Theta_e, bsq) corners of a table cell.
+        // Built while it stays L2-resident (default limit 64 MiB; COOL_QUAD_MAX_MB overrides, 0 disables).
+        if (nd == 3) {
+            size_t quad_max = (size_t)64 << 20;
+            if (const char *ev = getenv("COOL_QUAD_MAX_MB")) quad_max = (size_t)atoll(ev) << 20;
+            const size_t qbytes = (size_t)total * 4 * sizeof(float);
+            if (qbytes <= quad_max) {
+                std::vector<float> quad;
+                try { quad.resize((size_t)total * 4); } catch (...) { set_error("out of host memory"); return fail(COOL_ENOMEM); }
+                const int nr = ncan[CAX_RHO], ne = ncan[CAX_THE], nb = ncan[CAX_BSQ];
+                for (int ir = 0; ir < nr; ++ir)
+                    for (int ie = 0; ie < ne; ++ie) {
+                        const int ie1 = std::min(ie + 1, ne - 1);
+                        const float *row0 = &canon32[((size_t)ir * ne + ie) * nb], *row1 = &canon32[((size_t)ir * ne + ie1) * nb];
+                        float *q = &quad[((size_t)ir * ne + ie) * nb * 4];
+                        for (int ib = 0; ib < nb; ++ib) {
+                            const int ib1 = std::min(ib + 1, nb - 1);
+                            q[4 * ib + 0] = row0[ib]; q[4 * ib + 1] = row0[ib1]; q[4 * ib + 2] = row1[ib]; q[4 * ib + 3] = row1[ib1];
+                        }
+                    }
+                e = cudaMalloc(&t->d_q3, qbytes);
+                if (e == cudaSuccess) e = cudaMemcpy(t->d_q3, quad.data(), qbytes, cudaMemcpyHostToDevice);
+                if (e != cudaSuccess) { set_error("quad table upload: %s", cudaGetErrorString(e)); return fail(e == cudaErrorMemoryAllocation ? COOL_ENOMEM : COOL_ECUDA); }
+                D.q3 = (const float4 *)t->d_q3;
+            }
+        }
+
         // cudaArray + texture objects (x = bsq, y = theta_e | theta_i, z = rho | rho*n_the + i_the)
         const size_t ex = ncan[CAX_BSQ];
         const size_t ey = nd == 3 ? ncan[CAX_THE] : ncan[CAX_THI];
@@ -307,13 +338,25 @@ extern "C" cool_status cool_table_create(const cool_table_desc *desc, int device
         if (e == cudaSuccess) e = cudaMemcpy(t->d_coul, desc->host_coulomb, n * sizeof(float), cudaMemcpyHostToDevice);
         if (e != cudaSuccess) { set_error("Coulomb table upload: %s", cudaGetErrorString(e)); return fail(e == cudaErrorMemoryAllocation ? COOL_ENOMEM : COOL_ECUDA); }
         D.coul = t->d_coul;
-        {   // fp32 path: log2 C
-            std::vector<float> c2(n);
+        {   // fp32 path: log2 C, plain (padded to 16 B) and as quads {C(i,e), C(i,e+1), C(i+1,e), C(i+1,e+1)}
+            const size_t npad = (n + 3) & ~(size_t)3;
+            std::vector<float> c2(npad, 0.f), cq(n * 4);
             for (size_t k = 0; k < n; ++k) c2[k] = (float)(3.321928094887362 * (double)desc->host_coulomb[k]);
-            e = cudaMalloc(&t->d_fcoul, n * sizeof(float));
-            if (e == cudaSuccess) e = cudaMemcpy(t->d_fcoul, c2.data(), n * sizeof(float), cudaMemcpyHostToDevice);
+            const int n0 = desc->nc[0], n1 = desc->nc[1];
+            for (int i = 0; i < n0; ++i)
+                for (int j = 0; j < n1; ++j) {
+                    const int i1 = std::min(i + 1, n0 - 1), j1 = std::min(j + 1, n1 - 1);
+                    float *q = &cq[((size_t)i * n1 + j) * 4];
+                    q[0] = c2[(size_t)i * n1 + j]; q[1] = c2[(size_t)i * n1 + j1]; q[2] = c2[(size_t)i1 * n1 + j]; q[3] = c2[(size_t)i1 * n1 + j1];
+                }
+            e = cudaMalloc(&t->d_fcoul, npad * sizeof(float));
+            if (e == cudaSuccess) e = cudaMemcpy(t->d_fcoul, c2.data(), npad * sizeof(float), cudaMemcpyHostToDevice);
+            if (e == cudaSuccess) e = cudaMalloc(&t->d_fcoulq, cq.size() * sizeof(float));
+            if (e == cudaSuccess) e = cudaMemcpy(t->d_fcoulq, cq.data(), cq.size() * sizeof(float), cudaMemcpyHostToDevice);
             if (e != cudaSuccess) { set_error("Coulomb table upload: %s", cudaGetErrorString(e)); return fail(e == cudaErrorMemoryAllocation ? COOL_ENOMEM : COOL_ECUDA); }
             D.fcoul = t->d_fcoul;
+            D.fcoulq = (const float4 *)t->d_fcoulq;
+            D.coulq_bytes = (int)(cq.size() * sizeof(float));
         }
         D.cax[0] = make_axis(desc->nc[0], desc->clo[0], desc->chi[0]);
         D.cax[1] = make_axis(desc->nc[1], desc->clo[1], desc->chi[1]);

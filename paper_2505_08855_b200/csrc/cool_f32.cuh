@@ -1,21 +1,28 @@
 // cool_f32.cuh — the fp32 kernels of the cooling step (include/cool.h), written for sm_100a.
 //
-// Structure of one launch (persistent CTAs, one tile = THREADS*4 consecutive cells):
-//   * cell tiles (rho, bsq, Theta_e, Theta_i [, vol, r]) are staged into shared memory by 1-D TMA
-//     bulk copies (cp.async.bulk + mbarrier), double buffered, so HBM latency never sits on a
-//     warp's scoreboard; outputs leave as 128-bit streaming stores;
-//   * the table is read through one of four lookup policies (L1/L2-resident global gathers,
-//     shared-memory image, point texture, hardware-filtered texture);
+// Structure of one launch (one persistent CTA per SM; every WARP runs its own pipeline):
+//   * a warp tile = 128 consecutive cells (4 per lane).  The cell arrays of a tile (rho, bsq,
+//     Theta_e, Theta_i [, vol, r]) are staged into the warp's own shared-memory stages by 1-D TMA
+//     bulk copies (cp.async.bulk + one mbarrier per stage, NST stages deep), so HBM latency never
+//     sits on a warp's scoreboard and no CTA-wide barrier exists after the prologue; outputs leave
+//     as 128-bit streaming stores;
+//   * the table is read through one of five lookup policies: L1/L2-resident global gathers from
+//     the plain layout or from the quad layout (one float4 = the four (Theta_e, bsq) corners of a
+//     table cell: 2 LDG.128 instead of 8 LDG.32 per trilinear lookup, 2 instead of up to 8 sectors
+//     per cell from L2), shared-memory image, point texture, hardware-filtered texture;
+//   * the Coulomb coefficient table sits in shared memory, in the same quad layout (1 LDS.128);
 //   * the luminosity diagnostic is reduced warp -> block -> fixed-order last-block pass.
 // The step is a gather plus scalar arithmetic: no tensor cores.  On B200 it
-// is bound by instruction issue and the L1 data pipe, not by HBM, so the arithmetic is written to
-// minimise instructions:
+// is bound by the L1 data pipe and instruction issue, not by HBM, so the code is written to
+// minimise L1 wavefronts and instructions:
 //   * the table nodes are stored as T' = log2(rate / u_e at the node) (cool_internal.h), so that
 //     Lambda h / u_e = 2^(interp(T') + log2 h + clamp correction): no large-number cancellation, no
 //     compensated products;
 //   * log2 of a primitive is (exponent, log2 mantissa) folded straight into the node coordinate;
 //   * floor() is a round-down add of 1.5*2^23 whose mantissa bits are the node index, and the
 //     bias is folded into the address constant (no F2I/I2F, no masking);
+//   * the Coulomb table's coordinates are an affine map of the table's own node coordinates
+//     (one FMA instead of a second logarithm);
 //   * MODE 4: the (rho, bsq) contraction of the 16 corners is loop invariant over sub-steps, so a
 //     bilinear patch in (w_e, w_i) is cached per visited (i_e, i_i) table cell — 3 FMAs per channel
 //     per sub-step — and the Coulomb coefficient rides in the 4th texel channel;
@@ -35,8 +42,10 @@ struct F32Const {
     float hfloor2, spin;              // floor: (pi/2) h_floor^2 (Omega_K r)^2                          (eq 19)
     double lum_k;                     // lum = sum(dTheta_rad rho vol) * lum_k
     double ion_ratio;                 // theta_i of eq 15 = Theta_i / ion_ratio (analytic Coulomb only)
+    float cme_s, cme_o, cmi_s, cmi_o; // Coulomb-table node coordinate = table node coordinate * s + o (Theta_e; Theta_i in MODE 4)
     int nsub, coulomb, has_r, has_vol, use_tma, coul_smem, nf;
-    unsigned stage_bytes, coul_off, table_off;     // dynamic shared memory layout
+    unsigned wstage_bytes;            // bytes of one warp stage = nf * 512
+    unsigned stage_off, coul_off, table_off;       // dynamic shared memory layout
 };
 
 // ------------------------------------------------------------------------------------------
@@ -61,6 +70,13 @@ __device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity)
     asm volatile("{\n\t.reg .pred p;\n"
                  "COOL_WAIT:\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t@p bra COOL_DONE;\n\tbra COOL_WAIT;\n"
                  "COOL_DONE:\n\t}" ::"r"(bar), "r"(parity) : "memory");
+}
+// one elected lane of a converged warp (ptxas then keeps the TMA operands on the uniform datapath without a per-copy election loop)
+__device__ __forceinline__ bool elect_one()
+{
+    unsigned r;
+    asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(r));
+    return r != 0;
 }
 __device__ __forceinline__ float lg2_approx(float x)
 {
@@ -105,21 +121,25 @@ __device__ __forceinline__ float rsqrt_approx(float x)
 
 // ------------------------------------------------------------------------------------------
 // Node coordinate of a primitive along one table axis.
-//   tf : t_clamped + 1.5*2^23 rounded down; its bit pattern is 0x4B400000 + floor(t)
-//   fi : floor(t) as a float,  w = t_clamped - floor(t) in [0,1)
-//   d  : t_clamped - t (0 inside the table): the clamp correction of the T' form is d * d2f
+//   coord32 : t = (log2 q - lo)/Delta in node units, unclamped
+//   split32 : tf = t_clamped + 1.5*2^23 rounded down (bit pattern 0x4B400000 + floor(t)),
+//             fi = floor(t) as a float, w = t_clamped - floor(t) in [0,1),
+//             d  = t_clamped - t (0 inside the table): the clamp correction of the T' form is d * d2f
 // ------------------------------------------------------------------------------------------
 constexpr float kMagic = 12582912.0f;              // 1.5 * 2^23
 constexpr unsigned kMagicBits = 0x4B400000u;
 struct Loc32 { float tf, fi, w, d; };
-template <bool DIAG>
-__device__ __forceinline__ Loc32 locate32(const AxisCoef &a, float q, int &clamped, int one_bits)
+__device__ __forceinline__ float coord32(const AxisCoef &a, float q, int one_bits)
 {
     // non-positive (and negative-NaN) -> bits 0 -> exponent -127: below every table (lower-edge clamp)
     const int b = max(__float_as_int(q), 0);
     const float u = __int_as_float((b >> 23) | 0x4B000000);                     // 2^23 + biased exponent, exact
     const float lm = lg2_approx(__int_as_float(and_or(b, 0x007fffff, one_bits)));   // MUFU.LG2 on [1,2): abs err 2^-22
-    const float t = fmaf(u - a.ke, a.invf, fmaf(lm, a.invf, a.cf));
+    return fmaf(u - a.ke, a.invf, fmaf(lm, a.invf, a.cf));
+}
+template <bool DIAG>
+__device__ __forceinline__ Loc32 split32(const AxisCoef &a, float t, int &clamped)
+{
     if constexpr (DIAG) clamped |= (t < 0.f) | (t > a.nm1f);
     const float tc = fminf(fmaxf(t, 0.f), a.tmaxf);
     Loc32 L;
@@ -129,11 +149,36 @@ __device__ __forceinline__ Loc32 locate32(const AxisCoef &a, float q, int &clamp
     L.d = tc - t;
     return L;
 }
+template <bool DIAG>
+__device__ __forceinline__ Loc32 locate32(const AxisCoef &a, float q, int &clamped, int one_bits)
+{
+    return split32<DIAG>(a, coord32(a, q, one_bits), clamped);
+}
 __device__ __forceinline__ int loc_bits(const Loc32 &l) { return __float_as_int(l.tf); }
 __device__ __forceinline__ float lerp(float w, float a, float b) { return fmaf(w, b - a, a); }
 
+__device__ __forceinline__ float4 ldg_f4(const float4 *p)
+{
+    float4 v;
+    asm("ld.global.nc.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ float4 lds_f4(unsigned addr)
+{
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ float lds_f32(unsigned addr)
+{
+    float v;
+    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(addr));
+    return v;
+}
+
 // ------------------------------------------------------------------------------------------
-// Lookup policies over the T' tables.
+// Lookup policies over the T' tables.  corners3 returns c[cr*4 + ce*2 + cb]; every policy feeds the
+// same interpolation code, so the software variants agree bit for bit.
 // ------------------------------------------------------------------------------------------
 struct F32Global {
     static constexpr bool kHw = false, kSmem = false;
@@ -143,7 +188,6 @@ struct F32Global {
         c3 = (int)(0u - kMagicBits * (unsigned)(sr + se + 1));            // removes the bias of the three index words
         c4 = (int)(0u - kMagicBits * (unsigned)(sr + se + si + 1));
     }
-    // c[cr*4 + ce*2 + cb]
     __device__ __forceinline__ void corners3(const Loc32 &r, const Loc32 &e, const Loc32 &b, float (&c)[8]) const
     {
         const int off = loc_bits(r) * sr + (loc_bits(e) * se + (loc_bits(b) + c3));
@@ -161,9 +205,26 @@ struct F32Global {
             for (int ci = 0; ci < 2; ++ci) {
                 const int o = off + (ce ? se : 0) + (ci ? si : 0);
                 const float4 *a = elem_addr(p4, o), *u = elem_addr(p4, o + sr);
-                q[ce][ci][0] = __ldg(a); q[ce][ci][1] = __ldg(a + 1); q[ce][ci][2] = __ldg(u); q[ce][ci][3] = __ldg(u + 1);
+                q[ce][ci][0] = ldg_f4(a); q[ce][ci][1] = ldg_f4(a + 1); q[ce][ci][2] = ldg_f4(u); q[ce][ci][3] = ldg_f4(u + 1);
             }
     }
+};
+// MODE 3 quad layout: q3[r][e][b] = {T'(r,e,b), T'(r,e,b+1), T'(r,e+1,b), T'(r,e+1,b+1)} (same strides as the plain
+// layout): a trilinear lookup is two 128-bit gathers, each inside one 32-byte sector.
+struct F32GlobalQ {
+    static constexpr bool kHw = false, kSmem = false;
+    const float4 *pq; int sr, se, c3;
+    __device__ F32GlobalQ(const DevTable &T, const void *) : pq(T.q3), sr(T.s_rho), se(T.s_the)
+    {
+        c3 = (int)(0u - kMagicBits * (unsigned)(sr + se + 1));
+    }
+    __device__ __forceinline__ void corners3(const Loc32 &r, const Loc32 &e, const Loc32 &b, float (&c)[8]) const
+    {
+        const int off = loc_bits(r) * sr + (loc_bits(e) * se + (loc_bits(b) + c3));
+        const float4 lo = ldg_f4(elem_addr(pq, off)), hi = ldg_f4(elem_addr(pq, off + sr));
+        c[0] = lo.x; c[1] = lo.y; c[2] = lo.z; c[3] = lo.w; c[4] = hi.x; c[5] = hi.y; c[6] = hi.z; c[7] = hi.w;
+    }
+    __device__ __forceinline__ void corners4(const Loc32 &, const Loc32 &, const Loc32 &, const Loc32 &, float4 (&)[2][2][4]) const {}
 };
 struct F32Smem {
     static constexpr bool kHw = false, kSmem = true;
@@ -297,20 +358,19 @@ __device__ __forceinline__ float patch_eval(const Patch4 &P, int k, float we, fl
     return fmaf(we, fmaf(wi, P.c[k][3], P.c[k][1]), fmaf(wi, P.c[k][2], P.c[k][0]));
 }
 
-// Coulomb coefficient C = 2^(bilinear log2 C).  SMEM: `cs` is a shared-memory window address
-// (LDS, no generic loads); otherwise the table is read from global memory.
-__device__ __forceinline__ float lds_f32(unsigned addr)
-{
-    float v;
-    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(addr));
-    return v;
-}
-template <bool SMEM>
+// Coulomb coefficient C = 2^(bilinear log2 C) at (a = Theta_i, b = Theta_e) node coordinates.
+//   CM = 1, QUAD  : quad layout {C(i,e), C(i,e+1), C(i+1,e), C(i+1,e+1)} staged in shared memory, one LDS.128;
+//   CM = 1, !QUAD : plain layout staged in shared memory (SMEM variant: the table image leaves no room for quads);
+//   CM = 0        : plain layout in global memory (L1-resident).
+template <int CM, bool QUAD>
 __device__ __forceinline__ float coulomb_C32(int n1, const float *cg, unsigned cs, const Loc32 &a, const Loc32 &b)
 {
     const int off = loc_bits(a) * n1 + (loc_bits(b) + (int)(0u - kMagicBits * (unsigned)(n1 + 1)));
     float c00, c01, c10, c11;
-    if constexpr (SMEM) {
+    if constexpr (CM == 1 && QUAD) {
+        const float4 q = lds_f4(cs + 16u * (unsigned)off);
+        c00 = q.x; c01 = q.y; c10 = q.z; c11 = q.w;
+    } else if constexpr (CM == 1) {
         const unsigned p = cs + 4u * (unsigned)off, q = p + 4u * (unsigned)n1;
         c00 = lds_f32(p); c01 = lds_f32(p + 4); c10 = lds_f32(q); c11 = lds_f32(q + 4);
     } else {
@@ -320,12 +380,15 @@ __device__ __forceinline__ float coulomb_C32(int n1, const float *cg, unsigned c
     return ex2_approx(lerp(a.w, lerp(b.w, c00, c01), lerp(b.w, c10, c11)));
 }
 
-struct Ctx32 { const DevTable &T; const F32Const &S; unsigned coul_s; };      // coul_s: shared-memory address of the staged log2 C table
+struct Ctx32 { const DevTable &T; const F32Const &S; unsigned coul_s; };      // coul_s: shared-memory address of the staged Coulomb quads
 
 // ------------------------------------------------------------------------------------------
 // NV cells of one thread through all sub-steps, straight-line (no per-cell branches except the
 // MODE-4 patch rebuild), so the compiler interleaves them for ILP.
-//   CM: 1 = Coulomb from the coefficient table (fast path), 0 = runtime S.coulomb (off / table / analytic)
+//   CM: 1 = Coulomb from the coefficient table (shared-memory quads, or the 4th texel channel in
+//           MODE 4), 0 = runtime S.coulomb (off / table in global memory / analytic)
+// Cells with rho <= 0 pass through and cells with a NaN input give NaN (that cell only): they
+// run through the arithmetic like any other cell and are patched at the end.
 // ------------------------------------------------------------------------------------------
 template <int MODE, class Fetch, bool DIAG, int CM, bool NSUB1, int NV>
 __device__ __forceinline__ void step_cells_f32(const Ctx32 &X, const Fetch &F, const float *rho, const float *bsq, float *the, float *thi,
@@ -335,18 +398,19 @@ __device__ __forceinline__ void step_cells_f32(const Ctx32 &X, const Fetch &F, c
     const int coulomb = (CM == 1) ? 1 : S.coulomb;
     const int one_bits = opaque_const(0x3f800000);
     const bool use_floor = S.hfloor2 > 0.f;                 // warp-uniform
-    bool bad[NV]; float fb_e[NV], fb_i[NV];
+    bool bad[NV], any_bad = false;
+    float in_e[NV], in_i[NV], nanq[NV];
     Loc32 lr[NV], lb[NV];
     float kcell[NV], coul_kr[NV], tfloor[NV], lsum[NV][4];
     int clamped[NV], limited[NV], floored[NV];
     Patch4 P[(MODE == 4 && !Fetch::kHw) ? NV : 1];
 #pragma unroll
     for (int j = 0; j < NV; ++j) {
-        // rho <= 0: pass through; any NaN: NaN out (that cell only) — resolved by one select per output
-        const float chk = (rho[j] + bsq[j]) + (the[j] + thi[j]);
-        const float z = __fsub_rn(chk, chk);                      // 0, or NaN when any input is NaN (or the sum overflows)
-        bad[j] = !(rho[j] > 0.f) || z != 0.f;
-        fb_e[j] = the[j] + z; fb_i[j] = thi[j] + z;
+        const float chk = (bsq[j] + the[j]) + (thi[j] + rho[j]);      // NaN when any input is NaN (or the sum overflows)
+        nanq[j] = chk;
+        bad[j] = !(rho[j] > 0.f) || chk != chk;
+        any_bad |= bad[j];
+        in_e[j] = the[j]; in_i[j] = thi[j];
         clamped[j] = limited[j] = floored[j] = 0;
         lr[j] = locate32<DIAG>(T.ax[CAX_RHO], rho[j], clamped[j], one_bits);
         lb[j] = locate32<DIAG>(T.ax[CAX_BSQ], bsq[j], clamped[j], one_bits);
@@ -371,15 +435,17 @@ __device__ __forceinline__ void step_cells_f32(const Ctx32 &X, const Fetch &F, c
         float drad_last[NV], fr[NV][3];
 #pragma unroll
         for (int j = 0; j < NV; ++j) {
-            const Loc32 le = locate32<DIAG>(T.ax[CAX_THE], the[j], clamped[j], one_bits);
+            const float te = coord32(T.ax[CAX_THE], the[j], one_bits);
+            const Loc32 le = split32<DIAG>(T.ax[CAX_THE], te, clamped[j]);
             const float kk = fmaf(le.d, T.ax[CAX_THE].d2f, kcell[j]);
-            float rrad, yc = 0.f;
+            float rrad, yc = 0.f, ti = 0.f;
             fr[j][0] = fr[j][1] = fr[j][2] = 0.f;
             Loc32 li{0.f, 0.f, 0.f, 0.f};
             if constexpr (MODE == 3) {
                 rrad = ex2_approx(interp3_f32(F, lr[j], le, lb[j]) + kk);
             } else {
-                li = locate32<DIAG>(T.ax[CAX_THI], thi[j], clamped[j], one_bits);
+                ti = coord32(T.ax[CAX_THI], thi[j], one_bits);
+                li = split32<DIAG>(T.ax[CAX_THI], ti, clamped[j]);
                 float y0, y1, y2;
                 if constexpr (Fetch::kHw) {
                     const float4 v = F.hw4(lr[j], le, li, lb[j]);
@@ -422,10 +488,11 @@ __device__ __forceinline__ void step_cells_f32(const Ctx32 &X, const Fetch &F, c
                     } else {
                         int dummy = 0;
                         Loc32 ca, cb;                                   // Coulomb-table coordinates of Theta_i, Theta_e
-                        if (MODE == 4 && T.coul_share_thi) ca = li; else ca = locate32<false>(T.cax[0], thi[j], dummy, one_bits);
-                        if (T.coul_share_the) cb = le; else cb = locate32<false>(T.cax[1], the[j], dummy, one_bits);
-                        // CM = 1 is only launched with the table staged in shared memory
-                        C = (CM == 1) ? coulomb_C32<true>(T.cax[1].n, T.fcoul, X.coul_s, ca, cb) : coulomb_C32<false>(T.cax[1].n, T.fcoul, 0u, ca, cb);
+                        // branch-free (identical axes give s = 1, o = 0 and the same node coordinate): keeps the NV cells interleaved
+                        if (MODE == 4) ca = split32<false>(T.cax[0], fmaf(ti, S.cmi_s, S.cmi_o), dummy);
+                        else ca = locate32<false>(T.cax[0], thi[j], dummy, one_bits);
+                        cb = split32<false>(T.cax[1], fmaf(te, S.cme_s, S.cme_o), dummy);
+                        C = coulomb_C32<CM, !Fetch::kSmem>(T.cax[1].n, T.fcoul, X.coul_s, ca, cb);
                     }
                 } else {
                     C = (D != 0.f && !bad[j]) ? (float)coolphys::coulomb_C((double)the[j], (double)thi[j] / S.ion_ratio) : 0.f;
@@ -463,126 +530,142 @@ __device__ __forceinline__ void step_cells_f32(const Ctx32 &X, const Fetch &F, c
             }
         }
     }
+    if (any_bad) {                       // rare: rho <= 0 passes through, NaN inputs give NaN
 #pragma unroll
-    for (int j = 0; j < NV; ++j) {
-        if (bad[j]) { the[j] = fb_e[j]; thi[j] = fb_i[j]; }
-        if constexpr (DIAG) {
+        for (int j = 0; j < NV; ++j)
+            if (bad[j]) {
+                const float z = __fsub_rn(nanq[j], nanq[j]);          // 0, or NaN
+                the[j] = in_e[j] + z; thi[j] = in_i[j] + z;
+            }
+    }
+    if constexpr (DIAG) {
+#pragma unroll
+        for (int j = 0; j < NV; ++j)
             if (!bad[j]) {
                 const float wgt = rho[j] * vol[j];
 #pragma unroll
                 for (int k = 0; k < 4; ++k) acc.lum[k] += (double)(lsum[j][k] * wgt);
                 acc.lim += limited[j]; acc.flo += floored[j]; acc.cla += clamped[j];
             }
-        }
     }
 }
 
 // ------------------------------------------------------------------------------------------
-// The kernel.  Dynamic shared memory: [2 mbarriers | 2 stages x nf arrays x TILE floats |
-// Coulomb table (when small) | table image (SMEM variant)].
+// The kernel.  Dynamic shared memory:
+//   [NW*NST mbarriers | NW warps x NST stages x nf arrays x 128 floats | Coulomb quads | table image (SMEM variant)]
 // ------------------------------------------------------------------------------------------
 constexpr int kF32CellsPerThread = 4;
-constexpr unsigned kF32BarBytes = 16;
+constexpr int kWarpTile = 32 * kF32CellsPerThread;          // cells per warp tile
+constexpr unsigned kWarpArrBytes = kWarpTile * 4u;          // 512 B per array per stage
+constexpr unsigned kF32BarBytes = 512;                      // room for 16 warps x 4 stages of 8-byte mbarriers
 
-template <int MODE, class Fetch, bool DIAG, int CM, bool NSUB1, int THREADS, int MINB>
-__global__ void __launch_bounds__(THREADS, MINB)
+template <int MODE, class Fetch, bool DIAG, int CM, bool NSUB1, int THREADS, int NST>
+__global__ void __launch_bounds__(THREADS, 1)
 cool_f32_kernel(const DevTable T, const F32Const S, const CellPtrs C, double *partials, unsigned *ticket, cool_diag *d_diag)
 {
-    constexpr int TILE = THREADS * kF32CellsPerThread;
+    constexpr int NW = THREADS / 32;
     constexpr int G = (MODE == 4) ? 1 : kF32CellsPerThread;      // cells advanced together (MODE 4: the patch is 16 registers per cell)
+    static_assert(NW * NST * 8 <= (int)kF32BarBytes, "mbarrier area too small");
     extern __shared__ __align__(128) unsigned char smem_f32[];
-    const unsigned bar0 = smem_u32(smem_f32), bar1 = bar0 + 8;
-    float *stages = (float *)(smem_f32 + kF32BarBytes);
-    const unsigned stage_u32 = smem_u32(stages);
-    const int tid = threadIdx.x;
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);           // warp-uniform by construction: TMA operands stay in uniform registers
 
+    // ---- prologue (the only CTA-wide barrier): stage the Coulomb quads / table image, arm the warp's barriers
     if (CM == 1 && S.coul_smem) {
-        float *s_coul = (float *)(smem_f32 + S.coul_off);
-        for (int k = tid; k < (T.coul_bytes >> 2); k += THREADS) s_coul[k] = __ldg(T.fcoul + k);
+        float4 *dst = (float4 *)(smem_f32 + S.coul_off);
+        const float4 *src = Fetch::kSmem ? (const float4 *)T.fcoul : T.fcoulq;     // plain table padded to 16 B at create time
+        const unsigned n16 = (unsigned)(Fetch::kSmem ? ((T.coul_bytes + 15) >> 4) : (T.coulq_bytes >> 4));
+        for (unsigned k = tid; k < n16; k += THREADS) dst[k] = ldg_f4(src + k);
     }
     if constexpr (Fetch::kSmem) {
         const float4 *src = MODE == 3 ? (const float4 *)T.f1 : T.f4;
         float4 *dst = (float4 *)(smem_f32 + S.table_off);
         const unsigned n16 = T.table_bytes >> 4;                  // table_bytes is padded to 16 B at create time
-        for (unsigned k = tid; k < n16; k += THREADS) dst[k] = __ldg(src + k);
+        for (unsigned k = tid; k < n16; k += THREADS) dst[k] = ldg_f4(src + k);
     }
+    const unsigned bar_w = smem_u32(smem_f32) + (unsigned)(warp * NST) * 8u;              // this warp's mbarriers
+    const unsigned stg_w = smem_u32(smem_f32 + S.stage_off) + (unsigned)(warp * NST) * S.wstage_bytes;   // this warp's stages
+    if (lane == 0) {
+#pragma unroll
+        for (int s = 0; s < NST; ++s) mbar_init(bar_w + 8u * s, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    }
+    __syncthreads();
     const Fetch F(T, smem_f32 + S.table_off);
     const Ctx32 X{T, S, smem_u32(smem_f32 + S.coul_off)};
 
     const long long ncell = C.ncell;
-    const long long ntiles = (ncell + TILE - 1) / TILE;
-    const void *src[6] = {C.rho, C.bsq, C.the_in, C.thi_in, C.vol, C.r};     // staged in this order; vol / r only when present
+    const long long ntiles = (ncell + kWarpTile - 1) / kWarpTile;
+    const long long nfull = S.use_tma ? ncell / kWarpTile : 0;                // tiles that go through TMA
+    const long long GW = (long long)gridDim.x * NW;
     const int nf = S.nf;
-    const unsigned arr_bytes = TILE * 4u;
 
-    // one elected thread arms the stage's mbarrier and issues the bulk copies of one full tile
+    // lane 0 arms the stage's mbarrier and issues the bulk copies of one full warp tile
     auto issue = [&](long long tile, int s) {
-        const unsigned bar = s ? bar1 : bar0;
-        const unsigned dst = stage_u32 + (unsigned)s * S.stage_bytes;
-        const size_t goff = (size_t)tile * TILE * 4u;
-        mbar_expect_tx(bar, arr_bytes * (unsigned)nf);
-        int k = 0;
-#pragma unroll
-        for (int a = 0; a < 6; ++a) {
-            if (a == 4 && !S.has_vol) continue;
-            if (a == 5 && !S.has_r) continue;
-            tma_load_1d(dst + (unsigned)k * arr_bytes, (const char *)src[a] + goff, arr_bytes, bar);
-            ++k;
-        }
+        const unsigned bar = bar_w + 8u * (unsigned)s;
+        const unsigned dst = stg_w + (unsigned)s * S.wstage_bytes;
+        const size_t goff = (size_t)tile * kWarpArrBytes;
+        mbar_expect_tx(bar, kWarpArrBytes * (unsigned)nf);
+        tma_load_1d(dst, (const char *)C.rho + goff, kWarpArrBytes, bar);
+        tma_load_1d(dst + kWarpArrBytes, (const char *)C.bsq + goff, kWarpArrBytes, bar);
+        tma_load_1d(dst + 2 * kWarpArrBytes, (const char *)C.the_in + goff, kWarpArrBytes, bar);
+        tma_load_1d(dst + 3 * kWarpArrBytes, (const char *)C.thi_in + goff, kWarpArrBytes, bar);
+        unsigned k = 4;
+        if (S.has_vol) { tma_load_1d(dst + k * kWarpArrBytes, (const char *)C.vol + goff, kWarpArrBytes, bar); ++k; }
+        if (S.has_r) tma_load_1d(dst + k * kWarpArrBytes, (const char *)C.r + goff, kWarpArrBytes, bar);
     };
-    auto is_tma_tile = [&](long long tile) { return S.use_tma && tile < ntiles && (tile + 1) * TILE <= ncell; };
 
-    if (tid == 0) {
-        mbar_init(bar0, 1); mbar_init(bar1, 1);
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-        if (is_tma_tile(blockIdx.x)) issue(blockIdx.x, 0);
-        if (is_tma_tile((long long)blockIdx.x + gridDim.x)) issue((long long)blockIdx.x + gridDim.x, 1);
+    long long tile = (long long)blockIdx.x * NW + warp;
+    if (lane == 0) {
+#pragma unroll
+        for (int s = 0; s < NST; ++s)
+            if (tile + s * GW < nfull) issue(tile + s * GW, s);
     }
-    __syncthreads();
+    __syncwarp();
 
     DiagAcc acc;
-    int it = 0;
-    for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x, ++it) {
-        const int s = it & 1;
-        float *st = (float *)((unsigned char *)stages + (size_t)s * S.stage_bytes);
-        const long long c0 = tile * TILE;
-        const bool full = (tile + 1) * TILE <= ncell;
-        if (S.use_tma && full) {
-            mbar_wait(s ? bar1 : bar0, (unsigned)(it >> 1) & 1u);
-        } else {
-            // ragged last tile, or arrays that are not 16-byte aligned: cooperative plain loads (zero fill past the end)
-            int k = 0;
-#pragma unroll
-            for (int a = 0; a < 6; ++a) {
-                if (a == 4 && !S.has_vol) continue;
-                if (a == 5 && !S.has_r) continue;
-                const float *g = (const float *)src[a] + c0;
-                for (int i = tid; i < TILE; i += THREADS) st[k * TILE + i] = (c0 + i < ncell) ? __ldg(g + i) : 0.f;
-                ++k;
-            }
-            __syncthreads();
-        }
-        const float4 *s4 = (const float4 *)st;
-        float4 rho = s4[tid], bsq = s4[THREADS + tid], the = s4[2 * THREADS + tid], thi = s4[3 * THREADS + tid];
+    int s = 0; unsigned phase = 0;
+    for (; tile < ntiles; tile += GW) {
+        const long long c = tile * kWarpTile + (long long)lane * kF32CellsPerThread;
+        float4 rho, bsq, the, thi;
         float4 vv = make_float4(1.f, 1.f, 1.f, 1.f), rr = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (S.has_vol) vv = s4[4 * THREADS + tid];
-        if (S.has_r) rr = s4[(S.has_vol ? 5 : 4) * THREADS + tid];
-        __syncthreads();                                        // every thread holds its cells: the stage is free
-        if (tid == 0) {
-            const long long nxt = tile + 2ll * gridDim.x;
-            if (is_tma_tile(nxt)) {
-                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-                issue(nxt, s);
+        const bool tma = tile < nfull;
+        if (tma) {
+            mbar_wait(bar_w + 8u * (unsigned)s, phase);
+            const unsigned a = stg_w + (unsigned)s * S.wstage_bytes + 16u * (unsigned)lane;
+            // vol first: it feeds only the diagnostic sums, and shared-memory loads of a warp return in order, so once
+            // the outputs (which depend on every other array) are stored the whole stage has been read
+            if (S.has_vol) vv = lds_f4(a + 4 * kWarpArrBytes);
+            rho = lds_f4(a); bsq = lds_f4(a + kWarpArrBytes); the = lds_f4(a + 2 * kWarpArrBytes); thi = lds_f4(a + 3 * kWarpArrBytes);
+            if (S.has_r) rr = lds_f4(a + (S.has_vol ? 5u : 4u) * kWarpArrBytes);
+        } else {
+            // ragged last tile, or arrays that are not 16-byte aligned: guarded scalar loads (zeros past the end: rho = 0 passes through)
+#pragma unroll
+            for (int j = 0; j < kF32CellsPerThread; ++j) {
+                const bool in = c + j < ncell;
+                (&rho.x)[j] = in ? __ldg((const float *)C.rho + c + j) : 0.f;
+                (&bsq.x)[j] = in ? __ldg((const float *)C.bsq + c + j) : 0.f;
+                (&the.x)[j] = in ? __ldg((const float *)C.the_in + c + j) : 0.f;
+                (&thi.x)[j] = in ? __ldg((const float *)C.thi_in + c + j) : 0.f;
+                if (S.has_vol) (&vv.x)[j] = in ? __ldg((const float *)C.vol + c + j) : 1.f;
+                if (S.has_r) (&rr.x)[j] = in ? __ldg((const float *)C.r + c + j) : 0.f;
             }
         }
 #pragma unroll
         for (int j = 0; j < kF32CellsPerThread; j += G)
             step_cells_f32<MODE, Fetch, DIAG, CM, NSUB1, G>(X, F, &rho.x + j, &bsq.x + j, &the.x + j, &thi.x + j, &rr.x + j, &vv.x + j, acc);
-        const long long c = c0 + (long long)tid * kF32CellsPerThread;
-        if (full && S.use_tma) {
+        if (tma) {
             st_stream((float4 *)C.the_out + (c >> 2), the);
             st_stream((float4 *)C.thi_out + (c >> 2), thi);
+            // Re-arm the stage only now: the stores above depend on every value this warp read from it, so its
+            // LDS have all returned (read-before-overwrite across the generic and async proxies).  With NST
+            // stages the refill is still NST-1 tiles ahead of its use.
+            if (elect_one()) {
+                const long long nxt = tile + (long long)NST * GW;
+                if (nxt < nfull) issue(nxt, s);
+            }
+            if (++s == NST) { s = 0; phase ^= 1u; }
         } else {
 #pragma unroll
             for (int j = 0; j < kF32CellsPerThread; ++j)
@@ -597,58 +680,55 @@ cool_f32_kernel(const DevTable T, const F32Const S, const CellPtrs C, double *pa
 // ------------------------------------------------------------------------------------------
 struct LaunchCtx32 { const cool_table *t; F32Const S; const LaunchArgs *a; cudaStream_t st; };
 
-// fills the shared-memory layout fields of S for a launch with THREADS threads; returns the total
-inline size_t f32_smem_layout(F32Const &S, int threads, bool table_in_smem, const cool_table *t)
+constexpr int kF32Threads = 512, kF32Stages = 3;            // GLOBAL / texture variants: 16 warps, 3 stages each
+constexpr int kF32SmemThreads = 384, kF32SmemStages = 2;    // SMEM variant: the table image takes most of the shared memory
+constexpr int kCoulQuadSmemMax = 65536;                     // Coulomb quads up to 64^2 x 16 B are staged in shared memory
+
+// fills the shared-memory layout fields of S for a launch with `threads` threads; returns the total
+inline size_t f32_smem_layout(F32Const &S, int threads, int nst, bool table_in_smem, const cool_table *t)
 {
-    const size_t tile_bytes = (size_t)threads * kF32CellsPerThread * 4u;
-    S.stage_bytes = (unsigned)(tile_bytes * S.nf);
-    size_t off = kF32BarBytes + 2 * (size_t)S.stage_bytes;
+    S.wstage_bytes = kWarpArrBytes * (unsigned)S.nf;
+    S.stage_off = kF32BarBytes;
+    size_t off = kF32BarBytes + (size_t)(threads / 32) * nst * S.wstage_bytes;
     S.coul_off = (unsigned)off;
-    if (S.coul_smem) off += ((size_t)t->dev.coul_bytes + 15) & ~(size_t)15;
+    if (S.coul_smem) off += table_in_smem ? (((size_t)t->dev.coul_bytes + 15) & ~(size_t)15) : (size_t)t->dev.coulq_bytes;
     S.table_off = (unsigned)off;
     if (table_in_smem) off += t->dev.table_bytes;
     return off;
 }
 
-template <int MODE, class Fetch, bool DIAG, int CM, bool NSUB1, int THREADS, int MINB>
+template <int MODE, class Fetch, bool DIAG, int CM, bool NSUB1, int THREADS, int NST>
 static cudaError_t launch_f32_one(const LaunchCtx32 &L)
 {
     F32Const S = L.S;
-    const size_t smem = f32_smem_layout(S, THREADS, Fetch::kSmem, L.t);
-    auto kern = cool_f32_kernel<MODE, Fetch, DIAG, CM, NSUB1, THREADS, MINB>;
-    static int occ_cache = -1; static size_t occ_smem = ~(size_t)0;
+    const size_t smem = f32_smem_layout(S, THREADS, NST, Fetch::kSmem, L.t);
+    auto kern = cool_f32_kernel<MODE, Fetch, DIAG, CM, NSUB1, THREADS, NST>;
     if (smem > 48 * 1024) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
     }
-    if (occ_cache < 0 || occ_smem != smem) {
-        int occ = 0;
-        cudaError_t eo = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, THREADS, smem);
-        if (eo != cudaSuccess) return eo;
-        occ_cache = occ < 1 ? 1 : occ; occ_smem = smem;
-    }
     const LaunchArgs &a = *L.a;
-    constexpr long long TILE = (long long)THREADS * kF32CellsPerThread;
-    const long long ntiles = (a.ncell + TILE - 1) / TILE;
-    const long long cap = (long long)L.t->sm_count * occ_cache;
-    const int grid = (int)(ntiles < cap ? (ntiles < 1 ? 1 : ntiles) : cap);
+    constexpr long long CTA_TILE = (long long)(THREADS / 32) * kWarpTile;
+    const long long need = (a.ncell + CTA_TILE - 1) / CTA_TILE;
+    const int grid = (int)(need < L.t->sm_count ? (need < 1 ? 1 : need) : L.t->sm_count);     // one persistent CTA per SM
     CellPtrs C{a.rho, a.bsq, a.the_in, a.thi_in, a.r, a.vol, a.the_out, a.thi_out, a.ncell};
     kern<<<grid, THREADS, smem, L.st>>>(L.t->dev, S, C, a.partials, a.ticket, a.d_diag);
     return cudaGetLastError();
 }
 
-constexpr int kF32SmemThreads = 384;
-
-// dispatch over the four table variants for fixed <MODE, DIAG, CM, NSUB1>
+// dispatch over the table variants for fixed <MODE, DIAG, CM, NSUB1>
 template <int MODE, bool DIAG, int CM, bool NSUB1>
 static cudaError_t launch_f32_by_variant(const LaunchCtx32 &L, cool_variant v)
 {
-    constexpr int MB = 2;
     switch (v) {
-        case COOL_V_GLOBAL: return launch_f32_one<MODE, F32Global, DIAG, CM, NSUB1, 256, MB>(L);
-        case COOL_V_TEX_POINT: return launch_f32_one<MODE, F32TexPoint, DIAG, CM, NSUB1, 256, MB>(L);
-        case COOL_V_TEX_HWFILTER: return launch_f32_one<MODE, F32TexHw, DIAG, CM, NSUB1, 256, MB>(L);
-        case COOL_V_SMEM: return launch_f32_one<MODE, F32Smem, DIAG, CM, NSUB1, kF32SmemThreads, 1>(L);
+        case COOL_V_GLOBAL:
+            if constexpr (MODE == 3) {
+                if (L.t->dev.q3) return launch_f32_one<MODE, F32GlobalQ, DIAG, CM, NSUB1, kF32Threads, kF32Stages>(L);
+            }
+            return launch_f32_one<MODE, F32Global, DIAG, CM, NSUB1, kF32Threads, kF32Stages>(L);
+        case COOL_V_TEX_POINT: return launch_f32_one<MODE, F32TexPoint, DIAG, CM, NSUB1, kF32Threads, kF32Stages>(L);
+        case COOL_V_TEX_HWFILTER: return launch_f32_one<MODE, F32TexHw, DIAG, CM, NSUB1, kF32Threads, kF32Stages>(L);
+        case COOL_V_SMEM: return launch_f32_one<MODE, F32Smem, DIAG, CM, NSUB1, kF32SmemThreads, kF32SmemStages>(L);
         default: return cudaErrorInvalidValue;
     }
 }

@@ -28,6 +28,7 @@ struct AxisCoef {          // node-index coordinate t of a primitive q along one
     float nm1f, tmaxf;     // n-1 (clamp flag) and the largest float below n-1 (keeps floor(t) <= n-2)
     float ke;              // 2^23 + 127 + e0: (2^23 + biased exponent) - ke = e - e0, exactly
     float d2f;             // node spacing in log2 units (clamp correction of the fp32 path)
+    float c2f;             // t = log2(q)*invf + c2f (single-lg2 form)
 };
 
 struct DevTable {
@@ -45,8 +46,11 @@ struct DevTable {
     // so that Lambda h / u_e = 2^(interp + log2 h) without cancelling large fp32 numbers.
     const float *f1;
     const float4 *f4;
+    const float4 *q3;              // MODE 3 quad layout {T'(r,e,b), T'(r,e,b+1), T'(r,e+1,b), T'(r,e+1,b+1)}, plain strides; NULL when too large
     cudaTextureObject_t ftex_pt, ftex_lin;
-    const float *fcoul;            // log2 C [theta_i][theta_e]
+    const float *fcoul;            // log2 C [theta_i][theta_e] (allocation padded to 16 B)
+    const float4 *fcoulq;          // the same as quads {C(i,e), C(i,e+1), C(i+1,e), C(i+1,e+1)}
+    int coulq_bytes;
     int f4_has_coul;               // MODE 4: f4.w = log2 C (Coulomb axes identical to the table's Theta axes)
     // Coulomb coefficient table log10 C [theta_i][theta_e]
     const float *coul;
@@ -90,7 +94,7 @@ struct cool_table {
     cool::DevConst cst{};
     float *d_lin = nullptr;        // owns lin1 / lin4
     float *d_f32 = nullptr;        // owns f1 / f4
-    float *d_coul = nullptr, *d_fcoul = nullptr;
+    float *d_coul = nullptr, *d_fcoul = nullptr, *d_fcoulq = nullptr, *d_q3 = nullptr;
     cudaArray_t arr = nullptr, arr32 = nullptr;
     int sm_count = 148;
     int max_smem_optin = 0;

@@ -23,6 +23,15 @@ static StepConst make_step_const(const cool_table *t, cool_dtype dt, const Launc
     return S;
 }
 
+// Coulomb coefficient table staged in shared memory: quads (<= 64 KiB) for the GLOBAL / texture variants,
+// the plain layout (<= 16 KiB) for the SMEM variant; not needed when it rides in the 4-D texels.
+static bool coulomb_in_smem(const cool_table *t, const LaunchArgs &a, cool_variant v)
+{
+    const DevTable &D = t->dev;
+    if (a.coulomb != 1 || !D.fcoul || (D.mode == 4 && D.f4_has_coul)) return false;
+    return v == COOL_V_SMEM ? D.coul_bytes <= kCoulSmemMax : D.coulq_bytes <= kCoulQuadSmemMax;
+}
+
 static F32Const make_f32_const(const cool_table *t, const LaunchArgs &a)
 {
     const DevConst &K = t->cst;
@@ -46,7 +55,16 @@ static F32Const make_f32_const(const cool_table *t, const LaunchArgs &a)
     S.nf = 4 + S.has_r + S.has_vol;
     auto ok = [&](const void *p) { return p == nullptr || ((size_t)p % 16) == 0; };
     S.use_tma = ok(a.rho) && ok(a.bsq) && ok(a.the_in) && ok(a.thi_in) && ok(a.the_out) && ok(a.thi_out) && ok(a.r) && ok(a.vol);
-    S.coul_smem = a.coulomb == 1 && t->dev.fcoul && t->dev.coul_bytes <= kCoulSmemMax && !(t->dev.mode == 4 && t->dev.f4_has_coul);
+    // Coulomb-table node coordinates as an affine map of the table's own node coordinates
+    const DevTable &D = t->dev;
+    if (D.fcoul && D.mode != 0) {
+        const AxisCoef &te = D.ax[CAX_THE], &ce = D.cax[1];
+        S.cme_s = (float)(ce.inv10 / te.inv10); S.cme_o = (float)((te.lo10 - ce.lo10) * ce.inv10);
+        if (D.mode == 4) {
+            const AxisCoef &ti = D.ax[CAX_THI], &ci = D.cax[0];
+            S.cmi_s = (float)(ci.inv10 / ti.inv10); S.cmi_o = (float)((ti.lo10 - ci.lo10) * ci.inv10);
+        }
+    }
     return S;
 }
 
@@ -54,8 +72,8 @@ bool variant_supported(const cool_table *t, cool_variant v, cool_dtype, std::str
 {
     if (v == COOL_V_ANALYTIC) return true;
     if (t->dev.mode == 0) { if (why) *why = "table has no data (nproc = 0): only COOL_V_ANALYTIC applies"; return false; }
-    // SMEM variant: table image + two 6-array cell stages of the 512-thread kernel + Coulomb table + barriers
-    if (v == COOL_V_SMEM && (size_t)t->dev.table_bytes + kCoulSmemMax + 2 * 6 * (size_t)kF32SmemThreads * kF32CellsPerThread * 4 + 1024 > (size_t)t->max_smem_optin) {
+    // SMEM variant: table image + the warps' 6-array cell stages + plain Coulomb table + barriers
+    if (v == COOL_V_SMEM && (size_t)t->dev.table_bytes + kCoulSmemMax + (size_t)kF32SmemStages * 6 * (size_t)kF32SmemThreads * kF32CellsPerThread * 4 + kF32BarBytes > (size_t)t->max_smem_optin) {
         if (why) *why = "table does not fit in shared memory"; return false;
     }
     return true;
@@ -71,7 +89,8 @@ cool_status launch_step(const cool_table *t, cool_variant v, cool_dtype dt, cons
     if (v == COOL_V_ANALYTIC) e = launch_analytic(L, mode, dt, diag);
     else if (dt == COOL_F64) e = launch_f64(L, mode, v, diag);
     else {
-        const LaunchCtx32 L32{t, make_f32_const(t, a), &a, st};
+        LaunchCtx32 L32{t, make_f32_const(t, a), &a, st};
+        L32.S.coul_smem = coulomb_in_smem(t, a, v);
         // fast path: Coulomb from the coefficient table staged in shared memory (or riding in the 4-D texels)
         const int cm = (a.coulomb == 1 && (L32.S.coul_smem || (mode == 4 && t->dev.f4_has_coul))) ? 1 : 0;
         e = (mode == 3) ? launch_f32_m3(L32, v, diag, cm, a.nsub == 1) : launch_f32_m4(L32, v, diag, cm);
