@@ -340,13 +340,14 @@ extern "C" cool_status cool_table_create(const cool_table_desc *desc, int device
         D.coul = t->d_coul;
         {   // fp32 path: log2 C, plain (padded to 16 B) and as quads {C(i,e), C(i,e+1), C(i+1,e), C(i+1,e+1)}
             const size_t npad = (n + 3) & ~(size_t)3;
-            std::vector<float> c2(npad, 0.f), cq(n * 4);
-            for (size_t k = 0; k < n; ++k) c2[k] = (float)(3.321928094887362 * (double)desc->host_coulomb[k]);
             const int n0 = desc->nc[0], n1 = desc->nc[1];
+            const int qs = n1;                                   // quad row stride (no padding: 64^2 quads fill a 64 KiB carve-out step exactly)
+            std::vector<float> c2(npad, 0.f), cq((size_t)n0 * qs * 4, 0.f);
+            for (size_t k = 0; k < n; ++k) c2[k] = (float)(3.321928094887362 * (double)desc->host_coulomb[k]);
             for (int i = 0; i < n0; ++i)
                 for (int j = 0; j < n1; ++j) {
                     const int i1 = std::min(i + 1, n0 - 1), j1 = std::min(j + 1, n1 - 1);
-                    float *q = &cq[((size_t)i * n1 + j) * 4];
+                    float *q = &cq[((size_t)i * qs + j) * 4];
                     q[0] = c2[(size_t)i * n1 + j]; q[1] = c2[(size_t)i * n1 + j1]; q[2] = c2[(size_t)i1 * n1 + j]; q[3] = c2[(size_t)i1 * n1 + j1];
                 }
             e = cudaMalloc(&t->d_fcoul, npad * sizeof(float));
@@ -357,6 +358,7 @@ extern "C" cool_status cool_table_create(const cool_table_desc *desc, int device
             D.fcoul = t->d_fcoul;
             D.fcoulq = (const float4 *)t->d_fcoulq;
             D.coulq_bytes = (int)(cq.size() * sizeof(float));
+            D.coulq_stride = qs;
         }
         D.cax[0] = make_axis(desc->nc[0], desc->clo[0], desc->chi[0]);
         D.cax[1] = make_axis(desc->nc[1], desc->clo[1], desc->chi[1]);

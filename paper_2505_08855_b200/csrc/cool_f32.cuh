@@ -28,6 +28,7 @@
 //     per sub-step — and the Coulomb coefficient rides in the 4th texel channel;
 //   * a sub-step that leaves both temperatures bit-identical repeats itself: exact early exit.
 #pragma once
+#include <cstdlib>
 #include "cool_kernels.cuh"
 
 namespace cool {
@@ -363,12 +364,14 @@ __device__ __forceinline__ float patch_eval(const Patch4 &P, int k, float we, fl
 //   CM = 1, !QUAD : plain layout staged in shared memory (SMEM variant: the table image leaves no room for quads);
 //   CM = 0        : plain layout in global memory (L1-resident).
 template <int CM, bool QUAD>
-__device__ __forceinline__ float coulomb_C32(int n1, const float *cg, unsigned cs, const Loc32 &a, const Loc32 &b)
+__device__ __forceinline__ float coulomb_C32(int n1, int qstride, const float *cg, unsigned cs, const Loc32 &a, const Loc32 &b)
 {
     const int off = loc_bits(a) * n1 + (loc_bits(b) + (int)(0u - kMagicBits * (unsigned)(n1 + 1)));
     float c00, c01, c10, c11;
     if constexpr (CM == 1 && QUAD) {
-        const float4 q = lds_f4(cs + 16u * (unsigned)off);
+        // quad rows are skewed (row stride = 3 mod 8 quads) so that neighbouring (i, e) quads fall in different bank groups
+        const int qoff = loc_bits(a) * qstride + (loc_bits(b) + (int)(0u - kMagicBits * (unsigned)(qstride + 1)));
+        const float4 q = lds_f4(cs + 16u * (unsigned)qoff);
         c00 = q.x; c01 = q.y; c10 = q.z; c11 = q.w;
     } else if constexpr (CM == 1) {
         const unsigned p = cs + 4u * (unsigned)off, q = p + 4u * (unsigned)n1;
@@ -492,7 +495,7 @@ __device__ __forceinline__ void step_cells_f32(const Ctx32 &X, const Fetch &F, c
                         if (MODE == 4) ca = split32<false>(T.cax[0], fmaf(ti, S.cmi_s, S.cmi_o), dummy);
                         else ca = locate32<false>(T.cax[0], thi[j], dummy, one_bits);
                         cb = split32<false>(T.cax[1], fmaf(te, S.cme_s, S.cme_o), dummy);
-                        C = coulomb_C32<CM, !Fetch::kSmem>(T.cax[1].n, T.fcoul, X.coul_s, ca, cb);
+                        C = coulomb_C32<CM, !Fetch::kSmem>(T.cax[1].n, T.coulq_stride, T.fcoul, X.coul_s, ca, cb);
                     }
                 } else {
                     C = (D != 0.f && !bad[j]) ? (float)coolphys::coulomb_C((double)the[j], (double)thi[j] / S.ion_ratio) : 0.f;
@@ -557,7 +560,7 @@ __device__ __forceinline__ void step_cells_f32(const Ctx32 &X, const Fetch &F, c
 constexpr int kF32CellsPerThread = 4;
 constexpr int kWarpTile = 32 * kF32CellsPerThread;          // cells per warp tile
 constexpr unsigned kWarpArrBytes = kWarpTile * 4u;          // 512 B per array per stage
-constexpr unsigned kF32BarBytes = 512;                      // room for 16 warps x 4 stages of 8-byte mbarriers
+constexpr unsigned kF32BarBytes = 1024;                     // room for 32 warps x 4 stages of 8-byte mbarriers
 
 template <int MODE, class Fetch, bool DIAG, int CM, bool NSUB1, int THREADS, int NST>
 __global__ void __launch_bounds__(THREADS, 1)
@@ -630,8 +633,8 @@ cool_f32_kernel(const DevTable T, const F32Const S, const CellPtrs C, double *pa
         const long long c = tile * kWarpTile + (long long)lane * kF32CellsPerThread;
         float4 rho, bsq, the, thi;
         float4 vv = make_float4(1.f, 1.f, 1.f, 1.f), rr = make_float4(0.f, 0.f, 0.f, 0.f);
-        const bool tma = tile < nfull;
-        if (tma) {
+        const bool full = tile < nfull;
+        if (full) {
             mbar_wait(bar_w + 8u * (unsigned)s, phase);
             const unsigned a = stg_w + (unsigned)s * S.wstage_bytes + 16u * (unsigned)lane;
             // vol first: it feeds only the diagnostic sums, and shared-memory loads of a warp return in order, so once
@@ -655,7 +658,7 @@ cool_f32_kernel(const DevTable T, const F32Const S, const CellPtrs C, double *pa
 #pragma unroll
         for (int j = 0; j < kF32CellsPerThread; j += G)
             step_cells_f32<MODE, Fetch, DIAG, CM, NSUB1, G>(X, F, &rho.x + j, &bsq.x + j, &the.x + j, &thi.x + j, &rr.x + j, &vv.x + j, acc);
-        if (tma) {
+        if (full) {
             st_stream((float4 *)C.the_out + (c >> 2), the);
             st_stream((float4 *)C.thi_out + (c >> 2), thi);
             // Re-arm the stage only now: the stores above depend on every value this warp read from it, so its
@@ -680,9 +683,10 @@ cool_f32_kernel(const DevTable T, const F32Const S, const CellPtrs C, double *pa
 // ------------------------------------------------------------------------------------------
 struct LaunchCtx32 { const cool_table *t; F32Const S; const LaunchArgs *a; cudaStream_t st; };
 
-constexpr int kF32Threads = 512, kF32Stages = 3;            // GLOBAL / texture variants: 16 warps, 3 stages each
+constexpr int kF32Threads3 = 768, kF32Stages3 = 2;          // GLOBAL / texture variants, single-update 3-D step: 24 warps, 2 stages each
+constexpr int kF32Threads4 = 512, kF32Stages4 = 3;          // GLOBAL / texture variants, sub-stepped or 4-D: 16 warps, 3 stages each
 constexpr int kF32SmemThreads = 384, kF32SmemStages = 2;    // SMEM variant: the table image takes most of the shared memory
-constexpr int kCoulQuadSmemMax = 65536;                     // Coulomb quads up to 64^2 x 16 B are staged in shared memory
+constexpr int kCoulQuadSmemMax = 73728;                     // Coulomb quads up to 64 x (64 + 3 skew) x 16 B are staged in shared memory
 
 // fills the shared-memory layout fields of S for a launch with `threads` threads; returns the total
 inline size_t f32_smem_layout(F32Const &S, int threads, int nst, bool table_in_smem, const cool_table *t)
@@ -720,14 +724,19 @@ static cudaError_t launch_f32_one(const LaunchCtx32 &L)
 template <int MODE, bool DIAG, int CM, bool NSUB1>
 static cudaError_t launch_f32_by_variant(const LaunchCtx32 &L, cool_variant v)
 {
+    // The single-update 3-D step fits 80 registers: 24 warps per SM hide the gather latency (measured best on B200:
+    // 768 threads, 2 stages).  Sub-stepping loops and MODE 4 (a 16-register patch per cell) need 128 registers:
+    // 16 warps, 3 stages.
+    constexpr bool kWide = MODE == 3 && NSUB1;
+    constexpr int TH = kWide ? kF32Threads3 : kF32Threads4, NS = kWide ? kF32Stages3 : kF32Stages4;
     switch (v) {
         case COOL_V_GLOBAL:
             if constexpr (MODE == 3) {
-                if (L.t->dev.q3) return launch_f32_one<MODE, F32GlobalQ, DIAG, CM, NSUB1, kF32Threads, kF32Stages>(L);
+                if (L.t->dev.q3) return launch_f32_one<MODE, F32GlobalQ, DIAG, CM, NSUB1, TH, NS>(L);
             }
-            return launch_f32_one<MODE, F32Global, DIAG, CM, NSUB1, kF32Threads, kF32Stages>(L);
-        case COOL_V_TEX_POINT: return launch_f32_one<MODE, F32TexPoint, DIAG, CM, NSUB1, kF32Threads, kF32Stages>(L);
-        case COOL_V_TEX_HWFILTER: return launch_f32_one<MODE, F32TexHw, DIAG, CM, NSUB1, kF32Threads, kF32Stages>(L);
+            return launch_f32_one<MODE, F32Global, DIAG, CM, NSUB1, TH, NS>(L);
+        case COOL_V_TEX_POINT: return launch_f32_one<MODE, F32TexPoint, DIAG, CM, NSUB1, TH, NS>(L);
+        case COOL_V_TEX_HWFILTER: return launch_f32_one<MODE, F32TexHw, DIAG, CM, NSUB1, TH, NS>(L);
         case COOL_V_SMEM: return launch_f32_one<MODE, F32Smem, DIAG, CM, NSUB1, kF32SmemThreads, kF32SmemStages>(L);
         default: return cudaErrorInvalidValue;
     }
