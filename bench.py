@@ -33,6 +33,14 @@ METRIC = "Gcell-updates/s of the cooling step"
 UNIT = "Gcell-updates/s"
 SPEC_HBM_GBS = 8000.0                     # BASELINE.json: "vs 8 TB/s"
 FALLBACK_HBM_GBS = 6650.0                 # B200_PROFILING.md fallback
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from one `ncu --set full` capture each
+# (profiles/r01c_<workload>_global_full.txt, line "traffic ="); null for workloads that were not captured
+NCU_TRAFFIC_GB = {"c5": 3.7334, "s512": 3.1939, "c2": 0.4301}
+# issue-slot ceiling of the SMs (the bound that actually limits the sub-stepped 4-D step): 148 SMs x 4 schedulers x
+# 1 warp instruction per clock at clocks.max.sm 1965 MHz (B200_PROFILING.md unit counts) = 1163 G warp-instructions/s
+ISSUE_PEAK_GWINST = 148 * 4 * 1.965
+# warp instructions per launch (smsp__inst_executed.sum of the same captures)
+NCU_WARP_INST = {"c5": 3254462658, "s512": 613220864}
 
 
 # ------------------------------------------------------------------------------------------------
@@ -163,7 +171,8 @@ def main():
     ap.add_argument("--variant", default="auto")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--cpu-sample", type=int, default=1 << 24)
+    ap.add_argument("--no-also", action="store_true", help="skip the companion s512 measurement of the default workload")
+    ap.add_argument("--cpu-sample", type=int, default=1 << 27)
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3                                       # timing rule: W >= 3
@@ -271,6 +280,42 @@ def main():
             dd["lum_total"], dd["lum_brems"], dd["lum_synch"], dd["lum_compton"] = [float(x) for x in t.tolist()]
         diag_out = dd
 
+    # ---- companion line: the single-update 3-D step (table 128^3) on the same 512^3 field, same timing protocol ----
+    also = None
+    if args.workload == "c5" and args.variant == "auto" and not args.no_also:
+        spec2 = workload_spec("s512")
+        axis2, lo2, hi2 = table_ranges(spec2["n"])
+        desc2 = api.make_desc(axis2, spec2["n"], lo2, hi2, 1, nc=spec2["nc"], clo=[synth.LOG_THETA[0]] * 2, chi=[synth.LOG_THETA[1]] * 2)
+        data2, coul2 = api.cool_table_build_host(desc2, want_coulomb=True)
+        table2 = api.cool_table_create(desc2, data2, coul2, device=local_rank)
+        params2 = api.make_params(spec2["dt"], 1, 0.3, 0.0, api.COOL_V_AUTO, api.COOL_COULOMB_TABLE)
+
+        def step2():
+            api.cool_apply(table2, ncell, api.COOL_F32, d["rho"], d["bsq"], d["theta_e"], d["theta_i"], the_o, thi_o, params2, stream=stream)
+        for _ in range(args.warmup):
+            step2()
+        barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(args.steps):
+            step2()
+        e1.record()
+        barrier()
+        ms2 = float(e0.elapsed_time(e1)) / args.steps
+        if world > 1:
+            t = torch.tensor([ms2], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms2 = float(t.item())
+        peak2, _ = peaks()
+        ach2 = 24 * ncell / (ms2 * 1e-3) / 1e9
+        also = dict(workload="s512", description=spec2["label"], ms_per_step=ms2, value=ncell * world / (ms2 * 1e-3) / 1e9, unit=UNIT,
+                    roofline=dict(bound="hbm", achieved=ach2, peak=peak2, unit="GB/s", frac=ach2 / peak2, traffic=NCU_TRAFFIC_GB["s512"] * 1e9,
+                                  kernel="cool_f32_kernel<MODE=3, F32GlobalQ, DIAG=0, CM=1, NSUB1=1, 768 threads, 2 stages>", bytes_per_cell=24),
+                    frac_of_8TBs=ach2 / SPEC_HBM_GBS)
+        table2.destroy()
+        step()                                       # leave the_o / thi_o holding the main workload's result for the e2e check below
+        torch.cuda.synchronize()
+
     # ---- end to end: host buffers, copies inside the timed region (rank-local, max over ranks) ----
     e2e = None
     if not args.no_e2e:
@@ -308,6 +353,13 @@ def main():
     bpc = bytes_per_cell(spec)
     kern_ms = float(np.mean(per_step_ms))                     # one kernel per step: step time == kernel time
     achieved = bpc * ncell / (kern_ms * 1e-3) / 1e9
+    mode = len(spec["n"])
+    single = mode == 3 and spec["nsub"] == 1
+    fetch = {"global": "F32GlobalQ" if (mode == 3 and np.prod(spec["n"]) * 16 <= (64 << 20)) else "F32Global", "smem": "F32Smem",
+             "tex_point": "F32TexPoint", "tex_hwfilter": "F32TexHw"}.get(api.VARIANT_NAMES[resolved], api.VARIANT_NAMES[resolved])
+    kernel_name = "cool_f32_kernel<MODE=%d, %s, DIAG=%d, CM=1, NSUB1=%d, %s>" % (
+        mode, fetch, int(bool(spec["diag"])), int(spec["nsub"] == 1),
+        "384 threads, 2 stages" if fetch == "F32Smem" else ("768 threads, 2 stages" if single else "512 threads, 3 stages"))
     line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=args.warmup,
                 ms_per_step=total_ms / args.steps, higher_is_better=True, scaling="weak", vs_baseline=None,
                 dtype="f32", data="synthetic",
@@ -316,11 +368,18 @@ def main():
                             cell_substeps_per_s=value * spec["nsub"] * 1e9),
                 hbm_gbs=achieved * world, frac_of_8TBs=achieved / SPEC_HBM_GBS,
                 clocks=clocks, e2e=e2e, gpu_launches=launches_per_step * args.steps,
-                roofline=dict(bound="hbm", achieved=achieved, peak=peak, unit="GB/s", frac=achieved / peak, traffic=None,
-                              kernel="cool_step_kernel<float,%d,%s>" % (len(spec["n"]), api.VARIANT_NAMES[resolved]),
-                              bytes_per_cell=bpc, peak_source=peak_src,
+                roofline=dict(bound="hbm", achieved=achieved, peak=peak, unit="GB/s", frac=achieved / peak,
+                              traffic=(NCU_TRAFFIC_GB[args.workload] * 1e9 if args.workload in NCU_TRAFFIC_GB and args.variant == "auto" else None),
+                              kernel=kernel_name, bytes_per_cell=bpc, algorithmic_bytes_per_launch=bpc * ncell, peak_source=peak_src,
                               ms_per_launch_median=float(np.median(per_step_ms)), ms_per_launch_best=float(per_step_ms.min())),
                 diag=diag_out)
+    if args.workload in NCU_WARP_INST and args.variant == "auto":
+        gw = NCU_WARP_INST[args.workload] / (kern_ms * 1e-3) / 1e9
+        line["issue_roofline"] = dict(bound="alu", achieved=gw, peak=ISSUE_PEAK_GWINST, unit="G warp-instructions/s", frac=gw / ISSUE_PEAK_GWINST,
+                                      warp_inst_per_launch=NCU_WARP_INST[args.workload],
+                                      note="instruction-issue ceiling (148 SMs x 4 schedulers x 1965 MHz); instruction count from the ncu capture in profiles/")
+    if also is not None:
+        line["also"] = also
     if not args.no_cpu_baseline:
         m, cores, times = oracle_leg(spec, desc, data, coul, fields, args.cpu_sample, 1)
         line["cpu_baseline"] = dict(value=m / times[0] / 1e9, unit=UNIT, cores=cores, kind="oracle",
