@@ -557,9 +557,6 @@ __device__ __forceinline__ void step_cells_f32(const Ctx32 &X, const Fetch &F, c
 // The kernel.  Dynamic shared memory:
 //   [NW*NST mbarriers | NW warps x NST stages x nf arrays x 128 floats | Coulomb quads | table image (SMEM variant)]
 // ------------------------------------------------------------------------------------------
-#ifndef COOL_G4
-#define COOL_G4 1
-#endif
 constexpr int kF32CellsPerThread = 4;
 constexpr int kWarpTile = 32 * kF32CellsPerThread;          // cells per warp tile
 constexpr unsigned kWarpArrBytes = kWarpTile * 4u;          // 512 B per array per stage
@@ -570,7 +567,6 @@ __global__ void __launch_bounds__(THREADS, 1)
 cool_f32_kernel(const DevTable T, const F32Const S, const CellPtrs C, double *partials, unsigned *ticket, cool_diag *d_diag)
 {
     constexpr int NW = THREADS / 32;
-    constexpr int G = (MODE == 4) ? COOL_G4 : kF32CellsPerThread;      // cells advanced together (MODE 4: the patch is 16 registers per cell)
     static_assert(NW * NST * 8 <= (int)kF32BarBytes, "mbarrier area too small");
     extern __shared__ __align__(128) unsigned char smem_f32[];
     const int tid = threadIdx.x, lane = tid & 31;
@@ -658,9 +654,18 @@ cool_f32_kernel(const DevTable T, const F32Const S, const CellPtrs C, double *pa
                 if (S.has_r) (&rr.x)[j] = in ? __ldg((const float *)C.r + c + j) : 0.f;
             }
         }
-#pragma unroll
-        for (int j = 0; j < kF32CellsPerThread; j += G)
-            step_cells_f32<MODE, Fetch, DIAG, CM, NSUB1, G>(X, F, &rho.x + j, &bsq.x + j, &the.x + j, &thi.x + j, &rr.x + j, &vv.x + j, acc);
+        if constexpr (MODE == 4) {
+            // the 16-register patch allows one cell at a time: one copy of the cell code, run four times with the
+            // vectors rotated (a quarter of the instruction footprint of the unrolled form)
+            auto rot = [](float4 &v) { const float t = v.x; v.x = v.y; v.y = v.z; v.z = v.w; v.w = t; };
+#pragma unroll 1
+            for (int j = 0; j < kF32CellsPerThread; ++j) {
+                step_cells_f32<MODE, Fetch, DIAG, CM, NSUB1, 1>(X, F, &rho.x, &bsq.x, &the.x, &thi.x, &rr.x, &vv.x, acc);
+                rot(rho); rot(bsq); rot(the); rot(thi); rot(rr); rot(vv);
+            }
+        } else {
+            step_cells_f32<MODE, Fetch, DIAG, CM, NSUB1, kF32CellsPerThread>(X, F, &rho.x, &bsq.x, &the.x, &thi.x, &rr.x, &vv.x, acc);
+        }
         if (full) {
             st_stream((float4 *)C.the_out + (c >> 2), the);
             st_stream((float4 *)C.thi_out + (c >> 2), thi);
@@ -687,11 +692,7 @@ cool_f32_kernel(const DevTable T, const F32Const S, const CellPtrs C, double *pa
 struct LaunchCtx32 { const cool_table *t; F32Const S; const LaunchArgs *a; cudaStream_t st; };
 
 constexpr int kF32Threads3 = 768, kF32Stages3 = 2;          // GLOBAL / texture variants, single-update 3-D step: 24 warps, 2 stages each
-#ifndef COOL_T4
-#define COOL_T4 512
-#define COOL_S4 3
-#endif
-constexpr int kF32Threads4 = COOL_T4, kF32Stages4 = COOL_S4;          // GLOBAL / texture variants, sub-stepped or 4-D: 16 warps, 3 stages each
+constexpr int kF32Threads4 = 512, kF32Stages4 = 3;          // GLOBAL / texture variants, sub-stepped or 4-D: 16 warps, 3 stages each
 constexpr int kF32SmemThreads = 384, kF32SmemStages = 2;    // SMEM variant: the table image takes most of the shared memory
 constexpr int kCoulQuadSmemMax = 73728;                     // Coulomb quads up to 64 x (64 + 3 skew) x 16 B are staged in shared memory
 
