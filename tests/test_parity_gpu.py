@@ -328,3 +328,37 @@ def test_bad_arguments(tab3):
     with pytest.raises(api.CoolError) as e:
         api.cool_table_create(bad, data)
     assert e.value.status == api.COOL_EINVAL
+
+
+THETA_K2_SWITCH = 1.0e8 / 5.929896575e9        # C-12: K2(1/theta) -> 2 theta^2 at T_e <= 1e8 K
+
+
+@pytest.mark.parametrize("dt,nsub,cfg", [(10.0, 4, 1), (1000.0, 4, 2), (3.0, 8, 5)])
+def test_large_sample_fp32_and_the_k2_switch_interval(oracle, tab3, dt, nsub, cfg):
+    """200 003 cells at aggressive dt.  The table interval of Theta_e that contains the paper's K2 -> 2 theta^2
+    switch (C-12) holds a 1e23 jump of the synchrotron rate between two neighbouring nodes, i.e. a slope of
+    ~76 log2 units per node: there the fp32 quantisation of the INPUT alone (5.5e-7 nodes) moves the rate by
+    3e-5, and the fp32 node coordinate (<= 4e-6 nodes) by 2e-4.  Cells whose Theta_e may visit that interval
+    during the update are held to 3e-4 and counted; every other cell to the 1e-5 bar of north_star."""
+    table, otab, un = tab3
+    f = synth.log_uniform_cells(200003, dtype=np.float32, config=cfg, outlier_frac=0.01)
+    ref = cm.oracle_step(oracle, otab, un, f, dt, nsub=nsub)
+    got = cm.gpu_step(table, f, np.float32, dt, nsub=nsub, variant=api.COOL_V_GLOBAL)
+    ee = cm.rel_err(got["theta_e"], ref["theta_e"]); ei = cm.rel_err(got["theta_i"], ref["theta_i"])
+    lo, hi, n = cm.LO3[1], cm.HI3[1], 64
+    k = int(np.floor((np.log10(THETA_K2_SWITCH) - lo) / ((hi - lo) / (n - 1))))
+    node_lo, node_hi = 10.0 ** (lo + k * (hi - lo) / (n - 1)), 10.0 ** (lo + (k + 1) * (hi - lo) / (n - 1))
+    assert node_lo <= THETA_K2_SWITCH < node_hi
+    t0 = f["theta_e"].astype(np.float64)
+    tmin, tmax = np.minimum(t0, ref["theta_e"]), np.maximum(t0, ref["theta_e"])
+    # a sub-step moves Theta_e by at most ~30 % (limiter) and the path need not be monotone (Coulomb heating), so cells whose
+    # start..end range comes within a factor 1.5 of the interval may have visited it
+    crossing = (tmin <= node_hi * 1.5) & (tmax >= node_lo / 1.5)
+    out = ~crossing
+    print(f"\ndt={dt} nsub={nsub}: {int(crossing.sum())} cells cross the K2-switch interval "
+          f"[{node_lo:.5f}, {node_hi:.5f}]: max err {max(ee[crossing].max(), ei[crossing].max()):.2e}, "
+          f"{int(((ee > 1e-5) | (ei > 1e-5)).sum())} above 1e-5; elsewhere max {max(ee[out].max(), ei[out].max()):.2e}")
+    assert crossing.sum() > 500 and out.sum() > 150000
+    assert ee[out].max() <= 1e-5 and ei[out].max() <= 1e-5
+    assert ee[crossing].max() <= 3e-4 and ei[crossing].max() <= 3e-4
+    assert ((ee > 1e-5) | (ei > 1e-5)).sum() <= 40          # a handful of cells, all inside the switch interval
