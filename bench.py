@@ -67,6 +67,12 @@ def workload_spec(name: str):
     if name == "s512":
         return dict(label="512^3 fp32 MAD-like field, single update, table 128^3 + 64^2 Coulomb (3-D step of configs[2] at 512^3)",
                     n=[128, 128, 128], nc=[64, 64], nsub=1, dt=1e-3, field=("mad", 512, 512, 512), diag=False, vol=False)
+    if name == "s512d":
+        return dict(label="s512 with the luminosity diagnostic and volume weights", n=[128, 128, 128], nc=[64, 64], nsub=1, dt=1e-3,
+                    field=("mad", 512, 512, 512), diag=True, vol=True)
+    if name == "s512f":
+        return dict(label="s512 with luminosity, volume weights and the temperature floor (the 3-D step of configs[2] at 512^3)",
+                    n=[128, 128, 128], nc=[64, 64], nsub=1, dt=1e-3, field=("mad", 512, 512, 512), diag=True, vol=True, floor=0.1)
     raise SystemExit(f"unknown workload {name}")
 
 

@@ -511,8 +511,11 @@ __device__ __forceinline__ void step_cells_f32(const Ctx32 &X, const Fetch &F, c
             const float thi_n = __fmaf_rn(-dthe, S.gi1_over_ge1, thi[j]);
             if constexpr (DIAG) {
                 drad_last[j] = drad;
-                lsum[j][0] += drad; lsum[j][1] = fmaf(drad, fr[j][0], lsum[j][1]);
-                lsum[j][2] = fmaf(drad, fr[j][1], lsum[j][2]); lsum[j][3] = fmaf(drad, fr[j][2], lsum[j][3]);
+                lsum[j][0] += drad;
+                if constexpr (MODE == 4) {                       // per-process split exists only for the three process tables
+                    lsum[j][1] = fmaf(drad, fr[j][0], lsum[j][1]);
+                    lsum[j][2] = fmaf(drad, fr[j][1], lsum[j][2]); lsum[j][3] = fmaf(drad, fr[j][2], lsum[j][3]);
+                }
             }
             if constexpr (!NSUB1) changed |= (the_n != the[j]) | (thi_n != thi[j]);
             the[j] = the_n; thi[j] = thi_n;
@@ -525,8 +528,10 @@ __device__ __forceinline__ void step_cells_f32(const Ctx32 &X, const Fetch &F, c
 #pragma unroll
                     for (int j = 0; j < NV; ++j) {
                         lsum[j][0] = fmaf(rem, drad_last[j], lsum[j][0]);
+                        if constexpr (MODE == 4) {
 #pragma unroll
-                        for (int k = 0; k < 3; ++k) lsum[j][k + 1] = fmaf(rem, drad_last[j] * fr[j][k], lsum[j][k + 1]);
+                            for (int k = 0; k < 3; ++k) lsum[j][k + 1] = fmaf(rem, drad_last[j] * fr[j][k], lsum[j][k + 1]);
+                        }
                     }
                 }
                 break;
@@ -542,14 +547,23 @@ __device__ __forceinline__ void step_cells_f32(const Ctx32 &X, const Fetch &F, c
             }
     }
     if constexpr (DIAG) {
+        // the NV cells are summed in fp32 first (one fp64 add per sum per call): the fp64 pipe is narrow
+        float part[4] = {0.f, 0.f, 0.f, 0.f};
 #pragma unroll
-        for (int j = 0; j < NV; ++j)
-            if (!bad[j]) {
-                const float wgt = rho[j] * vol[j];
+        for (int j = 0; j < NV; ++j) {
+            const float wgt = rho[j] * vol[j];                  // bad cells (possibly NaN) contribute an exact 0
+            part[0] += bad[j] ? 0.f : lsum[j][0] * wgt;
+            if constexpr (MODE == 4) {
 #pragma unroll
-                for (int k = 0; k < 4; ++k) acc.lum[k] += (double)(lsum[j][k] * wgt);
-                acc.lim += limited[j]; acc.flo += floored[j]; acc.cla += clamped[j];
+                for (int k = 1; k < 4; ++k) part[k] += bad[j] ? 0.f : lsum[j][k] * wgt;
             }
+            if (!bad[j]) { acc.lim += limited[j]; acc.flo += floored[j]; acc.cla += clamped[j]; }
+        }
+        acc.lum[0] += (double)part[0];
+        if constexpr (MODE == 4) {
+#pragma unroll
+            for (int k = 1; k < 4; ++k) acc.lum[k] += (double)part[k];
+        }
     }
 }
 

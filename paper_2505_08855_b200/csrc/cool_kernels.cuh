@@ -325,12 +325,15 @@ __device__ __forceinline__ double warp_sum(double v)
     for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
     return v;
 }
-static __device__ __noinline__ void reduce_diag(const DiagAcc &acc, double lum_k, double *partials, unsigned *ticket, cool_diag *out)
+// Takes the sums BY VALUE: passing the accumulator by reference to this non-inlined function would pin it in local
+// memory for the whole kernel (one st.local per accumulation).
+static __device__ __noinline__ void reduce_diag_vals(double l0, double l1, double l2, double l3, int lim, int flo, int cla,
+                                                     double lum_k, double *partials, unsigned *ticket, cool_diag *out)
 {
     __shared__ double sh[32][8];
     __shared__ unsigned s_last;
     __shared__ double fin[256];
-    double v[7] = {acc.lum[0], acc.lum[1], acc.lum[2], acc.lum[3], (double)acc.lim, (double)acc.flo, (double)acc.cla};
+    double v[7] = {l0, l1, l2, l3, (double)lim, (double)flo, (double)cla};
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
 #pragma unroll
     for (int k = 0; k < 7; ++k) {
@@ -368,6 +371,10 @@ static __device__ __noinline__ void reduce_diag(const DiagAcc &acc, double lum_k
         __syncthreads();
     }
     if (threadIdx.x == 0) *ticket = 0;       // ready for the next launch on this stream
+}
+__device__ __forceinline__ void reduce_diag(const DiagAcc &acc, double lum_k, double *partials, unsigned *ticket, cool_diag *out)
+{
+    reduce_diag_vals(acc.lum[0], acc.lum[1], acc.lum[2], acc.lum[3], acc.lim, acc.flo, acc.cla, lum_k, partials, ticket, out);
 }
 
 // ------------------------------------------------------------------------------------------
