@@ -107,6 +107,9 @@ def lib():
                                C.POINTER(d), C.POINTER(i)]),
             "orc_step": (None, [C.POINTER(_Table), UP, C.c_longlong, p, p, p, p, p, p,
                                 d, i, d, d, i, i, p, p, p, p, p, i]),
+            "orc_step_implicit": (None, [C.POINTER(_Table), UP, C.c_longlong, p, p, p, p, p, p,
+                                         d, i, d, i, p, p, p, i]),
+            "orc_implicit_residual": (d, [C.POINTER(_Table), UP, d, d, d, d, d, d, i, d, i, d]),
             "orc_fill_total3": (None, [UP, C.POINTER(i), C.POINTER(d), C.POINTER(d), p, i]),
             "orc_fill_coulomb2": (None, [UP, C.POINTER(i), C.POINTER(d), C.POINTER(d), p]),
             "orc_max_threads": (i, []),
@@ -230,3 +233,30 @@ def step(table: Table, un: Units, rho, bsq, theta_e, theta_i, dt, nsub=1, f_limi
     if want_rates:
         out["lam0"] = lam0; out["qcc0"] = qcc0
     return out
+
+
+def step_implicit(table: Table, un: Units, rho, bsq, theta_e, theta_i, dt, nsub=1, h_floor=0.0, r=None, vol=None,
+                  coulomb_mode=None, nthreads=1):
+    """Part B' (implicit scheme, PAPER.md L185 (ii), reading C-18) over a field.  Returns dict(theta_e, theta_i, diag)."""
+    f64 = lambda a: None if a is None else np.ascontiguousarray(a, dtype=np.float64).ravel()
+    rho, bsq, the, thi, r, vol = map(f64, (rho, bsq, theta_e, theta_i, r, vol))
+    n = rho.size
+    if coulomb_mode is None:
+        coulomb_mode = COULOMB_TABLE if table.coul is not None else COULOMB_ANALYTIC
+    the_o = np.empty(n); thi_o = np.empty(n)
+    diag = np.zeros(7)
+    ptr = lambda a: None if a is None else a.ctypes.data
+    lib().orc_step_implicit(C.byref(table._c), C.byref(un), n, ptr(rho), ptr(bsq), ptr(the), ptr(thi), ptr(r), ptr(vol),
+                            float(dt), int(nsub), float(h_floor), int(coulomb_mode), ptr(the_o), ptr(thi_o), ptr(diag), int(nthreads))
+    return dict(theta_e=the_o, theta_i=thi_o,
+                diag=dict(lum_total=diag[0], lum_brems=diag[1], lum_synch=diag[2], lum_compton=diag[3],
+                          n_limited=int(diag[4]), n_floored=int(diag[5]), n_clamped=int(diag[6])))
+
+
+def implicit_residual(table: Table, un: Units, rho, bsq, theta_e, theta_i, dt, theta_trial, nsub=1, h_floor=0.0, r=0.0,
+                      coulomb_mode=None):
+    """F(theta_trial) of the first implicit sub-step of one cell (0 at a root)."""
+    if coulomb_mode is None:
+        coulomb_mode = COULOMB_TABLE if table.coul is not None else COULOMB_ANALYTIC
+    return lib().orc_implicit_residual(C.byref(table._c), C.byref(un), float(rho), float(bsq), float(theta_e), float(theta_i),
+                                       float(r), float(dt), int(nsub), float(h_floor), int(coulomb_mode), float(theta_trial))

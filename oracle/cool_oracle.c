@@ -516,6 +516,178 @@ void orc_step(const orc_table *tab, const orc_units *un, long long ncell,
     if (diag7) memcpy(diag7, acc, sizeof acc);
 }
 
+/* ================================================================================
+ * Part B'  the implicit scheme (PAPER.md L185 (ii): "an implicit solver for the cooling
+ * step ... adapted [from] the implicit-explicit (IMEX) solver ... used in the M1
+ * radiation scheme"; L369: ~1.8x the cost).  The paper gives no equations; this is
+ * reading C-18 of DESIGN.md, step by step:
+ *
+ *   per sub-step h = dt/nsub, from the start state (Theta_e, Theta_i):
+ *     a   = h K C(Theta_e, Theta_i),  K C (Theta_i - Theta_e) = dTheta_e/dt of eq 15;
+ *           the coefficient C is taken at the start state (the explicit half of IMEX),
+ *           the driving difference at the end state (linearly implicit):
+ *             x = a (Theta_i' - theta),  Theta_i' = Theta_i - g x,  g = (gamma_i-1)/(gamma_e-1)
+ *           =>  x = a (Theta_i - theta) / (1 + a g)
+ *     rhat(theta) = Lambda(rho, theta_c, bsq, Theta_i) (gamma_e-1) / (m_e/m_p rho theta_c),
+ *           theta_c = theta clamped to the table's Theta_e range: outside the range the
+ *           cooling TIME u_e/Lambda is held at its edge value (this is what makes the
+ *           root positive); Theta_i inside Lambda (4-D tables, through H) is the start
+ *           value; the floor test (eq 19) is taken at the start state
+ *     backward Euler for the radiative sink:  theta is the root of
+ *       F(theta) = theta - Theta_e + h theta rhat(theta) - a (Theta_i - theta)/(1 + a g)
+ *     in (0, Theta_e + a Theta_i/(1 + a g)]  (F(0) < 0 <= F(upper end)), found by bisection
+ *     Theta_e' = theta,  Theta_i' = Theta_i - g x(theta);  no limiter.
+ *   diagnostic: dE = h Lambda at the end state (= h theta rhat(theta) in Theta units).
+ *
+ * Pins (tests/test_oracle_implicit.py): residual of the root, dt -> 0 agrees with the
+ * unlimited explicit step, closed form for a constant cooling time (theta' = theta/(1+h/t_c)),
+ * Coulomb-only closed form (linear 2x2 backward Euler), positivity for h Lambda >> u_e,
+ * energy balance, no temperature crossing, zero exchange at equality.
+ * ============================================================================== */
+typedef struct {
+    const orc_table *tab; const orc_units *un;
+    double rho, bsq, the0, thi0, h, a, g, floored;
+} orc_imp_ctx;
+
+/* rhat(theta) * h * theta: the radiative loss of Theta_e over h at trial state theta;
+ * lam_out/frac/cl (optional) return Lambda (code units), process shares, clamp flag. */
+static double orc_imp_loss(const orc_imp_ctx *c, double theta, double *lam_out, double *frac, int *cl_out)
+{
+    const orc_table *tab = c->tab;
+    const double mr = ORC_ME / ORC_MP, ge1 = c->un->gamma_e - 1.0;
+    if (lam_out) *lam_out = 0.0;
+    if (frac) { frac[0] = frac[1] = frac[2] = 0.0; }
+    if (cl_out) *cl_out = 0;
+    if (c->floored != 0.0 || !(theta > 0.0)) return 0.0;
+    /* Theta_e range of the table */
+    double tlo = 0.0, thi_edge = INFINITY;
+    for (int k = 0; k < tab->ndim; ++k)
+        if (tab->axis[k] == ORC_AX_LOG_THETA_E) { tlo = pow(10.0, tab->lo[k]); thi_edge = pow(10.0, tab->hi[k]); }
+    double thc = theta < tlo ? tlo : (theta > thi_edge ? thi_edge : theta);
+    double prim[4], x[4]; int cl = 0;
+    prim[ORC_AX_LOG_RHO] = c->rho; prim[ORC_AX_LOG_THETA_E] = thc;
+    prim[ORC_AX_LOG_BSQ] = c->bsq; prim[ORC_AX_LOG_THETA_I] = c->thi0;
+    for (int k = 0; k < tab->ndim; ++k) {
+        double q = prim[tab->axis[k]];
+        x[k] = (q > 0.0) ? log10(q) : -INFINITY;
+    }
+    double lam;
+    if (tab->nproc == 1) {
+        lam = pow(10.0, orc_interp(tab->ndim, tab->n, tab->lo, tab->hi, tab->data[0], x, &cl));
+    } else {
+        double q[3];
+        for (int p = 0; p < 3; ++p)
+            q[p] = pow(10.0, orc_interp(tab->ndim, tab->n, tab->lo, tab->hi, tab->data[p], x, &cl));
+        lam = orc_combine_code(c->un, c->rho, thc, c->thi0, q[0], q[1], q[2], frac);
+    }
+    if (theta != thc) cl = 1;
+    if (cl_out) *cl_out = cl;
+    double rhat = lam * ge1 / (mr * c->rho * thc);
+    if (lam_out) *lam_out = rhat * theta * mr * c->rho / ge1;      /* Lambda at the trial state */
+    return c->h * theta * rhat;
+}
+static double orc_imp_F(const orc_imp_ctx *c, double theta)
+{
+    return theta - c->the0 + orc_imp_loss(c, theta, NULL, NULL, NULL) - c->a * (c->thi0 - theta) / (1.0 + c->a * c->g);
+}
+
+static void orc_imp_setup(orc_imp_ctx *c, const orc_table *tab, const orc_units *un, double rho, double bsq,
+                          double the, double thi, double r, double h, double h_floor, int coulomb_mode)
+{
+    const double mr = ORC_ME / ORC_MP, ge1 = un->gamma_e - 1.0, gi1 = un->gamma_i - 1.0;
+    c->tab = tab; c->un = un; c->rho = rho; c->bsq = bsq; c->the0 = the; c->thi0 = thi; c->h = h; c->g = gi1 / ge1;
+    c->floored = 0.0;
+    if (h_floor > 0.0 && r > 0.0) {
+        double tfloor = 0.5 * ORC_PI * pow(h_floor * orc_omega_k(r, un->spin) * r, 2.0);
+        if ((the + thi) * mr < tfloor) c->floored = 1.0;
+    }
+    double C = 0.0;
+    if (coulomb_mode == 1) {
+        double xc[2] = { thi > 0.0 ? log10(thi) : -INFINITY, the > 0.0 ? log10(the) : -INFINITY };
+        C = pow(10.0, orc_interp(2, tab->nc, tab->clo, tab->chi, tab->coul, xc, NULL));
+    } else if (coulomb_mode == 2) {
+        C = orc_coulomb_C(the, thi / un->ion_theta_mass_ratio);
+    }
+    /* dTheta_e/dt = K C (Theta_i - Theta_e),  K = pref conv rho (gamma_e-1)/(m_e/m_p) */
+    c->a = h * orc_coulomb_pref_cgs(un) * orc_rate_conv(un) * rho * C * ge1 / mr;
+}
+
+/* F(theta) of the FIRST sub-step for one cell: lets a test check that a result which differs from the
+ * oracle's root is still a root (several roots can exist where Lambda is not monotone in Theta_e). */
+double orc_implicit_residual(const orc_table *tab, const orc_units *un, double rho, double bsq, double the, double thi,
+                             double r, double dt, int nsub, double h_floor, int coulomb_mode, double theta_trial)
+{
+    orc_imp_ctx c;
+    orc_imp_setup(&c, tab, un, rho, bsq, the, thi, r, dt / nsub, h_floor, coulomb_mode);
+    return orc_imp_F(&c, theta_trial);
+}
+
+static void orc_step_cell_implicit(const orc_table *tab, const orc_units *un,
+                                   double rho, double bsq, double *the_io, double *thi_io,
+                                   double r, double vol, double dt, int nsub, double h_floor, int coulomb_mode, double *diag7)
+{
+    const double mr = ORC_ME / ORC_MP, ge1 = un->gamma_e - 1.0;
+    const double h = dt / nsub;
+    double the = *the_io, thi = *thi_io;
+    double de_sum[4] = {0, 0, 0, 0};
+    int floored = 0, clamped = 0;
+    for (int s = 0; s < nsub; ++s) {
+        orc_imp_ctx c;
+        orc_imp_setup(&c, tab, un, rho, bsq, the, thi, r, h, h_floor, coulomb_mode);
+        if (c.floored != 0.0) floored = 1;
+        double lo = 0.0, hi = the + c.a * thi / (1.0 + c.a * c.g);
+        if (!(hi > 0.0)) {              /* Theta_e = 0 and nothing to gain: nothing to do */
+            continue;
+        }
+        for (int it = 0; it < 200; ++it) {
+            double m = 0.5 * (lo + hi);
+            if (m == lo || m == hi) break;
+            if (orc_imp_F(&c, m) < 0.0) lo = m; else hi = m;
+        }
+        double theta = hi;                                  /* F(hi) >= 0: the first representable point at or past the root */
+        double lam, frac[3]; int cl;
+        double loss = orc_imp_loss(&c, theta, &lam, frac, &cl);
+        (void)loss;
+        clamped |= cl;
+        double x = c.a * (thi - theta) / (1.0 + c.a * c.g);
+        double de = lam * h;                                /* energy radiated, code units */
+        de_sum[0] += de; de_sum[1] += de * frac[0]; de_sum[2] += de * frac[1]; de_sum[3] += de * frac[2];
+        the = theta;
+        thi = thi - c.g * x;
+    }
+    (void)mr; (void)ge1;
+    *the_io = the; *thi_io = thi;
+    for (int k = 0; k < 4; ++k) diag7[k] = de_sum[k] * vol / dt;
+    diag7[4] = 0.0; diag7[5] = floored; diag7[6] = clamped;
+}
+
+/* Whole field, implicit scheme.  r, vol may be NULL.  diag7 is the sum over cells. */
+void orc_step_implicit(const orc_table *tab, const orc_units *un, long long ncell,
+                       const double *rho, const double *bsq, const double *the_in, const double *thi_in,
+                       const double *r, const double *vol, double dt, int nsub, double h_floor, int coulomb_mode,
+                       double *the_out, double *thi_out, double *diag7, int nthreads)
+{
+    double acc[7] = {0, 0, 0, 0, 0, 0, 0};
+    if (nthreads < 1) nthreads = 1;
+#pragma omp parallel num_threads(nthreads)
+    {
+        double loc[7] = {0, 0, 0, 0, 0, 0, 0};
+#pragma omp for schedule(dynamic, 256)
+        for (long long c = 0; c < ncell; ++c) {
+            double the = the_in[c], thi = thi_in[c], d7[7];
+            if (isnan(rho[c]) || isnan(bsq[c]) || isnan(the) || isnan(thi)) { the_out[c] = NAN; thi_out[c] = NAN; continue; }
+            if (!(rho[c] > 0.0)) { the_out[c] = the; thi_out[c] = thi; continue; }
+            orc_step_cell_implicit(tab, un, rho[c], bsq[c], &the, &thi, r ? r[c] : 0.0, vol ? vol[c] : 1.0,
+                                   dt, nsub, h_floor, coulomb_mode, d7);
+            the_out[c] = the; thi_out[c] = thi;
+            for (int k = 0; k < 7; ++k) loc[k] += d7[k];
+        }
+#pragma omp critical
+        for (int k = 0; k < 7; ++k) acc[k] += loc[k];
+    }
+    if (diag7) memcpy(diag7, acc, sizeof acc);
+}
+
 /* Fill tables node by node from Part A (used by tests to check the product's builder
  * and to build tiny brute-force tables).  Node coordinate = lo + i*(hi-lo)/(n-1). */
 void orc_fill_total3(const orc_units *un, const int *n, const double *lo, const double *hi, float *out, int nthreads)
