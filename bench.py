@@ -104,7 +104,7 @@ def peaks():
 # ------------------------------------------------------------------------------------------------
 # oracle legs (cpu_baseline and --impl reference): the only places bench.py touches oracle/
 # ------------------------------------------------------------------------------------------------
-def oracle_leg(spec, desc, data, coul, fields, sample_cells, steps=1):
+def oracle_leg(spec, desc, data, coul, fields, sample_cells, steps=1, scheme="explicit"):
     import oracle as O
     O.build()
     nd = desc.ndim
@@ -120,9 +120,10 @@ def oracle_leg(spec, desc, data, coul, fields, sample_cells, steps=1):
     times = []
     for _ in range(steps):
         t0 = time.perf_counter()
-        O.step(otab, un, fields["rho"][sl], fields["bsq"][sl], fields["theta_e"][sl], fields["theta_i"][sl], spec["dt"],
-               nsub=spec["nsub"], h_floor=spec.get("floor", 0.0), r=fields["r"][sl] if spec.get("floor") else None,
-               vol=fields["vol"][sl] if spec.get("vol") else None, nthreads=cores)
+        step = O.step_implicit if scheme == "implicit" else O.step
+        step(otab, un, fields["rho"][sl], fields["bsq"][sl], fields["theta_e"][sl], fields["theta_i"][sl], spec["dt"],
+             nsub=spec["nsub"], h_floor=spec.get("floor", 0.0), r=fields["r"][sl] if spec.get("floor") else None,
+             vol=fields["vol"][sl] if spec.get("vol") else None, nthreads=cores)
         times.append(time.perf_counter() - t0)
     return m, cores, times
 
@@ -175,6 +176,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="c5")
     ap.add_argument("--variant", default="auto")
+    ap.add_argument("--scheme", default="explicit", choices=["explicit", "implicit"], help="PAPER.md L185: (i) limiter or (ii) implicit solver")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-also", action="store_true", help="skip the companion s512 measurement of the default workload")
@@ -205,8 +207,8 @@ def main():
         fields = make_fields(small)
         sample = min(fields["rho"].size, 1 << 22)
         for _ in range(min(args.warmup, 1)):
-            oracle_leg(spec, desc, data, coul, fields, sample, 1)
-        m, cores, times = oracle_leg(spec, desc, data, coul, fields, sample, args.steps)
+            oracle_leg(spec, desc, data, coul, fields, sample, 1, args.scheme)
+        m, cores, times = oracle_leg(spec, desc, data, coul, fields, sample, args.steps, args.scheme)
         tot = float(np.sum(times))
         val = m * args.steps / tot / 1e9
         line = dict(metric=METRIC, value=val, unit=UNIT, n_gpus=args.gpus, steps=args.steps, warmup=args.warmup,
@@ -245,7 +247,8 @@ def main():
     the_o = torch.empty(ncell, dtype=torch.float32, device=dev)
     thi_o = torch.empty(ncell, dtype=torch.float32, device=dev)
     d_diag = torch.zeros(api.DIAG_BYTES, dtype=torch.uint8, device=dev) if spec["diag"] else None
-    params = api.make_params(spec["dt"], spec["nsub"], 0.3, spec.get("floor", 0.0), variant, api.COOL_COULOMB_TABLE)
+    scheme = api.COOL_SCHEME_IMPLICIT if args.scheme == "implicit" else api.COOL_SCHEME_EXPLICIT
+    params = api.make_params(spec["dt"], spec["nsub"], 0.3, spec.get("floor", 0.0), variant, api.COOL_COULOMB_TABLE, scheme)
     stream = torch.cuda.current_stream().cuda_stream
 
     def step():
@@ -288,7 +291,7 @@ def main():
 
     # ---- companion line: the single-update 3-D step (table 128^3) on the same 512^3 field, same timing protocol ----
     also = None
-    if args.workload == "c5" and args.variant == "auto" and not args.no_also:
+    if args.workload == "c5" and args.variant == "auto" and not args.no_also and args.scheme == "explicit":
         spec2 = workload_spec("s512")
         axis2, lo2, hi2 = table_ranges(spec2["n"])
         desc2 = api.make_desc(axis2, spec2["n"], lo2, hi2, 1, nc=spec2["nc"], clo=[synth.LOG_THETA[0]] * 2, chi=[synth.LOG_THETA[1]] * 2)
@@ -363,23 +366,24 @@ def main():
     single = mode == 3 and spec["nsub"] == 1
     fetch = {"global": "F32GlobalQ" if (mode == 3 and np.prod(spec["n"]) * 16 <= (64 << 20)) else "F32Global", "smem": "F32Smem",
              "tex_point": "F32TexPoint", "tex_hwfilter": "F32TexHw"}.get(api.VARIANT_NAMES[resolved], api.VARIANT_NAMES[resolved])
-    kernel_name = "cool_f32_kernel<MODE=%d, %s, DIAG=%d, CM=1, NSUB1=%d, %s>" % (
+    explicit = args.scheme == "explicit"
+    kernel_name = ("cool_implicit_kernel<float, MODE=%d, %s>" % (mode, api.VARIANT_NAMES[resolved])) if not explicit else "cool_f32_kernel<MODE=%d, %s, DIAG=%d, CM=1, NSUB1=%d, %s>" % (
         mode, fetch, int(bool(spec["diag"])), int(spec["nsub"] == 1),
         "384 threads, 2 stages" if fetch == "F32Smem" else ("768 threads, 2 stages" if single else "512 threads, 3 stages"))
     line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=args.warmup,
                 ms_per_step=total_ms / args.steps, higher_is_better=True, scaling="weak", vs_baseline=None,
-                dtype="f32", data="synthetic",
+                dtype="f32" if explicit else "f64", data="synthetic",
                 config=dict(workload=args.workload, description=spec["label"], cells_per_gpu=ncell, nsub=spec["nsub"],
-                            variant=api.VARIANT_NAMES[resolved], l2="inputs (%.2f GB per step) larger than L2" % (bpc * ncell / 1e9),
+                            variant=api.VARIANT_NAMES[resolved], scheme=args.scheme, l2="inputs (%.2f GB per step) larger than L2" % (bpc * ncell / 1e9),
                             cell_substeps_per_s=value * spec["nsub"] * 1e9),
                 hbm_gbs=achieved * world, frac_of_8TBs=achieved / SPEC_HBM_GBS,
                 clocks=clocks, e2e=e2e, gpu_launches=launches_per_step * args.steps,
                 roofline=dict(bound="hbm", achieved=achieved, peak=peak, unit="GB/s", frac=achieved / peak,
-                              traffic=(NCU_TRAFFIC_GB[args.workload] * 1e9 if args.workload in NCU_TRAFFIC_GB and args.variant == "auto" else None),
+                              traffic=(NCU_TRAFFIC_GB[args.workload] * 1e9 if args.workload in NCU_TRAFFIC_GB and args.variant == "auto" and explicit else None),
                               kernel=kernel_name, bytes_per_cell=bpc, algorithmic_bytes_per_launch=bpc * ncell, peak_source=peak_src,
                               ms_per_launch_median=float(np.median(per_step_ms)), ms_per_launch_best=float(per_step_ms.min())),
                 diag=diag_out)
-    if args.workload in NCU_WARP_INST and args.variant == "auto":
+    if args.workload in NCU_WARP_INST and args.variant == "auto" and explicit:
         gw = NCU_WARP_INST[args.workload] / (kern_ms * 1e-3) / 1e9
         line["issue_roofline"] = dict(bound="alu", achieved=gw, peak=ISSUE_PEAK_GWINST, unit="G warp-instructions/s", frac=gw / ISSUE_PEAK_GWINST,
                                       warp_inst_per_launch=NCU_WARP_INST[args.workload],
@@ -387,7 +391,7 @@ def main():
     if also is not None:
         line["also"] = also
     if not args.no_cpu_baseline:
-        m, cores, times = oracle_leg(spec, desc, data, coul, fields, args.cpu_sample, 1)
+        m, cores, times = oracle_leg(spec, desc, data, coul, fields, args.cpu_sample if explicit else min(args.cpu_sample, 1 << 23), 1, args.scheme)
         line["cpu_baseline"] = dict(value=m / times[0] / 1e9, unit=UNIT, cores=cores, kind="oracle",
                                     sample=f"{m} contiguous cells from the middle of the workload, one pass, {times[0]:.1f} s")
     print(json.dumps(line))

@@ -55,6 +55,15 @@ typedef enum {
 typedef enum { COOL_COULOMB_AUTO = 0, /* coefficient table if the cool_table has one, else analytic */
                COOL_COULOMB_OFF = 1, COOL_COULOMB_TABLE = 2, COOL_COULOMB_ANALYTIC = 3 } cool_coulomb_mode;
 
+/* Time integration of the radiative sink: (i) explicit with the 30 % limiter, or (ii) implicit.
+ * The paper gives no equations for (ii); the implicit scheme here is backward Euler per sub-step (reading
+ * C-18): Theta_e' solves  th - Theta_e + h th Lambda(th_c)/u_e(th_c) - q (Theta_i - th) = 0  with th_c = th clamped to
+ * the table's Theta_e range, q = a/(1 + a g), a = h K C(Theta_e, Theta_i) (Coulomb coefficient at the start state,
+ * driving difference at the end state), Theta_i' = Theta_i - g q (Theta_i - Theta_e').  No limiter (f_limit is
+ * ignored); always positive.  fp64 arithmetic for either cell dtype.  Variants: GLOBAL, SMEM, TEX_POINT (AUTO picks);
+ * TEX_HWFILTER and ANALYTIC return COOL_EUNSUPPORTED. */
+typedef enum { COOL_SCHEME_EXPLICIT = 0, COOL_SCHEME_IMPLICIT = 1 } cool_scheme;
+
 /* Unit system and fixed parameters of the physics (Table I). */
 typedef struct {
     double rho_scale_cgs;        /* g cm^-3 per code density unit (Table I)                      */
@@ -112,6 +121,7 @@ typedef struct {
     double h_floor;              /* (H/R)_floor of eq 19; 0 = off; needs cells.r */
     cool_variant variant;
     cool_coulomb_mode coulomb;
+    cool_scheme scheme;          /* COOL_SCHEME_EXPLICIT (0) or COOL_SCHEME_IMPLICIT */
 } cool_params;
 
 /* Diagnostics of one call (sums over the cells of the call; overwritten, not accumulated).

@@ -22,6 +22,7 @@ COOL_F32, COOL_F64 = 0, 1
 COOL_AX_LOG_RHO, COOL_AX_LOG_THETA_E, COOL_AX_LOG_BSQ, COOL_AX_LOG_THETA_I = range(4)
 COOL_V_AUTO, COOL_V_TEX_POINT, COOL_V_TEX_HWFILTER, COOL_V_SMEM, COOL_V_GLOBAL, COOL_V_ANALYTIC = range(6)
 COOL_COULOMB_AUTO, COOL_COULOMB_OFF, COOL_COULOMB_TABLE, COOL_COULOMB_ANALYTIC = range(4)
+COOL_SCHEME_EXPLICIT, COOL_SCHEME_IMPLICIT = range(2)
 VARIANT_NAMES = {COOL_V_AUTO: "auto", COOL_V_TEX_POINT: "tex_point", COOL_V_TEX_HWFILTER: "tex_hwfilter",
                  COOL_V_SMEM: "smem", COOL_V_GLOBAL: "global", COOL_V_ANALYTIC: "analytic"}
 VARIANTS = {v: k for k, v in VARIANT_NAMES.items()}
@@ -56,7 +57,7 @@ class cool_cells(C.Structure):
 
 class cool_params(C.Structure):
     _fields_ = [("dt", C.c_double), ("nsub", C.c_int), ("f_limit", C.c_double), ("h_floor", C.c_double),
-                ("variant", C.c_int), ("coulomb", C.c_int)]
+                ("variant", C.c_int), ("coulomb", C.c_int), ("scheme", C.c_int)]
 
 
 class cool_diag(C.Structure):
@@ -208,8 +209,9 @@ def _cells(ncell, dtype, rho, bsq, theta_e_in, theta_i_in, theta_e_out, theta_i_
     return c
 
 
-def make_params(dt, nsub=1, f_limit=0.3, h_floor=0.0, variant=COOL_V_AUTO, coulomb=COOL_COULOMB_AUTO) -> cool_params:
-    return cool_params(float(dt), int(nsub), float(f_limit), float(h_floor), int(variant), int(coulomb))
+def make_params(dt, nsub=1, f_limit=0.3, h_floor=0.0, variant=COOL_V_AUTO, coulomb=COOL_COULOMB_AUTO,
+                scheme=COOL_SCHEME_EXPLICIT) -> cool_params:
+    return cool_params(float(dt), int(nsub), float(f_limit), float(h_floor), int(variant), int(coulomb), int(scheme))
 
 
 def cool_apply(table: CoolTable, ncell, dtype, rho, bsq, theta_e_in, theta_i_in, theta_e_out, theta_i_out,

@@ -157,6 +157,10 @@ static cool_status check_args(const cool_table *t, const cool_cells *c, const co
         case COOL_COULOMB_ANALYTIC: cm = 2; break;
         default: set_error("unknown coulomb mode"); return COOL_EINVAL;
     }
+    if (p->scheme != COOL_SCHEME_EXPLICIT && p->scheme != COOL_SCHEME_IMPLICIT) { set_error("unknown scheme"); return COOL_EINVAL; }
+    if (p->scheme == COOL_SCHEME_IMPLICIT && (vv == COOL_V_TEX_HWFILTER || vv == COOL_V_ANALYTIC)) {
+        set_error("variant unsupported: the implicit scheme runs on the GLOBAL, SMEM and TEX_POINT lookups"); return COOL_EUNSUPPORTED;
+    }
     *v = vv; *coul = cm;
     return COOL_OK;
 }
@@ -389,7 +393,7 @@ extern "C" cool_status cool_apply(const cool_table *t, const cool_cells *c, cons
     LaunchArgs a{};
     a.ncell = c->ncell; a.rho = c->rho; a.bsq = c->bsq; a.the_in = c->theta_e_in; a.thi_in = c->theta_i_in;
     a.r = c->r; a.vol = c->vol; a.the_out = c->theta_e_out; a.thi_out = c->theta_i_out;
-    a.dt = p->dt; a.nsub = p->nsub; a.f_limit = p->f_limit; a.h_floor = p->h_floor; a.coulomb = coul;
+    a.dt = p->dt; a.nsub = p->nsub; a.f_limit = p->f_limit; a.h_floor = p->h_floor; a.coulomb = coul; a.scheme = p->scheme;
     a.want_diag = d_diag != nullptr; a.d_diag = d_diag;
     if (d_diag) {
         DiagWorkspace w;
@@ -454,7 +458,7 @@ extern "C" cool_status cool_apply_host(const cool_table *t, const cool_cells *c,
         a.ncell = (long long)n; a.rho = sg.buf[0]; a.bsq = sg.buf[1]; a.the_in = sg.buf[2]; a.thi_in = sg.buf[3];
         a.r = c->r ? sg.buf[4] : nullptr; a.vol = c->vol ? sg.buf[5] : nullptr;
         a.the_out = sg.buf[6]; a.thi_out = sg.buf[7];
-        a.dt = p->dt; a.nsub = p->nsub; a.f_limit = p->f_limit; a.h_floor = p->h_floor; a.coulomb = coul;
+        a.dt = p->dt; a.nsub = p->nsub; a.f_limit = p->f_limit; a.h_floor = p->h_floor; a.coulomb = coul; a.scheme = p->scheme;
         a.want_diag = h_diag != nullptr; a.d_diag = h_diag ? sg.d_diag : nullptr;
         if (h_diag) {
             DiagWorkspace w;

@@ -77,6 +77,7 @@ struct LaunchArgs {
     void *the_out, *thi_out;
     double dt; int nsub; double f_limit, h_floor;
     int coulomb;                   // 0 off, 1 table, 2 analytic
+    int scheme;                    // 0 explicit, 1 implicit
     int want_diag;
     double *partials;              // [grid][8]
     unsigned *ticket;

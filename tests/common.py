@@ -49,7 +49,8 @@ def oracle_table(oracle, desc, data, coul):
 
 
 def gpu_step(table, fields, dtype, dt, nsub=1, f_limit=0.3, h_floor=0.0, variant=api.COOL_V_AUTO,
-             coulomb=api.COOL_COULOMB_AUTO, want_diag=True, use_r=False, use_vol=False, inplace=False, offset=0):
+             coulomb=api.COOL_COULOMB_AUTO, want_diag=True, use_r=False, use_vol=False, inplace=False, offset=0,
+             scheme=api.COOL_SCHEME_EXPLICIT):
     """One cool_apply on cuda:0 through the C ABI.  ``offset`` (elements) misaligns the arrays."""
     import torch
     tdt = torch.float32 if dtype == np.float32 else torch.float64
@@ -72,7 +73,7 @@ def gpu_step(table, fields, dtype, dt, nsub=1, f_limit=0.3, h_floor=0.0, variant
         the_o = torch.empty(n + offset, dtype=tdt, device=dev)[offset:]
         thi_o = torch.empty(n + offset, dtype=tdt, device=dev)[offset:]
     d_diag = torch.zeros(api.DIAG_BYTES, dtype=torch.uint8, device=dev) if want_diag else None
-    params = api.make_params(dt, nsub, f_limit, h_floor, variant, coulomb)
+    params = api.make_params(dt, nsub, f_limit, h_floor, variant, coulomb, scheme)
     stream = torch.cuda.current_stream().cuda_stream
     api.cool_apply(table, n, cdt, rho, bsq, the, thi, the_o, thi_o, params, r=r, vol=vol, d_diag=d_diag, stream=stream)
     torch.cuda.synchronize()
@@ -90,6 +91,12 @@ def oracle_step(oracle, otab, un, fields, dt, nsub=1, f_limit=0.3, h_floor=0.0, 
                        f_limit=f_limit, h_floor=h_floor, r=fields["r"] if use_r else None,
                        vol=fields["vol"] if use_vol else None, rate_mode=rate_mode, coulomb_mode=coulomb_mode,
                        nthreads=nthreads or oracle.max_threads())
+
+
+def oracle_step_implicit(oracle, otab, un, fields, dt, nsub=1, h_floor=0.0, use_r=False, use_vol=False, coulomb_mode=None, nthreads=0):
+    return oracle.step_implicit(otab, un, fields["rho"], fields["bsq"], fields["theta_e"], fields["theta_i"], dt, nsub=nsub,
+                                h_floor=h_floor, r=fields["r"] if use_r else None, vol=fields["vol"] if use_vol else None,
+                                coulomb_mode=coulomb_mode, nthreads=nthreads or oracle.max_threads())
 
 
 def rel_err(a, b):
