@@ -9,37 +9,51 @@
 //              Theta_e range (the cooling time is held outside the range, which keeps the root positive)
 //   theta    = root of  F(th) = th - Theta_e + loss(th) - q (Theta_i - th)  in (0, Theta_e + q Theta_i]
 //   Theta_e' = theta,  Theta_i' = Theta_i - g q (Theta_i - theta);  no limiter.
-// The root is bracketed from the start (F(0) < 0 <= F(upper end)) and refined by Illinois-type false position with a
-// bisection safeguard until the bracket is two ulps wide; F' >= 1 wherever the loss does not decrease with Theta_e, so
-// the answer is then within rounding of the root.
+// F(0) < 0 <= F(Theta_e + q Theta_i) always.  Inside one Theta_e interval of the table every channel is linear in the
+// interval coordinate once (rho, bsq[, Theta_i]) are contracted, so the solve is: (1) a binary search over the table's
+// Theta_e NODES for the interval that brackets the root (one contraction per probed node), (2) inside that interval,
+// Illinois-type false position with a bisection safeguard on values that need no further table access, until the bracket
+// is two ulps wide (outside the table range F is linear: closed form).  F' >= 1 wherever the loss does not decrease
+// with Theta_e, so the answer is within rounding of the root; where Lambda is not monotone several roots can exist
+// and any of them is a solution of the scheme.
 #pragma once
 #include "cool_kernels.cuh"
 
 namespace cool {
 
-struct ImpCell {            // what F needs, fixed over one sub-step
-    double rho, the0, thi0, q, tmin, tmax;
-    Loc64 lr, lb, li;
-    bool floored;
-};
-
-// loss(th) in Theta units; optionally the process shares of Q_thin and the clamp flag of the Theta_e coordinate
+// The (rho, bsq[, Theta_i]) contraction of the table at Theta_e node i: within one Theta_e interval every channel is
+// linear in the interval coordinate w, so a root solve needs the table only at the two nodes of the interval.
 template <int MODE, class Fetch>
-__device__ __forceinline__ double imp_loss(const DevTable &T, const StepConst &S, const Fetch &F, const ImpCell &c, double th,
-                                           double *frac, int *clamped)
+__device__ __forceinline__ void imp_node(const Fetch &F, const Loc64 &r, const Loc64 &b, const Loc64 &ii, int i, double (&y)[3])
 {
-    if (frac) { frac[0] = frac[1] = frac[2] = 0.0; }
-    if (clamped) *clamped = 0;
-    if (c.floored || !(th > 0.0)) return 0.0;
-    const double thc = fmin(fmax(th, c.tmin), c.tmax);
-    Loc64 le = locate64(T.ax[CAX_THE], thc);
-    if (clamped) *clamped = le.clamped | (thc != th);
+    y[0] = y[1] = y[2] = 0.0;
+    if constexpr (MODE == 3) {
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+            const int cr = c >> 1, cb = c & 1;
+            y[0] += (cr ? r.w : 1.0 - r.w) * (cb ? b.w : 1.0 - b.w) * (double)F.at1(r.i + cr, i, b.i + cb);
+        }
+    } else {
+#pragma unroll
+        for (int c = 0; c < 8; ++c) {
+            const int cr = c >> 2, ci = (c >> 1) & 1, cb = c & 1;
+            const double pw = (cr ? r.w : 1.0 - r.w) * (ci ? ii.w : 1.0 - ii.w) * (cb ? b.w : 1.0 - b.w);
+            const float4 v = F.at4(r.i + cr, i, ii.i + ci, b.i + cb);
+            y[0] += pw * v.x; y[1] += pw * v.y; y[2] += pw * v.z;
+        }
+    }
+}
+
+struct ImpStep { double rho, thi0, q, R; };      // fixed over one sub-step: R = Theta_e + q Theta_i
+
+// Radiative loss of Theta_e over h at trial state th, from the channel logs y at th_c (th clamped to the table range)
+template <int MODE>
+__device__ __forceinline__ double imp_loss_y(const StepConst &S, const ImpStep &c, double th, double thc, const double (&y)[3], double *frac)
+{
     double lam;
     if constexpr (MODE == 3) {
-        lam = exp10(interp3_f64(F, c.lr, le, c.lb));
+        lam = exp10(y[0]);
     } else {
-        double y[3];
-        interp4_f64(F, c.lr, le, c.li, c.lb, y);
         const double qbr = exp10(y[0]), qsy = exp10(y[1]), eta = exp10(y[2]);
         const double qthin = qbr + eta * qsy;                                               // eq 10
         const double cs2 = (S.ae * thc + S.ai * c.thi0) / (1.0 + S.be * thc + S.bi * c.thi0);   // eq 14
@@ -54,62 +68,98 @@ __device__ __forceinline__ double imp_loss(const DevTable &T, const StepConst &S
 }
 
 template <int MODE, class Fetch>
-__device__ __forceinline__ double imp_F(const DevTable &T, const StepConst &S, const Fetch &F, const ImpCell &c, double th)
-{
-    return (th - c.the0) + imp_loss<MODE>(T, S, F, c, th, nullptr, nullptr) - c.q * (c.thi0 - th);
-}
-
-template <int MODE, class Fetch>
 __device__ void implicit_cell(const DevTable &T, const DevConst &K, const StepConst &S, const Fetch &F,
                               double rho, double bsq, double &the, double &thi, double r, double vol, DiagAcc &acc)
 {
     if (isnan(rho) || isnan(bsq) || isnan(the) || isnan(thi)) { the = thi = __longlong_as_double(0x7ff8000000000000LL); return; }
     if (!(rho > 0.0)) return;
-    ImpCell c;
-    c.rho = rho;
-    c.lr = locate64(T.ax[CAX_RHO], rho); c.lb = locate64(T.ax[CAX_BSQ], bsq);
-    c.tmin = exp10(T.ax[CAX_THE].lo10); c.tmax = exp10(T.ax[CAX_THE].lo10 + (T.ax[CAX_THE].n - 1) / T.ax[CAX_THE].inv10);
+    const AxisCoef &ax = T.ax[CAX_THE];
+    const int n = ax.n;
+    const Loc64 lr = locate64(T.ax[CAX_RHO], rho), lb = locate64(T.ax[CAX_BSQ], bsq);
+    Loc64 li{0, 0.0, 0};
     const double g = S.gi1 / S.ge1;
-    int floored = 0, clamped = c.lr.clamped | c.lb.clamped;
+    int floored = 0, clamped = lr.clamped | lb.clamped;
     double de_sum[4] = {0, 0, 0, 0};
+    auto node_theta = [&](int i) { return exp10(ax.lo10 + (double)i / ax.inv10); };
     for (int s = 0; s < S.nsub; ++s) {
-        c.the0 = the; c.thi0 = thi;
-        c.floored = false;
+        bool flo = false;
         if (S.hfloor2 > 0.0 && r > 0.0) {
             const double ok = r / (r * sqrt(r) + S.spin);            // Omega_K r
-            if ((the + thi) * S.mr < S.hfloor2 * ok * ok) { c.floored = true; floored = 1; }
+            if ((the + thi) * S.mr < S.hfloor2 * ok * ok) { flo = true; floored = 1; }
         }
-        if constexpr (MODE == 4) { c.li = locate64(T.ax[CAX_THI], thi); clamped |= c.li.clamped; }
+        if constexpr (MODE == 4) { li = locate64(T.ax[CAX_THI], thi); clamped |= li.clamped; }
         double C = 0.0;
         if (S.coulomb == 1) C = coulomb_C_table64(T, the, thi);
         else if (S.coulomb == 2) C = coolphys::coulomb_C(the, thi / K.units.ion_theta_mass_ratio);
         const double a = S.coul_kh * rho * C;
-        c.q = a / (1.0 + a * g);
+        ImpStep c{rho, thi, a / (1.0 + a * g), 0.0};
+        c.R = the + c.q * thi;
+        if (!(c.R > 0.0)) continue;
+        const double opq = 1.0 + c.q;
 
-        double lo = 0.0, hi = the + c.q * thi;
-        if (!(hi > 0.0)) continue;
-        double flo = -hi, fhi = imp_F<MODE>(T, S, F, c, hi);         // F(0) = -Theta_e - q Theta_i
-        int side = 0;
-        for (int it = 0; it < 200 && fhi != 0.0; ++it) {
-            const double width = hi - lo;
-            if (!(width > 4.4408920985006262e-16 * hi)) break;       // two ulps
-            double m = hi - fhi * (width / (fhi - flo));
-            if (!(m > lo && m < hi) || (it % 3) == 2) m = lo + 0.5 * width;
-            if (m == lo || m == hi) break;
-            const double fm = imp_F<MODE>(T, S, F, c, m);
-            if (fm < 0.0) { lo = m; flo = fm; if (side == -1) fhi *= 0.5; side = -1; }
-            else { hi = m; fhi = fm; if (side == 1) flo *= 0.5; side = 1; }
+        double theta, de = 0.0, frac[3] = {0.0, 0.0, 0.0};
+        if (flo) {
+            theta = c.R / opq;                                       // no radiative sink this sub-step
+        } else {
+            // 1. the Theta_e interval that brackets the root: binary search over the nodes below R
+            //    (F(0) < 0 and F(th >= R) >= 0 always; index -1 stands for theta = 0, imax + 1 for min(node, R))
+            int imax = -1;
+            if (c.R > exp10(ax.lo10)) {
+                const double tR = (log10(c.R) - ax.lo10) * ax.inv10;
+                imax = tR >= (double)(n - 1) ? n - 1 : (int)tR;
+            }
+            int ilo = -1, ihi = imax + 1;
+            double ya[3] = {0, 0, 0}, yb[3] = {0, 0, 0};
+            bool have_b = false;
+            while (ihi - ilo > 1) {
+                const int m = (ilo + ihi) >> 1;
+                double ym[3];
+                imp_node<MODE>(F, lr, lb, li, m, ym);
+                const double tm = node_theta(m);
+                const double fm = tm * opq - c.R + imp_loss_y<MODE>(S, c, tm, tm, ym, nullptr);
+                if (fm < 0.0) { ilo = m; ya[0] = ym[0]; ya[1] = ym[1]; ya[2] = ym[2]; }
+                else { ihi = m; yb[0] = ym[0]; yb[1] = ym[1]; yb[2] = ym[2]; have_b = true; }
+            }
+            if (ilo == -1 || ilo == n - 1) {
+                // 2a. outside the table range the cooling time is held: F is linear, closed form
+                const int e = ilo == -1 ? 0 : n - 1;
+                double ye[3];
+                if (ilo == -1 && have_b && ihi == 0) { ye[0] = yb[0]; ye[1] = yb[1]; ye[2] = yb[2]; }
+                else if (ilo == n - 1) { ye[0] = ya[0]; ye[1] = ya[1]; ye[2] = ya[2]; }
+                else imp_node<MODE>(F, lr, lb, li, e, ye);
+                const double te = node_theta(e);
+                const double hr = imp_loss_y<MODE>(S, c, te, te, ye, frac) / te;      // h rhat at the edge
+                theta = c.R / (opq + hr);
+                de = theta * hr;
+                clamped |= (theta != te);
+            } else {
+                // 2b. inside interval ilo: channels linear in w; Illinois false position with a bisection safeguard
+                if (!(have_b && ihi == ilo + 1)) imp_node<MODE>(F, lr, lb, li, ilo + 1, yb);
+                const double dy[3] = {yb[0] - ya[0], yb[1] - ya[1], yb[2] - ya[2]};
+                auto Fseg = [&](double th, double *fr) {
+                    double w = (log10(th) - ax.lo10) * ax.inv10 - (double)ilo;
+                    w = fmin(fmax(w, 0.0), 1.0);
+                    const double y[3] = {ya[0] + w * dy[0], ya[1] + w * dy[1], ya[2] + w * dy[2]};
+                    return imp_loss_y<MODE>(S, c, th, th, y, fr);
+                };
+                double lo = node_theta(ilo), hi = fmin(node_theta(ilo + 1), c.R);
+                double flo_ = lo * opq - c.R + Fseg(lo, nullptr), fhi = hi * opq - c.R + Fseg(hi, nullptr);
+                if (!(flo_ < 0.0)) { hi = lo; fhi = 0.0; }           // rounding at the node: the node is the root
+                int side = 0;
+                for (int it = 0; it < 200 && fhi != 0.0; ++it) {
+                    const double width = hi - lo;
+                    if (!(width > 4.4408920985006262e-16 * hi)) break;       // two ulps
+                    double m = hi - fhi * (width / (fhi - flo_));
+                    if (!(m > lo && m < hi) || (it % 3) == 2) m = lo + 0.5 * width;
+                    if (m == lo || m == hi) break;
+                    const double fm = m * opq - c.R + Fseg(m, nullptr);
+                    if (fm < 0.0) { lo = m; flo_ = fm; if (side == -1) fhi *= 0.5; side = -1; }
+                    else { hi = m; fhi = fm; if (side == 1) flo_ *= 0.5; side = 1; }
+                }
+                theta = hi;
+                de = Fseg(theta, frac);
+            }
         }
-        // polish the last two ulps by bisection so that hi is the first representable point with F >= 0
-        for (int it = 0; it < 4; ++it) {
-            const double m = lo + 0.5 * (hi - lo);
-            if (m == lo || m == hi) break;
-            if (imp_F<MODE>(T, S, F, c, m) < 0.0) lo = m; else hi = m;
-        }
-        const double theta = hi;
-        double frac[3]; int cl;
-        const double de = imp_loss<MODE>(T, S, F, c, theta, frac, &cl);
-        clamped |= cl;
         de_sum[0] += de; de_sum[1] += de * frac[0]; de_sum[2] += de * frac[1]; de_sum[3] += de * frac[2];
         thi = thi - g * (c.q * (thi - theta));
         the = theta;
