@@ -106,9 +106,9 @@ def lib():
             "orc_interp": (d, [i, C.POINTER(i), C.POINTER(d), C.POINTER(d), C.POINTER(C.c_float),
                                C.POINTER(d), C.POINTER(i)]),
             "orc_step": (None, [C.POINTER(_Table), UP, C.c_longlong, p, p, p, p, p, p,
-                                d, i, d, d, i, i, p, p, p, p, p, i]),
+                                d, i, d, d, i, i, p, p, p, p, p, p, i]),
             "orc_step_implicit": (None, [C.POINTER(_Table), UP, C.c_longlong, p, p, p, p, p, p,
-                                         d, i, d, i, p, p, p, i]),
+                                         d, i, d, i, p, p, p, p, i]),
             "orc_implicit_residual": (d, [C.POINTER(_Table), UP, d, d, d, d, d, d, i, d, i, d]),
             "orc_fill_total3": (None, [UP, C.POINTER(i), C.POINTER(d), C.POINTER(d), p, i]),
             "orc_fill_coulomb2": (None, [UP, C.POINTER(i), C.POINTER(d), C.POINTER(d), p]),
@@ -208,7 +208,7 @@ COULOMB_OFF, COULOMB_TABLE, COULOMB_ANALYTIC = 0, 1, 2
 
 def step(table: Table, un: Units, rho, bsq, theta_e, theta_i, dt, nsub=1, f_limit=0.3,
          h_floor=0.0, r=None, vol=None, rate_mode=RATE_TABLE, coulomb_mode=None, nthreads=1,
-         want_rates=False):
+         want_rates=False, want_cell_lum=False):
     """Part B over a field.  Inputs are converted to float64 exactly (float32 inputs are
     representable).  Returns dict(theta_e, theta_i, diag[, lam0, qcc0])."""
     f64 = lambda a: None if a is None else np.ascontiguousarray(a, dtype=np.float64).ravel()
@@ -222,21 +222,24 @@ def step(table: Table, un: Units, rho, bsq, theta_e, theta_i, dt, nsub=1, f_limi
     lam0 = np.empty(n) if want_rates else None
     qcc0 = np.empty(n) if want_rates else None
     diag = np.zeros(7)
+    cell_lum = np.zeros((n, 4)) if want_cell_lum else None
     ptr = lambda a: None if a is None else a.ctypes.data
     lib().orc_step(C.byref(table._c), C.byref(un), n, ptr(rho), ptr(bsq), ptr(the), ptr(thi),
                    ptr(r), ptr(vol), float(dt), int(nsub), float(f_limit), float(h_floor),
                    int(rate_mode), int(coulomb_mode), ptr(the_o), ptr(thi_o), ptr(lam0), ptr(qcc0),
-                   ptr(diag), int(nthreads))
+                   ptr(cell_lum), ptr(diag), int(nthreads))
     out = dict(theta_e=the_o, theta_i=thi_o,
                diag=dict(lum_total=diag[0], lum_brems=diag[1], lum_synch=diag[2], lum_compton=diag[3],
                          n_limited=int(diag[4]), n_floored=int(diag[5]), n_clamped=int(diag[6])))
     if want_rates:
         out["lam0"] = lam0; out["qcc0"] = qcc0
+    if want_cell_lum:
+        out["cell_lum"] = cell_lum
     return out
 
 
 def step_implicit(table: Table, un: Units, rho, bsq, theta_e, theta_i, dt, nsub=1, h_floor=0.0, r=None, vol=None,
-                  coulomb_mode=None, nthreads=1):
+                  coulomb_mode=None, nthreads=1, want_cell_lum=False):
     """Part B' (implicit scheme, PAPER.md L185 (ii), reading C-18) over a field.  Returns dict(theta_e, theta_i, diag)."""
     f64 = lambda a: None if a is None else np.ascontiguousarray(a, dtype=np.float64).ravel()
     rho, bsq, the, thi, r, vol = map(f64, (rho, bsq, theta_e, theta_i, r, vol))
@@ -245,12 +248,25 @@ def step_implicit(table: Table, un: Units, rho, bsq, theta_e, theta_i, dt, nsub=
         coulomb_mode = COULOMB_TABLE if table.coul is not None else COULOMB_ANALYTIC
     the_o = np.empty(n); thi_o = np.empty(n)
     diag = np.zeros(7)
+    cell_lum = np.zeros((n, 4)) if want_cell_lum else None
     ptr = lambda a: None if a is None else a.ctypes.data
     lib().orc_step_implicit(C.byref(table._c), C.byref(un), n, ptr(rho), ptr(bsq), ptr(the), ptr(thi), ptr(r), ptr(vol),
-                            float(dt), int(nsub), float(h_floor), int(coulomb_mode), ptr(the_o), ptr(thi_o), ptr(diag), int(nthreads))
-    return dict(theta_e=the_o, theta_i=thi_o,
-                diag=dict(lum_total=diag[0], lum_brems=diag[1], lum_synch=diag[2], lum_compton=diag[3],
-                          n_limited=int(diag[4]), n_floored=int(diag[5]), n_clamped=int(diag[6])))
+                            float(dt), int(nsub), float(h_floor), int(coulomb_mode), ptr(the_o), ptr(thi_o), ptr(cell_lum),
+                            ptr(diag), int(nthreads))
+    out = dict(theta_e=the_o, theta_i=thi_o,
+               diag=dict(lum_total=diag[0], lum_brems=diag[1], lum_synch=diag[2], lum_compton=diag[3],
+                         n_limited=int(diag[4]), n_floored=int(diag[5]), n_clamped=int(diag[6])))
+    if want_cell_lum:
+        out["cell_lum"] = cell_lum
+    return out
+
+
+def shell_sums(cell_lum, shell_cells):
+    """Radial luminosity profile (eq 25, numerator): partial sums of the per-cell terms over consecutive groups of
+    ``shell_cells`` cells (one radial shell = all (theta, phi) cells of one r index; phi fastest)."""
+    n = cell_lum.shape[0]
+    starts = np.arange(0, n, int(shell_cells))
+    return np.add.reduceat(cell_lum, starts, axis=0)
 
 
 def implicit_residual(table: Table, un: Units, rho, bsq, theta_e, theta_i, dt, theta_trial, nsub=1, h_floor=0.0, r=0.0,

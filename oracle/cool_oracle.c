@@ -477,12 +477,13 @@ static void orc_step_cell(const orc_table *tab, const orc_units *un,
     diag7[4] = limited; diag7[5] = floored; diag7[6] = clamped;
 }
 
-/* Whole field.  r, vol, lam0, qcc0 may be NULL.  diag7 is the sum over cells. */
+/* Whole field.  r, vol, lam0, qcc0, cell_lum may be NULL.  diag7 is the sum over cells; cell_lum[c][0..3] is cell c's
+ * own term of the luminosity sums (eq 22), from which radial profiles (eq 25) are plain partial sums. */
 void orc_step(const orc_table *tab, const orc_units *un, long long ncell,
               const double *rho, const double *bsq, const double *the_in, const double *thi_in,
               const double *r, const double *vol,
               double dt, int nsub, double f_limit, double h_floor, int rate_mode, int coulomb_mode,
-              double *the_out, double *thi_out, double *lam0, double *qcc0, double *diag7, int nthreads)
+              double *the_out, double *thi_out, double *lam0, double *qcc0, double *cell_lum, double *diag7, int nthreads)
 {
     double acc[7] = {0, 0, 0, 0, 0, 0, 0};
     if (nthreads < 1) nthreads = 1;
@@ -492,6 +493,7 @@ void orc_step(const orc_table *tab, const orc_units *un, long long ncell,
 #pragma omp for schedule(static)
         for (long long c = 0; c < ncell; ++c) {
             double the = the_in[c], thi = thi_in[c], d7[7];
+            if (cell_lum) for (int k = 0; k < 4; ++k) cell_lum[4 * c + k] = 0.0;
             if (isnan(rho[c]) || isnan(bsq[c]) || isnan(the) || isnan(thi)) {
                 the_out[c] = NAN; thi_out[c] = NAN;
                 if (lam0) lam0[c] = NAN;
@@ -508,6 +510,7 @@ void orc_step(const orc_table *tab, const orc_units *un, long long ncell,
                           dt, nsub, f_limit, h_floor, rate_mode, coulomb_mode,
                           lam0 ? &lam0[c] : NULL, qcc0 ? &qcc0[c] : NULL, d7);
             the_out[c] = the; thi_out[c] = thi;
+            if (cell_lum) for (int k = 0; k < 4; ++k) cell_lum[4 * c + k] = d7[k];
             for (int k = 0; k < 7; ++k) loc[k] += d7[k];
         }
 #pragma omp critical
@@ -665,7 +668,7 @@ static void orc_step_cell_implicit(const orc_table *tab, const orc_units *un,
 void orc_step_implicit(const orc_table *tab, const orc_units *un, long long ncell,
                        const double *rho, const double *bsq, const double *the_in, const double *thi_in,
                        const double *r, const double *vol, double dt, int nsub, double h_floor, int coulomb_mode,
-                       double *the_out, double *thi_out, double *diag7, int nthreads)
+                       double *the_out, double *thi_out, double *cell_lum, double *diag7, int nthreads)
 {
     double acc[7] = {0, 0, 0, 0, 0, 0, 0};
     if (nthreads < 1) nthreads = 1;
@@ -675,11 +678,13 @@ void orc_step_implicit(const orc_table *tab, const orc_units *un, long long ncel
 #pragma omp for schedule(dynamic, 256)
         for (long long c = 0; c < ncell; ++c) {
             double the = the_in[c], thi = thi_in[c], d7[7];
+            if (cell_lum) for (int k = 0; k < 4; ++k) cell_lum[4 * c + k] = 0.0;
             if (isnan(rho[c]) || isnan(bsq[c]) || isnan(the) || isnan(thi)) { the_out[c] = NAN; thi_out[c] = NAN; continue; }
             if (!(rho[c] > 0.0)) { the_out[c] = the; thi_out[c] = thi; continue; }
             orc_step_cell_implicit(tab, un, rho[c], bsq[c], &the, &thi, r ? r[c] : 0.0, vol ? vol[c] : 1.0,
                                    dt, nsub, h_floor, coulomb_mode, d7);
             the_out[c] = the; thi_out[c] = thi;
+            if (cell_lum) for (int k = 0; k < 4; ++k) cell_lum[4 * c + k] = d7[k];
             for (int k = 0; k < 7; ++k) loc[k] += d7[k];
         }
 #pragma omp critical

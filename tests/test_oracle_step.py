@@ -294,3 +294,32 @@ def test_process_tables_and_luminosity_split(oracle):
     d = a["diag"]
     assert d["lum_brems"] + d["lum_synch"] + d["lum_compton"] == pytest.approx(d["lum_total"], rel=1e-12)
     assert d["lum_brems"] > 0 and d["lum_synch"] > 0 and d["lum_compton"] >= 0
+
+
+def test_cell_luminosity_terms_and_shell_sums(oracle):
+    """Per-cell terms of eq 22 (L222) and their shell sums (eq 25): each cell's term equals the energy it lost
+    (energy leaves only through radiation), the terms add up to the whole-field diagnostic, the per-process terms add up
+    to the total, and shell sums are partial sums."""
+    un = oracle.Units()
+    rng = np.random.default_rng(31)
+    n = [4, 5, 3, 4]
+    data = [rng.uniform(-12.0, -7.0, size=n).astype(np.float32), rng.uniform(-12.0, -7.0, size=n).astype(np.float32),
+            rng.uniform(0.0, 1.0, size=n).astype(np.float32)]
+    tab = oracle.Table(AX4, n, [-6.0, -3.0, -8.0, -3.0], [0.0, 1.5, 0.0, 1.5], data,
+                       coul=np.zeros((3, 3), np.float32), clo=[-3.0, -3.0], chi=[1.5, 1.5])
+    rho, bsq, the, thi = _cells(1200, seed=32)
+    vol = rng.uniform(0.5, 2.0, rho.size)
+    dt = 7.0
+    for fn, kw in ((oracle.step, dict(nsub=3)), (oracle.step_implicit, dict(nsub=2))):
+        o = fn(tab, un, rho, bsq, the, thi, dt, vol=vol, want_cell_lum=True, **kw)
+        cl = o["cell_lum"]
+        lost = (_u(rho, the) + _u(rho, thi)) - (_u(rho, o["theta_e"]) + _u(rho, o["theta_i"]))
+        assert cl[:, 0] == pytest.approx(lost * vol / dt, rel=1e-9, abs=1e-14 * float((lost * vol / dt).max()))
+        assert cl[:, 1:].sum(axis=1) == pytest.approx(cl[:, 0], rel=1e-12)
+        assert (cl >= 0).all() and (cl[:, 0] > 0).sum() > 1000
+        d = o["diag"]
+        assert cl.sum(axis=0) == pytest.approx([d["lum_total"], d["lum_brems"], d["lum_synch"], d["lum_compton"]], rel=1e-12)
+        sh = oracle.shell_sums(cl, 256)
+        assert sh.shape == (5, 4)
+        assert sh[2] == pytest.approx(cl[512:768].sum(axis=0), rel=1e-13)
+        assert sh[4] == pytest.approx(cl[1024:].sum(axis=0), rel=1e-13)          # ragged last shell
