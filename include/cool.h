@@ -112,6 +112,15 @@ typedef struct {
     void *theta_e_out, *theta_i_out;
     const void *r;                             /* optional radius [r_g] per cell; NULL: no floor */
     const void *vol;                           /* optional sqrt(-g) dV weights; NULL: 1 */
+    /* Optional radial luminosity profile (numerator of eq 25): cells are grouped into consecutive shells of
+     * shell_cells cells (all (theta, phi) cells of one radial index when phi is fastest); lum_shell receives
+     * 4 doubles per shell, [shell][total, brems, synch, compton] = sum over the shell of dE vol/dt (overwritten).
+     * lum_shell is a DEVICE array for cool_apply and a HOST array for cool_apply_host, of 4 ceil(ncell/shell_cells)
+     * doubles; NULL: no profile.  shell_cells must be a positive multiple of 128 and the call must also ask for the
+     * diagnostics (d_diag / h_diag != NULL).  The shell sums are accumulated with fp64 atomics (order dependent in the
+     * last bits); their total equals cool_diag.lum_* to rounding. */
+    long long shell_cells;
+    double *lum_shell;
 } cool_cells;
 
 typedef struct {

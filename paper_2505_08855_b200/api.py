@@ -52,7 +52,7 @@ class cool_cells(C.Structure):
                 ("rho", C.c_void_p), ("bsq", C.c_void_p),
                 ("theta_e_in", C.c_void_p), ("theta_i_in", C.c_void_p),
                 ("theta_e_out", C.c_void_p), ("theta_i_out", C.c_void_p),
-                ("r", C.c_void_p), ("vol", C.c_void_p)]
+                ("r", C.c_void_p), ("vol", C.c_void_p), ("shell_cells", C.c_longlong), ("lum_shell", C.c_void_p)]
 
 
 class cool_params(C.Structure):
@@ -199,8 +199,9 @@ def cool_table_create(desc: cool_table_desc, data, coulomb=None, device: int = 0
     return CoolTable(h, desc)
 
 
-def _cells(ncell, dtype, rho, bsq, theta_e_in, theta_i_in, theta_e_out, theta_i_out, r, vol):
+def _cells(ncell, dtype, rho, bsq, theta_e_in, theta_i_in, theta_e_out, theta_i_out, r, vol, shell_cells=0, lum_shell=None):
     c = cool_cells()
+    c.shell_cells = int(shell_cells); c.lum_shell = _ptr(lum_shell)
     c.ncell = int(ncell); c.dtype = int(dtype)
     c.rho, c.bsq = _ptr(rho), _ptr(bsq)
     c.theta_e_in, c.theta_i_in = _ptr(theta_e_in), _ptr(theta_i_in)
@@ -215,16 +216,18 @@ def make_params(dt, nsub=1, f_limit=0.3, h_floor=0.0, variant=COOL_V_AUTO, coulo
 
 
 def cool_apply(table: CoolTable, ncell, dtype, rho, bsq, theta_e_in, theta_i_in, theta_e_out, theta_i_out,
-               params: cool_params, r=None, vol=None, d_diag=None, stream=None):
-    """Asynchronous update of DEVICE arrays on ``stream`` (a cudaStream_t address; None = default)."""
-    c = _cells(ncell, dtype, rho, bsq, theta_e_in, theta_i_in, theta_e_out, theta_i_out, r, vol)
+               params: cool_params, r=None, vol=None, d_diag=None, stream=None, shell_cells=0, lum_shell=None):
+    """Asynchronous update of DEVICE arrays on ``stream`` (a cudaStream_t address; None = default).
+    ``lum_shell``: optional device float64 array of 4*ceil(ncell/shell_cells) (radial luminosity profile)."""
+    c = _cells(ncell, dtype, rho, bsq, theta_e_in, theta_i_in, theta_e_out, theta_i_out, r, vol, shell_cells, lum_shell)
     _check(lib().cool_apply(table.handle, C.byref(c), C.byref(params), _ptr(d_diag), stream))
 
 
 def cool_apply_host(table: CoolTable, ncell, dtype, rho, bsq, theta_e_in, theta_i_in, theta_e_out, theta_i_out,
-                    params: cool_params, r=None, vol=None, want_diag=False):
-    """Synchronous update of HOST arrays (copies staged and overlapped inside the library)."""
-    c = _cells(ncell, dtype, rho, bsq, theta_e_in, theta_i_in, theta_e_out, theta_i_out, r, vol)
+                    params: cool_params, r=None, vol=None, want_diag=False, shell_cells=0, lum_shell=None):
+    """Synchronous update of HOST arrays (copies staged and overlapped inside the library).
+    ``lum_shell``: optional host float64 array of 4*ceil(ncell/shell_cells) (radial luminosity profile)."""
+    c = _cells(ncell, dtype, rho, bsq, theta_e_in, theta_i_in, theta_e_out, theta_i_out, r, vol, shell_cells, lum_shell)
     d = cool_diag() if want_diag else None
     _check(lib().cool_apply_host(table.handle, C.byref(c), C.byref(params), None if d is None else C.byref(d)))
     return None if d is None else d.as_dict()

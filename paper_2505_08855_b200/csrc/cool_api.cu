@@ -110,6 +110,7 @@ static void free_table(cool_table *t)
         if (s.s) cudaStreamDestroy(s.s);
     }
     if (t->h_diag_pinned) cudaFreeHost(t->h_diag_pinned);
+    if (t->d_shell) cudaFree(t->d_shell);
     delete t;
 }
 
@@ -137,6 +138,7 @@ static cool_status check_args(const cool_table *t, const cool_cells *c, const co
     if (c->ncell > 0 && (!c->rho || !c->bsq || !c->theta_e_in || !c->theta_i_in || !c->theta_e_out || !c->theta_i_out)) {
         set_error("NULL cell array"); return COOL_EINVAL;
     }
+    if (c->lum_shell && (c->shell_cells <= 0 || c->shell_cells % 128 != 0)) { set_error("lum_shell needs shell_cells > 0 and a multiple of 128"); return COOL_EINVAL; }
     if (!(p->dt > 0.0) || !std::isfinite(p->dt)) { set_error("dt must be finite and > 0"); return COOL_EINVAL; }
     if (p->nsub < 1 || p->nsub > 1024) { set_error("nsub must be in [1, 1024]"); return COOL_EINVAL; }
     if (!(p->f_limit > 0.0 && p->f_limit < 0.5)) { set_error("f_limit must be in (0, 0.5)"); return COOL_EINVAL; }
@@ -395,6 +397,12 @@ extern "C" cool_status cool_apply(const cool_table *t, const cool_cells *c, cons
     a.r = c->r; a.vol = c->vol; a.the_out = c->theta_e_out; a.thi_out = c->theta_i_out;
     a.dt = p->dt; a.nsub = p->nsub; a.f_limit = p->f_limit; a.h_floor = p->h_floor; a.coulomb = coul; a.scheme = p->scheme;
     a.want_diag = d_diag != nullptr; a.d_diag = d_diag;
+    if (c->lum_shell) {
+        if (!d_diag) { set_error("lum_shell needs d_diag"); return COOL_EINVAL; }
+        const long long nshell = (c->ncell + c->shell_cells - 1) / c->shell_cells;
+        if (nshell > 0) CUDA_TRY(cudaMemsetAsync(c->lum_shell, 0, (size_t)nshell * 4 * sizeof(double), st), "cudaMemsetAsync(lum_shell)");
+        a.lum_shell = c->ncell > 0 ? c->lum_shell : nullptr; a.shell_cells = c->shell_cells; a.cell_offset = 0;
+    }
     if (d_diag) {
         DiagWorkspace w;
         s = get_diag_ws(t, st, &w);
@@ -416,6 +424,7 @@ extern "C" cool_status cool_apply_host(const cool_table *t, const cool_cells *c,
     if (s != COOL_OK) return s;
     CUDA_TRY(cudaSetDevice(t->device), "cudaSetDevice");
     if (h_diag) memset(h_diag, 0, sizeof *h_diag);
+    if (c->lum_shell && !h_diag) { set_error("lum_shell needs h_diag"); return COOL_EINVAL; }
     if (c->ncell == 0) return COOL_OK;
 
     std::lock_guard<std::mutex> lk_host(t->host_mu);
@@ -447,6 +456,14 @@ extern "C" cool_status cool_apply_host(const cool_table *t, const cool_cells *c,
         t->h_diag_cap = nchunks;
     }
     const void *src[6] = {c->rho, c->bsq, c->theta_e_in, c->theta_i_in, c->r, c->vol};
+    const size_t shell_bytes = c->lum_shell ? (size_t)((c->ncell + c->shell_cells - 1) / c->shell_cells) * 4 * sizeof(double) : 0;
+    if (shell_bytes > t->d_shell_cap) {
+        if (t->d_shell) cudaFree(t->d_shell);
+        t->d_shell = nullptr; t->d_shell_cap = 0;
+        CUDA_TRY(cudaMalloc(&t->d_shell, shell_bytes), "cudaMalloc(shell sums)");
+        t->d_shell_cap = shell_bytes;
+    }
+    if (shell_bytes) CUDA_TRY(cudaMemset(t->d_shell, 0, shell_bytes), "cudaMemset(shell sums)");     // synchronous: done before any chunk's kernel
     int nl = 0;
     for (size_t k = 0; k < nchunks; ++k) {
         auto &sg = t->stages[k % NST];
@@ -460,6 +477,7 @@ extern "C" cool_status cool_apply_host(const cool_table *t, const cool_cells *c,
         a.the_out = sg.buf[6]; a.thi_out = sg.buf[7];
         a.dt = p->dt; a.nsub = p->nsub; a.f_limit = p->f_limit; a.h_floor = p->h_floor; a.coulomb = coul; a.scheme = p->scheme;
         a.want_diag = h_diag != nullptr; a.d_diag = h_diag ? sg.d_diag : nullptr;
+        if (shell_bytes) { a.lum_shell = t->d_shell; a.shell_cells = c->shell_cells; a.cell_offset = (long long)off; }
         if (h_diag) {
             DiagWorkspace w;
             s = get_diag_ws(t, sg.s, &w);
@@ -473,6 +491,7 @@ extern "C" cool_status cool_apply_host(const cool_table *t, const cool_cells *c,
         if (h_diag) CUDA_TRY(cudaMemcpyAsync(&t->h_diag_pinned[k], sg.d_diag, sizeof(cool_diag), cudaMemcpyDeviceToHost, sg.s), "cudaMemcpyAsync(diag)");
     }
     for (auto &sg : t->stages) CUDA_TRY(cudaStreamSynchronize(sg.s), "cudaStreamSynchronize");
+    if (shell_bytes) CUDA_TRY(cudaMemcpy(c->lum_shell, t->d_shell, shell_bytes, cudaMemcpyDeviceToHost), "cudaMemcpy(shell sums)");
     g_launches = nl;
     if (h_diag)
         for (size_t k = 0; k < nchunks; ++k) {

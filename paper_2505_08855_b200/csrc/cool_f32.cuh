@@ -47,6 +47,7 @@ struct F32Const {
     int nsub, coulomb, has_r, has_vol, use_tma, coul_smem, nf;
     unsigned wstage_bytes;            // bytes of one warp stage = nf * 512
     unsigned stage_off, coul_off, table_off;       // dynamic shared memory layout
+    double *lum_shell; unsigned shell_tiles, tile_offset;    // radial profile (eq 25): shell = (tile_offset + warp tile)/shell_tiles
 };
 
 // ------------------------------------------------------------------------------------------
@@ -395,7 +396,7 @@ struct Ctx32 { const DevTable &T; const F32Const &S; unsigned coul_s; };      //
 // ------------------------------------------------------------------------------------------
 template <int MODE, class Fetch, bool DIAG, int CM, bool NSUB1, int NV>
 __device__ __forceinline__ void step_cells_f32(const Ctx32 &X, const Fetch &F, const float *rho, const float *bsq, float *the, float *thi,
-                                               const float *rr, const float *vol, DiagAcc &acc)
+                                               const float *rr, const float *vol, DiagAcc &acc, unsigned wtile)
 {
     const DevTable &T = X.T; const F32Const &S = X.S;
     const int coulomb = (CM == 1) ? 1 : S.coulomb;
@@ -564,6 +565,18 @@ __device__ __forceinline__ void step_cells_f32(const Ctx32 &X, const Fetch &F, c
 #pragma unroll
             for (int k = 1; k < 4; ++k) acc.lum[k] += (double)part[k];
         }
+        if (S.lum_shell) {
+            // radial profile (eq 25): the warp's cells of this call lie in one shell (shell_cells is a multiple of the
+            // warp tile): one warp sum and one fp64 atomic per luminosity term
+            double *shell = S.lum_shell + 4u * ((S.tile_offset + wtile) / S.shell_tiles);
+#pragma unroll
+            for (int k = 0; k < (MODE == 4 ? 4 : 1); ++k) {
+                float t = part[k];
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+                if ((threadIdx.x & 31) == 0) atomicAdd(shell + k, (double)t * S.lum_k);
+            }
+        }
     }
 }
 
@@ -674,11 +687,11 @@ cool_f32_kernel(const DevTable T, const F32Const S, const CellPtrs C, double *pa
             auto rot = [](float4 &v) { const float t = v.x; v.x = v.y; v.y = v.z; v.z = v.w; v.w = t; };
 #pragma unroll 1
             for (int j = 0; j < kF32CellsPerThread; ++j) {
-                step_cells_f32<MODE, Fetch, DIAG, CM, NSUB1, 1>(X, F, &rho.x, &bsq.x, &the.x, &thi.x, &rr.x, &vv.x, acc);
+                step_cells_f32<MODE, Fetch, DIAG, CM, NSUB1, 1>(X, F, &rho.x, &bsq.x, &the.x, &thi.x, &rr.x, &vv.x, acc, (unsigned)tile);
                 rot(rho); rot(bsq); rot(the); rot(thi); rot(rr); rot(vv);
             }
         } else {
-            step_cells_f32<MODE, Fetch, DIAG, CM, NSUB1, kF32CellsPerThread>(X, F, &rho.x, &bsq.x, &the.x, &thi.x, &rr.x, &vv.x, acc);
+            step_cells_f32<MODE, Fetch, DIAG, CM, NSUB1, kF32CellsPerThread>(X, F, &rho.x, &bsq.x, &the.x, &thi.x, &rr.x, &vv.x, acc, (unsigned)tile);
         }
         if (full) {
             st_stream((float4 *)C.the_out + (c >> 2), the);

@@ -69,7 +69,7 @@ __device__ __forceinline__ double imp_loss_y(const StepConst &S, const ImpStep &
 
 template <int MODE, class Fetch>
 __device__ void implicit_cell(const DevTable &T, const DevConst &K, const StepConst &S, const Fetch &F,
-                              double rho, double bsq, double &the, double &thi, double r, double vol, DiagAcc &acc)
+                              double rho, double bsq, double &the, double &thi, double r, double vol, DiagAcc &acc, long long cell)
 {
     if (isnan(rho) || isnan(bsq) || isnan(the) || isnan(thi)) { the = thi = __longlong_as_double(0x7ff8000000000000LL); return; }
     if (!(rho > 0.0)) return;
@@ -168,6 +168,7 @@ __device__ void implicit_cell(const DevTable &T, const DevConst &K, const StepCo
 #pragma unroll
     for (int k = 0; k < 4; ++k) acc.lum[k] += de_sum[k] * wgt;
     acc.flo += floored; acc.cla += clamped;
+    shell_add(S, cell, de_sum, wgt, MODE == 4);
 }
 
 template <class Real, int MODE, class Fetch, int THREADS>
@@ -183,7 +184,7 @@ cool_implicit_kernel(const DevTable T, const DevConst K, const StepConst S, cons
         double the = (double)((const Real *)C.the_in)[c], thi = (double)((const Real *)C.thi_in)[c];
         const double rho = (double)((const Real *)C.rho)[c], bsq = (double)((const Real *)C.bsq)[c];
         const double rr = S.has_r ? (double)((const Real *)C.r)[c] : 0.0, vv = S.has_vol ? (double)((const Real *)C.vol)[c] : 1.0;
-        implicit_cell<MODE, Fetch>(T, K, S, F, rho, bsq, the, thi, rr, vv, acc);
+        implicit_cell<MODE, Fetch>(T, K, S, F, rho, bsq, the, thi, rr, vv, acc, c);
         ((Real *)C.the_out)[c] = (Real)the;
         ((Real *)C.thi_out)[c] = (Real)thi;
     }

@@ -82,6 +82,8 @@ struct LaunchArgs {
     double *partials;              // [grid][8]
     unsigned *ticket;
     cool_diag *d_diag;
+    double *lum_shell;             // device [nshell][4] or NULL (zeroed by the caller of launch_step)
+    long long shell_cells, cell_offset;
 };
 
 struct DiagWorkspace { double *partials = nullptr; unsigned *ticket = nullptr; int capacity_blocks = 0; };
@@ -108,6 +110,8 @@ struct cool_table {
     mutable size_t stage_bytes = 0;         // per staging buffer
     mutable cool_diag *h_diag_pinned = nullptr;
     mutable size_t h_diag_cap = 0;
+    mutable double *d_shell = nullptr;       // host path: device copy of the radial profile
+    mutable size_t d_shell_cap = 0;
 };
 
 namespace cool {

@@ -25,6 +25,7 @@ struct StepConst {
     double hfloor2, spin;          // floor: (pi/2) h_floor^2 (Omega_K r)^2                     (eq 19)
     double lum_k;                  // lum = sum(dTheta_rad rho vol) * lum_k,  lum_k = mr/(ge1 dt)
     int nsub, coulomb, has_r, has_vol, aligned;
+    double *lum_shell; long long shell_cells, cell_offset;   // radial profile (eq 25): shell = (cell_offset + cell)/shell_cells
 };
 
 // ------------------------------------------------------------------------------------------
@@ -152,6 +153,14 @@ struct DiagAcc {
     int lim, flo, cla;
     __device__ DiagAcc() : lum{0, 0, 0, 0}, lim(0), flo(0), cla(0) {}
 };
+// one cell's luminosity terms into its radial shell (fp64 / analytic / implicit kernels: one atomic per term)
+__device__ __forceinline__ void shell_add(const StepConst &S, long long cell, const double de_sum[4], double wgt, bool split)
+{
+    if (!S.lum_shell) return;
+    double *p = S.lum_shell + 4 * ((S.cell_offset + cell) / S.shell_cells);
+    atomicAdd(p, de_sum[0] * wgt * S.lum_k);
+    if (split) { atomicAdd(p + 1, de_sum[1] * wgt * S.lum_k); atomicAdd(p + 2, de_sum[2] * wgt * S.lum_k); atomicAdd(p + 3, de_sum[3] * wgt * S.lum_k); }
+}
 
 // ==========================================================================================
 // fp64 path: mirrors the definition step by step (tolerance 1e-12 against the oracle).
@@ -251,7 +260,7 @@ __device__ __forceinline__ void update64(const DevTable &T, const DevConst &K, c
 
 template <int MODE, class Fetch, bool DIAG>
 __device__ __forceinline__ void step_cell_f64(const DevTable &T, const DevConst &K, const StepConst &S, const Fetch &F,
-                                              double rho, double bsq, double &the, double &thi, double r, double vol, DiagAcc &acc)
+                                              double rho, double bsq, double &the, double &thi, double r, double vol, DiagAcc &acc, long long cell)
 {
     if (isnan(rho) || isnan(bsq) || isnan(the) || isnan(thi)) { the = thi = __longlong_as_double(0x7ff8000000000000LL); return; }
     if (!(rho > 0.0)) return;
@@ -286,13 +295,14 @@ __device__ __forceinline__ void step_cell_f64(const DevTable &T, const DevConst 
 #pragma unroll
         for (int k = 0; k < 4; ++k) acc.lum[k] += de_sum[k] * wgt;
         acc.lim += limited; acc.flo += floored; acc.cla += clamped;
+        shell_add(S, cell, de_sum, wgt, MODE == 4);
     }
 }
 
 // analytic variant (COOL_V_ANALYTIC): eqs 1-12 per cell, fp64 regardless of the cell dtype
 template <int MODE, bool DIAG>
 __device__ __noinline__ void step_cell_analytic(const DevTable &T, const DevConst &K, const StepConst &S,
-                                                double rho, double bsq, double &the, double &thi, double r, double vol, DiagAcc &acc)
+                                                double rho, double bsq, double &the, double &thi, double r, double vol, DiagAcc &acc, long long cell)
 {
     if (isnan(rho) || isnan(bsq) || isnan(the) || isnan(thi)) { the = thi = __longlong_as_double(0x7ff8000000000000LL); return; }
     if (!(rho > 0.0)) return;
@@ -312,6 +322,7 @@ __device__ __noinline__ void step_cell_analytic(const DevTable &T, const DevCons
 #pragma unroll
         for (int k = 0; k < 4; ++k) acc.lum[k] += de_sum[k] * wgt;
         acc.lim += limited; acc.flo += floored;
+        shell_add(S, cell, de_sum, wgt, true);
     }
 }
 
@@ -385,19 +396,19 @@ struct CellPtrs { const void *rho, *bsq, *the_in, *thi_in, *r, *vol; void *the_o
 // NV cells of one thread through the right path
 template <class Real, int MODE, class Fetch, bool ANALYTIC, bool DIAG, int CM, int NV>
 __device__ __forceinline__ void do_cells(const DevTable &T, const DevConst &K, const StepConst &S, const Fetch &F, const float *coul,
-                                         const Real *rho, const Real *bsq, Real *the, Real *thi, const Real *r, const Real *vol, DiagAcc &acc)
+                                         const Real *rho, const Real *bsq, Real *the, Real *thi, const Real *r, const Real *vol, DiagAcc &acc, long long cell0)
 {
     if constexpr (ANALYTIC) {
 #pragma unroll 1
         for (int j = 0; j < NV; ++j) {
             double te = (double)the[j], ti = (double)thi[j];
-            step_cell_analytic<MODE, DIAG>(T, K, S, (double)rho[j], (double)bsq[j], te, ti, (double)r[j], (double)vol[j], acc);
+            step_cell_analytic<MODE, DIAG>(T, K, S, (double)rho[j], (double)bsq[j], te, ti, (double)r[j], (double)vol[j], acc, cell0 + j);
             the[j] = (Real)te; thi[j] = (Real)ti;
         }
     } else {
         static_assert(sizeof(Real) == 8, "fp32 table variants live in cool_f32.cuh");
 #pragma unroll
-        for (int j = 0; j < NV; ++j) step_cell_f64<MODE, Fetch, DIAG>(T, K, S, F, rho[j], bsq[j], the[j], thi[j], r[j], vol[j], acc);
+        for (int j = 0; j < NV; ++j) step_cell_f64<MODE, Fetch, DIAG>(T, K, S, F, rho[j], bsq[j], the[j], thi[j], r[j], vol[j], acc, cell0 + j);
     }
 }
 
@@ -425,7 +436,7 @@ cool_step_kernel(const DevTable T, const DevConst K, const StepConst S, const Ce
         for (int j = 0; j < N; ++j) { vget(rr, j) = (Real)0; vget(vv, j) = (Real)1; }
         if (S.has_r) rr = ld_stream((const V *)C.r + v);
         if (S.has_vol) vv = ld_stream((const V *)C.vol + v);
-        do_cells<Real, MODE, Fetch, ANALYTIC, DIAG, CM, N>(T, K, S, F, coul, &rho.x, &bsq.x, &the.x, &thi.x, &rr.x, &vv.x, acc);
+        do_cells<Real, MODE, Fetch, ANALYTIC, DIAG, CM, N>(T, K, S, F, coul, &rho.x, &bsq.x, &the.x, &thi.x, &rr.x, &vv.x, acc, v * N);
         st_stream((V *)C.the_out + v, the);
         st_stream((V *)C.thi_out + v, thi);
     }
@@ -434,7 +445,7 @@ cool_step_kernel(const DevTable T, const DevConst K, const StepConst S, const Ce
         Real the = ((const Real *)C.the_in)[c], thi = ((const Real *)C.thi_in)[c];
         const Real rho = ((const Real *)C.rho)[c], bsq = ((const Real *)C.bsq)[c];
         const Real rr = S.has_r ? ((const Real *)C.r)[c] : (Real)0, vv = S.has_vol ? ((const Real *)C.vol)[c] : (Real)1;
-        do_cells<Real, MODE, Fetch, ANALYTIC, DIAG, CM, 1>(T, K, S, F, coul, &rho, &bsq, &the, &thi, &rr, &vv, acc);
+        do_cells<Real, MODE, Fetch, ANALYTIC, DIAG, CM, 1>(T, K, S, F, coul, &rho, &bsq, &the, &thi, &rr, &vv, acc, c);
         ((Real *)C.the_out)[c] = the;
         ((Real *)C.thi_out)[c] = thi;
     }

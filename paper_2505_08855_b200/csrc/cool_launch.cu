@@ -20,6 +20,7 @@ static StepConst make_step_const(const cool_table *t, cool_dtype dt, const Launc
     S.nsub = a.nsub; S.coulomb = a.coulomb;
     S.has_r = a.r != nullptr; S.has_vol = a.vol != nullptr;
     auto ok = [&](const void *p) { return p == nullptr || ((size_t)p % 16) == 0; };
+    S.lum_shell = a.lum_shell; S.shell_cells = a.shell_cells > 0 ? a.shell_cells : 1; S.cell_offset = a.cell_offset;
     S.aligned = ok(a.rho) && ok(a.bsq) && ok(a.the_in) && ok(a.thi_in) && ok(a.the_out) && ok(a.thi_out) && ok(a.r) && ok(a.vol);
     return S;
 }
@@ -54,6 +55,7 @@ static F32Const make_f32_const(const cool_table *t, const LaunchArgs &a)
     S.nsub = a.nsub; S.coulomb = a.coulomb;
     S.has_r = a.r != nullptr; S.has_vol = a.vol != nullptr;
     S.nf = 4 + S.has_r + S.has_vol;
+    S.lum_shell = a.lum_shell; S.shell_tiles = a.shell_cells > 0 ? (unsigned)(a.shell_cells / kWarpTile) : 1u; S.tile_offset = (unsigned)(a.cell_offset / kWarpTile);
     auto ok = [&](const void *p) { return p == nullptr || ((size_t)p % 16) == 0; };
     S.use_tma = ok(a.rho) && ok(a.bsq) && ok(a.the_in) && ok(a.thi_in) && ok(a.the_out) && ok(a.thi_out) && ok(a.r) && ok(a.vol);
     // Coulomb-table node coordinates as an affine map of the table's own node coordinates

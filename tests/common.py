@@ -50,7 +50,7 @@ def oracle_table(oracle, desc, data, coul):
 
 def gpu_step(table, fields, dtype, dt, nsub=1, f_limit=0.3, h_floor=0.0, variant=api.COOL_V_AUTO,
              coulomb=api.COOL_COULOMB_AUTO, want_diag=True, use_r=False, use_vol=False, inplace=False, offset=0,
-             scheme=api.COOL_SCHEME_EXPLICIT):
+             scheme=api.COOL_SCHEME_EXPLICIT, shell_cells=0):
     """One cool_apply on cuda:0 through the C ABI.  ``offset`` (elements) misaligns the arrays."""
     import torch
     tdt = torch.float32 if dtype == np.float32 else torch.float64
@@ -75,13 +75,19 @@ def gpu_step(table, fields, dtype, dt, nsub=1, f_limit=0.3, h_floor=0.0, variant
     d_diag = torch.zeros(api.DIAG_BYTES, dtype=torch.uint8, device=dev) if want_diag else None
     params = api.make_params(dt, nsub, f_limit, h_floor, variant, coulomb, scheme)
     stream = torch.cuda.current_stream().cuda_stream
-    api.cool_apply(table, n, cdt, rho, bsq, the, thi, the_o, thi_o, params, r=r, vol=vol, d_diag=d_diag, stream=stream)
+    lum_shell = None
+    if shell_cells:
+        lum_shell = torch.full((4 * ((n + shell_cells - 1) // shell_cells),), -1.0, dtype=torch.float64, device=dev)   # must be overwritten
+    api.cool_apply(table, n, cdt, rho, bsq, the, thi, the_o, thi_o, params, r=r, vol=vol, d_diag=d_diag, stream=stream,
+                   shell_cells=shell_cells, lum_shell=lum_shell)
     torch.cuda.synchronize()
     out = dict(theta_e=the_o.cpu().numpy().astype(np.float64), theta_i=thi_o.cpu().numpy().astype(np.float64),
                launches=api.cool_last_launch_count())
     if want_diag:
         raw = d_diag.cpu().numpy().tobytes()
         out["diag"] = api.cool_diag.from_buffer_copy(raw).as_dict()
+    if lum_shell is not None:
+        out["lum_shell"] = lum_shell.cpu().numpy().reshape(-1, 4)
     return out
 
 
