@@ -177,6 +177,7 @@ def main():
     ap.add_argument("--workload", default="c5")
     ap.add_argument("--variant", default="auto")
     ap.add_argument("--scheme", default="explicit", choices=["explicit", "implicit"], help="PAPER.md L185: (i) limiter or (ii) implicit solver")
+    ap.add_argument("--shells", action="store_true", help="also compute the radial luminosity profile (eq 25) in the same launch (MAD-like workloads with diagnostics)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-also", action="store_true", help="skip the companion s512 measurement of the default workload")
@@ -250,10 +251,16 @@ def main():
     scheme = api.COOL_SCHEME_IMPLICIT if args.scheme == "implicit" else api.COOL_SCHEME_EXPLICIT
     params = api.make_params(spec["dt"], spec["nsub"], 0.3, spec.get("floor", 0.0), variant, api.COOL_COULOMB_TABLE, scheme)
     stream = torch.cuda.current_stream().cuda_stream
+    shell_cells, lum_shell = 0, None
+    if args.shells:
+        if spec["field"][0] != "mad" or not spec["diag"]:
+            raise SystemExit("--shells needs a MAD-like workload with diagnostics (c5, c3, s512d, s512f)")
+        shell_cells = spec["field"][2] * spec["field"][3]                      # all (theta, phi) cells of one radial index
+        lum_shell = torch.zeros(4 * spec["field"][1], dtype=torch.float64, device=dev)
 
     def step():
         api.cool_apply(table, ncell, api.COOL_F32, d["rho"], d["bsq"], d["theta_e"], d["theta_i"], the_o, thi_o, params,
-                       r=d.get("r"), vol=d.get("vol"), d_diag=d_diag, stream=stream)
+                       r=d.get("r"), vol=d.get("vol"), d_diag=d_diag, stream=stream, shell_cells=shell_cells, lum_shell=lum_shell)
 
     def barrier():
         if world > 1:
@@ -374,7 +381,7 @@ def main():
                 ms_per_step=total_ms / args.steps, higher_is_better=True, scaling="weak", vs_baseline=None,
                 dtype="f32" if explicit else "f64", data="synthetic",
                 config=dict(workload=args.workload, description=spec["label"], cells_per_gpu=ncell, nsub=spec["nsub"],
-                            variant=api.VARIANT_NAMES[resolved], scheme=args.scheme, l2="inputs (%.2f GB per step) larger than L2" % (bpc * ncell / 1e9),
+                            variant=api.VARIANT_NAMES[resolved], scheme=args.scheme, radial_profile=bool(args.shells), l2="inputs (%.2f GB per step) larger than L2" % (bpc * ncell / 1e9),
                             cell_substeps_per_s=value * spec["nsub"] * 1e9),
                 hbm_gbs=achieved * world, frac_of_8TBs=achieved / SPEC_HBM_GBS,
                 clocks=clocks, e2e=e2e, gpu_launches=launches_per_step * args.steps,

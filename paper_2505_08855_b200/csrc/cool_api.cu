@@ -103,7 +103,7 @@ static void free_table(cool_table *t)
     if (t->d_fcoul) cudaFree(t->d_fcoul);
     if (t->d_fcoulq) cudaFree(t->d_fcoulq);
     if (t->d_q3) cudaFree(t->d_q3);
-    for (auto &kv : t->diag_ws) { cudaFree(kv.second.partials); cudaFree(kv.second.ticket); }
+    for (auto &kv : t->diag_ws) { cudaFree(kv.second.partials); cudaFree(kv.second.ticket); if (kv.second.shell_rep) cudaFree(kv.second.shell_rep); }
     for (auto &s : t->stages) {
         for (void *b : s.buf) if (b) cudaFree(b);
         if (s.d_diag) cudaFree(s.d_diag);
@@ -114,7 +114,10 @@ static void free_table(cool_table *t)
     delete t;
 }
 
-static cool_status get_diag_ws(const cool_table *t, cudaStream_t st, DiagWorkspace *out)
+// fills the radial-profile fields of `a` for a launch over cells [off, off + n) and zeroes the replica workspace on `st`
+static cool_status prepare_shells(const cool_table *t, cudaStream_t st, LaunchArgs &a, double *d_out, long long shell_cells, long long off, long long n);
+
+static cool_status get_diag_ws(const cool_table *t, cudaStream_t st, DiagWorkspace *out, size_t shell_bytes = 0)
 {
     std::lock_guard<std::mutex> lk(t->mu);
     auto it = t->diag_ws.find(st);
@@ -126,7 +129,32 @@ static cool_status get_diag_ws(const cool_table *t, cudaStream_t st, DiagWorkspa
         CUDA_TRY(cudaMemset(w.ticket, 0, sizeof(unsigned)), "cudaMemset(diag ticket)");
         it = t->diag_ws.emplace(st, w).first;
     }
+    if (shell_bytes > it->second.shell_cap) {
+        // growing the workspace of a stream that may still be running an earlier launch: wait for it first
+        CUDA_TRY(cudaStreamSynchronize(st), "cudaStreamSynchronize(shell workspace)");
+        if (it->second.shell_rep) cudaFree(it->second.shell_rep);
+        it->second.shell_rep = nullptr; it->second.shell_cap = 0;
+        CUDA_TRY(cudaMalloc(&it->second.shell_rep, shell_bytes), "cudaMalloc(shell workspace)");
+        it->second.shell_cap = shell_bytes;
+    }
     *out = it->second;
+    return COOL_OK;
+}
+
+static cool_status prepare_shells(const cool_table *t, cudaStream_t st, LaunchArgs &a, double *d_out, long long shell_cells, long long off, long long n)
+{
+    a.lum_shell = d_out; a.shell_cells = shell_cells; a.cell_offset = off;
+    a.shell0 = off / shell_cells;
+    const long long nloc = (off + n - 1) / shell_cells - a.shell0 + 1;
+    a.shell_nloc4 = (unsigned)(4 * nloc);
+    const int nrep = n >= (1ll << 24) ? kShellReplicasLarge : kShellReplicasSmall;
+    a.shell_rmask = (unsigned)(nrep - 1);
+    const size_t bytes = (size_t)nrep * a.shell_nloc4 * sizeof(double);
+    DiagWorkspace w;
+    cool_status s = get_diag_ws(t, st, &w, bytes);
+    if (s != COOL_OK) return s;
+    a.shell_rep = w.shell_rep;
+    CUDA_TRY(cudaMemsetAsync(a.shell_rep, 0, bytes, st), "cudaMemsetAsync(shell workspace)");
     return COOL_OK;
 }
 
@@ -139,6 +167,7 @@ static cool_status check_args(const cool_table *t, const cool_cells *c, const co
         set_error("NULL cell array"); return COOL_EINVAL;
     }
     if (c->lum_shell && (c->shell_cells <= 0 || c->shell_cells % 128 != 0)) { set_error("lum_shell needs shell_cells > 0 and a multiple of 128"); return COOL_EINVAL; }
+    if (c->lum_shell && (c->ncell / 128 + 1) * (c->shell_cells / 128) >= (1ll << 40)) { set_error("lum_shell: ncell x shell_cells too large"); return COOL_EINVAL; }
     if (!(p->dt > 0.0) || !std::isfinite(p->dt)) { set_error("dt must be finite and > 0"); return COOL_EINVAL; }
     if (p->nsub < 1 || p->nsub > 1024) { set_error("nsub must be in [1, 1024]"); return COOL_EINVAL; }
     if (!(p->f_limit > 0.0 && p->f_limit < 0.5)) { set_error("f_limit must be in (0, 0.5)"); return COOL_EINVAL; }
@@ -401,7 +430,10 @@ extern "C" cool_status cool_apply(const cool_table *t, const cool_cells *c, cons
         if (!d_diag) { set_error("lum_shell needs d_diag"); return COOL_EINVAL; }
         const long long nshell = (c->ncell + c->shell_cells - 1) / c->shell_cells;
         if (nshell > 0) CUDA_TRY(cudaMemsetAsync(c->lum_shell, 0, (size_t)nshell * 4 * sizeof(double), st), "cudaMemsetAsync(lum_shell)");
-        a.lum_shell = c->ncell > 0 ? c->lum_shell : nullptr; a.shell_cells = c->shell_cells; a.cell_offset = 0;
+        if (c->ncell > 0) {
+            s = prepare_shells(t, st, a, c->lum_shell, c->shell_cells, 0, c->ncell);
+            if (s != COOL_OK) return s;
+        }
     }
     if (d_diag) {
         DiagWorkspace w;
@@ -477,7 +509,10 @@ extern "C" cool_status cool_apply_host(const cool_table *t, const cool_cells *c,
         a.the_out = sg.buf[6]; a.thi_out = sg.buf[7];
         a.dt = p->dt; a.nsub = p->nsub; a.f_limit = p->f_limit; a.h_floor = p->h_floor; a.coulomb = coul; a.scheme = p->scheme;
         a.want_diag = h_diag != nullptr; a.d_diag = h_diag ? sg.d_diag : nullptr;
-        if (shell_bytes) { a.lum_shell = t->d_shell; a.shell_cells = c->shell_cells; a.cell_offset = (long long)off; }
+        if (shell_bytes) {
+            s = prepare_shells(t, sg.s, a, t->d_shell, c->shell_cells, (long long)off, (long long)n);
+            if (s != COOL_OK) return s;
+        }
         if (h_diag) {
             DiagWorkspace w;
             s = get_diag_ws(t, sg.s, &w);

@@ -47,7 +47,10 @@ struct F32Const {
     int nsub, coulomb, has_r, has_vol, use_tma, coul_smem, nf;
     unsigned wstage_bytes;            // bytes of one warp stage = nf * 512
     unsigned stage_off, coul_off, table_off;       // dynamic shared memory layout
-    double *lum_shell; unsigned shell_tiles, tile_offset;    // radial profile (eq 25): shell = (tile_offset + warp tile)/shell_tiles
+    // radial profile (eq 25): shell = (tile_offset + warp tile)/shell_tiles; sums go to replica (warp index & shell_rmask) of lum_shell
+    // (this launch's workspace, local shell index), shell_reduce_kernel then adds the replicas into the caller's array
+    double *lum_shell; unsigned shell_tiles, tile_offset, shell0, shell_nloc4, shell_rmask;
+    unsigned long long shell_magic;                          // ceil(2^40 / shell_tiles): (t * magic) >> 40 == t / shell_tiles for t * shell_tiles < 2^40
 };
 
 // ------------------------------------------------------------------------------------------
@@ -384,6 +387,22 @@ __device__ __forceinline__ float coulomb_C32(int n1, int qstride, const float *c
     return ex2_approx(lerp(a.w, lerp(b.w, c00, c01), lerp(b.w, c10, c11)));
 }
 
+// Radial profile (eq 25): the warp tile lies in one shell (shell_cells is a multiple of the tile): one warp sum and one
+// fp64 atomic per luminosity term, into the warp's replica of this launch's shells.
+template <int MODE>
+__device__ __forceinline__ void shell_flush(const F32Const &S, const float (&part)[4], unsigned wtile)
+{
+    double *shell = S.lum_shell + (size_t)((blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5)) & S.shell_rmask) * S.shell_nloc4
+                    + 4u * ((unsigned)(((unsigned long long)(S.tile_offset + wtile) * S.shell_magic) >> 40) - S.shell0);
+#pragma unroll
+    for (int k = 0; k < (MODE == 4 ? 4 : 1); ++k) {
+        float t = part[k];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+        if ((threadIdx.x & 31) == 0) atomicAdd(shell + k, (double)t * S.lum_k);
+    }
+}
+
 struct Ctx32 { const DevTable &T; const F32Const &S; unsigned coul_s; };      // coul_s: shared-memory address of the staged Coulomb quads
 
 // ------------------------------------------------------------------------------------------
@@ -396,7 +415,7 @@ struct Ctx32 { const DevTable &T; const F32Const &S; unsigned coul_s; };      //
 // ------------------------------------------------------------------------------------------
 template <int MODE, class Fetch, bool DIAG, int CM, bool NSUB1, int NV>
 __device__ __forceinline__ void step_cells_f32(const Ctx32 &X, const Fetch &F, const float *rho, const float *bsq, float *the, float *thi,
-                                               const float *rr, const float *vol, DiagAcc &acc, unsigned wtile)
+                                               const float *rr, const float *vol, DiagAcc &acc, float (&tile_part)[4], unsigned wtile)
 {
     const DevTable &T = X.T; const F32Const &S = X.S;
     const int coulomb = (CM == 1) ? 1 : S.coulomb;
@@ -565,17 +584,12 @@ __device__ __forceinline__ void step_cells_f32(const Ctx32 &X, const Fetch &F, c
 #pragma unroll
             for (int k = 1; k < 4; ++k) acc.lum[k] += (double)part[k];
         }
-        if (S.lum_shell) {
-            // radial profile (eq 25): the warp's cells of this call lie in one shell (shell_cells is a multiple of the
-            // warp tile): one warp sum and one fp64 atomic per luminosity term
-            double *shell = S.lum_shell + 4u * ((S.tile_offset + wtile) / S.shell_tiles);
+        if constexpr (NV == 1) {
+            // one cell of the tile (4-D kernel): the caller gathers the tile's terms and flushes them once
 #pragma unroll
-            for (int k = 0; k < (MODE == 4 ? 4 : 1); ++k) {
-                float t = part[k];
-#pragma unroll
-                for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
-                if ((threadIdx.x & 31) == 0) atomicAdd(shell + k, (double)t * S.lum_k);
-            }
+            for (int k = 0; k < 4; ++k) tile_part[k] = part[k];
+        } else {
+            if (S.lum_shell) shell_flush<MODE>(S, part, wtile);
         }
     }
 }
@@ -681,17 +695,27 @@ cool_f32_kernel(const DevTable T, const F32Const S, const CellPtrs C, double *pa
                 if (S.has_r) (&rr.x)[j] = in ? __ldg((const float *)C.r + c + j) : 0.f;
             }
         }
+        float tp[4] = {0.f, 0.f, 0.f, 0.f};                 // this thread's luminosity terms of the tile (DIAG)
         if constexpr (MODE == 4) {
             // the 16-register patch allows one cell at a time: one copy of the cell code, run four times with the
             // vectors rotated (a quarter of the instruction footprint of the unrolled form)
             auto rot = [](float4 &v) { const float t = v.x; v.x = v.y; v.y = v.z; v.z = v.w; v.w = t; };
 #pragma unroll 1
             for (int j = 0; j < kF32CellsPerThread; ++j) {
-                step_cells_f32<MODE, Fetch, DIAG, CM, NSUB1, 1>(X, F, &rho.x, &bsq.x, &the.x, &thi.x, &rr.x, &vv.x, acc, (unsigned)tile);
+                step_cells_f32<MODE, Fetch, DIAG, CM, NSUB1, 1>(X, F, &rho.x, &bsq.x, &the.x, &thi.x, &rr.x, &vv.x, acc, tp, (unsigned)tile);
+                // a finished cell's rho, bsq, vol and r slots are dead: they carry its four luminosity terms to the end of the tile
+                if constexpr (DIAG) { rho.x = tp[0]; bsq.x = tp[1]; vv.x = tp[2]; rr.x = tp[3]; }
                 rot(rho); rot(bsq); rot(the); rot(thi); rot(rr); rot(vv);
             }
+            if constexpr (DIAG) {
+                tp[0] = (rho.x + rho.y) + (rho.z + rho.w); tp[1] = (bsq.x + bsq.y) + (bsq.z + bsq.w);
+                tp[2] = (vv.x + vv.y) + (vv.z + vv.w); tp[3] = (rr.x + rr.y) + (rr.z + rr.w);
+            }
         } else {
-            step_cells_f32<MODE, Fetch, DIAG, CM, NSUB1, kF32CellsPerThread>(X, F, &rho.x, &bsq.x, &the.x, &thi.x, &rr.x, &vv.x, acc, (unsigned)tile);
+            step_cells_f32<MODE, Fetch, DIAG, CM, NSUB1, kF32CellsPerThread>(X, F, &rho.x, &bsq.x, &the.x, &thi.x, &rr.x, &vv.x, acc, tp, (unsigned)tile);
+        }
+        if constexpr (DIAG && MODE == 4) {
+            if (S.lum_shell) shell_flush<MODE>(S, tp, (unsigned)tile);
         }
         if (full) {
             st_stream((float4 *)C.the_out + (c >> 2), the);

@@ -82,11 +82,17 @@ struct LaunchArgs {
     double *partials;              // [grid][8]
     unsigned *ticket;
     cool_diag *d_diag;
-    double *lum_shell;             // device [nshell][4] or NULL (zeroed by the caller of launch_step)
-    long long shell_cells, cell_offset;
+    double *lum_shell;             // device [nshell][4] or NULL (zeroed by the caller; the launch ADDS its shells)
+    double *shell_rep;             // workspace [kShellReplicas][shell_nloc4], zeroed per launch
+    long long shell_cells, cell_offset, shell0;   // shell0: first shell this launch touches
+    unsigned shell_nloc4;          // 4 x number of shells this launch touches
+    unsigned shell_rmask;          // number of replicas - 1
 };
 
-struct DiagWorkspace { double *partials = nullptr; unsigned *ticket = nullptr; int capacity_blocks = 0; };
+// radial-profile atomics are spread over 32 (small launches) or 256 copies (by block / warp index): at any moment nearly all
+// warps work in the same shell, and the L2 serialises atomics to one address
+constexpr int kShellReplicasSmall = 32, kShellReplicasLarge = 256;
+struct DiagWorkspace { double *partials = nullptr; unsigned *ticket = nullptr; int capacity_blocks = 0; double *shell_rep = nullptr; size_t shell_cap = 0; };
 
 }  // namespace cool
 

@@ -25,7 +25,9 @@ struct StepConst {
     double hfloor2, spin;          // floor: (pi/2) h_floor^2 (Omega_K r)^2                     (eq 19)
     double lum_k;                  // lum = sum(dTheta_rad rho vol) * lum_k,  lum_k = mr/(ge1 dt)
     int nsub, coulomb, has_r, has_vol, aligned;
-    double *lum_shell; long long shell_cells, cell_offset;   // radial profile (eq 25): shell = (cell_offset + cell)/shell_cells
+    // radial profile (eq 25): shell = (cell_offset + cell)/shell_cells; sums go to replica (block index & shell_rmask) of lum_shell
+    // (this launch's workspace, local shell index); shell_reduce_kernel then adds the replicas into the caller's array
+    double *lum_shell; long long shell_cells, cell_offset, shell0; unsigned shell_nloc4, shell_rmask;
 };
 
 // ------------------------------------------------------------------------------------------
@@ -157,7 +159,7 @@ struct DiagAcc {
 __device__ __forceinline__ void shell_add(const StepConst &S, long long cell, const double de_sum[4], double wgt, bool split)
 {
     if (!S.lum_shell) return;
-    double *p = S.lum_shell + 4 * ((S.cell_offset + cell) / S.shell_cells);
+    double *p = S.lum_shell + (size_t)(blockIdx.x & S.shell_rmask) * S.shell_nloc4 + 4 * ((S.cell_offset + cell) / S.shell_cells - S.shell0);
     atomicAdd(p, de_sum[0] * wgt * S.lum_k);
     if (split) { atomicAdd(p + 1, de_sum[1] * wgt * S.lum_k); atomicAdd(p + 2, de_sum[2] * wgt * S.lum_k); atomicAdd(p + 3, de_sum[3] * wgt * S.lum_k); }
 }
@@ -387,7 +389,6 @@ __device__ __forceinline__ void reduce_diag(const DiagAcc &acc, double lum_k, do
 {
     reduce_diag_vals(acc.lum[0], acc.lum[1], acc.lum[2], acc.lum[3], acc.lim, acc.flo, acc.cla, lum_k, partials, ticket, out);
 }
-
 // ------------------------------------------------------------------------------------------
 // The kernel
 // ------------------------------------------------------------------------------------------

@@ -4,6 +4,18 @@
 
 namespace cool {
 
+// Radial profile, second (tiny) launch: add the replicas of the step launch's shells into the caller's array, in a fixed
+// order over the replicas.  Kept out of reduce_diag_vals on purpose: growing that non-inlined function cost the step
+// kernels that call it 8 % more instructions in their hot loops (measured).
+static __global__ void shell_reduce_kernel(const double *rep, double *out, unsigned nloc4, long long shell0, unsigned rmask)
+{
+    const unsigned idx = blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= nloc4) return;
+    double s = 0.0;
+    for (unsigned r = 0; r <= rmask; ++r) s += rep[(size_t)r * nloc4 + idx];
+    if (s != 0.0) atomicAdd(out + 4 * shell0 + idx, s);
+}
+
 static StepConst make_step_const(const cool_table *t, cool_dtype dt, const LaunchArgs &a)
 {
     const DevConst &K = t->cst;
@@ -20,7 +32,8 @@ static StepConst make_step_const(const cool_table *t, cool_dtype dt, const Launc
     S.nsub = a.nsub; S.coulomb = a.coulomb;
     S.has_r = a.r != nullptr; S.has_vol = a.vol != nullptr;
     auto ok = [&](const void *p) { return p == nullptr || ((size_t)p % 16) == 0; };
-    S.lum_shell = a.lum_shell; S.shell_cells = a.shell_cells > 0 ? a.shell_cells : 1; S.cell_offset = a.cell_offset;
+    S.lum_shell = a.lum_shell ? a.shell_rep : nullptr; S.shell_cells = a.shell_cells > 0 ? a.shell_cells : 1;
+    S.cell_offset = a.cell_offset; S.shell0 = a.shell0; S.shell_nloc4 = a.shell_nloc4; S.shell_rmask = a.shell_rmask;
     S.aligned = ok(a.rho) && ok(a.bsq) && ok(a.the_in) && ok(a.thi_in) && ok(a.the_out) && ok(a.thi_out) && ok(a.r) && ok(a.vol);
     return S;
 }
@@ -55,7 +68,10 @@ static F32Const make_f32_const(const cool_table *t, const LaunchArgs &a)
     S.nsub = a.nsub; S.coulomb = a.coulomb;
     S.has_r = a.r != nullptr; S.has_vol = a.vol != nullptr;
     S.nf = 4 + S.has_r + S.has_vol;
-    S.lum_shell = a.lum_shell; S.shell_tiles = a.shell_cells > 0 ? (unsigned)(a.shell_cells / kWarpTile) : 1u; S.tile_offset = (unsigned)(a.cell_offset / kWarpTile);
+    S.lum_shell = a.lum_shell ? a.shell_rep : nullptr;
+    S.shell_tiles = a.shell_cells > 0 ? (unsigned)(a.shell_cells / kWarpTile) : 1u; S.tile_offset = (unsigned)(a.cell_offset / kWarpTile);
+    S.shell0 = (unsigned)a.shell0; S.shell_nloc4 = a.shell_nloc4; S.shell_rmask = a.shell_rmask;
+    S.shell_magic = ((1ull << 40) + S.shell_tiles - 1) / S.shell_tiles;
     auto ok = [&](const void *p) { return p == nullptr || ((size_t)p % 16) == 0; };
     S.use_tma = ok(a.rho) && ok(a.bsq) && ok(a.the_in) && ok(a.thi_in) && ok(a.the_out) && ok(a.thi_out) && ok(a.r) && ok(a.vol);
     // Coulomb-table node coordinates as an affine map of the table's own node coordinates
@@ -101,6 +117,12 @@ cool_status launch_step(const cool_table *t, cool_variant v, cool_dtype dt, cons
     }
     if (e != cudaSuccess) { set_error("kernel launch failed: %s", cudaGetErrorString(e)); return COOL_ECUDA; }
     if (nlaunch) *nlaunch += 1;
+    if (a.lum_shell) {                       // radial profile: fold this launch's replicas into the caller's array
+        shell_reduce_kernel<<<(a.shell_nloc4 + 255) / 256, 256, 0, st>>>(a.shell_rep, a.lum_shell, a.shell_nloc4, a.shell0, a.shell_rmask);
+        e = cudaGetLastError();
+        if (e != cudaSuccess) { set_error("kernel launch failed: %s", cudaGetErrorString(e)); return COOL_ECUDA; }
+        if (nlaunch) *nlaunch += 1;
+    }
     return COOL_OK;
 }
 
