@@ -34,13 +34,13 @@ UNIT = "Gcell-updates/s"
 SPEC_HBM_GBS = 8000.0                     # BASELINE.json: "vs 8 TB/s"
 FALLBACK_HBM_GBS = 6650.0                 # B200_PROFILING.md fallback
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from one `ncu --set full` capture each
-# (profiles/r01c_<workload>_global_full.txt, line "traffic ="); null for workloads that were not captured
-NCU_TRAFFIC_GB = {"c5": 3.7334, "s512": 3.1939, "c2": 0.4301}
+# (profiles/r01d_<workload>_global_full.txt, c2: r01c; line "traffic ="); null for workloads that were not captured
+NCU_TRAFFIC_GB = {"c5": 3.7330, "s512": 3.1940, "s512f": 4.2761, "c2": 0.4301}
 # issue-slot ceiling of the SMs (the bound that actually limits the sub-stepped 4-D step): 148 SMs x 4 schedulers x
 # 1 warp instruction per clock at clocks.max.sm 1965 MHz (B200_PROFILING.md unit counts) = 1163 G warp-instructions/s
 ISSUE_PEAK_GWINST = 148 * 4 * 1.965
 # warp instructions per launch (smsp__inst_executed.sum of the same captures)
-NCU_WARP_INST = {"c5": 3254462658, "s512": 613220864}
+NCU_WARP_INST = {"c5": 3379873027, "s512": 613224416, "s512f": 815038674}
 
 
 # ------------------------------------------------------------------------------------------------
@@ -386,7 +386,7 @@ def main():
                 hbm_gbs=achieved * world, frac_of_8TBs=achieved / SPEC_HBM_GBS,
                 clocks=clocks, e2e=e2e, gpu_launches=launches_per_step * args.steps,
                 roofline=dict(bound="hbm", achieved=achieved, peak=peak, unit="GB/s", frac=achieved / peak,
-                              traffic=(NCU_TRAFFIC_GB[args.workload] * 1e9 if args.workload in NCU_TRAFFIC_GB and args.variant == "auto" and explicit else None),
+                              traffic=(NCU_TRAFFIC_GB[args.workload] * 1e9 if args.workload in NCU_TRAFFIC_GB and args.variant == "auto" and explicit and not args.shells else None),
                               kernel=kernel_name, bytes_per_cell=bpc, algorithmic_bytes_per_launch=bpc * ncell, peak_source=peak_src,
                               ms_per_launch_median=float(np.median(per_step_ms)), ms_per_launch_best=float(per_step_ms.min())),
                 diag=diag_out)
