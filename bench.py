@@ -371,7 +371,8 @@ def main():
     achieved = bpc * ncell / (kern_ms * 1e-3) / 1e9
     mode = len(spec["n"])
     single = mode == 3 and spec["nsub"] == 1
-    fetch = {"global": "F32GlobalQ" if (mode == 3 and np.prod(spec["n"]) * 16 <= (64 << 20)) else "F32Global", "smem": "F32Smem",
+    fetch = {"global": ("F32GlobalO" if np.prod(spec["n"]) * 32 <= (16 << 20) else "F32GlobalQ" if np.prod(spec["n"]) * 16 <= (64 << 20) else "F32Global") if mode == 3 else "F32Global",
+             "smem": "F32Smem",
              "tex_point": "F32TexPoint", "tex_hwfilter": "F32TexHw"}.get(api.VARIANT_NAMES[resolved], api.VARIANT_NAMES[resolved])
     explicit = args.scheme == "explicit"
     kernel_name = ("cool_implicit_kernel<float, MODE=%d, %s>" % (mode, api.VARIANT_NAMES[resolved])) if not explicit else "cool_f32_kernel<MODE=%d, %s, DIAG=%d, CM=1, NSUB1=%d, %s>" % (

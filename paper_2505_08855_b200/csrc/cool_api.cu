@@ -103,6 +103,7 @@ static void free_table(cool_table *t)
     if (t->d_fcoul) cudaFree(t->d_fcoul);
     if (t->d_fcoulq) cudaFree(t->d_fcoulq);
     if (t->d_q3) cudaFree(t->d_q3);
+    if (t->d_o3) cudaFree(t->d_o3);
     for (auto &kv : t->diag_ws) { cudaFree(kv.second.partials); cudaFree(kv.second.ticket); if (kv.second.shell_rep) cudaFree(kv.second.shell_rep); }
     for (auto &s : t->stages) {
         for (void *b : s.buf) if (b) cudaFree(b);
@@ -352,6 +353,31 @@ extern "C" cool_status cool_table_create(const cool_table_desc *desc, int device
                 if (e == cudaSuccess) e = cudaMemcpy(t->d_q3, quad.data(), qbytes, cudaMemcpyHostToDevice);
                 if (e != cudaSuccess) { set_error("quad table upload: %s", cudaGetErrorString(e)); return fail(e == cudaErrorMemoryAllocation ? COOL_ENOMEM : COOL_ECUDA); }
                 D.q3 = (const float4 *)t->d_q3;
+            }
+            // oct layout (8x the bytes): all eight corners of a table cell in one 32-byte sector, one 256-bit gather per
+            // lookup.  Wins while it sits comfortably in L2 (64^3: 8 MiB, 0.61 -> 0.40 ms on 2^26 log-uniform cells); at 128^3
+            // (64 MiB) it ties with the quads and costs L1 when the diagnostics shrink it, so the default limit is 16 MiB
+            // (COOL_OCT_MAX_MB overrides, 0 disables).
+            size_t oct_max = (size_t)16 << 20;
+            if (const char *ev = getenv("COOL_OCT_MAX_MB")) oct_max = (size_t)atoll(ev) << 20;
+            const size_t obytes = (size_t)total * 8 * sizeof(float);
+            if (obytes <= oct_max) {
+                std::vector<float> oct;
+                try { oct.resize((size_t)total * 8); } catch (...) { set_error("out of host memory"); return fail(COOL_ENOMEM); }
+                const int nr = ncan[CAX_RHO], ne = ncan[CAX_THE], nb = ncan[CAX_BSQ];
+                for (int ir = 0; ir < nr; ++ir)
+                    for (int ie = 0; ie < ne; ++ie)
+                        for (int ib = 0; ib < nb; ++ib) {
+                            float *o = &oct[((((size_t)ir * ne + ie) * nb) + ib) * 8];
+                            for (int c = 0; c < 8; ++c) {
+                                const int jr = std::min(ir + (c >> 2), nr - 1), je = std::min(ie + ((c >> 1) & 1), ne - 1), jb = std::min(ib + (c & 1), nb - 1);
+                                o[c] = canon32[((size_t)jr * ne + je) * nb + jb];
+                            }
+                        }
+                e = cudaMalloc(&t->d_o3, obytes);
+                if (e == cudaSuccess) e = cudaMemcpy(t->d_o3, oct.data(), obytes, cudaMemcpyHostToDevice);
+                if (e != cudaSuccess) { set_error("oct table upload: %s", cudaGetErrorString(e)); return fail(e == cudaErrorMemoryAllocation ? COOL_ENOMEM : COOL_ECUDA); }
+                D.o3 = (const float4 *)t->d_o3;
             }
         }
 

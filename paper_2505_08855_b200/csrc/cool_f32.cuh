@@ -231,6 +231,24 @@ struct F32GlobalQ {
     }
     __device__ __forceinline__ void corners4(const Loc32 &, const Loc32 &, const Loc32 &, const Loc32 &, float4 (&)[2][2][4]) const {}
 };
+// MODE 3 oct layout: o3[r][e][b] = the eight corners of table cell (r, e, b) in one 32-byte sector
+// {T'(r,e,b), T'(r,e,b+1), T'(r,e+1,b), T'(r,e+1,b+1), T'(r+1,e,b), ...}: a trilinear lookup is ONE 256-bit gather.
+struct F32GlobalO {
+    static constexpr bool kHw = false, kSmem = false;
+    const float4 *po; int sr, se, c3;
+    __device__ F32GlobalO(const DevTable &T, const void *) : po(T.o3), sr(T.s_rho), se(T.s_the)
+    {
+        c3 = (int)(0u - kMagicBits * (unsigned)(sr + se + 1));
+    }
+    __device__ __forceinline__ void corners3(const Loc32 &r, const Loc32 &e, const Loc32 &b, float (&c)[8]) const
+    {
+        const int off = loc_bits(r) * sr + (loc_bits(e) * se + (loc_bits(b) + c3));
+        const float4 *p = po + 2u * (unsigned)off;
+        asm("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+            : "=f"(c[0]), "=f"(c[1]), "=f"(c[2]), "=f"(c[3]), "=f"(c[4]), "=f"(c[5]), "=f"(c[6]), "=f"(c[7]) : "l"(p));
+    }
+    __device__ __forceinline__ void corners4(const Loc32 &, const Loc32 &, const Loc32 &, const Loc32 &, float4 (&)[2][2][4]) const {}
+};
 struct F32Smem {
     static constexpr bool kHw = false, kSmem = true;
     const float *p1; const float4 *p4; int sr, se, si, c3, c4;
@@ -791,6 +809,7 @@ static cudaError_t launch_f32_by_variant(const LaunchCtx32 &L, cool_variant v)
     switch (v) {
         case COOL_V_GLOBAL:
             if constexpr (MODE == 3) {
+                if (L.t->dev.o3) return launch_f32_one<MODE, F32GlobalO, DIAG, CM, NSUB1, TH, NS>(L);
                 if (L.t->dev.q3) return launch_f32_one<MODE, F32GlobalQ, DIAG, CM, NSUB1, TH, NS>(L);
             }
             return launch_f32_one<MODE, F32Global, DIAG, CM, NSUB1, TH, NS>(L);

@@ -46,6 +46,7 @@ struct DevTable {
     // so that Lambda h / u_e = 2^(interp + log2 h) without cancelling large fp32 numbers.
     const float *f1;
     const float4 *f4;
+    const float4 *o3;              // MODE 3 oct layout: 8 corners of a table cell per 32-byte element (2 float4), plain strides; NULL when too large
     const float4 *q3;              // MODE 3 quad layout {T'(r,e,b), T'(r,e,b+1), T'(r,e+1,b), T'(r,e+1,b+1)}, plain strides; NULL when too large
     cudaTextureObject_t ftex_pt, ftex_lin;
     const float *fcoul;            // log2 C [theta_i][theta_e] (allocation padded to 16 B)
@@ -103,7 +104,7 @@ struct cool_table {
     cool::DevConst cst{};
     float *d_lin = nullptr;        // owns lin1 / lin4
     float *d_f32 = nullptr;        // owns f1 / f4
-    float *d_coul = nullptr, *d_fcoul = nullptr, *d_fcoulq = nullptr, *d_q3 = nullptr;
+    float *d_coul = nullptr, *d_fcoul = nullptr, *d_fcoulq = nullptr, *d_q3 = nullptr, *d_o3 = nullptr;
     cudaArray_t arr = nullptr, arr32 = nullptr;
     int sm_count = 148;
     int max_smem_optin = 0;
