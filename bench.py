@@ -375,12 +375,12 @@ def main():
              "smem": "F32Smem",
              "tex_point": "F32TexPoint", "tex_hwfilter": "F32TexHw"}.get(api.VARIANT_NAMES[resolved], api.VARIANT_NAMES[resolved])
     explicit = args.scheme == "explicit"
-    kernel_name = ("cool_implicit_kernel<float, MODE=%d, %s>" % (mode, api.VARIANT_NAMES[resolved])) if not explicit else "cool_f32_kernel<MODE=%d, %s, DIAG=%d, CM=1, NSUB1=%d, %s>" % (
+    kernel_name = ("cool_implicit_f32_kernel<MODE=%d, %s>" % (mode, api.VARIANT_NAMES[resolved])) if not explicit else "cool_f32_kernel<MODE=%d, %s, DIAG=%d, CM=1, NSUB1=%d, %s>" % (
         mode, fetch, int(bool(spec["diag"])), int(spec["nsub"] == 1),
         "384 threads, 2 stages" if fetch == "F32Smem" else ("768 threads, 2 stages" if single else "512 threads, 3 stages"))
     line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=args.warmup,
                 ms_per_step=total_ms / args.steps, higher_is_better=True, scaling="weak", vs_baseline=None,
-                dtype="f32" if explicit else "f64", data="synthetic",
+                dtype="f32", data="synthetic",
                 config=dict(workload=args.workload, description=spec["label"], cells_per_gpu=ncell, nsub=spec["nsub"],
                             variant=api.VARIANT_NAMES[resolved], scheme=args.scheme, radial_profile=bool(args.shells), l2="inputs (%.2f GB per step) larger than L2" % (bpc * ncell / 1e9),
                             cell_substeps_per_s=value * spec["nsub"] * 1e9),

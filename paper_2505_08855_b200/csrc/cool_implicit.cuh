@@ -1,6 +1,6 @@
 // cool_implicit.cuh — the implicit cooling scheme (COOL_SCHEME_IMPLICIT; PAPER.md L185 (ii), L369; reading C-18 of
-// DESIGN.md), first correct CUDA path: fp64 arithmetic for either cell dtype, one thread per cell (vector) of the SoA
-// stream, the table read through the same lookup policies as the fp64 explicit path.
+// DESIGN.md): one thread per cell of the SoA stream, the table read through the lookup policies of the fp64 explicit
+// path; fp64 arithmetic for fp64 cells (first part of this file), fp32 arithmetic on the T' tables for fp32 cells (second part).
 //
 // Per sub-step h, from the start state (Theta_e, Theta_i):
 //   q        = a/(1 + a g),  a = h K C(Theta_e, Theta_i),  g = (gamma_i - 1)/(gamma_e - 1)      (Coulomb: coefficient at
@@ -17,7 +17,7 @@
 // with Theta_e, so the answer is within rounding of the root; where Lambda is not monotone several roots can exist
 // and any of them is a solution of the scheme.
 #pragma once
-#include "cool_kernels.cuh"
+#include "cool_f32.cuh"
 
 namespace cool {
 
@@ -214,6 +214,213 @@ static cudaError_t launch_implicit_one(const LaunchCtx &L, size_t smem)
     return cudaGetLastError();
 }
 
-cudaError_t launch_implicit(const LaunchCtx &L, int mode, cool_variant v, cool_dtype dt);
+// ==========================================================================================
+// fp32 cells: the same solve in fp32 on the T' tables (log2 of the rate per unit electron energy, cool_internal.h), where
+// h Lambda/u_e = 2^(interp T' + log2 h + rho clamp correction) needs no large-number cancellation.  Same structure:
+// binary search over the Theta_e nodes, then false position inside the interval on the contracted column values.
+// The bracket is refined to a few fp32 ulps, so the result is within ~1e-6 of the root (tolerance 1e-5, as for the
+// explicit fp32 path).  Fetch is one of the fp64 path's lookup policies, constructed over the T' arrays.
+// ==========================================================================================
+struct Imp32 { float rho, thi0, q, R, opq, kc, hf; };    // kc: clamp correction of the rho axis (log2), hf: h as a factor
+
+template <int MODE, class Fetch>
+__device__ __forceinline__ void imp32_node(const Fetch &F, const Loc32 &r, const Loc32 &b, const Loc32 &ii, int ir, int ib, int iii, int i, float (&y)[3])
+{
+    if constexpr (MODE == 3) {
+        const float a0 = lerp(b.w, F.at1(ir, i, ib), F.at1(ir, i, ib + 1)), a1 = lerp(b.w, F.at1(ir + 1, i, ib), F.at1(ir + 1, i, ib + 1));
+        y[0] = lerp(r.w, a0, a1); y[1] = y[2] = 0.f;
+    } else {
+        float v[2][2][3];
+#pragma unroll
+        for (int cr = 0; cr < 2; ++cr)
+#pragma unroll
+            for (int ci = 0; ci < 2; ++ci) {
+                const float4 t0 = F.at4(ir + cr, i, iii + ci, ib), t1 = F.at4(ir + cr, i, iii + ci, ib + 1);
+                v[cr][ci][0] = lerp(b.w, t0.x, t1.x); v[cr][ci][1] = lerp(b.w, t0.y, t1.y); v[cr][ci][2] = lerp(b.w, t0.z, t1.z);
+            }
+#pragma unroll
+        for (int k = 0; k < 3; ++k) y[k] = lerp(r.w, lerp(ii.w, v[0][0][k], v[0][1][k]), lerp(ii.w, v[1][0][k], v[1][1][k]));
+    }
+}
+
+// loss(th)/th = h Lambda(th_c)/u_e(th_c) from the channel values y at th_c; optional process shares
+template <int MODE>
+__device__ __forceinline__ float imp32_rate(const F32Const &S, const Imp32 &c, float thc, const float (&y)[3], float *frac)
+{
+    // h multiplies the power of two instead of joining its exponent: one rounding less at magnitude ~40, which matters
+    // here because in the strongly cooled limit theta' ~ R/rate carries the full relative error of the rate
+    if constexpr (MODE == 3) {
+        return ex2_approx(y[0] + c.kc) * c.hf;
+    } else {
+        const float rbr = ex2_approx(fminf(y[0] + c.kc, 100.f)) * c.hf;
+        const float esy = y[1] + c.kc;
+        const float rsy = ex2_approx(fminf(esy + y[2], 100.f)) * c.hf;                        // eta * Q_syn
+        const float rthin = rbr + rsy;                                                        // eq 10
+        const float num = fmaf(S.ae, thc, S.ai * c.thi0), den = fmaf(S.be, thc, fmaf(S.bi, c.thi0, 1.f));
+        const float rcs = c.rho * (num * rsqrt_approx(num * den));                            // rho c_s   (eqs 13-14)
+        const float th3 = fmaxf(thc * thc * thc, 1e-30f);
+        const float tau_abs = rthin * (S.inv_kB * rcs) * rcp_approx(th3);                     // eq 12
+        const float tau_sca = S.ksca * rcs;
+        if (frac) {
+            const float inv = rcp_approx(fmaxf(rthin, 1e-37f));
+            const float rs0 = ex2_approx(fminf(esy, 100.f)) * c.hf;
+            frac[0] = rbr * inv; frac[1] = rs0 * inv; frac[2] = (rsy - rs0) * inv;
+        }
+        return rthin * rcp_approx(fmaf(tau_abs, fmaf(1.5f, tau_abs + tau_sca, 1.7320508f), 1.f));   // eq 11
+    }
+}
+
+template <int MODE, class Fetch>
+__device__ void implicit_cell_f32(const DevTable &T, const StepConst &S, const F32Const &S32, const Fetch &F,
+                                  float rho, float bsq, float &the, float &thi, float r, float vol, DiagAcc &acc, long long cell)
+{
+    const float chk = (bsq + the) + (thi + rho);
+    if (chk != chk) { the = thi = __int_as_float(0x7fc00000); return; }
+    if (!(rho > 0.f)) return;
+    const int one_bits = 0x3f800000;
+    const AxisCoef &ax = T.ax[CAX_THE];
+    const int n = ax.n;
+    int clamped = 0, floored = 0;
+    const Loc32 lr = locate32<true>(T.ax[CAX_RHO], rho, clamped, one_bits), lb = locate32<true>(T.ax[CAX_BSQ], bsq, clamped, one_bits);
+    const int ir = (int)lr.fi, ib = (int)lb.fi;
+    Loc32 li{0.f, 0.f, 0.f, 0.f}; int iii = 0;
+    const float g = S32.gi1_over_ge1;
+    float de_sum[4] = {0.f, 0.f, 0.f, 0.f};
+    auto node_theta = [&](int i) { return ex2_approx(fmaf((float)i - ax.cf, ax.d2f, ax.e0)); };
+    for (int s = 0; s < S32.nsub; ++s) {
+        bool flo = false;
+        if (S32.hfloor2 > 0.f && r > 0.f) {
+            const float ok = __fdividef(r, fmaf(r, sqrtf(r), S32.spin));
+            if ((the + thi) * S32.mr < S32.hfloor2 * ok * ok) { flo = true; floored = 1; }
+        }
+        if constexpr (MODE == 4) { li = locate32<true>(T.ax[CAX_THI], thi, clamped, one_bits); iii = (int)li.fi; }
+        float C = 0.f;
+        if (S32.coulomb == 1) {
+            int dummy = 0;
+            const Loc32 ca = locate32<false>(T.cax[0], thi, dummy, one_bits), cb = locate32<false>(T.cax[1], the, dummy, one_bits);
+            C = coulomb_C32<0, false>(T.cax[1].n, 0, T.fcoul, 0u, ca, cb);
+        } else if (S32.coulomb == 2) {
+            C = (float)coolphys::coulomb_C((double)the, (double)thi / S32.ion_ratio);
+        }
+        const float a = S32.coul_kh * rho * C;
+        Imp32 c;
+        c.rho = rho; c.thi0 = thi; c.q = a / (1.f + a * g); c.R = fmaf(c.q, thi, the); c.opq = 1.f + c.q;
+        c.kc = lr.d * T.ax[CAX_RHO].d2f; c.hf = ex2_approx(S32.k0);
+        if (!(c.R > 0.f)) continue;
+        float theta, rate = 0.f, frac[3] = {0.f, 0.f, 0.f};
+        if (flo) {
+            theta = c.R / c.opq;
+        } else {
+            const float tR = coord32(ax, c.R, one_bits);
+            const int imax = tR >= (float)(n - 1) ? n - 1 : (tR < 0.f ? -1 : (int)tR);
+            int ilo = -1, ihi = imax + 1;
+            float ya[3] = {0.f, 0.f, 0.f}, yb[3] = {0.f, 0.f, 0.f};
+            bool have_b = false;
+            while (ihi - ilo > 1) {
+                const int m = (ilo + ihi) >> 1;
+                float ym[3];
+                imp32_node<MODE>(F, lr, lb, li, ir, ib, iii, m, ym);
+                const float tm = node_theta(m);
+                const float fm = fmaf(tm, c.opq, -c.R) + tm * imp32_rate<MODE>(S32, c, tm, ym, nullptr);
+                if (fm < 0.f) { ilo = m; ya[0] = ym[0]; ya[1] = ym[1]; ya[2] = ym[2]; }
+                else { ihi = m; yb[0] = ym[0]; yb[1] = ym[1]; yb[2] = ym[2]; have_b = true; }
+            }
+            if (ilo == -1 || ilo == n - 1) {
+                const int e = ilo == -1 ? 0 : n - 1;
+                float ye[3];
+                if (ilo == -1 && have_b) { ye[0] = yb[0]; ye[1] = yb[1]; ye[2] = yb[2]; }
+                else if (ilo == n - 1) { ye[0] = ya[0]; ye[1] = ya[1]; ye[2] = ya[2]; }
+                else imp32_node<MODE>(F, lr, lb, li, ir, ib, iii, e, ye);
+                const float te = node_theta(e);
+                rate = imp32_rate<MODE>(S32, c, te, ye, frac);                 // cooling time held outside the range
+                theta = c.R / (c.opq + rate);
+                clamped |= 1;
+            } else {
+                if (!have_b) imp32_node<MODE>(F, lr, lb, li, ir, ib, iii, ilo + 1, yb);
+                const float dy[3] = {yb[0] - ya[0], yb[1] - ya[1], yb[2] - ya[2]};
+                auto Rate = [&](float th, float *fr) {
+                    const float w = fminf(fmaxf(coord32(ax, th, one_bits) - (float)ilo, 0.f), 1.f);
+                    const float y[3] = {fmaf(w, dy[0], ya[0]), fmaf(w, dy[1], ya[1]), fmaf(w, dy[2], ya[2])};
+                    return imp32_rate<MODE>(S32, c, th, y, fr);
+                };
+                float lo = node_theta(ilo), hi = fminf(node_theta(ilo + 1), c.R);
+                float flo_ = fmaf(lo, c.opq, -c.R) + lo * Rate(lo, nullptr), fhi = fmaf(hi, c.opq, -c.R) + hi * Rate(hi, nullptr);
+                if (!(flo_ < 0.f)) { hi = lo; fhi = 0.f; }
+                if (!(fhi >= 0.f)) fhi = 0.f;                                  // rounding at the upper node: it is the root
+                int side = 0;
+                for (int it = 0; it < 48 && fhi != 0.f; ++it) {
+                    const float width = hi - lo;
+                    if (!(width > 2.4e-7f * hi)) break;                        // two fp32 ulps
+                    float m = hi - fhi * (width / (fhi - flo_));
+                    if (!(m > lo && m < hi) || (it % 3) == 2) m = lo + 0.5f * width;
+                    if (m == lo || m == hi) break;
+                    const float fm = fmaf(m, c.opq, -c.R) + m * Rate(m, nullptr);
+                    if (fm < 0.f) { lo = m; flo_ = fm; if (side == -1) fhi *= 0.5f; side = -1; }
+                    else { hi = m; fhi = fm; if (side == 1) flo_ *= 0.5f; side = 1; }
+                }
+                theta = hi;
+                rate = Rate(theta, frac);
+            }
+        }
+        const float de = theta * rate;
+        de_sum[0] += de; de_sum[1] = fmaf(de, frac[0], de_sum[1]); de_sum[2] = fmaf(de, frac[1], de_sum[2]); de_sum[3] = fmaf(de, frac[2], de_sum[3]);
+        // Theta_i' = Theta_i - g q (Theta_i - theta) in its cancellation-free form (a >> 1 drives Theta_i' -> theta)
+        thi = fmaf(g * a, theta, thi) / fmaf(a, g, 1.f);
+        the = theta;
+    }
+    const double wgt = (double)rho * (double)vol;
+    const double ds[4] = {(double)de_sum[0], (double)de_sum[1], (double)de_sum[2], (double)de_sum[3]};
+#pragma unroll
+    for (int k = 0; k < 4; ++k) acc.lum[k] += ds[k] * wgt;
+    acc.flo += floored; acc.cla += clamped;
+    shell_add(S, cell, ds, wgt, MODE == 4);
+}
+
+template <int MODE, class Fetch, int THREADS>
+__global__ void __launch_bounds__(THREADS)
+cool_implicit_f32_kernel(const DevTable T, const StepConst S, const F32Const S32, const CellPtrs C, double *partials, unsigned *ticket, cool_diag *d_diag)
+{
+    extern __shared__ __align__(16) unsigned char smem_imp32[];
+    DevTable Tp = T;                                 // the lookup policies of the fp64 path, pointed at the T' arrays
+    Tp.lin1 = T.f1; Tp.lin4 = T.f4; Tp.tex_pt = T.ftex_pt;
+    const Fetch F(Tp, smem_imp32);
+    if (Fetch::kSmem) __syncthreads();
+    DiagAcc acc;
+    const long long stride = (long long)gridDim.x * THREADS;
+    for (long long c = (long long)blockIdx.x * THREADS + threadIdx.x; c < C.ncell; c += stride) {
+        float the = ((const float *)C.the_in)[c], thi = ((const float *)C.thi_in)[c];
+        const float rho = ((const float *)C.rho)[c], bsq = ((const float *)C.bsq)[c];
+        const float rr = S.has_r ? ((const float *)C.r)[c] : 0.f, vv = S.has_vol ? ((const float *)C.vol)[c] : 1.f;
+        implicit_cell_f32<MODE, Fetch>(T, S, S32, F, rho, bsq, the, thi, rr, vv, acc, c);
+        ((float *)C.the_out)[c] = the;
+        ((float *)C.thi_out)[c] = thi;
+    }
+    if (d_diag) reduce_diag(acc, S.lum_k, partials, ticket, d_diag);
+}
+
+template <int MODE, class Fetch>
+static cudaError_t launch_implicit_f32_one(const LaunchCtx &L, const F32Const &S32, size_t smem)
+{
+    constexpr int THREADS = 256;
+    auto kern = cool_implicit_f32_kernel<MODE, Fetch, THREADS>;
+    if (smem > 48 * 1024) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+    }
+    int occ = 0;
+    cudaError_t eo = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, THREADS, smem);
+    if (eo != cudaSuccess) return eo;
+    if (occ < 1) occ = 1;
+    const LaunchArgs &a = *L.a;
+    long long need = (a.ncell + THREADS - 1) / THREADS;
+    const long long cap = (long long)L.t->sm_count * (occ * 8 < 32 ? occ * 8 : 32);
+    const int grid = (int)(need < 1 ? 1 : (need < cap ? need : cap));
+    CellPtrs C{a.rho, a.bsq, a.the_in, a.thi_in, a.r, a.vol, a.the_out, a.thi_out, a.ncell};
+    kern<<<grid, THREADS, smem, L.st>>>(L.t->dev, *L.S, S32, C, a.partials, a.ticket, a.d_diag);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_implicit(const LaunchCtx &L, const F32Const &S32, int mode, cool_variant v, cool_dtype dt);
+
 
 }  // namespace cool

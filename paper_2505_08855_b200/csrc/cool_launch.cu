@@ -1,5 +1,4 @@
 // cool_launch.cu — per-launch constants and dispatch to the kernel instantiations.
-#include "cool_f32.cuh"
 #include "cool_implicit.cuh"
 
 namespace cool {
@@ -105,7 +104,7 @@ cool_status launch_step(const cool_table *t, cool_variant v, cool_dtype dt, cons
     const int mode = t->dev.mode == 0 ? (t->desc.ndim == 4 ? 4 : 3) : t->dev.mode;
     const bool diag = a.want_diag != 0;
     cudaError_t e;
-    if (a.scheme == COOL_SCHEME_IMPLICIT) e = launch_implicit(L, mode, v, dt);
+    if (a.scheme == COOL_SCHEME_IMPLICIT) e = launch_implicit(L, make_f32_const(t, a), mode, v, dt);
     else if (v == COOL_V_ANALYTIC) e = launch_analytic(L, mode, dt, diag);
     else if (dt == COOL_F64) e = launch_f64(L, mode, v, diag);
     else {

@@ -1,6 +1,7 @@
 """Parity of the implicit scheme (COOL_SCHEME_IMPLICIT; PAPER.md L185 (ii), reading C-18) through the C ABI against
-oracle Part B'.  The CUDA path finds the root by safeguarded false position, the oracle by plain bisection; both stop
-within an ulp or two of the root, so fp64 cells agree to 1e-10 and fp32 cells to the rounding of the stored result.
+oracle Part B'.  The CUDA path finds the root by a node search plus safeguarded false position, the oracle by plain
+bisection.  fp64 cells: fp64 solve, both stop within an ulp or two of the root (1e-10).  fp32 cells: fp32 solve on the
+T' tables, refined to a few fp32 ulps (5e-5: see TOL).
 Where Lambda is not monotone in Theta_e several roots can exist: a cell that differs from the oracle must then still
 satisfy the oracle's residual (checked, and such cells must be rare)."""
 import numpy as np
@@ -11,7 +12,10 @@ from paper_2505_08855_b200 import api, synth
 
 pytestmark = pytest.mark.gpu
 
-TOL = {np.float32: 2e-7, np.float64: 1e-10}
+# fp64 cells: fp64 solve.  fp32 cells: fp32 solve on the T' tables; in the strongly cooled limit theta' ~ R/rate carries the
+# full relative error of rate = 2^y with |y| up to ~30 (ulp 1.9e-6, a few roundings, x ln 2: ~4e-6 per sub-step, measured),
+# and it adds over sub-steps (4 sub-steps: measured max 1.6e-5): 5e-5
+TOL = {np.float32: 5e-5, np.float64: 1e-10}
 IMP = api.COOL_SCHEME_IMPLICIT
 
 
@@ -46,7 +50,7 @@ def test_implicit_config1_variants(oracle, dtype, dt, nsub):
         err, nbad = _check(oracle, otab, un, f, got, ref, dtype, dt, nsub, api.VARIANT_NAMES[v])
         print(f"\nimplicit {np.dtype(dtype).name} dt={dt} nsub={nsub} {api.VARIANT_NAMES[v]}: max rel err {err:.2e}, {nbad} cells on another root")
         d, r = got["diag"], ref["diag"]
-        assert d["lum_total"] == pytest.approx(r["lum_total"], rel=1e-6 if dtype == np.float32 else 1e-9)
+        assert d["lum_total"] == pytest.approx(r["lum_total"], rel=2e-5 if dtype == np.float32 else 1e-9)   # a cell on another root moves the sum too
         assert d["n_limited"] == 0 and d["n_clamped"] == r["n_clamped"]
         assert got["launches"] == 1
         if base is None:
@@ -95,7 +99,7 @@ def test_implicit_process_tables_mad_field_floor(oracle, dtype):
         ref = cm.oracle_step_implicit(oracle, otab, un, f, dt, nsub=nsub, h_floor=0.12, use_r=True, use_vol=True)
         got = cm.gpu_step(table, f, dtype, dt, nsub=nsub, h_floor=0.12, use_r=True, use_vol=True, scheme=IMP, variant=api.COOL_V_GLOBAL)
         _check(oracle, otab, un, f, got, ref, dtype, dt, nsub, f"mad dt={dt}")
-        rt = 1e-6 if dtype == np.float32 else 1e-9
+        rt = 2e-5 if dtype == np.float32 else 1e-9
         for k in ("lum_total", "lum_brems", "lum_synch", "lum_compton"):
             assert got["diag"][k] == pytest.approx(ref["diag"][k], rel=rt, abs=1e-300), k
         assert 0 < got["diag"]["n_floored"] == ref["diag"]["n_floored"] < f["rho"].size     # h_floor = 0.12 floors part of this field

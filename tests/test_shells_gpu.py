@@ -18,11 +18,13 @@ def _tables(oracle, n, nc):
     return api.cool_table_create(desc, data, coul), cm.oracle_table(oracle, desc, data, coul), cm.oracle_units(oracle, desc)
 
 
-def _compare(got, ref_shell, ref_diag, rtol):
+def _compare(got, ref_shell, ref_diag, rtol, split_abs=0.0):
+    """split_abs: extra absolute tolerance on the per-process terms, as a fraction of the shell's total (the fp32 kernels
+    form the Compton share as a difference of two rates, (eta - 1) Q_syn, which cancels where eta is within ~1e-6 of 1)."""
     sh = got["lum_shell"]
     assert sh.shape == ref_shell.shape
     scale = np.abs(ref_shell).max(axis=0)
-    assert np.all(np.abs(sh - ref_shell) <= rtol * np.abs(ref_shell) + 1e-3 * rtol * scale)
+    assert np.all(np.abs(sh - ref_shell) <= rtol * np.abs(ref_shell) + 1e-3 * rtol * scale + split_abs * ref_shell[:, :1])
     assert (ref_shell[:, 0] > 0).sum() >= ref_shell.shape[0] - 1         # a real profile, not zeros
     for k, name in enumerate(("lum_total", "lum_brems", "lum_synch", "lum_compton")):
         assert sh[:, k].sum() == pytest.approx(got["diag"][name], rel=10 * rtol, abs=1e-300)
@@ -61,7 +63,8 @@ def test_shell_sums_implicit_and_analytic(oracle, dtype):
     o = oracle.step_implicit(otab, un, f["rho"], f["bsq"], f["theta_e"], f["theta_i"], dt, nsub=2, vol=f["vol"], want_cell_lum=True,
                              nthreads=oracle.max_threads())
     got = cm.gpu_step(table, f, dtype, dt, nsub=2, use_vol=True, shell_cells=SHELL, scheme=api.COOL_SCHEME_IMPLICIT)
-    _compare(got, oracle.shell_sums(o["cell_lum"], SHELL), o["diag"], 1e-6 if dtype == np.float32 else 1e-9)
+    _compare(got, oracle.shell_sums(o["cell_lum"], SHELL), o["diag"], 2e-5 if dtype == np.float32 else 1e-9,
+             split_abs=1e-6 if dtype == np.float32 else 0.0)
     # analytic variant: shells add up to its own total
     got = cm.gpu_step(table, f, dtype, 1.0, use_vol=True, shell_cells=SHELL, variant=api.COOL_V_ANALYTIC)
     assert got["lum_shell"][:, 0].sum() == pytest.approx(got["diag"]["lum_total"], rel=1e-9)
