@@ -145,16 +145,18 @@ __device__ void implicit_cell(const DevTable &T, const DevConst &K, const StepCo
                 double lo = node_theta(ilo), hi = fmin(node_theta(ilo + 1), c.R);
                 double flo_ = lo * opq - c.R + Fseg(lo, nullptr), fhi = hi * opq - c.R + Fseg(hi, nullptr);
                 if (!(flo_ < 0.0)) { hi = lo; fhi = 0.0; }           // rounding at the node: the node is the root
-                int side = 0;
+                int side = 0, stall = 0;
                 for (int it = 0; it < 200 && fhi != 0.0; ++it) {
                     const double width = hi - lo;
                     if (!(width > 4.4408920985006262e-16 * hi)) break;       // two ulps
                     double m = hi - fhi * (width / (fhi - flo_));
-                    if (!(m > lo && m < hi) || (it % 3) == 2) m = lo + 0.5 * width;
+                    if (!(m > lo && m < hi) || stall >= 2) { m = lo + 0.5 * width; stall = 0; }   // bisect when the bracket stalls
                     if (m == lo || m == hi) break;
                     const double fm = m * opq - c.R + Fseg(m, nullptr);
+                    if (fabs(fm) <= 2.3e-16 * c.R) { hi = m; break; }        // below ulp(R) the sign of F is rounding noise
                     if (fm < 0.0) { lo = m; flo_ = fm; if (side == -1) fhi *= 0.5; side = -1; }
                     else { hi = m; fhi = fm; if (side == 1) flo_ *= 0.5; side = 1; }
+                    stall = (hi - lo > 0.5 * width) ? stall + 1 : 0;
                 }
                 theta = hi;
                 de = Fseg(theta, frac);
@@ -347,16 +349,21 @@ __device__ void implicit_cell_f32(const DevTable &T, const StepConst &S, const F
                 float flo_ = fmaf(lo, c.opq, -c.R) + lo * Rate(lo, nullptr), fhi = fmaf(hi, c.opq, -c.R) + hi * Rate(hi, nullptr);
                 if (!(flo_ < 0.f)) { hi = lo; fhi = 0.f; }
                 if (!(fhi >= 0.f)) fhi = 0.f;                                  // rounding at the upper node: it is the root
-                int side = 0;
+                int side = 0, stall = 0;
                 for (int it = 0; it < 48 && fhi != 0.f; ++it) {
                     const float width = hi - lo;
                     if (!(width > 2.4e-7f * hi)) break;                        // two fp32 ulps
                     float m = hi - fhi * (width / (fhi - flo_));
-                    if (!(m > lo && m < hi) || (it % 3) == 2) m = lo + 0.5f * width;
+                    if (!(m > lo && m < hi) || stall >= 2) { m = lo + 0.5f * width; stall = 0; }   // bisect when the bracket stalls
                     if (m == lo || m == hi) break;
                     const float fm = fmaf(m, c.opq, -c.R) + m * Rate(m, nullptr);
+                    // F is a difference of terms of size R: below ~ulp(R) its sign is rounding noise and m is as good a
+                    // root as fp32 can tell (F' >= opq + rate where the rate does not fall with Theta_e, so the error in
+                    // theta is <= ulp(theta))
+                    if (fabsf(fm) <= 1.2e-7f * c.R) { hi = m; break; }
                     if (fm < 0.f) { lo = m; flo_ = fm; if (side == -1) fhi *= 0.5f; side = -1; }
                     else { hi = m; fhi = fm; if (side == 1) flo_ *= 0.5f; side = 1; }
+                    stall = (hi - lo > 0.5f * width) ? stall + 1 : 0;
                 }
                 theta = hi;
                 rate = Rate(theta, frac);
