@@ -362,3 +362,50 @@ def test_large_sample_fp32_and_the_k2_switch_interval(oracle, tab3, dt, nsub, cf
     assert ee[out].max() <= 1e-5 and ei[out].max() <= 1e-5
     assert ee[crossing].max() <= 3e-4 and ei[crossing].max() <= 3e-4
     assert ((ee > 1e-5) | (ei > 1e-5)).sum() <= 40          # a handful of cells, all inside the switch interval
+
+
+def test_table_layouts_agree_bit_for_bit(oracle, monkeypatch):
+    """The GLOBAL variant reads 3-D tables through the oct (<= 16 MiB), quad (<= 64 MiB) or plain layout, chosen at
+    cool_table_create by size; all three feed the same interpolation code and must give identical bits."""
+    desc, data, coul = cm.build_tables([64, 64, 64], nc=[64, 64])
+    f = synth.log_uniform_cells(70001, dtype=np.float32, config=2, outlier_frac=0.01)
+    outs = []
+    for env in ({}, {"COOL_OCT_MAX_MB": "0"}, {"COOL_OCT_MAX_MB": "0", "COOL_QUAD_MAX_MB": "0"}):
+        for k in ("COOL_OCT_MAX_MB", "COOL_QUAD_MAX_MB"):
+            monkeypatch.delenv(k, raising=False)
+        for k, v in env.items():
+            monkeypatch.setenv(k, v)
+        t = api.cool_table_create(desc, data, coul)
+        outs.append(cm.gpu_step(t, f, np.float32, 5.0, nsub=2, variant=api.COOL_V_GLOBAL))
+        t.destroy()
+    for o in outs[1:]:
+        assert np.array_equal(outs[0]["theta_e"], o["theta_e"]) and np.array_equal(outs[0]["theta_i"], o["theta_i"])
+        assert outs[0]["diag"] == o["diag"]
+
+
+def test_concurrent_streams_share_one_table(oracle, tab3):
+    """cool_apply is asynchronous and safe on different streams with the same table (each stream has its own diagnostics
+    workspace): interleaved launches on three streams give the results of the same launches run one after another."""
+    import torch
+    table, otab, un = tab3
+    dev = torch.device("cuda:0")
+    fields = [synth.log_uniform_cells(300007, dtype=np.float32, config=c) for c in (1, 2, 4)]
+    serial = [cm.gpu_step(table, f, np.float32, 2.0, nsub=2, variant=api.COOL_V_GLOBAL) for f in fields]
+    streams = [torch.cuda.Stream(device=dev) for _ in fields]
+    bufs = []
+    for f in fields:
+        d = {k: torch.from_numpy(f[k]).to(dev) for k in ("rho", "bsq", "theta_e", "theta_i")}
+        d["oe"] = torch.empty_like(d["rho"]); d["oi"] = torch.empty_like(d["rho"])
+        d["diag"] = torch.zeros(api.DIAG_BYTES, dtype=torch.uint8, device=dev)
+        bufs.append(d)
+    torch.cuda.synchronize()
+    p = api.make_params(2.0, 2, 0.3, 0.0, api.COOL_V_GLOBAL, api.COOL_COULOMB_AUTO)
+    for rep in range(3):                                   # several rounds of interleaved launches
+        for d, s in zip(bufs, streams):
+            api.cool_apply(table, d["rho"].numel(), api.COOL_F32, d["rho"], d["bsq"], d["theta_e"], d["theta_i"], d["oe"], d["oi"], p,
+                           d_diag=d["diag"], stream=s.cuda_stream)
+    torch.cuda.synchronize()
+    for d, ref in zip(bufs, serial):
+        assert np.array_equal(d["oe"].cpu().numpy().astype(np.float64), ref["theta_e"])
+        assert np.array_equal(d["oi"].cpu().numpy().astype(np.float64), ref["theta_i"])
+        assert api.cool_diag.from_buffer_copy(d["diag"].cpu().numpy().tobytes()).as_dict() == ref["diag"]
