@@ -10,7 +10,7 @@
 //   theta    = root of  F(th) = th - Theta_e + loss(th) - q (Theta_i - th)  in (0, Theta_e + q Theta_i]
 //   Theta_e' = theta,  Theta_i' = Theta_i - g q (Theta_i - theta);  no limiter.
 // F(0) < 0 <= F(Theta_e + q Theta_i) always.  Inside one Theta_e interval of the table every channel is linear in the
-// interval coordinate once (rho, bsq[, Theta_i]) are contracted, so the solve is: (1) a binary search over the table's
+// interval coordinate once (rho, bsq[, Theta_i]) are contracted, so the solve is: (1) a galloping, then binary, search over the table's
 // Theta_e NODES for the interval that brackets the root (one contraction per probed node), (2) inside that interval,
 // Illinois-type false position with a bisection safeguard on values that need no further table access, until the bracket
 // is two ulps wide (outside the table range F is linear: closed form).  F' >= 1 wherever the loss does not decrease
@@ -111,15 +111,20 @@ __device__ void implicit_cell(const DevTable &T, const DevConst &K, const StepCo
             int ilo = -1, ihi = imax + 1;
             double ya[3] = {0, 0, 0}, yb[3] = {0, 0, 0};
             bool have_b = false;
-            while (ihi - ilo > 1) {
-                const int m = (ilo + ihi) >> 1;
+            auto probe = [&](int m) {                        // F at node m; narrows [ilo, ihi]; true when F < 0 there
                 double ym[3];
                 imp_node<MODE>(F, lr, lb, li, m, ym);
                 const double tm = node_theta(m);
                 const double fm = tm * opq - c.R + imp_loss_y<MODE>(S, c, tm, tm, ym, nullptr);
-                if (fm < 0.0) { ilo = m; ya[0] = ym[0]; ya[1] = ym[1]; ya[2] = ym[2]; }
-                else { ihi = m; yb[0] = ym[0]; yb[1] = ym[1]; yb[2] = ym[2]; have_b = true; }
-            }
+                if (fm < 0.0) { ilo = m; ya[0] = ym[0]; ya[1] = ym[1]; ya[2] = ym[2]; return true; }
+                ihi = m; yb[0] = ym[0]; yb[1] = ym[1]; yb[2] = ym[2]; have_b = true;
+                return false;
+            };
+            // gallop down from the node just below R (weak cooling leaves the root in the interval that holds R: one probe),
+            // then bisect what is left
+            for (int m = imax, step = 1; m >= 0; m -= step, step <<= 1)
+                if (probe(m)) break;
+            while (ihi - ilo > 1) probe((ilo + ihi) >> 1);
             if (ilo == -1 || ilo == n - 1) {
                 // 2a. outside the table range the cooling time is held: F is linear, closed form
                 const int e = ilo == -1 ? 0 : n - 1;
@@ -318,15 +323,20 @@ __device__ void implicit_cell_f32(const DevTable &T, const StepConst &S, const F
             int ilo = -1, ihi = imax + 1;
             float ya[3] = {0.f, 0.f, 0.f}, yb[3] = {0.f, 0.f, 0.f};
             bool have_b = false;
-            while (ihi - ilo > 1) {
-                const int m = (ilo + ihi) >> 1;
+            auto probe = [&](int m) {                        // F at node m; narrows [ilo, ihi]; true when F < 0 there
                 float ym[3];
                 imp32_node<MODE>(F, lr, lb, li, ir, ib, iii, m, ym);
                 const float tm = node_theta(m);
                 const float fm = fmaf(tm, c.opq, -c.R) + tm * imp32_rate<MODE>(S32, c, tm, ym, nullptr);
-                if (fm < 0.f) { ilo = m; ya[0] = ym[0]; ya[1] = ym[1]; ya[2] = ym[2]; }
-                else { ihi = m; yb[0] = ym[0]; yb[1] = ym[1]; yb[2] = ym[2]; have_b = true; }
-            }
+                if (fm < 0.f) { ilo = m; ya[0] = ym[0]; ya[1] = ym[1]; ya[2] = ym[2]; return true; }
+                ihi = m; yb[0] = ym[0]; yb[1] = ym[1]; yb[2] = ym[2]; have_b = true;
+                return false;
+            };
+            // gallop down from the node just below R (weak cooling leaves the root in the interval that holds R: one probe),
+            // then bisect what is left
+            for (int m = imax, step = 1; m >= 0; m -= step, step <<= 1)
+                if (probe(m)) break;
+            while (ihi - ilo > 1) probe((ilo + ihi) >> 1);
             if (ilo == -1 || ilo == n - 1) {
                 const int e = ilo == -1 ? 0 : n - 1;
                 float ye[3];
