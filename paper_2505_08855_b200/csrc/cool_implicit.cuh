@@ -356,24 +356,48 @@ __device__ void implicit_cell_f32(const DevTable &T, const StepConst &S, const F
                     return imp32_rate<MODE>(S32, c, th, y, fr);
                 };
                 float lo = node_theta(ilo), hi = fminf(node_theta(ilo + 1), c.R);
-                float flo_ = fmaf(lo, c.opq, -c.R) + lo * Rate(lo, nullptr), fhi = fmaf(hi, c.opq, -c.R) + hi * Rate(hi, nullptr);
-                if (!(flo_ < 0.f)) { hi = lo; fhi = 0.f; }
-                if (!(fhi >= 0.f)) fhi = 0.f;                                  // rounding at the upper node: it is the root
-                int side = 0, stall = 0;
-                for (int it = 0; it < 48 && fhi != 0.f; ++it) {
-                    const float width = hi - lo;
-                    if (!(width > 2.4e-7f * hi)) break;                        // two fp32 ulps
-                    float m = hi - fhi * (width / (fhi - flo_));
-                    if (!(m > lo && m < hi) || stall >= 2) { m = lo + 0.5f * width; stall = 0; }   // bisect when the bracket stalls
-                    if (m == lo || m == hi) break;
-                    const float fm = fmaf(m, c.opq, -c.R) + m * Rate(m, nullptr);
-                    // F is a difference of terms of size R: below ~ulp(R) its sign is rounding noise and m is as good a
-                    // root as fp32 can tell (F' >= opq + rate where the rate does not fall with Theta_e, so the error in
-                    // theta is <= ulp(theta))
-                    if (fabsf(fm) <= 1.2e-7f * c.R) { hi = m; break; }
-                    if (fm < 0.f) { lo = m; flo_ = fm; if (side == -1) fhi *= 0.5f; side = -1; }
-                    else { hi = m; fhi = fm; if (side == 1) flo_ *= 0.5f; side = 1; }
-                    stall = (hi - lo > 0.5f * width) ? stall + 1 : 0;
+                const float noise = 1.2e-7f * c.R;              // F is a difference of terms of size R: below ~ulp(R) its sign is
+                                                                // rounding noise and the point is as good a root as fp32 can tell
+                                                                // (F' >= opq + rate where the rate does not fall with Theta_e, so
+                                                                // the error in theta is <= ulp(theta))
+                float rhi = Rate(hi, nullptr);
+                float fhi = fmaf(hi, c.opq, -c.R) + hi * rhi;
+                if (fhi > noise) {
+                    const float flo0 = fmaf(lo, c.opq, -c.R) + lo * Rate(lo, nullptr);
+                    if (!(flo0 < 0.f)) { hi = lo; fhi = 0.f; }                  // rounding at the lower node: it is the root
+                    if constexpr (MODE == 3) {
+                        // inside the interval the rate is an exact power law, rate ~ theta^p with p = dy invf, so
+                        // F' = opq + rate (1 + p): Newton steps, kept inside the bracket
+                        const float p1 = fmaf(dy[0], ax.invf, 1.f);
+                        float x = hi, fx = fhi, rx = rhi;
+                        for (int it = 0; it < 40 && fabsf(fx) > noise; ++it) {
+                            const float d = fmaf(rx, p1, c.opq);
+                            float m = d > 0.25f * c.opq ? x - fx / d : lo + 0.5f * (hi - lo);
+                            if (!(m > lo && m < hi)) m = lo + 0.5f * (hi - lo);
+                            if (m == lo || m == hi) break;
+                            const float rm = Rate(m, nullptr), fm = fmaf(m, c.opq, -c.R) + m * rm;
+                            if (fm < 0.f) lo = m; else hi = m;
+                            const bool done = fabsf(m - x) <= 1.2e-7f * m;
+                            x = m; fx = fm; rx = rm;
+                            if (done) break;
+                        }
+                        hi = x;
+                    } else {
+                        float flo_ = flo0;
+                        int side = 0, stall = 0;
+                        for (int it = 0; it < 48 && fhi != 0.f; ++it) {
+                            const float width = hi - lo;
+                            if (!(width > 2.4e-7f * hi)) break;                        // two fp32 ulps
+                            float m = hi - fhi * (width / (fhi - flo_));
+                            if (!(m > lo && m < hi) || stall >= 2) { m = lo + 0.5f * width; stall = 0; }   // bisect when the bracket stalls
+                            if (m == lo || m == hi) break;
+                            const float fm = fmaf(m, c.opq, -c.R) + m * Rate(m, nullptr);
+                            if (fabsf(fm) <= noise) { hi = m; break; }
+                            if (fm < 0.f) { lo = m; flo_ = fm; if (side == -1) fhi *= 0.5f; side = -1; }
+                            else { hi = m; fhi = fm; if (side == 1) flo_ *= 0.5f; side = 1; }
+                            stall = (hi - lo > 0.5f * width) ? stall + 1 : 0;
+                        }
+                    }
                 }
                 theta = hi;
                 rate = Rate(theta, frac);
