@@ -428,13 +428,23 @@ cool_implicit_f32_kernel(const DevTable T, const StepConst S, const F32Const S32
     if (Fetch::kSmem) __syncthreads();
     DiagAcc acc;
     const long long stride = (long long)gridDim.x * THREADS;
-    for (long long c = (long long)blockIdx.x * THREADS + threadIdx.x; c < C.ncell; c += stride) {
-        float the = ((const float *)C.the_in)[c], thi = ((const float *)C.thi_in)[c];
-        const float rho = ((const float *)C.rho)[c], bsq = ((const float *)C.bsq)[c];
-        const float rr = S.has_r ? ((const float *)C.r)[c] : 0.f, vv = S.has_vol ? ((const float *)C.vol)[c] : 1.f;
+    long long c = (long long)blockIdx.x * THREADS + threadIdx.x;
+    // the next cell's values are requested before the current cell is solved: the solve hides the HBM latency
+    float n_the = 0.f, n_thi = 0.f, n_rho = 0.f, n_bsq = 0.f, n_rr = 0.f, n_vv = 1.f;
+    auto fetch = [&](long long k) {
+        n_the = __ldcs((const float *)C.the_in + k); n_thi = __ldcs((const float *)C.thi_in + k);
+        n_rho = __ldcs((const float *)C.rho + k); n_bsq = __ldcs((const float *)C.bsq + k);
+        if (S.has_r) n_rr = __ldcs((const float *)C.r + k);
+        if (S.has_vol) n_vv = __ldcs((const float *)C.vol + k);
+    };
+    if (c < C.ncell) fetch(c);
+    for (; c < C.ncell; c += stride) {
+        float the = n_the, thi = n_thi;
+        const float rho = n_rho, bsq = n_bsq, rr = n_rr, vv = n_vv;
+        if (c + stride < C.ncell) fetch(c + stride);
         implicit_cell_f32<MODE, Fetch>(T, S, S32, F, rho, bsq, the, thi, rr, vv, acc, c);
-        ((float *)C.the_out)[c] = the;
-        ((float *)C.thi_out)[c] = thi;
+        __stcs((float *)C.the_out + c, the);
+        __stcs((float *)C.thi_out + c, thi);
     }
     if (d_diag) reduce_diag(acc, S.lum_k, partials, ticket, d_diag);
 }
