@@ -270,8 +270,6 @@ extern "C" cool_status cool_table_create(const cool_table_desc *desc, int device
         if (bytes > 0xffffffffull) { set_error("table too large"); return fail(COOL_EINVAL); }
         std::vector<float> canon;
         try { canon.assign(bytes / sizeof(float), 0.f); } catch (...) { set_error("out of host memory"); return fail(COOL_ENOMEM); }
-        long long sstride[4];
-        { long long s = 1; for (int k = nd - 1; k >= 0; --k) { sstride[k] = s; s *= desc->n[k]; } }
         long long cstride_of_src[4];          // canonical stride (in nodes) for source axis k
         for (int k = 0; k < nd; ++k) {
             const int slot = canon_slot(desc->axis[k]);
@@ -288,7 +286,6 @@ extern "C" cool_status cool_table_create(const cool_table_desc *desc, int device
             }
             for (int k = nd - 1; k >= 0; --k) { if (++idx[k] < desc->n[k]) break; idx[k] = 0; }
         }
-        (void)sstride;
         cudaError_t e = cudaMalloc(&t->d_lin, bytes);
         if (e != cudaSuccess) { set_error("cudaMalloc(table): %s", cudaGetErrorString(e)); return fail(e == cudaErrorMemoryAllocation ? COOL_ENOMEM : COOL_ECUDA); }
         e = cudaMemcpy(t->d_lin, canon.data(), bytes, cudaMemcpyHostToDevice);
