@@ -150,6 +150,7 @@ __device__ void implicit_cell(const DevTable &T, const DevConst &K, const StepCo
                 double lo = node_theta(ilo), hi = fmin(node_theta(ilo + 1), c.R);
                 double flo_ = lo * opq - c.R + Fseg(lo, nullptr), fhi = hi * opq - c.R + Fseg(hi, nullptr);
                 if (!(flo_ < 0.0)) { hi = lo; fhi = 0.0; }           // rounding at the node: the node is the root
+                if (fhi <= 2.3e-16 * c.R) fhi = 0.0;                 // weak cooling: F at the bracket end is already rounding noise
                 int side = 0, stall = 0;
                 for (int it = 0; it < 200 && fhi != 0.0; ++it) {
                     const double width = hi - lo;
