@@ -390,12 +390,12 @@ __device__ __forceinline__ float coulomb_C32(int n1, int qstride, const float *c
 {
     const int off = loc_bits(a) * n1 + (loc_bits(b) + (int)(0u - kMagicBits * (unsigned)(n1 + 1)));
     float c00, c01, c10, c11;
-    if constexpr (CM == 1 && QUAD) {
+    if constexpr (CM >= 1 && QUAD) {
         // quad rows are skewed (row stride = 3 mod 8 quads) so that neighbouring (i, e) quads fall in different bank groups
         const int qoff = loc_bits(a) * qstride + (loc_bits(b) + (int)(0u - kMagicBits * (unsigned)(qstride + 1)));
         const float4 q = lds_f4(cs + 16u * (unsigned)qoff);
         c00 = q.x; c01 = q.y; c10 = q.z; c11 = q.w;
-    } else if constexpr (CM == 1) {
+    } else if constexpr (CM >= 1) {
         const unsigned p = cs + 4u * (unsigned)off, q = p + 4u * (unsigned)n1;
         c00 = lds_f32(p); c01 = lds_f32(p + 4); c10 = lds_f32(q); c11 = lds_f32(q + 4);
     } else {
@@ -421,6 +421,13 @@ __device__ __forceinline__ void shell_flush(const F32Const &S, const float (&par
     }
 }
 
+// Layout of the Coulomb table in shared memory, chosen by the launcher through CM: CM = 1 quads (64 KiB for 64^2, one
+// LDS.128 per cell) — except for the SMEM variant, whose table image leaves no room: plain there too; CM = 2 the plain
+// table (16 KiB, four LDS.32), used for small launches with diagnostics (configs[2]-sized: 8 M cells), where it measures
+// 13 % faster (0.089 -> 0.077 ms) while at 512^3 the quads win by 6 %.
+template <class Fetch, int CM>
+__host__ __device__ constexpr bool coul_quads() { return CM == 1 && !Fetch::kSmem; }
+
 struct Ctx32 { const DevTable &T; const F32Const &S; unsigned coul_s; };      // coul_s: shared-memory address of the staged Coulomb quads
 
 // ------------------------------------------------------------------------------------------
@@ -436,7 +443,7 @@ __device__ __forceinline__ void step_cells_f32(const Ctx32 &X, const Fetch &F, c
                                                const float *rr, const float *vol, DiagAcc &acc, float (&tile_part)[4], unsigned wtile)
 {
     const DevTable &T = X.T; const F32Const &S = X.S;
-    const int coulomb = (CM == 1) ? 1 : S.coulomb;
+    const int coulomb = (CM >= 1) ? 1 : S.coulomb;
     const int one_bits = opaque_const(0x3f800000);
     const bool use_floor = S.hfloor2 > 0.f;                 // warp-uniform
     bool bad[NV], any_bad = false;
@@ -533,7 +540,7 @@ __device__ __forceinline__ void step_cells_f32(const Ctx32 &X, const Fetch &F, c
                         if (MODE == 4) ca = split32<false>(T.cax[0], fmaf(ti, S.cmi_s, S.cmi_o), dummy);
                         else ca = locate32<false>(T.cax[0], thi[j], dummy, one_bits);
                         cb = split32<false>(T.cax[1], fmaf(te, S.cme_s, S.cme_o), dummy);
-                        C = coulomb_C32<CM, !Fetch::kSmem>(T.cax[1].n, T.coulq_stride, T.fcoul, X.coul_s, ca, cb);
+                        C = coulomb_C32<CM, coul_quads<Fetch, CM>()>(T.cax[1].n, T.coulq_stride, T.fcoul, X.coul_s, ca, cb);
                     }
                 } else {
                     C = (D != 0.f && !bad[j]) ? (float)coolphys::coulomb_C((double)the[j], (double)thi[j] / S.ion_ratio) : 0.f;
@@ -626,17 +633,25 @@ __global__ void __launch_bounds__(THREADS, 1)
 cool_f32_kernel(const DevTable T, const F32Const S, const CellPtrs C, double *partials, unsigned *ticket, cool_diag *d_diag)
 {
     constexpr int NW = THREADS / 32;
-    static_assert(NW * NST * 8 <= (int)kF32BarBytes, "mbarrier area too small");
+    static_assert(NW * NST * 8 <= (int)kF32BarBytes - 8, "mbarrier area too small");
     extern __shared__ __align__(128) unsigned char smem_f32[];
     const int tid = threadIdx.x, lane = tid & 31;
     const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);           // warp-uniform by construction: TMA operands stay in uniform registers
 
     // ---- prologue (the only CTA-wide barrier): stage the Coulomb quads / table image, arm the warp's barriers
-    if (CM == 1 && S.coul_smem) {
-        float4 *dst = (float4 *)(smem_f32 + S.coul_off);
-        const float4 *src = Fetch::kSmem ? (const float4 *)T.fcoul : T.fcoulq;     // plain table padded to 16 B at create time
-        const unsigned n16 = (unsigned)(Fetch::kSmem ? ((T.coul_bytes + 15) >> 4) : (T.coulq_bytes >> 4));
-        for (unsigned k = tid; k < n16; k += THREADS) dst[k] = ldg_f4(src + k);
+    // The Coulomb table comes in by TMA bulk copies on a barrier of its own (last slot of the barrier area): the warps
+    // arm their cell pipelines meanwhile and wait for it only just before the first tile
+    const unsigned cbar = smem_u32(smem_f32) + kF32BarBytes - 8u;
+    if (CM >= 1 && S.coul_smem && tid == 0) {
+        constexpr bool kQuads = coul_quads<Fetch, CM>();
+        const char *src = kQuads ? (const char *)T.fcoulq : (const char *)T.fcoul;  // plain table padded to 16 B at create time
+        const unsigned bytes = kQuads ? (unsigned)T.coulq_bytes : (((unsigned)T.coul_bytes + 15u) & ~15u);
+        mbar_init(cbar, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        mbar_expect_tx(cbar, bytes);
+        const unsigned dst = smem_u32(smem_f32 + S.coul_off);
+        for (unsigned o = 0; o < bytes; o += 16384u) tma_load_1d(dst + o, src + o, min(16384u, bytes - o), cbar);
     }
     if constexpr (Fetch::kSmem) {
         const float4 *src = MODE == 3 ? (const float4 *)T.f1 : T.f4;
@@ -685,6 +700,7 @@ cool_f32_kernel(const DevTable T, const F32Const S, const CellPtrs C, double *pa
     }
     __syncwarp();
 
+    if (CM >= 1 && S.coul_smem) mbar_wait(cbar, 0);
     DiagAcc acc;
     int s = 0; unsigned phase = 0;
     for (; tile < ntiles; tile += GW) {
@@ -766,13 +782,13 @@ constexpr int kF32SmemThreads = 384, kF32SmemStages = 2;    // SMEM variant: the
 constexpr int kCoulQuadSmemMax = 73728;                     // Coulomb quads up to 64 x (64 + 3 skew) x 16 B are staged in shared memory
 
 // fills the shared-memory layout fields of S for a launch with `threads` threads; returns the total
-inline size_t f32_smem_layout(F32Const &S, int threads, int nst, bool table_in_smem, const cool_table *t)
+inline size_t f32_smem_layout(F32Const &S, int threads, int nst, bool table_in_smem, bool coul_quad, const cool_table *t)
 {
     S.wstage_bytes = kWarpArrBytes * (unsigned)S.nf;
     S.stage_off = kF32BarBytes;
     size_t off = kF32BarBytes + (size_t)(threads / 32) * nst * S.wstage_bytes;
     S.coul_off = (unsigned)off;
-    if (S.coul_smem) off += table_in_smem ? (((size_t)t->dev.coul_bytes + 15) & ~(size_t)15) : (size_t)t->dev.coulq_bytes;
+    if (S.coul_smem) off += coul_quad ? (size_t)t->dev.coulq_bytes : (((size_t)t->dev.coul_bytes + 15) & ~(size_t)15);
     S.table_off = (unsigned)off;
     if (table_in_smem) off += t->dev.table_bytes;
     return off;
@@ -782,7 +798,7 @@ template <int MODE, class Fetch, bool DIAG, int CM, bool NSUB1, int THREADS, int
 static cudaError_t launch_f32_one(const LaunchCtx32 &L)
 {
     F32Const S = L.S;
-    const size_t smem = f32_smem_layout(S, THREADS, NST, Fetch::kSmem, L.t);
+    const size_t smem = f32_smem_layout(S, THREADS, NST, Fetch::kSmem, coul_quads<Fetch, CM>(), L.t);
     auto kern = cool_f32_kernel<MODE, Fetch, DIAG, CM, NSUB1, THREADS, NST>;
     if (smem > 48 * 1024) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);

@@ -8,7 +8,7 @@ static cudaError_t go(const LaunchCtx32 &L, cool_variant v, bool nsub1)
 }
 cudaError_t launch_f32_m3(const LaunchCtx32 &L, cool_variant v, bool diag, int cm, bool nsub1)
 {
-    if (diag) return cm ? go<true, 1>(L, v, nsub1) : go<true, 0>(L, v, nsub1);
+    if (diag) return cm == 2 ? go<true, 2>(L, v, nsub1) : cm ? go<true, 1>(L, v, nsub1) : go<true, 0>(L, v, nsub1);
     return cm ? go<false, 1>(L, v, nsub1) : go<false, 0>(L, v, nsub1);
 }
 }  // namespace cool

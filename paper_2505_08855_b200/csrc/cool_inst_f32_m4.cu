@@ -3,7 +3,7 @@
 namespace cool {
 cudaError_t launch_f32_m4(const LaunchCtx32 &L, cool_variant v, bool diag, int cm)
 {
-    if (diag) return cm ? launch_f32_by_variant<4, true, 1, false>(L, v) : launch_f32_by_variant<4, true, 0, false>(L, v);
+    if (diag) return cm == 2 ? launch_f32_by_variant<4, true, 2, false>(L, v) : cm ? launch_f32_by_variant<4, true, 1, false>(L, v) : launch_f32_by_variant<4, true, 0, false>(L, v);
     return cm ? launch_f32_by_variant<4, false, 1, false>(L, v) : launch_f32_by_variant<4, false, 0, false>(L, v);
 }
 }  // namespace cool

@@ -37,13 +37,17 @@ static StepConst make_step_const(const cool_table *t, cool_dtype dt, const Launc
     return S;
 }
 
-// Coulomb coefficient table staged in shared memory: quads (<= 64 KiB) for the GLOBAL / texture variants,
-// the plain layout (<= 16 KiB) for the SMEM variant; not needed when it rides in the 4-D texels.
-static bool coulomb_in_smem(const cool_table *t, const LaunchArgs &a, cool_variant v)
+// Coulomb coefficient table staged in shared memory (not needed when it rides in the 4-D texels): returns the kernels'
+// CM — 0 not staged, 1 quads (<= 72 KiB; the SMEM variant stores the plain table under CM = 1), 2 plain table (<= 16 KiB)
+// for small launches with diagnostics.
+constexpr long long kCoulPlainBelowCells = 1ll << 25;
+static int coulomb_smem_mode(const cool_table *t, const LaunchArgs &a, cool_variant v)
 {
     const DevTable &D = t->dev;
-    if (a.coulomb != 1 || !D.fcoul || (D.mode == 4 && D.f4_has_coul)) return false;
-    return v == COOL_V_SMEM ? D.coul_bytes <= kCoulSmemMax : D.coulq_bytes <= kCoulQuadSmemMax;
+    if (a.coulomb != 1 || !D.fcoul || (D.mode == 4 && D.f4_has_coul)) return 0;
+    if (v == COOL_V_SMEM) return D.coul_bytes <= kCoulSmemMax ? 1 : 0;
+    if (a.want_diag && a.ncell < kCoulPlainBelowCells && D.coul_bytes <= kCoulSmemMax) return 2;
+    return D.coulq_bytes <= kCoulQuadSmemMax ? 1 : 0;
 }
 
 static F32Const make_f32_const(const cool_table *t, const LaunchArgs &a)
@@ -109,9 +113,10 @@ cool_status launch_step(const cool_table *t, cool_variant v, cool_dtype dt, cons
     else if (dt == COOL_F64) e = launch_f64(L, mode, v, diag);
     else {
         LaunchCtx32 L32{t, make_f32_const(t, a), &a, st};
-        L32.S.coul_smem = coulomb_in_smem(t, a, v);
+        const int csm = coulomb_smem_mode(t, a, v);
+        L32.S.coul_smem = csm != 0;
         // fast path: Coulomb from the coefficient table staged in shared memory (or riding in the 4-D texels)
-        const int cm = (a.coulomb == 1 && (L32.S.coul_smem || (mode == 4 && t->dev.f4_has_coul))) ? 1 : 0;
+        const int cm = a.coulomb == 1 ? (csm ? csm : (mode == 4 && t->dev.f4_has_coul ? 1 : 0)) : 0;
         e = (mode == 3) ? launch_f32_m3(L32, v, diag, cm, a.nsub == 1) : launch_f32_m4(L32, v, diag, cm);
     }
     if (e != cudaSuccess) { set_error("kernel launch failed: %s", cudaGetErrorString(e)); return COOL_ECUDA; }
