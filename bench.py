@@ -377,7 +377,7 @@ def main():
     explicit = args.scheme == "explicit"
     kernel_name = ("cool_implicit_f32_kernel<MODE=%d, %s>" % (mode, api.VARIANT_NAMES[resolved])) if not explicit else "cool_f32_kernel<MODE=%d, %s, DIAG=%d, CM=1, NSUB1=%d, %s>" % (
         mode, fetch, int(bool(spec["diag"])), int(spec["nsub"] == 1),
-        "384 threads, 2 stages" if fetch == "F32Smem" else ("768 threads, 2 stages" if single else "512 threads, 3 stages"))
+        "384 threads, 2 stages" if fetch == "F32Smem" else ("768 threads, 2 stages" if single else "512 threads, 2 stages"))
     line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=args.warmup,
                 ms_per_step=total_ms / args.steps, higher_is_better=True, scaling="weak", vs_baseline=None,
                 dtype="f32", data="synthetic",

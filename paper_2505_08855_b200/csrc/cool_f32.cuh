@@ -777,7 +777,7 @@ cool_f32_kernel(const DevTable T, const F32Const S, const CellPtrs C, double *pa
 struct LaunchCtx32 { const cool_table *t; F32Const S; const LaunchArgs *a; cudaStream_t st; };
 
 constexpr int kF32Threads3 = 768, kF32Stages3 = 2;          // GLOBAL / texture variants, single-update 3-D step: 24 warps, 2 stages each
-constexpr int kF32Threads4 = 512, kF32Stages4 = 3;          // GLOBAL / texture variants, sub-stepped or 4-D: 16 warps, 3 stages each
+constexpr int kF32Threads4 = 512, kF32Stages4 = 2;          // GLOBAL / texture variants, sub-stepped or 4-D: 16 warps, 2 stages each
 constexpr int kF32SmemThreads = 384, kF32SmemStages = 2;    // SMEM variant: the table image takes most of the shared memory
 constexpr int kCoulQuadSmemMax = 73728;                     // Coulomb quads up to 64 x (64 + 3 skew) x 16 B are staged in shared memory
 
@@ -819,7 +819,7 @@ static cudaError_t launch_f32_by_variant(const LaunchCtx32 &L, cool_variant v)
 {
     // The single-update 3-D step fits 80 registers: 24 warps per SM hide the gather latency (measured best on B200:
     // 768 threads, 2 stages).  Sub-stepping loops and MODE 4 (a 16-register patch per cell) need 128 registers:
-    // 16 warps, 3 stages.
+    // 16 warps, 2 stages (3 stages measure 1-4 % slower: less L1 under the gathers).
     constexpr bool kWide = MODE == 3 && NSUB1;
     constexpr int TH = kWide ? kF32Threads3 : kF32Threads4, NS = kWide ? kF32Stages3 : kF32Stages4;
     switch (v) {
