@@ -20,6 +20,7 @@ import os
 import subprocess
 import sys
 import tempfile
+import threading
 import time
 
 import numpy as np
@@ -129,43 +130,101 @@ def oracle_leg(spec, desc, data, coul, fields, sample_cells, steps=1, scheme="ex
 
 
 # ------------------------------------------------------------------------------------------------
-def clocks_monitor_start(gpu_index):
-    f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
-    q = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
-        "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
-    try:
-        p = subprocess.Popen(["nvidia-smi", f"--id={gpu_index}", f"--query-gpu={q}", "--format=csv,noheader,nounits", "-lms", "100"],
-                             stdout=f, stderr=subprocess.DEVNULL)
-    except OSError:
-        return None, f.name
-    return p, f.name
+class ClocksMonitor:
+    """SM clock and clock-event reasons sampled DURING the timed region (B200_PROFILING.md, clocks line).  The timed region
+    of the default run is ~80 ms, shorter than nvidia-smi's start-up, so the samples come from NVML (the library nvidia-smi
+    reads) on a thread of this process, every 2 ms; `nvidia-smi -lms` is the fallback when NVML cannot be loaded."""
+    REASONS = (("hw_slowdown", 0x8), ("hw_thermal_slowdown", 0x40), ("sw_thermal_slowdown", 0x20), ("sw_power_cap", 0x4))
 
-
-def clocks_monitor_stop(p, path):
-    out = dict(sm_mhz=None, sm_max_mhz=None, reasons=[], samples=0)
-    if p is not None:
-        p.terminate()
+    def __init__(self, uuid):
+        self.rows, self.max_mhz, self.source = [], None, None
+        self._stop, self._thread, self._proc, self._path = threading.Event(), None, None, None
         try:
-            p.wait(timeout=5)
+            import pynvml
+            pynvml.nvmlInit()
+            uuid = str(uuid)
+            uuid = uuid if uuid.startswith("GPU-") else "GPU-" + uuid
+            try:
+                self._h = pynvml.nvmlDeviceGetHandleByUUID(uuid)
+            except Exception:
+                self._h = pynvml.nvmlDeviceGetHandleByUUID(uuid.encode())
+            self._nv = pynvml
+            self._reasons = getattr(pynvml, "nvmlDeviceGetCurrentClocksEventReasons", None) or pynvml.nvmlDeviceGetCurrentClocksThrottleReasons
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self._h, pynvml.NVML_CLOCK_SM))
+            self._sample()                       # fails here, not on the thread, if the queries are not supported
+            self.rows.clear()
+            self.source = "nvml"
         except Exception:
-            p.kill()
-    try:
-        rows = [r.strip().split(",") for r in open(path) if r.strip()]
-        sm = [float(r[0]) for r in rows if len(r) >= 7]
-        if sm:
-            out["sm_mhz"] = float(np.median(sm)); out["sm_max_mhz"] = float(rows[0][1]); out["samples"] = len(sm)
-            names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-            for k, nm in enumerate(names):
-                if any(r[3 + k].strip().lower().startswith("active") for r in rows if len(r) >= 7):
-                    out["reasons"].append(nm)
-    except Exception:
-        pass
-    finally:
+            self._nv = None
+
+    def _sample(self):
+        nv = self._nv
+        self.rows.append((float(nv.nvmlDeviceGetClockInfo(self._h, nv.NVML_CLOCK_SM)), int(self._reasons(self._h))))
+
+    def _run(self):
+        while not self._stop.is_set():
+            try:
+                self._sample()
+            except Exception:
+                break
+            self._stop.wait(0.002)
+
+    def start(self, gpu_index):
+        if self._nv is not None:
+            self._thread = threading.Thread(target=self._run, daemon=True)
+            self._thread.start()
+            return
+        f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self._path = f.name
+        q = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
+            "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
         try:
-            os.unlink(path)
+            self._proc = subprocess.Popen(["nvidia-smi", f"--id={gpu_index}", f"--query-gpu={q}", "--format=csv,noheader,nounits", "-lms", "20"],
+                                          stdout=f, stderr=subprocess.DEVNULL)
+            self.source = "nvidia-smi"
+            t0 = time.time()                     # wait for its first row so that the timed region is covered
+            while time.time() - t0 < 5.0 and os.path.getsize(self._path) == 0:
+                time.sleep(0.01)
         except OSError:
+            self._proc = None
+
+    def stop(self):
+        out = dict(sm_mhz=None, sm_max_mhz=self.max_mhz, reasons=[], samples=0, source=self.source)
+        if self._thread is not None:
+            self._stop.set()
+            self._thread.join(timeout=2)
+            if self.rows:
+                out["sm_mhz"] = float(np.median([r[0] for r in self.rows])); out["samples"] = len(self.rows)
+                out["sm_min_mhz"] = float(min(r[0] for r in self.rows))
+                bits = 0
+                for r in self.rows:
+                    bits |= r[1]
+                out["reasons"] = [nm for nm, b in self.REASONS if bits & b]
+            return out
+        if self._proc is not None:
+            self._proc.terminate()
+            try:
+                self._proc.wait(timeout=5)
+            except Exception:
+                self._proc.kill()
+        try:
+            rows = [r.strip().split(",") for r in open(self._path) if r.strip()]
+            rows = [r for r in rows if len(r) >= 7]
+            if rows:
+                sm = [float(r[0]) for r in rows]
+                out["sm_mhz"] = float(np.median(sm)); out["sm_min_mhz"] = float(min(sm)); out["sm_max_mhz"] = float(rows[0][1]); out["samples"] = len(sm)
+                for k, (nm, _) in enumerate(self.REASONS):
+                    if any(r[3 + k].strip().lower().startswith("active") for r in rows):
+                        out["reasons"].append(nm)
+        except Exception:
             pass
-    return out
+        finally:
+            try:
+                if self._path:
+                    os.unlink(self._path)
+            except OSError:
+                pass
+        return out
 
 
 def main():
@@ -271,15 +330,17 @@ def main():
         step()
     launches_per_step = api.cool_last_launch_count()
     barrier()
-    mon, mon_path = clocks_monitor_start(local_rank) if rank == 0 else (None, None)
+    mon = ClocksMonitor(torch.cuda.get_device_properties(dev).uuid) if rank == 0 else None
     ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
     barrier()
+    if mon is not None:
+        mon.start(local_rank)
     ev[0].record()
     for k in range(args.steps):
         step()
         ev[k + 1].record()
     barrier()
-    clocks = clocks_monitor_stop(mon, mon_path) if rank == 0 else None
+    clocks = mon.stop() if rank == 0 else None
     per_step_ms = np.array([ev[k].elapsed_time(ev[k + 1]) for k in range(args.steps)])
     total_ms = float(ev[0].elapsed_time(ev[-1]))
     if world > 1:
