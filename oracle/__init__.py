@@ -113,6 +113,8 @@ def lib():
             "orc_fill_total3": (None, [UP, C.POINTER(i), C.POINTER(d), C.POINTER(d), p, i]),
             "orc_fill_coulomb2": (None, [UP, C.POINTER(i), C.POINTER(d), C.POINTER(d), p]),
             "orc_max_threads": (i, []),
+            "orc_tau_sca_cell": (d, [UP, d, d]),
+            "orc_radpress": (None, [UP, C.c_longlong, p, p, p, d, p, C.POINTER(C.c_longlong)]),
         }
         for name, (res, args) in sig.items():
             f = getattr(L, name); f.restype = res; f.argtypes = args
@@ -276,3 +278,18 @@ def implicit_residual(table: Table, un: Units, rho, bsq, theta_e, theta_i, dt, t
         coulomb_mode = COULOMB_TABLE if table.coul is not None else COULOMB_ANALYTIC
     return lib().orc_implicit_residual(C.byref(table._c), C.byref(un), float(rho), float(bsq), float(theta_e), float(theta_i),
                                        float(r), float(dt), int(nsub), float(h_floor), int(coulomb_mode), float(theta_trial))
+
+
+# ---- Part C: radiation-pressure temperature correction (eq 29) ---------------------------
+def tau_sca(un, rho, hscale_rg): return lib().orc_tau_sca_cell(C.byref(un), rho, hscale_rg)
+
+
+def radpress(un: Units, rho, theta_e, hscale_rg, tau_crit=1.0):
+    """Theta_e corrected for radiation pressure where tau_sca = n_e sigma_T H > tau_crit (eq 29; C-20).
+    Returns (theta_e_out, n_corrected)."""
+    rho, the, hs = (np.ascontiguousarray(a, dtype=np.float64) for a in (rho, theta_e, hscale_rg))
+    out = np.empty_like(the)
+    cnt = C.c_longlong(0)
+    lib().orc_radpress(C.byref(un), rho.size, rho.ctypes.data, the.ctypes.data, hs.ctypes.data, float(tau_crit),
+                       out.ctypes.data, C.byref(cnt))
+    return out, int(cnt.value)

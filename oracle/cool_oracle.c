@@ -9,11 +9,14 @@
  * Part A  analytic physics, §II eqs 1-15 (L57-L147)
  * Part B  the table-interpolated, limited, sub-stepped update (PAPER.md L122-L124,
  *         L181, L185, L197; readings C-1..C-17 of SURVEY.md §8(c) / DESIGN.md)
+ * Part B' the implicit scheme (L185 (ii), L369; reading C-18)
+ * Part C  the radiation-pressure temperature correction (eq 29; reading C-20)
  *
  * Pins (tests/test_oracle_*.py): closed-form brems scaling, incomplete-gamma closed
  * form of the synchrotron integral, scipy.special.kve for the Bessel functions,
  * residual of eq 5, limits of eqs 7 and 11, node-exact / linear-exact interpolation,
- * conservation / positivity / no-crossing of the update, brute force on tiny tables.
+ * conservation / positivity / no-crossing of the update, brute force on tiny tables;
+ * Part C: manufactured roots of eq 29, mpmath roots of the unreduced quartic, both limits.
  * Nothing here is "parity unpinned".
  *
  * Everything is double precision; no blocking, fusion or reordering beyond what the
@@ -723,4 +726,58 @@ int orc_max_threads(void)
 #else
     return 1;
 #endif
+}
+
+/* ======================================================================================
+ * Part C — radiation-pressure temperature correction (eq 29;
+ * DESIGN.md reading C-20).  Post-processing, cell by cell.
+ *
+ *   P = P_rad + P_gas = a T_e^4 + N k_B T_gas,   T_gas = T_e + T_i          (eq 29)
+ *
+ * P is the pressure the simulation holds for the cell, which has no radiation term (L332:
+ * "our simulations do not take radiation pressure into account"): P = N k_B (T_e + T_i)
+ * with the simulated temperatures.  The paper recalculates T_e only (L345), so T_i is the
+ * simulated one on both sides and N k_B T_i cancels:
+ *
+ *   a T^4 + N k_B (T - T_e) = 0,     0 < T <= T_e                             (one root)
+ *
+ * solved where the in-cell scattering depth tau_sca = n_e sigma_T H(r) (L353) exceeds a
+ * threshold (1 for Fig. 9(b); 4.6 for Fig. 10); other cells keep T_e.
+ * a = 7.5646e-15 erg cm^-3 K^-4 is the value the paper prints (L345), not 4 sigma_SB/c.
+ * N = n_e (C-14: fully ionised hydrogen).  The root is found by bisection on [0, T_e].
+ * ====================================================================================== */
+#define ORC_ARAD 7.5646e-15           /* erg cm^-3 K^-4, as printed (L345) */
+
+double orc_tau_sca_cell(const orc_units *u, double rho, double hscale_rg)     /* L353 */
+{
+    return orc_ne_cgs(u, rho) * ORC_SIGT * (hscale_rg * orc_rg(u));
+}
+
+/* Returns the corrected Theta_e; *corrected = 1 if the quartic was solved for this cell. */
+double orc_radpress_cell(const orc_units *u, double rho, double the, double hscale_rg, double tau_crit, int *corrected)
+{
+    *corrected = 0;
+    if (!(rho > 0.0) || !(the > 0.0) || !(orc_tau_sca_cell(u, rho, hscale_rg) > tau_crit)) return the;
+    double N = orc_ne_cgs(u, rho);
+    double Te = the * ORC_ME * ORC_C * ORC_C / ORC_KB;          /* K */
+    double lo = 0.0, hi = Te;                                   /* f(0) = -N k T_e < 0 <= a T_e^4 = f(T_e) */
+    for (int it = 0; it < 200; ++it) {
+        double T = 0.5 * (lo + hi);
+        double f = ORC_ARAD * T * T * T * T + N * ORC_KB * (T - Te);
+        if (f > 0.0) hi = T; else lo = T;
+    }
+    *corrected = 1;
+    return 0.5 * (lo + hi) * ORC_KB / (ORC_ME * ORC_C * ORC_C);
+}
+
+void orc_radpress(const orc_units *u, long long ncell, const double *rho, const double *the, const double *hscale_rg,
+                  double tau_crit, double *the_out, long long *ncorrected)
+{
+    long long cnt = 0;
+    for (long long k = 0; k < ncell; ++k) {
+        int c;
+        the_out[k] = orc_radpress_cell(u, rho[k], the[k], hscale_rg[k], tau_crit, &c);
+        cnt += c;
+    }
+    *ncorrected = cnt;
 }
