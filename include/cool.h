@@ -181,6 +181,23 @@ int cool_last_launch_count(void);
 
 cool_status cool_table_destroy(cool_table *table);
 
+/* Radiation-pressure temperature correction (eq 29; post-processing of the high-accretion-rate
+ * runs, Figs 9(b) and 10).  Eq 29, P = a T_e^4 + N k_B (T_e + T_i), with P the simulated gas pressure
+ * N k_B (T_e + T_i) and only T_e recalculated (L345: T_i cancels), is  a T^4 + N k_B (T - T_e) = 0; its one root in
+ * (0, T_e] replaces Theta_e in every cell whose in-cell scattering depth tau_sca = n_e sigma_T H (L353) exceeds
+ * tau_crit (the paper uses 1 for Fig. 9(b) and 4.6 for Fig. 10).  a = 7.5646e-15 erg cm^-3 K^-4 as printed (L345),
+ * N = n_e = rho rho_scale_cgs/m_p.  Other cells, and cells with rho <= 0, Theta_e <= 0 or NaN, are copied unchanged.
+ * Only units->rho_scale_cgs and units->mbh_msun are used; no table is needed.
+ * d_rho, d_theta_e, d_hscale (scale height H of the cell's radius, in r_g), d_theta_e_out: DEVICE arrays of ncell
+ * elements of `dtype` on the CURRENT device, owned by the caller; d_theta_e_out may alias d_theta_e; 16-byte
+ * alignment of all four enables 128-bit accesses, other alignments take a scalar path.  d_ncorrected: DEVICE pointer
+ * to one long long that receives the number of corrected cells (overwritten), or NULL.  Asynchronous on
+ * `cuda_stream`; does not synchronise.  One kernel launch.  Errors: COOL_EINVAL (NULL arrays with ncell > 0, ncell < 0,
+ * tau_crit < 0 or not finite, non-positive units), COOL_ECUDA. */
+cool_status cool_radpress_correct(const cool_units *units, long long ncell, cool_dtype dtype, const void *d_rho,
+                                  const void *d_theta_e, const void *d_hscale, double tau_crit, void *d_theta_e_out,
+                                  long long *d_ncorrected, void *cuda_stream);
+
 const char *cool_last_error(void);         /* thread-local, never NULL */
 const char *cool_version(void);
 

@@ -72,7 +72,7 @@ class cool_diag(C.Structure):
 DIAG_BYTES = C.sizeof(cool_diag)
 EXPORTS = ("cool_table_build_host", "cool_table_create", "cool_apply", "cool_apply_host",
            "cool_table_auto_variant", "cool_last_launch_count", "cool_table_destroy",
-           "cool_last_error", "cool_version")
+           "cool_last_error", "cool_version", "cool_radpress_correct")
 
 _lib = None
 
@@ -98,6 +98,9 @@ def lib():
         L.cool_last_launch_count.restype = C.c_int
         L.cool_table_destroy.restype = C.c_int
         L.cool_table_destroy.argtypes = [C.c_void_p]
+        L.cool_radpress_correct.restype = C.c_int
+        L.cool_radpress_correct.argtypes = [C.POINTER(cool_units), C.c_longlong, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p,
+                                            C.c_double, C.c_void_p, C.c_void_p, C.c_void_p]
         L.cool_last_error.restype = C.c_char_p
         L.cool_version.restype = C.c_char_p
         _lib = L
@@ -231,6 +234,12 @@ def cool_apply_host(table: CoolTable, ncell, dtype, rho, bsq, theta_e_in, theta_
     d = cool_diag() if want_diag else None
     _check(lib().cool_apply_host(table.handle, C.byref(c), C.byref(params), None if d is None else C.byref(d)))
     return None if d is None else d.as_dict()
+
+
+def cool_radpress_correct(units: cool_units, ncell, dtype, rho, theta_e, hscale, tau_crit, theta_e_out, d_ncorrected=None, stream=None):
+    """Radiation-pressure temperature correction (eq 29) of DEVICE arrays on the current device; see include/cool.h."""
+    _check(lib().cool_radpress_correct(C.byref(units), int(ncell), int(dtype), _ptr(rho), _ptr(theta_e), _ptr(hscale),
+                                       float(tau_crit), _ptr(theta_e_out), _ptr(d_ncorrected), stream))
 
 
 def cool_table_destroy(table: CoolTable):

@@ -23,6 +23,8 @@ void set_error(const char *fmt, ...)
     va_end(ap);
 }
 
+void note_launches(int n) { g_launches = n; }
+
 #define CUDA_TRY(call, what)                                                            \
     do {                                                                                \
         cudaError_t e_ = (call);                                                        \

@@ -123,6 +123,7 @@ struct cool_table {
 
 namespace cool {
 void set_error(const char *fmt, ...);
+void note_launches(int n);           // what cool_last_launch_count() reports for this thread
 bool desc_valid(const cool_table_desc *d, bool need_coulomb_shape, std::string *why);
 coolphys::Units to_units(const cool_units &u);
 cool_status launch_step(const cool_table *t, cool_variant v, cool_dtype dt, const LaunchArgs &a, cudaStream_t s, int *nlaunch);

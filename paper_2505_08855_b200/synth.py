@@ -99,6 +99,43 @@ def mad_like_cells(nr: int = 288, nth: int = 192, nph: int = 144, dtype=np.float
     return out
 
 
+def scale_height(r, r_tr: float = 50.0, thick: float = 0.3, thin: float = 0.05):
+    """Density scale height H(r) in r_g of a truncated disc as in the paper's Fig. 4: H/r = ``thick`` inside the
+    truncation radius ``r_tr``, falling to ``thin`` outside:  H = r (thin + (thick - thin)/(1 + (r/r_tr)^4))."""
+    r = np.asarray(r, dtype=np.float64)
+    return r * (thin + (thick - thin) / (1.0 + (r / r_tr) ** 4))
+
+
+def thick_disc_cells(nr: int = 288, nth: int = 192, nph: int = 144, dtype=np.float32, config: int = 6, rho0: float = 5.0,
+                     r_in: float = 1.2, r_out: float = 300.0, seed: int = MASTER_SEED):
+    """Input of the radiation-pressure correction (the high-accretion-rate runs after the disc has
+    collapsed): an (r, theta, phi) grid as in mad_like_cells with
+
+        rho     = rho0 exp(-(theta - pi/2)^2 / (2 (H/r)^2)),  H(r) = scale_height(r)     (code units of rho_scale)
+        Theta_e = 3 (r/r_in)^-1   (T_e ~ 1e9 K near r ~ 20 r_g)
+        hscale  = H(r) in r_g, the same for every cell of a radial shell
+        rho and Theta_e times exp(0.05 N(0,1))
+
+    With Table I's rho_scale = 3e-7 g/cm^3 and M = 10 Msun this gives tau_sca = n_e sigma_T H of a few in the midplane
+    (the paper quotes 2-8, L338) and << 1 off the midplane.  Returns dict(rho, theta_e, r, hscale, shape)."""
+    n = nr * nth * nph
+    r1 = np.exp(np.linspace(np.log(r_in), np.log(r_out), nr))
+    th1 = (np.arange(nth) + 0.5) * np.pi / nth
+    R = r1[:, None, None]
+    TH = th1[None, :, None]
+    H = scale_height(R)
+    rho = np.broadcast_to(rho0 * np.exp(-((TH - 0.5 * np.pi) ** 2) / (2.0 * (H / R) ** 2)), (nr, nth, nph))
+    the = np.broadcast_to(3.0 * r_in / R, (nr, nth, nph))
+    out = {}
+    for k, (name, arr) in enumerate((("rho", rho), ("theta_e", the))):
+        noise = _rng(config, (_F_NOISE << 4) | k, seed).standard_normal(n, dtype=np.float32)
+        out[name] = (arr.reshape(-1) * np.exp(0.05 * noise.astype(np.float64))).astype(dtype)
+    out["r"] = np.broadcast_to(R, (nr, nth, nph)).reshape(-1).astype(dtype)
+    out["hscale"] = np.broadcast_to(H, (nr, nth, nph)).reshape(-1).astype(dtype)
+    out["shape"] = (nr, nth, nph)
+    return out
+
+
 # rho_scale [g cm^-3] for the density-normalisation sweep of config 3: log-log
 # interpolation of (mdot, rho_scale) through PAPER.md Table I (L290-L294):
 # (2.6e-1, 3e-7), (5.1e-4, 1e-8), (4.7e-6, 1e-9).
