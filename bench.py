@@ -36,7 +36,7 @@ SPEC_HBM_GBS = 8000.0                     # BASELINE.json: "vs 8 TB/s"
 FALLBACK_HBM_GBS = 6650.0                 # B200_PROFILING.md fallback
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from one `ncu --set full` capture each
 # (profiles/r01d_<workload>_global_full.txt, c2: r01c; line "traffic ="); null for workloads that were not captured
-NCU_TRAFFIC_GB = {"c5": 3.7347, "s512": 3.1940, "s512f": 4.2761, "c2": 0.4301, "c3": 0.2361}
+NCU_TRAFFIC_GB = {"c5": 3.7347, "s512": 3.1940, "s512f": 4.2761, "c2": 0.4301, "c3": 0.2361, "rp512": 2.1180}   # rp512: profiles/r01e_rp512_radpress_full.txt
 # issue-slot ceiling of the SMs (the bound that actually limits the sub-stepped 4-D step): 148 SMs x 4 schedulers x
 # 1 warp instruction per clock at clocks.max.sm 1965 MHz (B200_PROFILING.md unit counts) = 1163 G warp-instructions/s
 ISSUE_PEAK_GWINST = 148 * 4 * 1.965
@@ -227,6 +227,129 @@ class ClocksMonitor:
         return out
 
 
+def run_radpress(args, rank, local_rank, world):
+    """--workload rp512: the radiation-pressure temperature correction (eq 29) on a 512^3 fp32 thick-disc
+    field: one streaming kernel per step, 16 B/cell (rho, Theta_e, H read; Theta_e written).  Not the default line."""
+    metric, unit = "Gcell/s of the radiation-pressure temperature correction (eq 29)", "Gcell/s"
+    label = "512^3 fp32 thick-disc field (synth.thick_disc_cells), tau_crit = 1 (Fig. 9(b))"
+    tau_crit = 1.0
+    if args.impl == "reference":
+        if rank != 0:
+            return 0
+        import oracle as O
+        O.build()
+        f = synth.thick_disc_cells(512, 512, 16)
+        un = O.Units()
+        times = []
+        for k in range(min(args.warmup, 1) + args.steps):
+            t0 = time.perf_counter()
+            O.radpress(un, f["rho"], f["theta_e"], f["hscale"], tau_crit)
+            if k >= min(args.warmup, 1):
+                times.append(time.perf_counter() - t0)
+        m, tot = f["rho"].size, float(np.sum(times))
+        val = m * args.steps / tot / 1e9
+        print(json.dumps(dict(metric=metric, value=val, unit=unit, n_gpus=args.gpus, steps=args.steps, warmup=args.warmup,
+                              ms_per_step=1e3 * tot / args.steps, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f64",
+                              data="synthetic", impl="reference", config=dict(workload="rp512", description=label, cells_per_step=m,
+                                                                              note="oracle Part C (bisection, one host thread) on a phi-slab of the workload"),
+                              cpu_baseline=dict(value=val, unit=unit, cores=1, kind="oracle", sample=f"{m} cells (a 512x512x16 phi-slab) per step"),
+                              e2e=dict(value=val, unit=unit, h2d_bytes_per_step=0, d2h_bytes_per_step=0), gpu_launches=0)))
+        return 0
+    import torch
+    from paper_2505_08855_b200 import api
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+    f = synth.thick_disc_cells(512, 512, 512, config=6 + 16 * rank)
+    ncell = f["rho"].size
+    keys = ("rho", "theta_e", "hscale")
+    host = {k: torch.from_numpy(f[k]).pin_memory() for k in keys}
+    d = {k: host[k].to(dev) for k in keys}
+    out = torch.empty_like(d["theta_e"])
+    d_cnt = torch.zeros(1, dtype=torch.int64, device=dev)
+    units = api.default_units()
+    stream = torch.cuda.current_stream().cuda_stream
+
+    def step():
+        api.cool_radpress_correct(units, ncell, api.COOL_F32, d["rho"], d["theta_e"], d["hscale"], tau_crit, out, d_cnt, stream)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    mon = ClocksMonitor(torch.cuda.get_device_properties(dev).uuid) if rank == 0 else None
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+    barrier()
+    if mon is not None:
+        mon.start(local_rank)
+    ev[0].record()
+    for k in range(args.steps):
+        step()
+        ev[k + 1].record()
+    barrier()
+    clocks = mon.stop() if rank == 0 else None
+    per_step_ms = np.array([ev[k].elapsed_time(ev[k + 1]) for k in range(args.steps)])
+    total_ms = float(ev[0].elapsed_time(ev[-1]))
+    # end to end: pinned host arrays in, corrected Theta_e and the counter out, every step
+    h_out = torch.empty(ncell, dtype=torch.float32).pin_memory()
+    e2e_steps = max(1, min(args.steps, 3))
+
+    def hstep():
+        for k in keys:
+            d[k].copy_(host[k], non_blocking=True)
+        step()
+        h_out.copy_(out, non_blocking=True)
+        return int(d_cnt.item())
+    hstep()
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        ncorr = hstep()
+    barrier()
+    dt_e2e = time.perf_counter() - t0
+    if world > 1:
+        t = torch.tensor([total_ms, dt_e2e], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms, dt_e2e = float(t[0].item()), float(t[1].item())
+        dist.destroy_process_group()
+    if rank != 0:
+        return 0
+    peak, peak_src = peaks()
+    kern_ms = float(np.mean(per_step_ms))
+    achieved = 16 * ncell / (kern_ms * 1e-3) / 1e9
+    value = ncell * world * args.steps / (total_ms * 1e-3) / 1e9
+    line = dict(metric=metric, value=value, unit=unit, n_gpus=world, steps=args.steps, warmup=args.warmup, ms_per_step=total_ms / args.steps,
+                higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f32", data="synthetic",
+                config=dict(workload="rp512", description=label, cells_per_gpu=ncell, tau_crit=tau_crit, corrected_cells=ncorr,
+                            l2="inputs (%.2f GB per step) larger than L2" % (12 * ncell / 1e9)),
+                clocks=clocks, gpu_launches=args.steps,
+                e2e=dict(value=ncell * world * e2e_steps / dt_e2e / 1e9, unit=unit, h2d_bytes_per_step=12 * ncell, d2h_bytes_per_step=4 * ncell + 8,
+                         steps=e2e_steps, api="cool_radpress_correct after 3 pinned host->device copies, device->host copy of the result"),
+                roofline=dict(bound="hbm", achieved=achieved, peak=peak, unit="GB/s", frac=achieved / peak,
+                              traffic=NCU_TRAFFIC_GB["rp512"] * 1e9 if "rp512" in NCU_TRAFFIC_GB else None,
+                              kernel="cool_radpress_kernel<float, VEC=1, COUNT=1>", bytes_per_cell=16, algorithmic_bytes_per_launch=16 * ncell,
+                              peak_source=peak_src, ms_per_launch_median=float(np.median(per_step_ms)), ms_per_launch_best=float(per_step_ms.min())))
+    if not args.no_cpu_baseline:
+        import oracle as O
+        O.build()
+        sl = slice(ncell // 2, ncell // 2 + (1 << 23))
+        t0 = time.perf_counter()
+        O.radpress(O.Units(), f["rho"][sl], f["theta_e"][sl], f["hscale"][sl], tau_crit)
+        t1 = time.perf_counter() - t0
+        line["cpu_baseline"] = dict(value=(1 << 23) / t1 / 1e9, unit=unit, cores=1, kind="oracle",
+                                    sample=f"{1 << 23} contiguous cells from the middle of the workload, one pass, {t1:.1f} s")
+    print(json.dumps(line))
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -248,6 +371,8 @@ def main():
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.workload == "rp512":
+        return run_radpress(args, rank, local_rank, world)
     spec = workload_spec(args.workload)
     axis, lo, hi = table_ranges(spec["n"])
 

@@ -13,7 +13,6 @@
 namespace {
 
 constexpr int kRpThreads = 256;
-constexpr int kRpCtasPerSm = 8;
 
 struct RpConst {
     double c_tau;        // tau_sca = c_tau rho hscale : (rho_scale/m_p) sigma_T r_g
@@ -114,18 +113,25 @@ cudaError_t rp_launch(const void *rho, const void *the, const void *hs, void *ou
     const bool vec = (((uintptr_t)rho | (uintptr_t)the | (uintptr_t)hs | (uintptr_t)out) & 15) == 0;
     const long long per_cta = (long long)kRpThreads * W * 2;
     long long grid = (ncell + per_cta - 1) / per_cta;
-    const long long cap = (long long)nsm * kRpCtasPerSm;
-    if (grid > cap) grid = cap;
-    if (grid < 1) grid = 1;
     auto *cnt = reinterpret_cast<unsigned long long *>(d_cnt);
     const Real *r = (const Real *)rho, *t = (const Real *)the, *h = (const Real *)hs;
     Real *o = (Real *)out;
+    // one wave: as many CTAs as are resident at once (registers decide: 5 per SM for the fp32 vector kernel), each
+    // striding over the whole array, so that no partial second wave runs on a part of the machine
+    auto go = [&](auto kern) {
+        int per_sm = 1;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, kRpThreads, 0) != cudaSuccess || per_sm < 1) per_sm = 1;
+        const long long cap = (long long)nsm * per_sm;
+        if (grid > cap) grid = cap;
+        if (grid < 1) grid = 1;
+        kern<<<(unsigned)grid, kRpThreads, 0, st>>>(r, t, h, o, ncell, K, cnt);
+    };
     if (vec) {
-        if (d_cnt) cool_radpress_kernel<Real, true, true><<<(unsigned)grid, kRpThreads, 0, st>>>(r, t, h, o, ncell, K, cnt);
-        else cool_radpress_kernel<Real, true, false><<<(unsigned)grid, kRpThreads, 0, st>>>(r, t, h, o, ncell, K, cnt);
+        if (d_cnt) go(cool_radpress_kernel<Real, true, true>);
+        else go(cool_radpress_kernel<Real, true, false>);
     } else {
-        if (d_cnt) cool_radpress_kernel<Real, false, true><<<(unsigned)grid, kRpThreads, 0, st>>>(r, t, h, o, ncell, K, cnt);
-        else cool_radpress_kernel<Real, false, false><<<(unsigned)grid, kRpThreads, 0, st>>>(r, t, h, o, ncell, K, cnt);
+        if (d_cnt) go(cool_radpress_kernel<Real, false, true>);
+        else go(cool_radpress_kernel<Real, false, false>);
     }
     return cudaGetLastError();
 }
