@@ -10,6 +10,14 @@
 
 #include "cool_internal.h"
 
+// Row skew of the Coulomb quads in float4 units: rows i and i+1 of one column would share their banks (a row of 64 quads is
+// 1024 B), and the cells of a warp straddle both; 2 quads keep the 2 x 2 neighbourhood of a lookup in distinct bank groups.
+// 64 x 66 quads + the stages of the 768-thread kernel fill the 163 KiB a CTA can have at the 164 KiB carve-out exactly
+// (measured at 512^3: skew 0 0.627 ms, 1 0.619 ms, 2 0.614 ms; 3 needs the next carve-out step and is slower).
+#ifndef COOL_COULQ_SKEW
+#define COOL_COULQ_SKEW 2
+#endif
+
 namespace cool {
 
 static thread_local char g_err[512] = "";
@@ -401,7 +409,7 @@ extern "C" cool_status cool_table_create(const cool_table_desc *desc, int device
         {   // fp32 path: log2 C, plain (padded to 16 B) and as quads {C(i,e), C(i,e+1), C(i+1,e), C(i+1,e+1)}
             const size_t npad = (n + 3) & ~(size_t)3;
             const int n0 = desc->nc[0], n1 = desc->nc[1];
-            const int qs = n1;                                   // quad row stride (no padding: 64^2 quads fill a 64 KiB carve-out step exactly)
+            const int qs = n1 + COOL_COULQ_SKEW;                 // quad row stride
             std::vector<float> c2(npad, 0.f), cq((size_t)n0 * qs * 4, 0.f);
             for (size_t k = 0; k < n; ++k) c2[k] = (float)(3.321928094887362 * (double)desc->host_coulomb[k]);
             for (int i = 0; i < n0; ++i)

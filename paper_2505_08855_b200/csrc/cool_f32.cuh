@@ -779,7 +779,7 @@ struct LaunchCtx32 { const cool_table *t; F32Const S; const LaunchArgs *a; cudaS
 constexpr int kF32Threads3 = 768, kF32Stages3 = 2;          // GLOBAL / texture variants, single-update 3-D step: 24 warps, 2 stages each
 constexpr int kF32Threads4 = 512, kF32Stages4 = 2;          // GLOBAL / texture variants, sub-stepped or 4-D: 16 warps, 2 stages each
 constexpr int kF32SmemThreads = 384, kF32SmemStages = 2;    // SMEM variant: the table image takes most of the shared memory
-constexpr int kCoulQuadSmemMax = 73728;                     // Coulomb quads up to 64 x (64 + 3 skew) x 16 B are staged in shared memory
+constexpr int kCoulQuadSmemMax = 73728;                     // Coulomb quads up to 64 x (64 + 2 skew) x 16 B (and a little more) are staged in shared memory
 
 // fills the shared-memory layout fields of S for a launch with `threads` threads; returns the total
 inline size_t f32_smem_layout(F32Const &S, int threads, int nst, bool table_in_smem, bool coul_quad, const cool_table *t)

@@ -51,7 +51,7 @@ struct DevTable {
     cudaTextureObject_t ftex_pt, ftex_lin;
     const float *fcoul;            // log2 C [theta_i][theta_e] (allocation padded to 16 B)
     const float4 *fcoulq;          // the same as quads {C(i,e), C(i,e+1), C(i+1,e), C(i+1,e+1)}
-    int coulq_bytes, coulq_stride;  // row stride of the quads in float4 units (= 3 mod 8: bank skew)
+    int coulq_bytes, coulq_stride;  // row stride of the quads in float4 units (nc[1] + 2: bank skew, see cool_api.cu)
     int f4_has_coul;               // MODE 4: f4.w = log2 C (Coulomb axes identical to the table's Theta axes)
     // Coulomb coefficient table log10 C [theta_i][theta_e]
     const float *coul;
