@@ -106,6 +106,14 @@ def test_no_gpu_means_loud_failure():
     with pytest.raises(api.CoolError) as e:
         api.cool_table_create(desc, data)
     assert e.value.status == api.COOL_ECUDA
+    # the eq 29 correction needs no table: it must fail just as loudly (argument errors come first)
+    x = np.ones(8, np.float32)
+    with pytest.raises(api.CoolError) as e:
+        api.cool_radpress_correct(api.default_units(), 8, api.COOL_F32, x, x, x, 1.0, x)
+    assert e.value.status == api.COOL_ECUDA
+    with pytest.raises(api.CoolError) as e:
+        api.cool_radpress_correct(api.default_units(), 8, api.COOL_F32, x, x, x, -1.0, x)
+    assert e.value.status == api.COOL_EINVAL
 
 
 def test_product_does_not_import_oracle():
