@@ -143,9 +143,11 @@ __device__ __forceinline__ float coord32(const AxisCoef &a, float q, int one_bit
     return fmaf(u - a.ke, a.invf, fmaf(lm, a.invf, a.cf));
 }
 template <bool DIAG>
-__device__ __forceinline__ Loc32 split32(const AxisCoef &a, float t, int &clamped)
+__device__ __forceinline__ Loc32 split32(const AxisCoef &a, float t, bool &clamped)
 {
-    if constexpr (DIAG) clamped |= (t < 0.f) | (t > a.nm1f);
+    // t < 0 or t > n-1 in one unsigned compare of the bit patterns (negative floats compare above every positive one;
+    // t is never -0: it is a sum that cancels to +0; a NaN t belongs to a cell that is not counted)
+    if constexpr (DIAG) clamped |= __float_as_uint(t) > __float_as_uint(a.nm1f);
     const float tc = fminf(fmaxf(t, 0.f), a.tmaxf);
     Loc32 L;
     L.tf = __fadd_rd(tc, kMagic);
@@ -155,7 +157,7 @@ __device__ __forceinline__ Loc32 split32(const AxisCoef &a, float t, int &clampe
     return L;
 }
 template <bool DIAG>
-__device__ __forceinline__ Loc32 locate32(const AxisCoef &a, float q, int &clamped, int one_bits)
+__device__ __forceinline__ Loc32 locate32(const AxisCoef &a, float q, bool &clamped, int one_bits)
 {
     return split32<DIAG>(a, coord32(a, q, one_bits), clamped);
 }
@@ -450,7 +452,7 @@ __device__ __forceinline__ void step_cells_f32(const Ctx32 &X, const Fetch &F, c
     float in_e[NV], in_i[NV], nanq[NV];
     Loc32 lr[NV], lb[NV];
     float kcell[NV], coul_kr[NV], tfloor[NV], lsum[NV][4];
-    int clamped[NV], limited[NV], floored[NV];
+    bool clamped[NV], limited[NV], floored[NV];
     Patch4 P[(MODE == 4 && !Fetch::kHw) ? NV : 1];
 #pragma unroll
     for (int j = 0; j < NV; ++j) {
@@ -459,7 +461,7 @@ __device__ __forceinline__ void step_cells_f32(const Ctx32 &X, const Fetch &F, c
         bad[j] = !(rho[j] > 0.f) || chk != chk;
         any_bad |= bad[j];
         in_e[j] = the[j]; in_i[j] = thi[j];
-        clamped[j] = limited[j] = floored[j] = 0;
+        clamped[j] = limited[j] = floored[j] = false;
         lr[j] = locate32<DIAG>(T.ax[CAX_RHO], rho[j], clamped[j], one_bits);
         lb[j] = locate32<DIAG>(T.ax[CAX_BSQ], bsq[j], clamped[j], one_bits);
         tfloor[j] = 0.f;
@@ -521,7 +523,7 @@ __device__ __forceinline__ void step_cells_f32(const Ctx32 &X, const Fetch &F, c
                 }
             }
             if (use_floor) {
-                if ((the[j] + thi[j]) * S.mr < tfloor[j]) { rrad = 0.f; floored[j] = 1; }
+                if ((the[j] + thi[j]) * S.mr < tfloor[j]) { rrad = 0.f; floored[j] = true; }
             }
             if constexpr (DIAG) limited[j] |= (rrad > S.f_limit);
             rrad = fminf(rrad, S.f_limit);
@@ -534,7 +536,7 @@ __device__ __forceinline__ void step_cells_f32(const Ctx32 &X, const Fetch &F, c
                     if (MODE == 4 && T.f4_has_coul) {
                         C = ex2_approx(yc);
                     } else {
-                        int dummy = 0;
+                        bool dummy = false;
                         Loc32 ca, cb;                                   // Coulomb-table coordinates of Theta_i, Theta_e
                         // branch-free (identical axes give s = 1, o = 0 and the same node coordinate): keeps the NV cells interleaved
                         if (MODE == 4) ca = split32<false>(T.cax[0], fmaf(ti, S.cmi_s, S.cmi_o), dummy);
@@ -602,7 +604,9 @@ __device__ __forceinline__ void step_cells_f32(const Ctx32 &X, const Fetch &F, c
 #pragma unroll
                 for (int k = 1; k < 4; ++k) part[k] += bad[j] ? 0.f : lsum[j][k] * wgt;
             }
-            if (!bad[j]) { acc.lim += limited[j]; acc.flo += floored[j]; acc.cla += clamped[j]; }
+            if (limited[j] && !bad[j]) ++acc.lim;               // predicated increments: the flags stay predicates
+            if (floored[j] && !bad[j]) ++acc.flo;
+            if (clamped[j] && !bad[j]) ++acc.cla;
         }
         acc.lum[0] += (double)part[0];
         if constexpr (MODE == 4) {

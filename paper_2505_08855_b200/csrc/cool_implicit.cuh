@@ -288,7 +288,7 @@ __device__ void implicit_cell_f32(const DevTable &T, const StepConst &S, const F
     const int one_bits = 0x3f800000;
     const AxisCoef &ax = T.ax[CAX_THE];
     const int n = ax.n;
-    int clamped = 0, floored = 0;
+    bool clamped = false; int floored = 0;
     const Loc32 lr = locate32<true>(T.ax[CAX_RHO], rho, clamped, one_bits), lb = locate32<true>(T.ax[CAX_BSQ], bsq, clamped, one_bits);
     const int ir = (int)lr.fi, ib = (int)lb.fi;
     Loc32 li{0.f, 0.f, 0.f, 0.f}; int iii = 0;
@@ -304,7 +304,7 @@ __device__ void implicit_cell_f32(const DevTable &T, const StepConst &S, const F
         if constexpr (MODE == 4) { li = locate32<true>(T.ax[CAX_THI], thi, clamped, one_bits); iii = (int)li.fi; }
         float C = 0.f;
         if (S32.coulomb == 1) {
-            int dummy = 0;
+            bool dummy = false;
             const Loc32 ca = locate32<false>(T.cax[0], thi, dummy, one_bits), cb = locate32<false>(T.cax[1], the, dummy, one_bits);
             C = coulomb_C32<0, false>(T.cax[1].n, 0, T.fcoul, 0u, ca, cb);
         } else if (S32.coulomb == 2) {
@@ -347,7 +347,7 @@ __device__ void implicit_cell_f32(const DevTable &T, const StepConst &S, const F
                 const float te = node_theta(e);
                 rate = imp32_rate<MODE>(S32, c, te, ye, frac);                 // cooling time held outside the range
                 theta = c.R / (c.opq + rate);
-                clamped |= 1;
+                clamped = true;
             } else {
                 if (!have_b) imp32_node<MODE>(F, lr, lb, li, ir, ib, iii, ilo + 1, yb);
                 const float dy[3] = {yb[0] - ya[0], yb[1] - ya[1], yb[2] - ya[2]};
@@ -414,7 +414,7 @@ __device__ void implicit_cell_f32(const DevTable &T, const StepConst &S, const F
     const double ds[4] = {(double)de_sum[0], (double)de_sum[1], (double)de_sum[2], (double)de_sum[3]};
 #pragma unroll
     for (int k = 0; k < 4; ++k) acc.lum[k] += ds[k] * wgt;
-    acc.flo += floored; acc.cla += clamped;
+    acc.flo += floored; acc.cla += clamped ? 1 : 0;
     shell_add(S, cell, ds, wgt, MODE == 4);
 }
 
