@@ -35,13 +35,13 @@ UNIT = "Gcell-updates/s"
 SPEC_HBM_GBS = 8000.0                     # BASELINE.json: "vs 8 TB/s"
 FALLBACK_HBM_GBS = 6650.0                 # B200_PROFILING.md fallback
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from one `ncu --set full` capture each
-# (profiles/r01d_<workload>_global_full.txt, s512: r01e, c2: r01c; line "traffic ="); null for workloads that were not captured
-NCU_TRAFFIC_GB = {"c5": 3.7347, "s512": 3.1948, "s512f": 4.2761, "c2": 0.4301, "c3": 0.2361, "rp512": 2.1180}   # rp512: profiles/r01e_rp512_radpress_full.txt
+# (profiles/r01e_<workload>_global_full.txt, rp512: r01e_rp512_radpress_full.txt, c2: r01c; line "traffic ="); null for workloads that were not captured
+NCU_TRAFFIC_GB = {"c5": 3.7339, "s512": 3.1948, "s512f": 4.2766, "c2": 0.4301, "c3": 0.2358, "rp512": 2.1180}   # rp512: profiles/r01e_rp512_radpress_full.txt
 # issue-slot ceiling of the SMs (the bound that actually limits the sub-stepped 4-D step): 148 SMs x 4 schedulers x
 # 1 warp instruction per clock at clocks.max.sm 1965 MHz (B200_PROFILING.md unit counts) = 1163 G warp-instructions/s
 ISSUE_PEAK_GWINST = 148 * 4 * 1.965
 # warp instructions per launch (smsp__inst_executed.sum of the same captures)
-NCU_WARP_INST = {"c5": 3361983299, "s512": 613040600, "s512f": 815038674, "c3": 50791210}
+NCU_WARP_INST = {"c5": 3322223572, "s512": 613040600, "s512f": 780244894, "c3": 48924970}
 
 
 # ------------------------------------------------------------------------------------------------
