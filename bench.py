@@ -561,8 +561,8 @@ def main():
              "smem": "F32Smem",
              "tex_point": "F32TexPoint", "tex_hwfilter": "F32TexHw"}.get(api.VARIANT_NAMES[resolved], api.VARIANT_NAMES[resolved])
     explicit = args.scheme == "explicit"
-    kernel_name = ("cool_implicit_f32_kernel<MODE=%d, %s>" % (mode, api.VARIANT_NAMES[resolved])) if not explicit else "cool_f32_kernel<MODE=%d, %s, DIAG=%d, CM=1, NSUB1=%d, %s>" % (
-        mode, fetch, int(bool(spec["diag"])), int(spec["nsub"] == 1),
+    kernel_name = ("cool_implicit_f32_kernel<MODE=%d, %s>" % (mode, api.VARIANT_NAMES[resolved])) if not explicit else "cool_f32_kernel<MODE=%d, %s, DIAG=%d, CM=%d, NSUB1=%d, %s>" % (
+        mode, fetch, int(bool(spec["diag"])), 2 if (mode == 3 and spec["diag"] and fetch != "F32Smem" and (ncell < (1 << 25) or not spec.get("floor"))) else 1, int(spec["nsub"] == 1),
         "384 threads, 2 stages" if fetch == "F32Smem" else ("768 threads, 2 stages" if single else "512 threads, 2 stages"))
     line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=args.warmup,
                 ms_per_step=total_ms / args.steps, higher_is_better=True, scaling="weak", vs_baseline=None,

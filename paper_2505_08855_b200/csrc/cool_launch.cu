@@ -39,14 +39,16 @@ static StepConst make_step_const(const cool_table *t, cool_dtype dt, const Launc
 
 // Coulomb coefficient table staged in shared memory (not needed when it rides in the 4-D texels): returns the kernels'
 // CM — 0 not staged, 1 quads (<= 72 KiB; the SMEM variant stores the plain table under CM = 1), 2 plain table (<= 16 KiB)
-// for small launches with diagnostics.
+// for launches with diagnostics that are small or stage no radius array.  Measured on B200 (table 128^3, Coulomb 64^2):
+// 288x192x144 cells with the floor 0.089 (quads) / 0.077 ms (plain); 512^3 with the floor (6 cell arrays) 0.910 / 0.927 ms;
+// 512^3 without it (5 arrays: the plain table keeps the CTA under the 164 KiB carve-out) 0.849 / 0.784 ms.
 constexpr long long kCoulPlainBelowCells = 1ll << 25;
 static int coulomb_smem_mode(const cool_table *t, const LaunchArgs &a, cool_variant v)
 {
     const DevTable &D = t->dev;
     if (a.coulomb != 1 || !D.fcoul || (D.mode == 4 && D.f4_has_coul)) return 0;
     if (v == COOL_V_SMEM) return D.coul_bytes <= kCoulSmemMax ? 1 : 0;
-    if (a.want_diag && a.ncell < kCoulPlainBelowCells && D.coul_bytes <= kCoulSmemMax) return 2;
+    if (a.want_diag && (a.ncell < kCoulPlainBelowCells || a.r == nullptr) && D.coul_bytes <= kCoulSmemMax) return 2;
     return D.coulq_bytes <= kCoulQuadSmemMax ? 1 : 0;
 }
 
