@@ -323,3 +323,108 @@ def test_cell_luminosity_terms_and_shell_sums(oracle):
         assert sh.shape == (5, 4)
         assert sh[2] == pytest.approx(cl[512:768].sum(axis=0), rel=1e-13)
         assert sh[4] == pytest.approx(cl[1024:].sum(axis=0), rel=1e-13)          # ragged last shell
+
+
+# ---------------------------------------------------------------- per-process luminosity split (reading C-21)
+# DESIGN.md C-21: the energy a cell radiates is attributed to bremsstrahlung, synchrotron and the Compton-added part in
+# proportion to their shares of Q_thin = Q_brem + eta Q_syn (eq 10): Q_brem, Q_syn, (eta - 1) Q_syn;
+# the optically-thick bridge of eqs 11-12 (L108-L118) and the limiter (L185) scale all three alike.
+def _proc_table(oracle, log_br, log_sy, log_eta, with_coul=False):
+    n = [3, 3, 3, 3]
+    lo, hi = [-6.0, -3.0, -8.0, -3.0], [0.0, 1.5, 0.0, 1.5]
+    data = [np.full(n, v, dtype=np.float32) for v in (log_br, log_sy, log_eta)]
+    if with_coul:
+        return oracle.Table(AX4, n, lo, hi, data, coul=np.zeros((3, 3), np.float32), clo=[-3.0, -3.0], chi=[1.5, 1.5])
+    return oracle.Table(AX4, n, lo, hi, data)
+
+
+def _both_schemes(oracle, tab, un, rho, bsq, the, thi, dt, vol, nsub):
+    yield "explicit", oracle.step(tab, un, rho, bsq, the, thi, dt, nsub=nsub, vol=vol, coulomb_mode=oracle.COULOMB_OFF, want_cell_lum=True)
+    yield "implicit", oracle.step_implicit(tab, un, rho, bsq, the, thi, dt, nsub=nsub, vol=vol, coulomb_mode=oracle.COULOMB_OFF, want_cell_lum=True)
+
+
+@pytest.mark.parametrize("nsub", [1, 3])
+def test_luminosity_split_single_process_limits(oracle, nsub):
+    """(i) no synchrotron (Q_syn = 1e-300, eta = 1): everything is bremsstrahlung; (ii) no bremsstrahlung, eta = 1:
+    everything is synchrotron, nothing Compton; (iii) no bremsstrahlung, eta = 3: Compton-added = (eta - 1) x synchrotron
+    = exactly twice the synchrotron share.  A swap of two shares, or shares of anything but Q_thin, fails one of these."""
+    un = oracle.Units()
+    rho, bsq, the, thi = _cells(400, seed=41)
+    vol = np.random.default_rng(42).uniform(0.5, 2.0, rho.size)
+    dt = 3.0
+    for name, o in _both_schemes(oracle, _proc_table(oracle, -9.0, -300.0, 0.0), un, rho, bsq, the, thi, dt, vol, nsub):
+        d = o["diag"]
+        assert d["lum_total"] > 0 and d["lum_brems"] == pytest.approx(d["lum_total"], rel=1e-14), name
+        assert d["lum_synch"] <= 1e-250 * d["lum_total"] and d["lum_compton"] == 0.0, name
+        assert o["cell_lum"][:, 1] == pytest.approx(o["cell_lum"][:, 0], rel=1e-14)
+    for name, o in _both_schemes(oracle, _proc_table(oracle, -300.0, -9.0, 0.0), un, rho, bsq, the, thi, dt, vol, nsub):
+        d = o["diag"]
+        assert d["lum_total"] > 0 and d["lum_synch"] == pytest.approx(d["lum_total"], rel=1e-14), name
+        assert d["lum_brems"] <= 1e-250 * d["lum_total"] and d["lum_compton"] == 0.0, name
+    log3 = float(np.float32(np.log10(3.0)))
+    eta = 10.0 ** log3                                          # the value the fp32 table actually holds
+    for name, o in _both_schemes(oracle, _proc_table(oracle, -300.0, -9.0, log3), un, rho, bsq, the, thi, dt, vol, nsub):
+        d = o["diag"]
+        assert d["lum_compton"] / d["lum_synch"] == pytest.approx(eta - 1.0, rel=1e-12), name
+        assert d["lum_synch"] + d["lum_compton"] == pytest.approx(d["lum_total"], rel=1e-12), name
+        cl = o["cell_lum"]
+        act = cl[:, 0] > 0
+        assert act.sum() > 300 and cl[act, 3] / cl[act, 2] == pytest.approx(eta - 1.0, rel=1e-12)
+
+
+def test_luminosity_split_ratios_survive_bridge_and_limiter(oracle):
+    """With constant process tables the shares are the same for every cell, Q_brem : Q_syn : (eta - 1) Q_syn, whether
+    the cell is optically thin or thick (eq 11 rescales Q_thin as a whole) and whether or not the 30 % limiter bites."""
+    un = oracle.Units()
+    rho, bsq, the, thi = _cells(600, seed=43)
+    rho = rho * 1e3                                             # some cells optically thick (tau_sca = 2 n_e sigma_T H > 1)
+    lb, ls, le = -1.0, -1.5, float(np.float32(0.25))    # strong enough for tau_abs ~ 1 in the cold cells
+    qbr, qsy, eta = 10.0 ** lb, 10.0 ** ls, 10.0 ** le
+    qthin = qbr + eta * qsy
+    tab = _proc_table(oracle, lb, ls, le)
+    for dt in (1e-12, 1e3):                                     # unlimited / mostly limited
+        o = oracle.step(tab, un, rho, bsq, the, thi, dt, nsub=2, coulomb_mode=oracle.COULOMB_OFF, want_cell_lum=True, want_rates=True)
+        cl = o["cell_lum"]
+        assert cl[:, 1] / cl[:, 0] == pytest.approx(qbr / qthin, rel=1e-12)
+        assert cl[:, 2] / cl[:, 0] == pytest.approx(qsy / qthin, rel=1e-12)
+        assert cl[:, 3] / cl[:, 0] == pytest.approx((eta - 1.0) * qsy / qthin, rel=1e-12)
+        # the bridge really is exercised: Q_total / Q_thin spans thin (-> 1) and thick (<< 1) cells
+        ratio = o["lam0"] / qthin
+        assert ratio.max() > 0.99 and ratio.min() < 0.5
+    assert 0 < o["diag"]["n_limited"] <= rho.size
+
+
+def test_luminosity_split_one_cell_by_hand(oracle):
+    """One cell written out from eqs 10-14 with unequal shares: H_th = c_s/Omega_K (eqs 13-14),
+    tau_sca = 2 n_e sigma_T H, tau_abs = H Q_thin/(4 sigma_SB T_e^4) (eq 12), Q_total of eq 11, then the shares of C-21."""
+    un = oracle.Units()
+    c, kB, me, mp, sigT, sigSB, GMsun = 2.99792458e10, 1.380649e-16, 9.1093837015e-28, 1.67262192369e-24, 6.6524587321e-25, 5.670374419e-5, 1.32712440018e26
+    rho, bsq, the, thi, vol, dt = 2e-2, 1e-4, 0.4, 5.0, 1.7, 1e-5
+    lb, ls, le = float(np.float32(-6.2)), float(np.float32(-7.1)), float(np.float32(0.6))
+    tab = _proc_table(oracle, lb, ls, le)
+    o = oracle.step(tab, un, np.array([rho]), np.array([bsq]), np.array([the]), np.array([thi]), dt, vol=np.array([vol]),
+                    coulomb_mode=oracle.COULOMB_OFF)
+    # by hand, cgs
+    rg = GMsun * 10.0 / c ** 2
+    tg = rg / c
+    conv = tg / (3e-7 * c ** 2)                                  # erg cm^-3 s^-1 -> code units
+    pe, pi = the * me / mp, thi * me / mp
+    cs2 = (5.0 / 3.0) * (pe + pi) / (1.0 + 1.5 * (pe + pi) + pe + pi)          # eq 14: gamma P/(rho + u + P), u = P/(gamma-1)
+    H = rg * math.sqrt(cs2) * (10.0 ** 1.5 + 0.9375)             # eq 13 at r_ref = 10 r_g: c_s / Omega_K
+    ne = rho * 3e-7 / mp
+    Te = the * me * c ** 2 / kB
+    qbr, qsy, eta = 10.0 ** lb / conv, 10.0 ** ls / conv, 10.0 ** le
+    qthin = qbr + eta * qsy                                      # eq 10
+    bb = 4.0 * sigSB * Te ** 4
+    tau_sca, tau_abs = 2.0 * ne * sigT * H, H * qthin / bb       # eq 12
+    qtot = (bb / H) / (1.5 * (tau_abs + tau_sca) + math.sqrt(3.0) + 1.0 / tau_abs) * conv     # eq 11
+    ue = rho * the * (me / mp) / (2.0 / 3.0)
+    assert qtot * dt < 0.3 * ue                                  # the limiter is idle for this cell
+    d = o["diag"]
+    assert d["lum_total"] == pytest.approx(qtot * vol, rel=1e-12)
+    assert d["lum_brems"] == pytest.approx(qtot * vol * qbr / qthin, rel=1e-12)
+    assert d["lum_synch"] == pytest.approx(qtot * vol * qsy / qthin, rel=1e-12)
+    assert d["lum_compton"] == pytest.approx(qtot * vol * (eta - 1.0) * qsy / qthin, rel=1e-12)
+    assert len({round(d[k] / d["lum_total"], 3) for k in ("lum_brems", "lum_synch", "lum_compton")}) == 3      # unequal shares
+    fr = oracle.combine_code(un, rho, the, thi, 10.0 ** lb, 10.0 ** ls, eta)[1]
+    assert fr == pytest.approx([qbr / qthin, qsy / qthin, (eta - 1.0) * qsy / qthin], rel=1e-13)
