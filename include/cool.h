@@ -121,6 +121,13 @@ typedef struct {
      * last bits); their total equals cool_diag.lum_* to rounding. */
     long long shell_cells;
     double *lum_shell;
+    /* Optional per-cell event flags, one byte per cell (overwritten): bit 0 = the 30 % limiter capped the radiative loss in
+     * some sub-step (L185), bit 1 = the temperature floor switched cooling off (eq 19), bit 2 = a table coordinate was
+     * clamped (C-7), bit 3 = the cell was recomputed by the precise pass (fp32 cells whose Theta_e visits a table interval
+     * too steep for fp32 coordinates, e.g. the K2 -> 2 theta^2 switch of L87).  Bits 0-2 are the per-cell
+     * terms of cool_diag.n_limited / n_floored / n_clamped.  DEVICE array for cool_apply, HOST array for cool_apply_host;
+     * NULL: not wanted.  Needs the diagnostics (d_diag / h_diag != NULL); 4-byte alignment enables 32-bit stores. */
+    unsigned char *flags;
 } cool_cells;
 
 typedef struct {
@@ -178,6 +185,11 @@ cool_variant cool_table_auto_variant(const cool_table *table);
 
 /* Number of kernel launches the last cool_apply / cool_apply_host on this thread issued. */
 int cool_last_launch_count(void);
+
+/* Name of the step kernel instantiation the last cool_apply / cool_apply_host on this thread launched (the dispatcher's own
+ * choice of lookup policy, Coulomb staging, thread count), e.g. "cool_f32_kernel<MODE=3,F32GlobalQ,DIAG=0,CM=1,NSUB1=1,768x2>".
+ * Thread-local, never NULL ("" before the first launch). */
+const char *cool_last_kernel_name(void);
 
 cool_status cool_table_destroy(cool_table *table);
 

@@ -106,7 +106,7 @@ def lib():
             "orc_interp": (d, [i, C.POINTER(i), C.POINTER(d), C.POINTER(d), C.POINTER(C.c_float),
                                C.POINTER(d), C.POINTER(i)]),
             "orc_step": (None, [C.POINTER(_Table), UP, C.c_longlong, p, p, p, p, p, p,
-                                d, i, d, d, i, i, p, p, p, p, p, p, i]),
+                                d, i, d, d, i, i, p, p, p, p, p, p, i, p]),
             "orc_step_implicit": (None, [C.POINTER(_Table), UP, C.c_longlong, p, p, p, p, p, p,
                                          d, i, d, i, p, p, p, p, i]),
             "orc_implicit_residual": (d, [C.POINTER(_Table), UP, d, d, d, d, d, d, i, d, i, d]),
@@ -210,7 +210,7 @@ COULOMB_OFF, COULOMB_TABLE, COULOMB_ANALYTIC = 0, 1, 2
 
 def step(table: Table, un: Units, rho, bsq, theta_e, theta_i, dt, nsub=1, f_limit=0.3,
          h_floor=0.0, r=None, vol=None, rate_mode=RATE_TABLE, coulomb_mode=None, nthreads=1,
-         want_rates=False, want_cell_lum=False):
+         want_rates=False, want_cell_lum=False, want_cell_flags=False):
     """Part B over a field.  Inputs are converted to float64 exactly (float32 inputs are
     representable).  Returns dict(theta_e, theta_i, diag[, lam0, qcc0])."""
     f64 = lambda a: None if a is None else np.ascontiguousarray(a, dtype=np.float64).ravel()
@@ -225,11 +225,12 @@ def step(table: Table, un: Units, rho, bsq, theta_e, theta_i, dt, nsub=1, f_limi
     qcc0 = np.empty(n) if want_rates else None
     diag = np.zeros(7)
     cell_lum = np.zeros((n, 4)) if want_cell_lum else None
+    cell_flags = np.zeros(n, dtype=np.uint8) if want_cell_flags else None
     ptr = lambda a: None if a is None else a.ctypes.data
     lib().orc_step(C.byref(table._c), C.byref(un), n, ptr(rho), ptr(bsq), ptr(the), ptr(thi),
                    ptr(r), ptr(vol), float(dt), int(nsub), float(f_limit), float(h_floor),
                    int(rate_mode), int(coulomb_mode), ptr(the_o), ptr(thi_o), ptr(lam0), ptr(qcc0),
-                   ptr(cell_lum), ptr(diag), int(nthreads))
+                   ptr(cell_lum), ptr(diag), int(nthreads), ptr(cell_flags))
     out = dict(theta_e=the_o, theta_i=thi_o,
                diag=dict(lum_total=diag[0], lum_brems=diag[1], lum_synch=diag[2], lum_compton=diag[3],
                          n_limited=int(diag[4]), n_floored=int(diag[5]), n_clamped=int(diag[6])))
@@ -237,6 +238,8 @@ def step(table: Table, un: Units, rho, bsq, theta_e, theta_i, dt, nsub=1, f_limi
         out["lam0"] = lam0; out["qcc0"] = qcc0
     if want_cell_lum:
         out["cell_lum"] = cell_lum
+    if want_cell_flags:
+        out["cell_flags"] = cell_flags            # bit 0 limited, bit 1 floored, bit 2 clamped (per-cell terms of the counts)
     return out
 
 

@@ -486,7 +486,8 @@ void orc_step(const orc_table *tab, const orc_units *un, long long ncell,
               const double *rho, const double *bsq, const double *the_in, const double *thi_in,
               const double *r, const double *vol,
               double dt, int nsub, double f_limit, double h_floor, int rate_mode, int coulomb_mode,
-              double *the_out, double *thi_out, double *lam0, double *qcc0, double *cell_lum, double *diag7, int nthreads)
+              double *the_out, double *thi_out, double *lam0, double *qcc0, double *cell_lum, double *diag7, int nthreads,
+              unsigned char *cell_flags)   /* optional, per cell: bit 0 limited, bit 1 floored, bit 2 clamped (diag7[4..6] of the cell) */
 {
     double acc[7] = {0, 0, 0, 0, 0, 0, 0};
     if (nthreads < 1) nthreads = 1;
@@ -497,6 +498,7 @@ void orc_step(const orc_table *tab, const orc_units *un, long long ncell,
         for (long long c = 0; c < ncell; ++c) {
             double the = the_in[c], thi = thi_in[c], d7[7];
             if (cell_lum) for (int k = 0; k < 4; ++k) cell_lum[4 * c + k] = 0.0;
+            if (cell_flags) cell_flags[c] = 0;
             if (isnan(rho[c]) || isnan(bsq[c]) || isnan(the) || isnan(thi)) {
                 the_out[c] = NAN; thi_out[c] = NAN;
                 if (lam0) lam0[c] = NAN;
@@ -514,6 +516,7 @@ void orc_step(const orc_table *tab, const orc_units *un, long long ncell,
                           lam0 ? &lam0[c] : NULL, qcc0 ? &qcc0[c] : NULL, d7);
             the_out[c] = the; thi_out[c] = thi;
             if (cell_lum) for (int k = 0; k < 4; ++k) cell_lum[4 * c + k] = d7[k];
+            if (cell_flags) cell_flags[c] = (unsigned char)((d7[4] != 0.0) | ((d7[5] != 0.0) << 1) | ((d7[6] != 0.0) << 2));
             for (int k = 0; k < 7; ++k) loc[k] += d7[k];
         }
 #pragma omp critical

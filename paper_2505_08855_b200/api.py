@@ -52,7 +52,8 @@ class cool_cells(C.Structure):
                 ("rho", C.c_void_p), ("bsq", C.c_void_p),
                 ("theta_e_in", C.c_void_p), ("theta_i_in", C.c_void_p),
                 ("theta_e_out", C.c_void_p), ("theta_i_out", C.c_void_p),
-                ("r", C.c_void_p), ("vol", C.c_void_p), ("shell_cells", C.c_longlong), ("lum_shell", C.c_void_p)]
+                ("r", C.c_void_p), ("vol", C.c_void_p), ("shell_cells", C.c_longlong), ("lum_shell", C.c_void_p),
+                ("flags", C.c_void_p)]
 
 
 class cool_params(C.Structure):
@@ -72,7 +73,7 @@ class cool_diag(C.Structure):
 DIAG_BYTES = C.sizeof(cool_diag)
 EXPORTS = ("cool_table_build_host", "cool_table_create", "cool_apply", "cool_apply_host",
            "cool_table_auto_variant", "cool_last_launch_count", "cool_table_destroy",
-           "cool_last_error", "cool_version", "cool_radpress_correct")
+           "cool_last_error", "cool_version", "cool_radpress_correct", "cool_last_kernel_name")
 
 _lib = None
 
@@ -96,6 +97,7 @@ def lib():
         L.cool_table_auto_variant.restype = C.c_int
         L.cool_table_auto_variant.argtypes = [C.c_void_p]
         L.cool_last_launch_count.restype = C.c_int
+        L.cool_last_kernel_name.restype = C.c_char_p
         L.cool_table_destroy.restype = C.c_int
         L.cool_table_destroy.argtypes = [C.c_void_p]
         L.cool_radpress_correct.restype = C.c_int
@@ -202,9 +204,9 @@ def cool_table_create(desc: cool_table_desc, data, coulomb=None, device: int = 0
     return CoolTable(h, desc)
 
 
-def _cells(ncell, dtype, rho, bsq, theta_e_in, theta_i_in, theta_e_out, theta_i_out, r, vol, shell_cells=0, lum_shell=None):
+def _cells(ncell, dtype, rho, bsq, theta_e_in, theta_i_in, theta_e_out, theta_i_out, r, vol, shell_cells=0, lum_shell=None, flags=None):
     c = cool_cells()
-    c.shell_cells = int(shell_cells); c.lum_shell = _ptr(lum_shell)
+    c.shell_cells = int(shell_cells); c.lum_shell = _ptr(lum_shell); c.flags = _ptr(flags)
     c.ncell = int(ncell); c.dtype = int(dtype)
     c.rho, c.bsq = _ptr(rho), _ptr(bsq)
     c.theta_e_in, c.theta_i_in = _ptr(theta_e_in), _ptr(theta_i_in)
@@ -219,18 +221,20 @@ def make_params(dt, nsub=1, f_limit=0.3, h_floor=0.0, variant=COOL_V_AUTO, coulo
 
 
 def cool_apply(table: CoolTable, ncell, dtype, rho, bsq, theta_e_in, theta_i_in, theta_e_out, theta_i_out,
-               params: cool_params, r=None, vol=None, d_diag=None, stream=None, shell_cells=0, lum_shell=None):
+               params: cool_params, r=None, vol=None, d_diag=None, stream=None, shell_cells=0, lum_shell=None, flags=None):
     """Asynchronous update of DEVICE arrays on ``stream`` (a cudaStream_t address; None = default).
-    ``lum_shell``: optional device float64 array of 4*ceil(ncell/shell_cells) (radial luminosity profile)."""
-    c = _cells(ncell, dtype, rho, bsq, theta_e_in, theta_i_in, theta_e_out, theta_i_out, r, vol, shell_cells, lum_shell)
+    ``lum_shell``: optional device float64 array of 4*ceil(ncell/shell_cells) (radial luminosity profile);
+    ``flags``: optional device uint8 array of ncell per-cell event flags (see include/cool.h)."""
+    c = _cells(ncell, dtype, rho, bsq, theta_e_in, theta_i_in, theta_e_out, theta_i_out, r, vol, shell_cells, lum_shell, flags)
     _check(lib().cool_apply(table.handle, C.byref(c), C.byref(params), _ptr(d_diag), stream))
 
 
 def cool_apply_host(table: CoolTable, ncell, dtype, rho, bsq, theta_e_in, theta_i_in, theta_e_out, theta_i_out,
-                    params: cool_params, r=None, vol=None, want_diag=False, shell_cells=0, lum_shell=None):
+                    params: cool_params, r=None, vol=None, want_diag=False, shell_cells=0, lum_shell=None, flags=None):
     """Synchronous update of HOST arrays (copies staged and overlapped inside the library).
-    ``lum_shell``: optional host float64 array of 4*ceil(ncell/shell_cells) (radial luminosity profile)."""
-    c = _cells(ncell, dtype, rho, bsq, theta_e_in, theta_i_in, theta_e_out, theta_i_out, r, vol, shell_cells, lum_shell)
+    ``lum_shell``: optional host float64 array of 4*ceil(ncell/shell_cells) (radial luminosity profile);
+    ``flags``: optional host uint8 array of ncell per-cell event flags."""
+    c = _cells(ncell, dtype, rho, bsq, theta_e_in, theta_i_in, theta_e_out, theta_i_out, r, vol, shell_cells, lum_shell, flags)
     d = cool_diag() if want_diag else None
     _check(lib().cool_apply_host(table.handle, C.byref(c), C.byref(params), None if d is None else C.byref(d)))
     return None if d is None else d.as_dict()
@@ -248,6 +252,10 @@ def cool_table_destroy(table: CoolTable):
 
 def cool_last_launch_count() -> int:
     return lib().cool_last_launch_count()
+
+
+def cool_last_kernel_name() -> str:
+    return lib().cool_last_kernel_name().decode()
 
 
 def cool_version() -> str:

@@ -33,6 +33,28 @@ void set_error(const char *fmt, ...)
 
 void note_launches(int n) { g_launches = n; }
 
+static thread_local char g_kernel[256] = "";
+void note_kernel(const char *fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_kernel, sizeof g_kernel, fmt, ap);
+    va_end(ap);
+}
+
+// restores the caller's current device when an entry point that had to switch to the table's device returns
+struct DeviceGuard {
+    int prev = -1;
+    cudaError_t enter(int dev)
+    {
+        cudaError_t e = cudaGetDevice(&prev);
+        if (e != cudaSuccess) { prev = -1; return e; }
+        if (prev == dev) { prev = -1; return cudaSuccess; }
+        return cudaSetDevice(dev);
+    }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
 #define CUDA_TRY(call, what)                                                            \
     do {                                                                                \
         cudaError_t e_ = (call);                                                        \
@@ -100,7 +122,8 @@ static cudaError_t make_textures(const float *host, int chan, size_t ex, size_t 
 static void free_table(cool_table *t)
 {
     if (!t) return;
-    cudaSetDevice(t->device);
+    DeviceGuard dg;
+    dg.enter(t->device);
     if (t->dev.tex_pt) cudaDestroyTextureObject(t->dev.tex_pt);
     if (t->dev.tex_lin) cudaDestroyTextureObject(t->dev.tex_lin);
     if (t->dev.ftex_pt) cudaDestroyTextureObject(t->dev.ftex_pt);
@@ -114,10 +137,11 @@ static void free_table(cool_table *t)
     if (t->d_fcoulq) cudaFree(t->d_fcoulq);
     if (t->d_q3) cudaFree(t->d_q3);
     if (t->d_o3) cudaFree(t->d_o3);
-    for (auto &kv : t->diag_ws) { cudaFree(kv.second.partials); cudaFree(kv.second.ticket); if (kv.second.shell_rep) cudaFree(kv.second.shell_rep); }
+    for (auto &kv : t->diag_ws) { cudaFree(kv.second.partials); cudaFree(kv.second.ticket); if (kv.second.shell_rep) cudaFree(kv.second.shell_rep); if (kv.second.fixmap) cudaFree(kv.second.fixmap); }
     for (auto &s : t->stages) {
         for (void *b : s.buf) if (b) cudaFree(b);
         if (s.d_diag) cudaFree(s.d_diag);
+        if (s.flags) cudaFree(s.flags);
         if (s.s) cudaStreamDestroy(s.s);
     }
     if (t->h_diag_pinned) cudaFreeHost(t->h_diag_pinned);
@@ -128,7 +152,7 @@ static void free_table(cool_table *t)
 // fills the radial-profile fields of `a` for a launch over cells [off, off + n) and zeroes the replica workspace on `st`
 static cool_status prepare_shells(const cool_table *t, cudaStream_t st, LaunchArgs &a, double *d_out, long long shell_cells, long long off, long long n);
 
-static cool_status get_diag_ws(const cool_table *t, cudaStream_t st, DiagWorkspace *out, size_t shell_bytes = 0)
+static cool_status get_diag_ws(const cool_table *t, cudaStream_t st, DiagWorkspace *out, size_t shell_bytes = 0, size_t fixmap_bytes = 0)
 {
     std::lock_guard<std::mutex> lk(t->mu);
     auto it = t->diag_ws.find(st);
@@ -136,9 +160,23 @@ static cool_status get_diag_ws(const cool_table *t, cudaStream_t st, DiagWorkspa
         DiagWorkspace w;
         w.capacity_blocks = t->sm_count * 32;
         CUDA_TRY(cudaMalloc(&w.partials, sizeof(double) * 8 * (size_t)w.capacity_blocks), "cudaMalloc(diag partials)");
-        CUDA_TRY(cudaMalloc(&w.ticket, sizeof(unsigned)), "cudaMalloc(diag ticket)");
-        CUDA_TRY(cudaMemset(w.ticket, 0, sizeof(unsigned)), "cudaMemset(diag ticket)");
+        cudaError_t e = cudaMalloc(&w.ticket, sizeof(unsigned));
+        // zeroed on the stream whose kernels use it (a plain cudaMemset runs on the legacy default stream, which
+        // non-blocking streams do not wait for); the kernels leave it at zero again
+        if (e == cudaSuccess) e = cudaMemsetAsync(w.ticket, 0, sizeof(unsigned), st);
+        if (e != cudaSuccess) {
+            set_error("diag ticket: %s", cudaGetErrorString(e));
+            cudaFree(w.partials); if (w.ticket) cudaFree(w.ticket);
+            return e == cudaErrorMemoryAllocation ? COOL_ENOMEM : COOL_ECUDA;
+        }
         it = t->diag_ws.emplace(st, w).first;
+    }
+    if (fixmap_bytes > it->second.fixmap_cap) {
+        CUDA_TRY(cudaStreamSynchronize(st), "cudaStreamSynchronize(precise-pass bitmap)");
+        if (it->second.fixmap) cudaFree(it->second.fixmap);
+        it->second.fixmap = nullptr; it->second.fixmap_cap = 0;
+        CUDA_TRY(cudaMalloc(&it->second.fixmap, fixmap_bytes), "cudaMalloc(precise-pass bitmap)");
+        it->second.fixmap_cap = fixmap_bytes;
     }
     if (shell_bytes > it->second.shell_cap) {
         // growing the workspace of a stream that may still be running an earlier launch: wait for it first
@@ -167,6 +205,14 @@ static cool_status prepare_shells(const cool_table *t, cudaStream_t st, LaunchAr
     a.shell_rep = w.shell_rep;
     CUDA_TRY(cudaMemsetAsync(a.shell_rep, 0, bytes, st), "cudaMemsetAsync(shell workspace)");
     return COOL_OK;
+}
+
+// work lists of the precise pass (cool_fix.cu): per fp32-kernel warp a count, and per listed tile its index and four 32-bit
+// words of cell bits.  Every warp owns ceil(ntiles / warps) slots, so ntiles + warps slots always suffice.
+static size_t fixmap_bytes(const cool_table *t, long long ncell)
+{
+    const size_t ntiles = (size_t)((ncell + 127) / 128), warps = (size_t)t->sm_count * kFixMaxWarpsPerSm;
+    return warps * 4 + (ntiles + warps) * 20 + 64;
 }
 
 static cool_status check_args(const cool_table *t, const cool_cells *c, const cool_params *p, cool_variant *v, int *coul)
@@ -214,6 +260,7 @@ using namespace cool;
 extern "C" const char *cool_last_error(void) { return g_err; }
 extern "C" const char *cool_version(void) { return "cool_b200 0.1 (sm_100a)"; }
 extern "C" int cool_last_launch_count(void) { return g_launches; }
+extern "C" const char *cool_last_kernel_name(void) { return g_kernel; }
 
 extern "C" cool_variant cool_table_auto_variant(const cool_table *t)
 {
@@ -330,6 +377,58 @@ extern "C" cool_status cool_table_create(const cool_table_desc *desc, int device
                             }
                         }
                 }
+        }
+        // Steep intervals of the fp32 tables (cool_internal.h, cool_fix.cu): along Theta_e they become bands whose cells the
+        // precise pass recomputes; a steep interval along any other axis sends every cell there (not seen in the paper's tables).
+        {
+            double steep = kSteepLog2;
+            if (const char *ev = getenv("COOL_STEEP_LOG2")) steep = atof(ev);          // experiments; <= 0 switches the pass off
+            const int nr = ncan[CAX_RHO], ne = ncan[CAX_THE], ni = ncan[CAX_THI], nb = ncan[CAX_BSQ];
+            std::vector<double> de(ne > 1 ? ne - 1 : 0, 0.0);
+            double dother = 0.0;
+            const size_t sb = chan, si = (size_t)nb * chan, se = (size_t)ni * si, sr = (size_t)ne * se;
+            // What counts is the sensitivity of the TOTAL rate to a coordinate error.  nproc = 3: Q_thin = Q_brem + eta Q_syn, so
+            // a channel's node-to-node step is weighted by its share of Q_thin (a synchrotron table that falls by 100 log2
+            // units where bremsstrahlung dominates a million-fold is harmless); the shares are monotone between two nodes
+            // (the ratio of two log-linear interpolants), so the larger of the two end-point values bounds the interval.
+            auto step = [&](size_t o, size_t o2) {
+                if (nd == 3) return std::fabs((double)canon32[o2] - (double)canon32[o]);
+                const double d0 = std::fabs((double)canon32[o2] - (double)canon32[o]);
+                const double d1 = std::fabs(((double)canon32[o2 + 1] + (double)canon32[o2 + 2]) - ((double)canon32[o + 1] + (double)canon32[o + 2]));
+                double m = 0.0;
+                for (size_t q : {o, o2}) {
+                    const double ssy = 1.0 / (1.0 + exp2((double)canon32[q] - ((double)canon32[q + 1] + (double)canon32[q + 2])));
+                    m = std::max(m, (1.0 - ssy) * d0 + ssy * d1);
+                }
+                return m;
+            };
+            for (int ir = 0; ir < nr; ++ir)
+                for (int ie = 0; ie < ne; ++ie)
+                    for (int ii = 0; ii < ni; ++ii)
+                        for (int ib = 0; ib < nb; ++ib) {
+                            const size_t o = ir * sr + ie * se + ii * si + ib * sb;
+                            if (ie + 1 < ne) de[ie] = std::max(de[ie], step(o, o + se));
+                            if (ir + 1 < nr) dother = std::max(dother, step(o, o + sr));
+                            if (ii + 1 < ni) dother = std::max(dother, step(o, o + si));
+                            if (ib + 1 < nb) dother = std::max(dother, step(o, o + sb));
+                        }
+            D.nband = 0;
+            if (steep > 0.0) {
+                int first = -1, last = -1;                            // first and last steep interval: one band covers them all (over-marking is safe)
+                D.band_step = 0.f;
+                for (int ie = 0; ie + 1 < ne; ++ie)
+                    if (de[ie] > steep) { if (first < 0) first = ie; last = ie; D.band_step = std::max(D.band_step, (float)de[ie]); }
+                const AxisCoef &axe = D.ax[CAX_THE];
+                auto node_theta = [&](double tnode) { return pow(10.0, axe.lo10 + tnode / axe.inv10); };
+                if (dother > steep) {                                 // every positive Theta_e is inside the band
+                    D.nband = 1; D.band_lo = 0.f; D.band_hi = INFINITY;
+                    D.band_step = std::max(D.band_step, (float)dother);
+                } else if (first >= 0) {
+                    D.nband = 1;
+                    D.band_lo = (float)node_theta(first - kBandMargin);
+                    D.band_hi = (float)node_theta(last + 1 + kBandMargin);
+                }
+            }
         }
         e = cudaMalloc(&t->d_f32, bytes);
         if (e == cudaSuccess) e = cudaMemcpy(t->d_f32, canon32.data(), bytes, cudaMemcpyHostToDevice);
@@ -452,13 +551,22 @@ extern "C" cool_status cool_apply(const cool_table *t, const cool_cells *c, cons
     cool_variant v; int coul;
     cool_status s = check_args(t, c, p, &v, &coul);
     if (s != COOL_OK) return s;
-    CUDA_TRY(cudaSetDevice(t->device), "cudaSetDevice");
+    DeviceGuard dg;
+    CUDA_TRY(dg.enter(t->device), "cudaSetDevice");
     cudaStream_t st = (cudaStream_t)stream;
     LaunchArgs a{};
     a.ncell = c->ncell; a.rho = c->rho; a.bsq = c->bsq; a.the_in = c->theta_e_in; a.thi_in = c->theta_i_in;
     a.r = c->r; a.vol = c->vol; a.the_out = c->theta_e_out; a.thi_out = c->theta_i_out;
     a.dt = p->dt; a.nsub = p->nsub; a.f_limit = p->f_limit; a.h_floor = p->h_floor; a.coulomb = coul; a.scheme = p->scheme;
     a.want_diag = d_diag != nullptr; a.d_diag = d_diag;
+    if (c->flags && !d_diag) { set_error("flags needs d_diag"); return COOL_EINVAL; }
+    a.flags = c->flags;
+    if (c->ncell > 0 && uses_fixmap(t, v, c->dtype, a)) {
+        DiagWorkspace w;
+        s = get_diag_ws(t, st, &w, 0, fixmap_bytes(t, c->ncell));
+        if (s != COOL_OK) return s;
+        a.fixmap = w.fixmap; a.partials = w.partials; a.ticket = w.ticket;
+    }
     if (c->lum_shell) {
         if (!d_diag) { set_error("lum_shell needs d_diag"); return COOL_EINVAL; }
         const long long nshell = (c->ncell + c->shell_cells - 1) / c->shell_cells;
@@ -487,9 +595,11 @@ extern "C" cool_status cool_apply_host(const cool_table *t, const cool_cells *c,
     cool_variant v; int coul;
     cool_status s = check_args(t, c, p, &v, &coul);
     if (s != COOL_OK) return s;
-    CUDA_TRY(cudaSetDevice(t->device), "cudaSetDevice");
+    DeviceGuard dg;
+    CUDA_TRY(dg.enter(t->device), "cudaSetDevice");
     if (h_diag) memset(h_diag, 0, sizeof *h_diag);
     if (c->lum_shell && !h_diag) { set_error("lum_shell needs h_diag"); return COOL_EINVAL; }
+    if (c->flags && !h_diag) { set_error("flags needs h_diag"); return COOL_EINVAL; }
     if (c->ncell == 0) return COOL_OK;
 
     std::lock_guard<std::mutex> lk_host(t->host_mu);
@@ -506,13 +616,27 @@ extern "C" cool_status cool_apply_host(const cool_table *t, const cool_cells *c,
         }
     }
     if (t->stage_bytes < need_bytes) {
-        for (auto &sg : t->stages)
+        for (auto &sg : t->stages) {
+            CUDA_TRY(cudaStreamSynchronize(sg.s), "cudaStreamSynchronize");
             for (void *&b : sg.buf) {
                 if (b) { cudaFree(b); b = nullptr; }
                 CUDA_TRY(cudaMalloc(&b, need_bytes), "cudaMalloc(stage buffer)");
             }
+            if (sg.flags) { cudaFree(sg.flags); sg.flags = nullptr; }
+            CUDA_TRY(cudaMalloc(&sg.flags, chunk), "cudaMalloc(stage flags)");
+        }
         t->stage_bytes = need_bytes;
     }
+    // a failure inside the chunk loop must not return while copies into the caller's buffers are still in flight
+    auto fail_sync = [&](cool_status st_) { for (auto &sg : t->stages) cudaStreamSynchronize(sg.s); return st_; };
+#define CUDA_TRY_SYNC(call, what)                                                       \
+    do {                                                                                \
+        cudaError_t e_ = (call);                                                        \
+        if (e_ != cudaSuccess) {                                                        \
+            set_error("%s: %s", what, cudaGetErrorString(e_));                          \
+            return fail_sync(e_ == cudaErrorMemoryAllocation ? COOL_ENOMEM : COOL_ECUDA); \
+        }                                                                               \
+    } while (0)
     const size_t nchunks = ((size_t)c->ncell + chunk - 1) / chunk;
     if (h_diag && t->h_diag_cap < nchunks) {
         if (t->h_diag_pinned) cudaFreeHost(t->h_diag_pinned);
@@ -528,36 +652,46 @@ extern "C" cool_status cool_apply_host(const cool_table *t, const cool_cells *c,
         CUDA_TRY(cudaMalloc(&t->d_shell, shell_bytes), "cudaMalloc(shell sums)");
         t->d_shell_cap = shell_bytes;
     }
-    if (shell_bytes) CUDA_TRY(cudaMemset(t->d_shell, 0, shell_bytes), "cudaMemset(shell sums)");     // synchronous: done before any chunk's kernel
+    if (shell_bytes) {
+        // zeroed on stage stream 0 and waited for: every stage stream (non-blocking: they do not wait for the legacy default
+        // stream a plain cudaMemset would run on) adds into these sums
+        CUDA_TRY(cudaMemsetAsync(t->d_shell, 0, shell_bytes, t->stages[0].s), "cudaMemsetAsync(shell sums)");
+        CUDA_TRY(cudaStreamSynchronize(t->stages[0].s), "cudaStreamSynchronize(shell sums)");
+    }
     int nl = 0;
     for (size_t k = 0; k < nchunks; ++k) {
         auto &sg = t->stages[k % NST];
         const size_t off = k * chunk;
         const size_t n = std::min(chunk, (size_t)c->ncell - off);
         for (int j = 0; j < 6; ++j)
-            if (src[j]) CUDA_TRY(cudaMemcpyAsync(sg.buf[j], (const char *)src[j] + off * es, n * es, cudaMemcpyHostToDevice, sg.s), "cudaMemcpyAsync(H2D)");
+            if (src[j]) CUDA_TRY_SYNC(cudaMemcpyAsync(sg.buf[j], (const char *)src[j] + off * es, n * es, cudaMemcpyHostToDevice, sg.s), "cudaMemcpyAsync(H2D)");
         LaunchArgs a{};
         a.ncell = (long long)n; a.rho = sg.buf[0]; a.bsq = sg.buf[1]; a.the_in = sg.buf[2]; a.thi_in = sg.buf[3];
         a.r = c->r ? sg.buf[4] : nullptr; a.vol = c->vol ? sg.buf[5] : nullptr;
         a.the_out = sg.buf[6]; a.thi_out = sg.buf[7];
         a.dt = p->dt; a.nsub = p->nsub; a.f_limit = p->f_limit; a.h_floor = p->h_floor; a.coulomb = coul; a.scheme = p->scheme;
         a.want_diag = h_diag != nullptr; a.d_diag = h_diag ? sg.d_diag : nullptr;
+        a.flags = c->flags ? sg.flags : nullptr;
         if (shell_bytes) {
             s = prepare_shells(t, sg.s, a, t->d_shell, c->shell_cells, (long long)off, (long long)n);
-            if (s != COOL_OK) return s;
+            if (s != COOL_OK) return fail_sync(s);
         }
-        if (h_diag) {
+        const bool fix = uses_fixmap(t, v, c->dtype, a);
+        if (h_diag || fix) {
             DiagWorkspace w;
-            s = get_diag_ws(t, sg.s, &w);
-            if (s != COOL_OK) return s;
-            a.partials = w.partials; a.ticket = w.ticket;
+            s = get_diag_ws(t, sg.s, &w, 0, fix ? fixmap_bytes(t, (long long)n) : 0);
+            if (s != COOL_OK) return fail_sync(s);
+            a.partials = w.partials; a.ticket = w.ticket; a.fixmap = fix ? w.fixmap : nullptr;
+            if (shell_bytes) a.shell_rep = w.shell_rep;
         }
         s = launch_step(t, v, c->dtype, a, sg.s, &nl);
-        if (s != COOL_OK) return s;
-        CUDA_TRY(cudaMemcpyAsync((char *)c->theta_e_out + off * es, sg.buf[6], n * es, cudaMemcpyDeviceToHost, sg.s), "cudaMemcpyAsync(D2H)");
-        CUDA_TRY(cudaMemcpyAsync((char *)c->theta_i_out + off * es, sg.buf[7], n * es, cudaMemcpyDeviceToHost, sg.s), "cudaMemcpyAsync(D2H)");
-        if (h_diag) CUDA_TRY(cudaMemcpyAsync(&t->h_diag_pinned[k], sg.d_diag, sizeof(cool_diag), cudaMemcpyDeviceToHost, sg.s), "cudaMemcpyAsync(diag)");
+        if (s != COOL_OK) return fail_sync(s);
+        CUDA_TRY_SYNC(cudaMemcpyAsync((char *)c->theta_e_out + off * es, sg.buf[6], n * es, cudaMemcpyDeviceToHost, sg.s), "cudaMemcpyAsync(D2H)");
+        CUDA_TRY_SYNC(cudaMemcpyAsync((char *)c->theta_i_out + off * es, sg.buf[7], n * es, cudaMemcpyDeviceToHost, sg.s), "cudaMemcpyAsync(D2H)");
+        if (c->flags) CUDA_TRY_SYNC(cudaMemcpyAsync(c->flags + off, sg.flags, n, cudaMemcpyDeviceToHost, sg.s), "cudaMemcpyAsync(flags)");
+        if (h_diag) CUDA_TRY_SYNC(cudaMemcpyAsync(&t->h_diag_pinned[k], sg.d_diag, sizeof(cool_diag), cudaMemcpyDeviceToHost, sg.s), "cudaMemcpyAsync(diag)");
     }
+#undef CUDA_TRY_SYNC
     for (auto &sg : t->stages) CUDA_TRY(cudaStreamSynchronize(sg.s), "cudaStreamSynchronize");
     if (shell_bytes) CUDA_TRY(cudaMemcpy(c->lum_shell, t->d_shell, shell_bytes, cudaMemcpyDeviceToHost), "cudaMemcpy(shell sums)");
     g_launches = nl;

@@ -51,6 +51,14 @@ struct F32Const {
     // (this launch's workspace, local shell index), shell_reduce_kernel then adds the replicas into the caller's array
     double *lum_shell; unsigned shell_tiles, tile_offset, shell0, shell_nloc4, shell_rmask;
     unsigned long long shell_magic;                          // ceil(2^40 / shell_tiles): (t * magic) >> 40 == t / shell_tiles for t * shell_tiles < 2^40
+    // precise pass (cool_fix.cu): cells whose Theta_e coordinate enters a steep band of the table (DevTable::band_*) are not
+    // stored and not counted here; every warp lists the tiles in which it marked such cells (cool_internal.h, fix_layout)
+    unsigned *fixmap;                 // NULL: no precise pass
+    FixLists fix;
+    // a cell goes to the precise pass when band_lo < Theta_e < band_hi (the table's steep band, DevTable) and fix_rmin < h Lambda/u_e
+    // < fix_rmax (cool_internal.h).  Both windows are tested on the bit patterns (positive floats order like their bits):
+    // bits(x) - lo_bits < width as unsigned, which is false for negative, zero and NaN x; width 0 = empty (no precise pass)
+    unsigned band_lo_bits, band_w, rmin_bits, r_w;
 };
 
 // ------------------------------------------------------------------------------------------
@@ -188,6 +196,7 @@ __device__ __forceinline__ float lds_f32(unsigned addr)
 // same interpolation code, so the software variants agree bit for bit.
 // ------------------------------------------------------------------------------------------
 struct F32Global {
+    static const char *name() { return "F32Global"; }
     static constexpr bool kHw = false, kSmem = false;
     const float *p1; const float4 *p4; int sr, se, si, c3, c4;
     __device__ F32Global(const DevTable &T, const void *) : p1(T.f1), p4(T.f4), sr(T.s_rho), se(T.s_the), si(T.s_thi)
@@ -219,6 +228,7 @@ struct F32Global {
 // MODE 3 quad layout: q3[r][e][b] = {T'(r,e,b), T'(r,e,b+1), T'(r,e+1,b), T'(r,e+1,b+1)} (same strides as the plain
 // layout): a trilinear lookup is two 128-bit gathers, each inside one 32-byte sector.
 struct F32GlobalQ {
+    static const char *name() { return "F32GlobalQ"; }
     static constexpr bool kHw = false, kSmem = false;
     const float4 *pq; int sr, se, c3;
     __device__ F32GlobalQ(const DevTable &T, const void *) : pq(T.q3), sr(T.s_rho), se(T.s_the)
@@ -236,6 +246,7 @@ struct F32GlobalQ {
 // MODE 3 oct layout: o3[r][e][b] = the eight corners of table cell (r, e, b) in one 32-byte sector
 // {T'(r,e,b), T'(r,e,b+1), T'(r,e+1,b), T'(r,e+1,b+1), T'(r+1,e,b), ...}: a trilinear lookup is ONE 256-bit gather.
 struct F32GlobalO {
+    static const char *name() { return "F32GlobalO"; }
     static constexpr bool kHw = false, kSmem = false;
     const float4 *po; int sr, se, c3;
     __device__ F32GlobalO(const DevTable &T, const void *) : po(T.o3), sr(T.s_rho), se(T.s_the)
@@ -252,6 +263,7 @@ struct F32GlobalO {
     __device__ __forceinline__ void corners4(const Loc32 &, const Loc32 &, const Loc32 &, const Loc32 &, float4 (&)[2][2][4]) const {}
 };
 struct F32Smem {
+    static const char *name() { return "F32Smem"; }
     static constexpr bool kHw = false, kSmem = true;
     const float *p1; const float4 *p4; int sr, se, si, c3, c4;
     __device__ F32Smem(const DevTable &T, const void *img) : p1((const float *)img), p4((const float4 *)img), sr(T.s_rho), se(T.s_the), si(T.s_thi)
@@ -279,6 +291,7 @@ struct F32Smem {
     }
 };
 struct F32TexPoint {
+    static const char *name() { return "F32TexPoint"; }
     static constexpr bool kHw = false, kSmem = false;
     cudaTextureObject_t tex; float nef;
     __device__ F32TexPoint(const DevTable &T, const void *) : tex(T.ftex_pt), nef((float)T.ax[CAX_THE].n) {}
@@ -306,6 +319,7 @@ struct F32TexPoint {
     }
 };
 struct F32TexHw {
+    static const char *name() { return "F32TexHw"; }
     static constexpr bool kHw = true, kSmem = false;
     cudaTextureObject_t tex; float nef;
     __device__ F32TexHw(const DevTable &T, const void *) : tex(T.ftex_lin), nef((float)T.ax[CAX_THE].n) {}
@@ -442,24 +456,25 @@ struct Ctx32 { const DevTable &T; const F32Const &S; unsigned coul_s; };      //
 // ------------------------------------------------------------------------------------------
 template <int MODE, class Fetch, bool DIAG, int CM, bool NSUB1, int NV>
 __device__ __forceinline__ void step_cells_f32(const Ctx32 &X, const Fetch &F, const float *rho, const float *bsq, float *the, float *thi,
-                                               const float *rr, const float *vol, DiagAcc &acc, float (&tile_part)[4], unsigned wtile)
+                                               const float *rr, const float *vol, DiagAcc &acc, float (&tile_part)[4], unsigned wtile,
+                                               unsigned &fixmask, unsigned &flagword)
 {
     const DevTable &T = X.T; const F32Const &S = X.S;
     const int coulomb = (CM >= 1) ? 1 : S.coulomb;
     const int one_bits = opaque_const(0x3f800000);
     const bool use_floor = S.hfloor2 > 0.f;                 // warp-uniform
-    bool bad[NV], any_bad = false;
+    unsigned badm = 0u;                                     // bit j: cell j has rho <= 0 or a NaN input (one integer: predicate registers are scarce)
     float in_e[NV], in_i[NV], nanq[NV];
     Loc32 lr[NV], lb[NV];
     float kcell[NV], coul_kr[NV], tfloor[NV], lsum[NV][4];
     bool clamped[NV], limited[NV], floored[NV];
+    unsigned fm = 0u;                                       // bit j: cell j is left to the precise pass (one integer: predicate registers are scarce)
     Patch4 P[(MODE == 4 && !Fetch::kHw) ? NV : 1];
 #pragma unroll
     for (int j = 0; j < NV; ++j) {
         const float chk = (bsq[j] + the[j]) + (thi[j] + rho[j]);      // NaN when any input is NaN (or the sum overflows)
         nanq[j] = chk;
-        bad[j] = !(rho[j] > 0.f) || chk != chk;
-        any_bad |= bad[j];
+        if (!(rho[j] > 0.f) || chk != chk) badm |= 1u << j;
         in_e[j] = the[j]; in_i[j] = thi[j];
         clamped[j] = limited[j] = floored[j] = false;
         lr[j] = locate32<DIAG>(T.ax[CAX_RHO], rho[j], clamped[j], one_bits);
@@ -525,6 +540,9 @@ __device__ __forceinline__ void step_cells_f32(const Ctx32 &X, const Fetch &F, c
             if (use_floor) {
                 if ((the[j] + thi[j]) * S.mr < tfloor[j]) { rrad = 0.f; floored[j] = true; }
             }
+            // inside the steep band of the table, radiating a fraction that is neither negligible nor certainly limited: left to
+            // the precise pass (cool_internal.h); the band is empty when no precise pass follows
+            if (((__float_as_uint(the[j]) - S.band_lo_bits) < S.band_w) & ((__float_as_uint(rrad) - S.rmin_bits) < S.r_w)) fm |= 1u << j;
             if constexpr (DIAG) limited[j] |= (rrad > S.f_limit);
             rrad = fminf(rrad, S.f_limit);
             // Coulomb exchange (eq 15), capped by f_limit of the donor and by the equalising transfer
@@ -545,7 +563,7 @@ __device__ __forceinline__ void step_cells_f32(const Ctx32 &X, const Fetch &F, c
                         C = coulomb_C32<CM, coul_quads<Fetch, CM>()>(T.cax[1].n, T.coulq_stride, T.fcoul, X.coul_s, ca, cb);
                     }
                 } else {
-                    C = (D != 0.f && !bad[j]) ? (float)coolphys::coulomb_C((double)the[j], (double)thi[j] / S.ion_ratio) : 0.f;
+                    C = (D != 0.f && !((badm >> j) & 1u)) ? (float)coolphys::coulomb_C((double)the[j], (double)thi[j] / S.ion_ratio) : 0.f;
                 }
                 const float raw = coul_kr[j] * C * fabsf(D);
                 const float cap1 = (D > 0.f) ? S.cap1i * thi[j] : S.cap1e * the[j];
@@ -585,10 +603,22 @@ __device__ __forceinline__ void step_cells_f32(const Ctx32 &X, const Fetch &F, c
             }
         }
     }
-    if (any_bad) {                       // rare: rho <= 0 passes through, NaN inputs give NaN
+    flagword = 0u;
+    if (fm != 0u) {                      // rare: cells of the precise pass pass through here (the outputs may alias the inputs), unsummed and uncounted
 #pragma unroll
         for (int j = 0; j < NV; ++j)
-            if (bad[j]) {
+            if ((fm >> j) & 1u) {
+                if ((badm >> j) & 1u) { fm &= ~(1u << j); continue; }
+                the[j] = in_e[j]; thi[j] = in_i[j];
+                lsum[j][0] = lsum[j][1] = lsum[j][2] = lsum[j][3] = 0.f;
+                limited[j] = floored[j] = clamped[j] = false;
+            }
+    }
+    fixmask = fm;
+    if (badm != 0u) {                    // rare: rho <= 0 passes through, NaN inputs give NaN
+#pragma unroll
+        for (int j = 0; j < NV; ++j)
+            if ((badm >> j) & 1u) {
                 const float z = __fsub_rn(nanq[j], nanq[j]);          // 0, or NaN
                 the[j] = in_e[j] + z; thi[j] = in_i[j] + z;
             }
@@ -599,14 +629,15 @@ __device__ __forceinline__ void step_cells_f32(const Ctx32 &X, const Fetch &F, c
 #pragma unroll
         for (int j = 0; j < NV; ++j) {
             const float wgt = rho[j] * vol[j];                  // bad cells (possibly NaN) contribute an exact 0
-            part[0] += bad[j] ? 0.f : lsum[j][0] * wgt;
+            const bool bad = (badm >> j) & 1u;
+            part[0] += bad ? 0.f : lsum[j][0] * wgt;
             if constexpr (MODE == 4) {
 #pragma unroll
-                for (int k = 1; k < 4; ++k) part[k] += bad[j] ? 0.f : lsum[j][k] * wgt;
+                for (int k = 1; k < 4; ++k) part[k] += bad ? 0.f : lsum[j][k] * wgt;
             }
-            if (limited[j] && !bad[j]) ++acc.lim;               // predicated increments: the flags stay predicates
-            if (floored[j] && !bad[j]) ++acc.flo;
-            if (clamped[j] && !bad[j]) ++acc.cla;
+            if (limited[j] && !bad) { ++acc.lim; flagword |= 1u << (8 * j); }      // predicated: the flags stay predicates
+            if (floored[j] && !bad) { ++acc.flo; flagword |= 2u << (8 * j); }
+            if (clamped[j] && !bad) { ++acc.cla; flagword |= 4u << (8 * j); }
         }
         acc.lum[0] += (double)part[0];
         if constexpr (MODE == 4) {
@@ -707,6 +738,7 @@ cool_f32_kernel(const DevTable T, const F32Const S, const CellPtrs C, double *pa
     if (CM >= 1 && S.coul_smem) mbar_wait(cbar, 0);
     DiagAcc acc;
     int s = 0; unsigned phase = 0;
+    unsigned fixcnt = 0;                                      // tiles this warp has listed for the precise pass (warp-uniform)
     for (; tile < ntiles; tile += GW) {
         const long long c = tile * kWarpTile + (long long)lane * kF32CellsPerThread;
         float4 rho, bsq, the, thi;
@@ -734,13 +766,16 @@ cool_f32_kernel(const DevTable T, const F32Const S, const CellPtrs C, double *pa
             }
         }
         float tp[4] = {0.f, 0.f, 0.f, 0.f};                 // this thread's luminosity terms of the tile (DIAG)
+        unsigned fixmask = 0u, flagword = 0u;               // bit j / byte j: cell j of this lane
         if constexpr (MODE == 4) {
             // the 16-register patch allows one cell at a time: one copy of the cell code, run four times with the
             // vectors rotated (a quarter of the instruction footprint of the unrolled form)
             auto rot = [](float4 &v) { const float t = v.x; v.x = v.y; v.y = v.z; v.z = v.w; v.w = t; };
 #pragma unroll 1
             for (int j = 0; j < kF32CellsPerThread; ++j) {
-                step_cells_f32<MODE, Fetch, DIAG, CM, NSUB1, 1>(X, F, &rho.x, &bsq.x, &the.x, &thi.x, &rr.x, &vv.x, acc, tp, (unsigned)tile);
+                unsigned fm1, fw1;
+                step_cells_f32<MODE, Fetch, DIAG, CM, NSUB1, 1>(X, F, &rho.x, &bsq.x, &the.x, &thi.x, &rr.x, &vv.x, acc, tp, (unsigned)tile, fm1, fw1);
+                fixmask |= fm1 << j; flagword |= fw1 << (8 * j);
                 // a finished cell's rho, bsq, vol and r slots are dead: they carry its four luminosity terms to the end of the tile
                 if constexpr (DIAG) { rho.x = tp[0]; bsq.x = tp[1]; vv.x = tp[2]; rr.x = tp[3]; }
                 rot(rho); rot(bsq); rot(the); rot(thi); rot(rr); rot(vv);
@@ -750,14 +785,14 @@ cool_f32_kernel(const DevTable T, const F32Const S, const CellPtrs C, double *pa
                 tp[2] = (vv.x + vv.y) + (vv.z + vv.w); tp[3] = (rr.x + rr.y) + (rr.z + rr.w);
             }
         } else {
-            step_cells_f32<MODE, Fetch, DIAG, CM, NSUB1, kF32CellsPerThread>(X, F, &rho.x, &bsq.x, &the.x, &thi.x, &rr.x, &vv.x, acc, tp, (unsigned)tile);
-        }
-        if constexpr (DIAG && MODE == 4) {
-            if (S.lum_shell) shell_flush<MODE>(S, tp, (unsigned)tile);
+            step_cells_f32<MODE, Fetch, DIAG, CM, NSUB1, kF32CellsPerThread>(X, F, &rho.x, &bsq.x, &the.x, &thi.x, &rr.x, &vv.x, acc, tp, (unsigned)tile, fixmask, flagword);
         }
         if (full) {
             st_stream((float4 *)C.the_out + (c >> 2), the);
             st_stream((float4 *)C.thi_out + (c >> 2), thi);
+            if constexpr (DIAG) {
+                if (C.flags) *((unsigned *)(C.flags + c)) = flagword;
+            }
             // Re-arm the stage only now: the stores above depend on every value this warp read from it, so its
             // LDS have all returned (read-before-overwrite across the generic and async proxies).  With NST
             // stages the refill is still NST-1 tiles ahead of its use.
@@ -769,9 +804,30 @@ cool_f32_kernel(const DevTable T, const F32Const S, const CellPtrs C, double *pa
         } else {
 #pragma unroll
             for (int j = 0; j < kF32CellsPerThread; ++j)
-                if (c + j < ncell) { ((float *)C.the_out)[c + j] = (&the.x)[j]; ((float *)C.thi_out)[c + j] = (&thi.x)[j]; }
+                if (c + j < ncell) {
+                    ((float *)C.the_out)[c + j] = (&the.x)[j]; ((float *)C.thi_out)[c + j] = (&thi.x)[j];
+                    if constexpr (DIAG) {
+                        if (C.flags) C.flags[c + j] = (unsigned char)(flagword >> (8 * j));
+                    }
+                }
+        }
+        if (S.fixmap) {                                     // cells left to the precise pass: list the tile
+            if (__any_sync(0xffffffffu, fixmask != 0u)) {
+                const unsigned w0 = __ballot_sync(0xffffffffu, fixmask & 1u), w1 = __ballot_sync(0xffffffffu, fixmask & 2u);
+                const unsigned w2 = __ballot_sync(0xffffffffu, fixmask & 4u), w3 = __ballot_sync(0xffffffffu, fixmask & 8u);
+                if (lane == 0) {
+                    const size_t slot = (size_t)(blockIdx.x * NW + warp) * S.fix.cap + fixcnt;
+                    S.fix.tile[slot] = (unsigned)tile;
+                    S.fix.words[slot] = make_uint4(w0, w1, w2, w3);
+                }
+                ++fixcnt;
+            }
+        }
+        if constexpr (DIAG && MODE == 4) {
+            if (S.lum_shell) shell_flush<MODE>(S, tp, (unsigned)tile);
         }
     }
+    if (S.fixmap && lane == 0) S.fix.count[blockIdx.x * NW + warp] = fixcnt;      // every warp, every launch: no memset needed
     if constexpr (DIAG) reduce_diag(acc, S.lum_k, partials, ticket, d_diag);
 }
 
@@ -812,7 +868,13 @@ static cudaError_t launch_f32_one(const LaunchCtx32 &L)
     constexpr long long CTA_TILE = (long long)(THREADS / 32) * kWarpTile;
     const long long need = (a.ncell + CTA_TILE - 1) / CTA_TILE;
     const int grid = (int)(need < L.t->sm_count ? (need < 1 ? 1 : need) : L.t->sm_count);     // one persistent CTA per SM
-    CellPtrs C{a.rho, a.bsq, a.the_in, a.thi_in, a.r, a.vol, a.the_out, a.thi_out, a.ncell};
+    if (a.fixmap) {
+        const unsigned warps = (unsigned)grid * (THREADS / 32);
+        S.fix = fix_layout(a.fixmap, warps, (a.ncell + kWarpTile - 1) / kWarpTile);
+        a.fix_warps = warps; a.fix_cap = S.fix.cap;
+    }
+    CellPtrs C{a.rho, a.bsq, a.the_in, a.thi_in, a.r, a.vol, a.the_out, a.thi_out, a.ncell, a.flags};
+    note_kernel("cool_f32_kernel<MODE=%d,%s,DIAG=%d,CM=%d,NSUB1=%d,%dx%d>", MODE, Fetch::name(), (int)DIAG, CM, (int)NSUB1, THREADS, NST);
     kern<<<grid, THREADS, smem, L.st>>>(L.t->dev, S, C, a.partials, a.ticket, a.d_diag);
     return cudaGetLastError();
 }
@@ -843,5 +905,7 @@ static cudaError_t launch_f32_by_variant(const LaunchCtx32 &L, cool_variant v)
 // one function per translation unit of instantiations (cool_inst_f32_*.cu)
 cudaError_t launch_f32_m3(const LaunchCtx32 &L, cool_variant v, bool diag, int cm, bool nsub1);
 cudaError_t launch_f32_m4(const LaunchCtx32 &L, cool_variant v, bool diag, int cm);
+// precise pass over the cells the fp32 launch listed in LaunchArgs::fixmap (cool_fix.cu)
+cudaError_t launch_fix(const LaunchCtx &L, int mode, bool diag);
 
 }  // namespace cool

@@ -69,8 +69,10 @@ __device__ __forceinline__ double imp_loss_y(const StepConst &S, const ImpStep &
 
 template <int MODE, class Fetch>
 __device__ void implicit_cell(const DevTable &T, const DevConst &K, const StepConst &S, const Fetch &F,
-                              double rho, double bsq, double &the, double &thi, double r, double vol, DiagAcc &acc, long long cell)
+                              double rho, double bsq, double &the, double &thi, double r, double vol, DiagAcc &acc, long long cell,
+                              unsigned char *flags)
 {
+    if (flags) flags[cell] = 0;
     if (isnan(rho) || isnan(bsq) || isnan(the) || isnan(thi)) { the = thi = __longlong_as_double(0x7ff8000000000000LL); return; }
     if (!(rho > 0.0)) return;
     const AxisCoef &ax = T.ax[CAX_THE];
@@ -177,6 +179,7 @@ __device__ void implicit_cell(const DevTable &T, const DevConst &K, const StepCo
     for (int k = 0; k < 4; ++k) acc.lum[k] += de_sum[k] * wgt;
     acc.flo += floored; acc.cla += clamped;
     shell_add(S, cell, de_sum, wgt, MODE == 4);
+    if (flags) flags[cell] = (unsigned char)((floored << 1) | (clamped << 2));
 }
 
 template <class Real, int MODE, class Fetch, int THREADS>
@@ -192,7 +195,7 @@ cool_implicit_kernel(const DevTable T, const DevConst K, const StepConst S, cons
         double the = (double)((const Real *)C.the_in)[c], thi = (double)((const Real *)C.thi_in)[c];
         const double rho = (double)((const Real *)C.rho)[c], bsq = (double)((const Real *)C.bsq)[c];
         const double rr = S.has_r ? (double)((const Real *)C.r)[c] : 0.0, vv = S.has_vol ? (double)((const Real *)C.vol)[c] : 1.0;
-        implicit_cell<MODE, Fetch>(T, K, S, F, rho, bsq, the, thi, rr, vv, acc, c);
+        implicit_cell<MODE, Fetch>(T, K, S, F, rho, bsq, the, thi, rr, vv, acc, c, d_diag ? C.flags : nullptr);
         ((Real *)C.the_out)[c] = (Real)the;
         ((Real *)C.thi_out)[c] = (Real)thi;
     }
@@ -217,7 +220,7 @@ static cudaError_t launch_implicit_one(const LaunchCtx &L, size_t smem)
     long long need = (a.ncell + THREADS - 1) / THREADS;
     const long long cap = (long long)L.t->sm_count * (occ * 8 < 32 ? occ * 8 : 32);     // <= the diagnostics workspace (32 blocks per SM)
     const int grid = (int)(need < 1 ? 1 : (need < cap ? need : cap));
-    CellPtrs C{a.rho, a.bsq, a.the_in, a.thi_in, a.r, a.vol, a.the_out, a.thi_out, a.ncell};
+    CellPtrs C{a.rho, a.bsq, a.the_in, a.thi_in, a.r, a.vol, a.the_out, a.thi_out, a.ncell, a.flags};
     kern<<<grid, THREADS, smem, L.st>>>(L.t->dev, L.t->cst, *L.S, C, a.partials, a.ticket, a.d_diag);
     return cudaGetLastError();
 }
@@ -280,8 +283,10 @@ __device__ __forceinline__ float imp32_rate(const F32Const &S, const Imp32 &c, f
 
 template <int MODE, class Fetch>
 __device__ void implicit_cell_f32(const DevTable &T, const StepConst &S, const F32Const &S32, const Fetch &F,
-                                  float rho, float bsq, float &the, float &thi, float r, float vol, DiagAcc &acc, long long cell)
+                                  float rho, float bsq, float &the, float &thi, float r, float vol, DiagAcc &acc, long long cell,
+                                  unsigned char *flags)
 {
+    if (flags) flags[cell] = 0;
     const float chk = (bsq + the) + (thi + rho);
     if (chk != chk) { the = thi = __int_as_float(0x7fc00000); return; }
     if (!(rho > 0.f)) return;
@@ -416,6 +421,7 @@ __device__ void implicit_cell_f32(const DevTable &T, const StepConst &S, const F
     for (int k = 0; k < 4; ++k) acc.lum[k] += ds[k] * wgt;
     acc.flo += floored; acc.cla += clamped ? 1 : 0;
     shell_add(S, cell, ds, wgt, MODE == 4);
+    if (flags) flags[cell] = (unsigned char)((floored << 1) | (clamped ? 4 : 0));
 }
 
 template <int MODE, class Fetch, int THREADS>
@@ -443,7 +449,7 @@ cool_implicit_f32_kernel(const DevTable T, const StepConst S, const F32Const S32
         float the = n_the, thi = n_thi;
         const float rho = n_rho, bsq = n_bsq, rr = n_rr, vv = n_vv;
         if (c + stride < C.ncell) fetch(c + stride);
-        implicit_cell_f32<MODE, Fetch>(T, S, S32, F, rho, bsq, the, thi, rr, vv, acc, c);
+        implicit_cell_f32<MODE, Fetch>(T, S, S32, F, rho, bsq, the, thi, rr, vv, acc, c, d_diag ? C.flags : nullptr);
         __stcs((float *)C.the_out + c, the);
         __stcs((float *)C.thi_out + c, thi);
     }
@@ -467,7 +473,7 @@ static cudaError_t launch_implicit_f32_one(const LaunchCtx &L, const F32Const &S
     long long need = (a.ncell + THREADS - 1) / THREADS;
     const long long cap = (long long)L.t->sm_count * (occ * 8 < 32 ? occ * 8 : 32);
     const int grid = (int)(need < 1 ? 1 : (need < cap ? need : cap));
-    CellPtrs C{a.rho, a.bsq, a.the_in, a.thi_in, a.r, a.vol, a.the_out, a.thi_out, a.ncell};
+    CellPtrs C{a.rho, a.bsq, a.the_in, a.thi_in, a.r, a.vol, a.the_out, a.thi_out, a.ncell, a.flags};
     kern<<<grid, THREADS, smem, L.st>>>(L.t->dev, *L.S, S32, C, a.partials, a.ticket, a.d_diag);
     return cudaGetLastError();
 }

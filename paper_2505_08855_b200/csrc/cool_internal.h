@@ -58,9 +58,21 @@ struct DevTable {
     AxisCoef cax[2];               // 0: theta_i, 1: theta_e
     int coul_bytes;                // size of the Coulomb table (staged in shared memory when small)
     int coul_share_the, coul_share_thi;   // Coulomb axis identical to the table's Theta_e / Theta_i axis
+    // Steep Theta_e intervals (fp32 path): where neighbouring Theta_e nodes of T' differ by more than kSteepLog2 (weighted by
+    // the channel's share of Q_thin for the process tables) the fp32 node coordinate (<= 5e-6 nodes) and the fp32 state
+    // carried between sub-steps cannot hold the 1e-5 tolerance: the K2 -> 2 theta^2 switch of PAPER.md L87 is a 16-19
+    // log2-unit step between two nodes, a local power-law index of 60-140.  All steep intervals together make one band
+    // band_lo < Theta_e < band_hi (a margin included; the paper's tables have exactly one steep interval).  A cell that is inside a band at the start of a
+    // sub-step in which it radiates a fraction r of its electron energy with fix_rmin < r < fix_rmax (F32Const) is left to
+    // the precise pass (cool_fix.cu: the fp64 step on the canonical log10 tables): below fix_rmin the steep rate cannot move
+    // the result by more than 1.5e-6, above fix_rmax the 30 % limiter decides whatever the rate.
+    int nband;                     // 0: none, 1: band_lo < Theta_e < band_hi
+    float band_lo, band_hi;
+    float band_step;               // steepest step of the bands [log2 units per node]
 };
+constexpr double kSteepLog2 = 6.0;        // |Delta T'| per Theta_e node above which an interval is steep (precision budget)
+constexpr double kBandMargin = 1.0 / 128; // nodes; far above the distance between the fp32 and the fp64 trajectory of a cell (<= 2e-4 nodes)
 
-// Unit-dependent constants, precomputed on the host in fp64 (and rounded copies for fp32).
 struct DevConst {
     coolphys::Units units;
     coolphys::Derived der;
@@ -88,12 +100,33 @@ struct LaunchArgs {
     long long shell_cells, cell_offset, shell0;   // shell0: first shell this launch touches
     unsigned shell_nloc4;          // 4 x number of shells this launch touches
     unsigned shell_rmask;          // number of replicas - 1
+    unsigned char *flags;          // per-cell event flags (device) or NULL
+    unsigned *fixmap;              // precise pass workspace (see fix_layout); NULL: no pass
+    mutable unsigned fix_warps, fix_cap;   // set by the fp32 launch: its number of warps and the list slots each of them owns
 };
+// Precise-pass work lists inside LaunchArgs::fixmap, for an fp32 launch of `warps` warps over `ntiles` warp tiles:
+//   count[warps] | tile[warps * cap] | words[warps * cap] (uint4, 16-byte aligned),  cap = ceil(ntiles / warps)
+// warp w lists the tiles in which it marked cells at slots [w * cap, w * cap + count[w]); bit `lane` of word j of a tile
+// stands for cell tile*128 + lane*4 + j.
+constexpr int kFixMaxWarpsPerSm = 32;
+struct FixLists { unsigned *count, *tile; uint4 *words; unsigned cap; };
+inline FixLists fix_layout(unsigned *base, unsigned warps, long long ntiles)
+{
+    FixLists f;
+    f.cap = (unsigned)((ntiles + warps - 1) / warps);
+    f.count = base;
+    f.tile = base + warps;
+    size_t off = ((size_t)warps + (size_t)warps * f.cap) * 4;
+    off = (off + 15) & ~(size_t)15;
+    f.words = (uint4 *)((char *)base + off);
+    return f;
+}
 
 // radial-profile atomics are spread over 32 (small launches) or 256 copies (by block / warp index): at any moment nearly all
 // warps work in the same shell, and the L2 serialises atomics to one address
 constexpr int kShellReplicasSmall = 32, kShellReplicasLarge = 256;
-struct DiagWorkspace { double *partials = nullptr; unsigned *ticket = nullptr; int capacity_blocks = 0; double *shell_rep = nullptr; size_t shell_cap = 0; };
+struct DiagWorkspace { double *partials = nullptr; unsigned *ticket = nullptr; int capacity_blocks = 0; double *shell_rep = nullptr; size_t shell_cap = 0;
+                       unsigned *fixmap = nullptr; size_t fixmap_cap = 0; };
 
 }  // namespace cool
 
@@ -112,7 +145,7 @@ struct cool_table {
     mutable std::mutex mu, host_mu;
     mutable std::map<cudaStream_t, cool::DiagWorkspace> diag_ws;     // per-stream, so concurrent streams never share
     // host-path staging (cool_apply_host), created lazily, used under mu
-    struct HostStage { cudaStream_t s = nullptr; void *buf[8] = {}; cool_diag *d_diag = nullptr; };
+    struct HostStage { cudaStream_t s = nullptr; void *buf[8] = {}; cool_diag *d_diag = nullptr; unsigned char *flags = nullptr; };
     mutable std::vector<HostStage> stages;
     mutable size_t stage_bytes = 0;         // per staging buffer
     mutable cool_diag *h_diag_pinned = nullptr;
@@ -124,8 +157,10 @@ struct cool_table {
 namespace cool {
 void set_error(const char *fmt, ...);
 void note_launches(int n);           // what cool_last_launch_count() reports for this thread
+void note_kernel(const char *fmt, ...);   // what cool_last_kernel_name() reports for this thread
 bool desc_valid(const cool_table_desc *d, bool need_coulomb_shape, std::string *why);
 coolphys::Units to_units(const cool_units &u);
 cool_status launch_step(const cool_table *t, cool_variant v, cool_dtype dt, const LaunchArgs &a, cudaStream_t s, int *nlaunch);
 bool variant_supported(const cool_table *t, cool_variant v, cool_dtype dt, std::string *why);
+bool uses_fixmap(const cool_table *t, cool_variant v, cool_dtype dt, const LaunchArgs &a);
 }

@@ -262,7 +262,8 @@ __device__ __forceinline__ void update64(const DevTable &T, const DevConst &K, c
 
 template <int MODE, class Fetch, bool DIAG>
 __device__ __forceinline__ void step_cell_f64(const DevTable &T, const DevConst &K, const StepConst &S, const Fetch &F,
-                                              double rho, double bsq, double &the, double &thi, double r, double vol, DiagAcc &acc, long long cell)
+                                              double rho, double bsq, double &the, double &thi, double r, double vol, DiagAcc &acc, long long cell,
+                                              int *cell_flags = nullptr)
 {
     if (isnan(rho) || isnan(bsq) || isnan(the) || isnan(thi)) { the = thi = __longlong_as_double(0x7ff8000000000000LL); return; }
     if (!(rho > 0.0)) return;
@@ -298,13 +299,15 @@ __device__ __forceinline__ void step_cell_f64(const DevTable &T, const DevConst 
         for (int k = 0; k < 4; ++k) acc.lum[k] += de_sum[k] * wgt;
         acc.lim += limited; acc.flo += floored; acc.cla += clamped;
         shell_add(S, cell, de_sum, wgt, MODE == 4);
+        if (cell_flags) *cell_flags = limited | (floored << 1) | (clamped << 2);
     }
 }
 
 // analytic variant (COOL_V_ANALYTIC): eqs 1-12 per cell, fp64 regardless of the cell dtype
 template <int MODE, bool DIAG>
 __device__ __noinline__ void step_cell_analytic(const DevTable &T, const DevConst &K, const StepConst &S,
-                                                double rho, double bsq, double &the, double &thi, double r, double vol, DiagAcc &acc, long long cell)
+                                                double rho, double bsq, double &the, double &thi, double r, double vol, DiagAcc &acc, long long cell,
+                                                int *cell_flags)
 {
     if (isnan(rho) || isnan(bsq) || isnan(the) || isnan(thi)) { the = thi = __longlong_as_double(0x7ff8000000000000LL); return; }
     if (!(rho > 0.0)) return;
@@ -325,6 +328,7 @@ __device__ __noinline__ void step_cell_analytic(const DevTable &T, const DevCons
         for (int k = 0; k < 4; ++k) acc.lum[k] += de_sum[k] * wgt;
         acc.lim += limited; acc.flo += floored;
         shell_add(S, cell, de_sum, wgt, true);
+        if (cell_flags) *cell_flags = limited | (floored << 1);
     }
 }
 
@@ -392,24 +396,31 @@ __device__ __forceinline__ void reduce_diag(const DiagAcc &acc, double lum_k, do
 // ------------------------------------------------------------------------------------------
 // The kernel
 // ------------------------------------------------------------------------------------------
-struct CellPtrs { const void *rho, *bsq, *the_in, *thi_in, *r, *vol; void *the_out, *thi_out; long long ncell; };
+struct CellPtrs { const void *rho, *bsq, *the_in, *thi_in, *r, *vol; void *the_out, *thi_out; long long ncell; unsigned char *flags; };
 
 // NV cells of one thread through the right path
 template <class Real, int MODE, class Fetch, bool ANALYTIC, bool DIAG, int CM, int NV>
 __device__ __forceinline__ void do_cells(const DevTable &T, const DevConst &K, const StepConst &S, const Fetch &F, const float *coul,
-                                         const Real *rho, const Real *bsq, Real *the, Real *thi, const Real *r, const Real *vol, DiagAcc &acc, long long cell0)
+                                         const Real *rho, const Real *bsq, Real *the, Real *thi, const Real *r, const Real *vol, DiagAcc &acc, long long cell0,
+                                         unsigned char *flags)
 {
     if constexpr (ANALYTIC) {
 #pragma unroll 1
         for (int j = 0; j < NV; ++j) {
             double te = (double)the[j], ti = (double)thi[j];
-            step_cell_analytic<MODE, DIAG>(T, K, S, (double)rho[j], (double)bsq[j], te, ti, (double)r[j], (double)vol[j], acc, cell0 + j);
+            int fl = 0;
+            step_cell_analytic<MODE, DIAG>(T, K, S, (double)rho[j], (double)bsq[j], te, ti, (double)r[j], (double)vol[j], acc, cell0 + j, &fl);
             the[j] = (Real)te; thi[j] = (Real)ti;
+            if (DIAG && flags) flags[cell0 + j] = (unsigned char)fl;
         }
     } else {
         static_assert(sizeof(Real) == 8, "fp32 table variants live in cool_f32.cuh");
 #pragma unroll
-        for (int j = 0; j < NV; ++j) step_cell_f64<MODE, Fetch, DIAG>(T, K, S, F, rho[j], bsq[j], the[j], thi[j], r[j], vol[j], acc, cell0 + j);
+        for (int j = 0; j < NV; ++j) {
+            int fl = 0;
+            step_cell_f64<MODE, Fetch, DIAG>(T, K, S, F, rho[j], bsq[j], the[j], thi[j], r[j], vol[j], acc, cell0 + j, &fl);
+            if (DIAG && flags) flags[cell0 + j] = (unsigned char)fl;
+        }
     }
 }
 
@@ -437,7 +448,7 @@ cool_step_kernel(const DevTable T, const DevConst K, const StepConst S, const Ce
         for (int j = 0; j < N; ++j) { vget(rr, j) = (Real)0; vget(vv, j) = (Real)1; }
         if (S.has_r) rr = ld_stream((const V *)C.r + v);
         if (S.has_vol) vv = ld_stream((const V *)C.vol + v);
-        do_cells<Real, MODE, Fetch, ANALYTIC, DIAG, CM, N>(T, K, S, F, coul, &rho.x, &bsq.x, &the.x, &thi.x, &rr.x, &vv.x, acc, v * N);
+        do_cells<Real, MODE, Fetch, ANALYTIC, DIAG, CM, N>(T, K, S, F, coul, &rho.x, &bsq.x, &the.x, &thi.x, &rr.x, &vv.x, acc, v * N, C.flags);
         st_stream((V *)C.the_out + v, the);
         st_stream((V *)C.thi_out + v, thi);
     }
@@ -446,7 +457,7 @@ cool_step_kernel(const DevTable T, const DevConst K, const StepConst S, const Ce
         Real the = ((const Real *)C.the_in)[c], thi = ((const Real *)C.thi_in)[c];
         const Real rho = ((const Real *)C.rho)[c], bsq = ((const Real *)C.bsq)[c];
         const Real rr = S.has_r ? ((const Real *)C.r)[c] : (Real)0, vv = S.has_vol ? ((const Real *)C.vol)[c] : (Real)1;
-        do_cells<Real, MODE, Fetch, ANALYTIC, DIAG, CM, 1>(T, K, S, F, coul, &rho, &bsq, &the, &thi, &rr, &vv, acc, c);
+        do_cells<Real, MODE, Fetch, ANALYTIC, DIAG, CM, 1>(T, K, S, F, coul, &rho, &bsq, &the, &thi, &rr, &vv, acc, c, C.flags);
         ((Real *)C.the_out)[c] = the;
         ((Real *)C.thi_out)[c] = thi;
     }
@@ -462,24 +473,22 @@ template <class Real, int MODE, class Fetch, bool ANALYTIC, bool DIAG, int CM, i
 static cudaError_t launch_one(const LaunchCtx &L, size_t smem)
 {
     auto kern = cool_step_kernel<Real, MODE, Fetch, ANALYTIC, DIAG, CM, THREADS, MINB>;
-    static int occ_cache = -1; static size_t occ_smem = ~(size_t)0;
     if (smem > 48 * 1024) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
     }
-    if (occ_cache < 0 || occ_smem != smem) {
-        int occ = 0;
-        cudaError_t eo = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, THREADS, smem);
-        if (eo != cudaSuccess) return eo;
-        occ_cache = occ < 1 ? 1 : occ; occ_smem = smem;
-    }
+    // asked per call (a host-side computation of a few microseconds): a cached value would be shared by threads and devices
+    int occ_cache = 0;
+    cudaError_t eo = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_cache, kern, THREADS, smem);
+    if (eo != cudaSuccess) return eo;
+    if (occ_cache < 1) occ_cache = 1;
     const LaunchArgs &a = *L.a;
     constexpr int N = VecT<Real>::N;
     long long need = (a.ncell / N + THREADS - 1) / THREADS;
     if (need < 1) need = 1;
     const long long cap = (long long)L.t->sm_count * occ_cache;
     const int grid = (int)(need < cap ? need : cap);
-    CellPtrs C{a.rho, a.bsq, a.the_in, a.thi_in, a.r, a.vol, a.the_out, a.thi_out, a.ncell};
+    CellPtrs C{a.rho, a.bsq, a.the_in, a.thi_in, a.r, a.vol, a.the_out, a.thi_out, a.ncell, a.flags};
     kern<<<grid, THREADS, smem, L.st>>>(L.t->dev, L.t->cst, *L.S, C, a.partials, a.ticket, a.d_diag);
     return cudaGetLastError();
 }
@@ -487,6 +496,7 @@ static cudaError_t launch_one(const LaunchCtx &L, size_t smem)
 // one function per translation unit of instantiations (cool_inst_*.cu)
 cudaError_t launch_f64(const LaunchCtx &L, int mode, cool_variant v, bool diag);
 cudaError_t launch_analytic(const LaunchCtx &L, int mode, cool_dtype dt, bool diag);
+
 
 constexpr int kSmemThreads = 512;
 

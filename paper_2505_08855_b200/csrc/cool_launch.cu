@@ -1,4 +1,7 @@
 // cool_launch.cu — per-launch constants and dispatch to the kernel instantiations.
+#include <algorithm>
+#include <cstring>
+
 #include "cool_implicit.cuh"
 
 namespace cool {
@@ -29,7 +32,7 @@ static StepConst make_step_const(const cool_table *t, cool_dtype dt, const Launc
     S.spin = K.units.spin;
     S.lum_k = K.mr / (K.ge1 * a.dt);
     S.nsub = a.nsub; S.coulomb = a.coulomb;
-    S.has_r = a.r != nullptr; S.has_vol = a.vol != nullptr;
+    S.has_r = a.r != nullptr && S.hfloor2 > 0.0; S.has_vol = a.vol != nullptr && a.want_diag;      // arrays nobody uses are not read
     auto ok = [&](const void *p) { return p == nullptr || ((size_t)p % 16) == 0; };
     S.lum_shell = a.lum_shell ? a.shell_rep : nullptr; S.shell_cells = a.shell_cells > 0 ? a.shell_cells : 1;
     S.cell_offset = a.cell_offset; S.shell0 = a.shell0; S.shell_nloc4 = a.shell_nloc4; S.shell_rmask = a.shell_rmask;
@@ -71,14 +74,29 @@ static F32Const make_f32_const(const cool_table *t, const LaunchArgs &a)
     S.lum_k = K.mr / (K.ge1 * a.dt);
     S.ion_ratio = K.units.ion_theta_mass_ratio;
     S.nsub = a.nsub; S.coulomb = a.coulomb;
-    S.has_r = a.r != nullptr; S.has_vol = a.vol != nullptr;
+    S.has_r = a.r != nullptr && S.hfloor2 > 0.f; S.has_vol = a.vol != nullptr && a.want_diag;      // arrays nobody uses are neither staged nor read
     S.nf = 4 + S.has_r + S.has_vol;
+    S.fixmap = a.fixmap;
+    {
+        // precise-pass criterion (cool_internal.h): a band cell left to the fp32 path errs by at most r/(1-r) x step x ln 2 x dt_nodes,
+        // dt_nodes = the fp32 path's worst node-coordinate error inside a band: 1e-5 (the tolerance itself) of Theta_e in
+        // node units plus the coordinate's own 1e-5
+        const DevTable &D0 = t->dev;
+        const double dt_nodes = 1e-5 * 1.4426950408889634 / (double)D0.ax[CAX_THE].d2f + 1e-5;
+        const double sens = 0.6931471805599453 * (double)D0.band_step * dt_nodes;
+        const bool on = a.fixmap != nullptr && D0.nband != 0;
+        auto bits = [](double x) { const float f = (float)x; unsigned u; memcpy(&u, &f, 4); return u; };
+        const float hi = std::min(D0.band_hi, 3.0e38f);               // keep the width a finite-float difference
+        const unsigned lo_b = bits(D0.band_lo), rmin_b = bits(1.5e-6 / sens), rmax_b = bits(a.f_limit * (1.0 + 2.0 * sens) + 1e-6);
+        S.band_lo_bits = lo_b; S.band_w = on ? bits(hi) - lo_b : 0u;
+        S.rmin_bits = rmin_b; S.r_w = (on && rmax_b > rmin_b) ? rmax_b - rmin_b : 0u;
+    }
     S.lum_shell = a.lum_shell ? a.shell_rep : nullptr;
     S.shell_tiles = a.shell_cells > 0 ? (unsigned)(a.shell_cells / kWarpTile) : 1u; S.tile_offset = (unsigned)(a.cell_offset / kWarpTile);
     S.shell0 = (unsigned)a.shell0; S.shell_nloc4 = a.shell_nloc4; S.shell_rmask = a.shell_rmask;
     S.shell_magic = ((1ull << 40) + S.shell_tiles - 1) / S.shell_tiles;
     auto ok = [&](const void *p) { return p == nullptr || ((size_t)p % 16) == 0; };
-    S.use_tma = ok(a.rho) && ok(a.bsq) && ok(a.the_in) && ok(a.thi_in) && ok(a.the_out) && ok(a.thi_out) && ok(a.r) && ok(a.vol);
+    S.use_tma = ok(a.rho) && ok(a.bsq) && ok(a.the_in) && ok(a.thi_in) && ok(a.the_out) && ok(a.thi_out) && ok(a.r) && ok(a.vol) && ((size_t)a.flags % 4) == 0;
     // Coulomb-table node coordinates as an affine map of the table's own node coordinates
     const DevTable &D = t->dev;
     if (D.fcoul && D.mode != 0) {
@@ -103,6 +121,14 @@ bool variant_supported(const cool_table *t, cool_variant v, cool_dtype, std::str
     return true;
 }
 
+// The precise pass follows the fp32 software-interpolation kernels of the explicit scheme when the table has steep Theta_e
+// intervals.  Not the hardware-filtered texture (its 8-bit weights miss the tolerance everywhere: reported, not gated), not
+// fp64 cells or the analytic variant (already fp64), not the implicit scheme (a root solve is insensitive to the coordinate).
+bool uses_fixmap(const cool_table *t, cool_variant v, cool_dtype dt, const LaunchArgs &a)
+{
+    return t->dev.nband != 0 && dt == COOL_F32 && a.scheme == COOL_SCHEME_EXPLICIT && (v == COOL_V_GLOBAL || v == COOL_V_SMEM || v == COOL_V_TEX_POINT);
+}
+
 cool_status launch_step(const cool_table *t, cool_variant v, cool_dtype dt, const LaunchArgs &a, cudaStream_t st, int *nlaunch)
 {
     const StepConst S = make_step_const(t, dt, a);
@@ -110,11 +136,23 @@ cool_status launch_step(const cool_table *t, cool_variant v, cool_dtype dt, cons
     const int mode = t->dev.mode == 0 ? (t->desc.ndim == 4 ? 4 : 3) : t->dev.mode;
     const bool diag = a.want_diag != 0;
     cudaError_t e;
-    if (a.scheme == COOL_SCHEME_IMPLICIT) e = launch_implicit(L, make_f32_const(t, a), mode, v, dt);
-    else if (v == COOL_V_ANALYTIC) e = launch_analytic(L, mode, dt, diag);
-    else if (dt == COOL_F64) e = launch_f64(L, mode, v, diag);
+    bool fix = false;
+    static const char *const vname[] = {"auto", "tex_point", "tex_hwfilter", "smem", "global", "analytic"};
+    if (a.scheme == COOL_SCHEME_IMPLICIT) {
+        note_kernel("%s<MODE=%d,%s>", dt == COOL_F64 ? "cool_implicit_kernel" : "cool_implicit_f32_kernel", mode, vname[v]);
+        e = launch_implicit(L, make_f32_const(t, a), mode, v, dt);
+    } else if (v == COOL_V_ANALYTIC) {
+        note_kernel("cool_step_kernel<%s,MODE=%d,analytic,DIAG=%d>", dt == COOL_F64 ? "double" : "float", mode, (int)diag);
+        e = launch_analytic(L, mode, dt, diag);
+    } else if (dt == COOL_F64) {
+        note_kernel("cool_step_kernel<double,MODE=%d,%s,DIAG=%d>", mode, vname[v], (int)diag);
+        e = launch_f64(L, mode, v, diag);
+    }
     else {
-        LaunchCtx32 L32{t, make_f32_const(t, a), &a, st};
+        fix = a.fixmap && uses_fixmap(t, v, dt, a);
+        LaunchArgs af = a;                                   // the fp32 kernels list cells for the precise pass only when it will run
+        if (!fix) af.fixmap = nullptr;
+        LaunchCtx32 L32{t, make_f32_const(t, af), &a, st};
         const int csm = coulomb_smem_mode(t, a, v);
         L32.S.coul_smem = csm != 0;
         // fast path: Coulomb from the coefficient table staged in shared memory (or riding in the 4-D texels)
@@ -123,6 +161,11 @@ cool_status launch_step(const cool_table *t, cool_variant v, cool_dtype dt, cons
     }
     if (e != cudaSuccess) { set_error("kernel launch failed: %s", cudaGetErrorString(e)); return COOL_ECUDA; }
     if (nlaunch) *nlaunch += 1;
+    if (fix) {                                           // precise pass over the cells the fp32 kernel listed (steep table intervals)
+        e = launch_fix(L, mode, diag);
+        if (e != cudaSuccess) { set_error("kernel launch failed: %s", cudaGetErrorString(e)); return COOL_ECUDA; }
+        if (nlaunch) *nlaunch += 1;
+    }
     if (a.lum_shell) {                       // radial profile: fold this launch's replicas into the caller's array
         shell_reduce_kernel<<<(a.shell_nloc4 + 255) / 256, 256, 0, st>>>(a.shell_rep, a.lum_shell, a.shell_nloc4, a.shell0, a.shell_rmask);
         e = cudaGetLastError();

@@ -50,7 +50,7 @@ def oracle_table(oracle, desc, data, coul):
 
 def gpu_step(table, fields, dtype, dt, nsub=1, f_limit=0.3, h_floor=0.0, variant=api.COOL_V_AUTO,
              coulomb=api.COOL_COULOMB_AUTO, want_diag=True, use_r=False, use_vol=False, inplace=False, offset=0,
-             scheme=api.COOL_SCHEME_EXPLICIT, shell_cells=0):
+             scheme=api.COOL_SCHEME_EXPLICIT, shell_cells=0, want_flags=False):
     """One cool_apply on cuda:0 through the C ABI.  ``offset`` (elements) misaligns the arrays."""
     import torch
     tdt = torch.float32 if dtype == np.float32 else torch.float64
@@ -78,11 +78,14 @@ def gpu_step(table, fields, dtype, dt, nsub=1, f_limit=0.3, h_floor=0.0, variant
     lum_shell = None
     if shell_cells:
         lum_shell = torch.full((4 * ((n + shell_cells - 1) // shell_cells),), -1.0, dtype=torch.float64, device=dev)   # must be overwritten
+    flags = torch.full((n + 4,), 255, dtype=torch.uint8, device=dev)[offset % 4:][:n] if want_flags else None   # must be overwritten
     api.cool_apply(table, n, cdt, rho, bsq, the, thi, the_o, thi_o, params, r=r, vol=vol, d_diag=d_diag, stream=stream,
-                   shell_cells=shell_cells, lum_shell=lum_shell)
+                   shell_cells=shell_cells, lum_shell=lum_shell, flags=flags)
     torch.cuda.synchronize()
     out = dict(theta_e=the_o.cpu().numpy().astype(np.float64), theta_i=thi_o.cpu().numpy().astype(np.float64),
-               launches=api.cool_last_launch_count())
+               launches=api.cool_last_launch_count(), kernel=api.cool_last_kernel_name())
+    if flags is not None:
+        out["flags"] = flags.cpu().numpy()
     if want_diag:
         raw = d_diag.cpu().numpy().tobytes()
         out["diag"] = api.cool_diag.from_buffer_copy(raw).as_dict()
@@ -92,11 +95,11 @@ def gpu_step(table, fields, dtype, dt, nsub=1, f_limit=0.3, h_floor=0.0, variant
 
 
 def oracle_step(oracle, otab, un, fields, dt, nsub=1, f_limit=0.3, h_floor=0.0, use_r=False, use_vol=False,
-                rate_mode=0, coulomb_mode=None, nthreads=0):
+                rate_mode=0, coulomb_mode=None, nthreads=0, **kw):
     return oracle.step(otab, un, fields["rho"], fields["bsq"], fields["theta_e"], fields["theta_i"], dt, nsub=nsub,
                        f_limit=f_limit, h_floor=h_floor, r=fields["r"] if use_r else None,
                        vol=fields["vol"] if use_vol else None, rate_mode=rate_mode, coulomb_mode=coulomb_mode,
-                       nthreads=nthreads or oracle.max_threads())
+                       nthreads=nthreads or oracle.max_threads(), **kw)
 
 
 def oracle_step_implicit(oracle, otab, un, fields, dt, nsub=1, h_floor=0.0, use_r=False, use_vol=False, coulomb_mode=None, nthreads=0):
