@@ -420,9 +420,11 @@ extern "C" cool_status cool_table_create(const cool_table_desc *desc, int device
                     if (de[ie] > steep) { if (first < 0) first = ie; last = ie; D.band_step = std::max(D.band_step, (float)de[ie]); }
                 const AxisCoef &axe = D.ax[CAX_THE];
                 auto node_theta = [&](double tnode) { return pow(10.0, axe.lo10 + tnode / axe.inv10); };
+                D.band_k0 = first; D.band_k1 = last;
                 if (dother > steep) {                                 // every positive Theta_e is inside the band
                     D.nband = 1; D.band_lo = 0.f; D.band_hi = INFINITY;
                     D.band_step = std::max(D.band_step, (float)dother);
+                    D.band_k0 = 0; D.band_k1 = ne - 2;
                 } else if (first >= 0) {
                     D.nband = 1;
                     D.band_lo = (float)node_theta(first - kBandMargin);

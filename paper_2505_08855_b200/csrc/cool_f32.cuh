@@ -51,14 +51,15 @@ struct F32Const {
     // (this launch's workspace, local shell index), shell_reduce_kernel then adds the replicas into the caller's array
     double *lum_shell; unsigned shell_tiles, tile_offset, shell0, shell_nloc4, shell_rmask;
     unsigned long long shell_magic;                          // ceil(2^40 / shell_tiles): (t * magic) >> 40 == t / shell_tiles for t * shell_tiles < 2^40
-    // precise pass (cool_fix.cu): cells whose Theta_e coordinate enters a steep band of the table (DevTable::band_*) are not
-    // stored and not counted here; every warp lists the tiles in which it marked such cells (cool_internal.h, fix_layout)
+    // precise pass (cool_fix.cu): a cell goes there when band_lo < Theta_e < band_hi (the table's steep band, DevTable) at the
+    // start of a sub-step in which fix_rmin < h Lambda/u_e < fix_rmax (cool_internal.h).  Both windows are tested on the bit
+    // patterns (positive floats order like their bits): bits(x) - lo_bits < width as unsigned, false for negative, zero and
+    // NaN x; width 0 = empty (no precise pass).  Such a cell is treated like a cell with rho <= 0 here (passed through,
+    // neither summed nor counted) and its tile is listed for the precise pass (cool_internal.h, fix_layout).
+    unsigned band_lo_bits, band_w, rmin_bits, r_w;
+    int kb_lo; unsigned kb_n;         // the band's Theta_e intervals and one neighbour each side, as node-index words (Loc32::tf bits): (bits - kb_lo) < kb_n
     unsigned *fixmap;                 // NULL: no precise pass
     FixLists fix;
-    // a cell goes to the precise pass when band_lo < Theta_e < band_hi (the table's steep band, DevTable) and fix_rmin < h Lambda/u_e
-    // < fix_rmax (cool_internal.h).  Both windows are tested on the bit patterns (positive floats order like their bits):
-    // bits(x) - lo_bits < width as unsigned, which is false for negative, zero and NaN x; width 0 = empty (no precise pass)
-    unsigned band_lo_bits, band_w, rmin_bits, r_w;
 };
 
 // ------------------------------------------------------------------------------------------
@@ -444,7 +445,7 @@ __device__ __forceinline__ void shell_flush(const F32Const &S, const float (&par
 template <class Fetch, int CM>
 __host__ __device__ constexpr bool coul_quads() { return CM == 1 && !Fetch::kSmem; }
 
-struct Ctx32 { const DevTable &T; const F32Const &S; unsigned coul_s; };      // coul_s: shared-memory address of the staged Coulomb quads
+struct Ctx32 { const DevTable &T; const F32Const &S; unsigned coul_s; bool want_flags; };      // coul_s: shared-memory address of the staged Coulomb quads
 
 // ------------------------------------------------------------------------------------------
 // NV cells of one thread through all sub-steps, straight-line (no per-cell branches except the
@@ -454,27 +455,54 @@ struct Ctx32 { const DevTable &T; const F32Const &S; unsigned coul_s; };      //
 // Cells with rho <= 0 pass through and cells with a NaN input give NaN (that cell only): they
 // run through the arithmetic like any other cell and are patched at the end.
 // ------------------------------------------------------------------------------------------
-template <int MODE, class Fetch, bool DIAG, int CM, bool NSUB1, int NV>
+// Single update of a cell whose INPUT Theta_e lies in the steep band (F32Const::band_*): the only thing fp32 cannot carry
+// there is the Theta_e node coordinate (the inputs are exact and no state is carried), so the rate is re-evaluated with
+//   * t_e = (log2 Theta_e - lo)/Delta and its interval weight in fp64,
+//   * the two Theta_e nodes contracted over (rho, bsq) in fp32, then y = a(e) + w_e (a(e+1) - a(e)) + log2 h + clamp terms in fp64,
+//   * 2^y with the integer part exact and the fraction (|f| <= 1/2) by MUFU.EX2.
+// Rare (a few cells in ten thousand) and out of line, so the step around it keeps its registers.  Reads the plain T' layout.
+static __device__ __noinline__ float precise_rate3(const float *f1, int s_rho, int s_the, int n, double lo10, double inv10,
+                                                   int ir, int ib, float wr, float wb, float the, float kcell)      // scalars only: no struct on the stack
+{
+    const double L10 = 3.321928094887362;
+    const double t = (log2((double)the) - lo10 * L10) * (inv10 / L10);
+    const double tc = fmin(fmax(t, 0.0), (double)(n - 1));
+    int ie = (int)tc;
+    if (ie > n - 2) ie = n - 2;
+    const double w = tc - (double)ie;
+    const float *p = f1 + ((size_t)ir * s_rho + (size_t)ie * s_the + ib), *q = p + s_the, *u = p + s_rho, *v = u + s_the;
+    const float a0 = lerp(wr, lerp(wb, __ldg(p), __ldg(p + 1)), lerp(wb, __ldg(u), __ldg(u + 1)));      // node e
+    const float a1 = lerp(wr, lerp(wb, __ldg(q), __ldg(q + 1)), lerp(wb, __ldg(v), __ldg(v + 1)));      // node e + 1
+    double y = fma(w, (double)a1 - (double)a0, (double)a0) + ((tc - t) * (L10 / inv10) + (double)kcell);
+    y = fmin(fmax(y, -1000.0), 1000.0);
+    const double yi = rint(y);
+    return (float)scalbn((double)ex2_approx((float)(y - yi)), (int)yi);
+}
+
+// FIXT: test every cell at every sub-step for the precise pass (F32Const::band_*).  MODE 3 only; the 4-D step tests inside its
+// patch-rebuild branch instead (cells in or next to the steep interval rebuild their patch every sub-step), which costs the
+// sub-step loop nothing.
+template <int MODE, class Fetch, bool DIAG, int CM, bool NSUB1, int NV, bool FIXT>
 __device__ __forceinline__ void step_cells_f32(const Ctx32 &X, const Fetch &F, const float *rho, const float *bsq, float *the, float *thi,
                                                const float *rr, const float *vol, DiagAcc &acc, float (&tile_part)[4], unsigned wtile,
-                                               unsigned &fixmask, unsigned &flagword)
+                                               unsigned &flagword)   // byte j: event flags of cell j (include/cool.h); bit 3 = left to the precise pass
 {
     const DevTable &T = X.T; const F32Const &S = X.S;
     const int coulomb = (CM >= 1) ? 1 : S.coulomb;
     const int one_bits = opaque_const(0x3f800000);
     const bool use_floor = S.hfloor2 > 0.f;                 // warp-uniform
-    unsigned badm = 0u;                                     // bit j: cell j has rho <= 0 or a NaN input (one integer: predicate registers are scarce)
+    bool bad[NV], any_bad = false;
     float in_e[NV], in_i[NV], nanq[NV];
     Loc32 lr[NV], lb[NV];
     float kcell[NV], coul_kr[NV], tfloor[NV], lsum[NV][4];
     bool clamped[NV], limited[NV], floored[NV];
-    unsigned fm = 0u;                                       // bit j: cell j is left to the precise pass (one integer: predicate registers are scarce)
     Patch4 P[(MODE == 4 && !Fetch::kHw) ? NV : 1];
 #pragma unroll
     for (int j = 0; j < NV; ++j) {
         const float chk = (bsq[j] + the[j]) + (thi[j] + rho[j]);      // NaN when any input is NaN (or the sum overflows)
         nanq[j] = chk;
-        if (!(rho[j] > 0.f) || chk != chk) badm |= 1u << j;
+        bad[j] = !(rho[j] > 0.f) || chk != chk;
+        any_bad |= bad[j];
         in_e[j] = the[j]; in_i[j] = thi[j];
         clamped[j] = limited[j] = floored[j] = false;
         lr[j] = locate32<DIAG>(T.ax[CAX_RHO], rho[j], clamped[j], one_bits);
@@ -516,7 +544,26 @@ __device__ __forceinline__ void step_cells_f32(const Ctx32 &X, const Fetch &F, c
                     const float4 v = F.hw4(lr[j], le, li, lb[j]);
                     y0 = v.x; y1 = v.y; y2 = v.z; yc = v.w;
                 } else {
-                    if (loc_bits(le) != P[j].ke || loc_bits(li) != P[j].ki) build_patch(F, lr[j], lb[j], le, li, P[j]);
+                    if (loc_bits(le) != P[j].ke || loc_bits(li) != P[j].ki) {
+                        build_patch(F, lr[j], lb[j], le, li, P[j]);
+                        // Precise pass (F32Const::band_*): a cell whose Theta_e interval is the steep one or a neighbour of it
+                        // keeps its patch invalid, so it comes back here every sub-step, and only here is it tested — the
+                        // sub-step loop itself carries no test.  The radiated fraction is evaluated once more on this rare path.
+                        if ((unsigned)(loc_bits(le) - S.kb_lo) < S.kb_n) {
+                            P[j].ke = -1;
+                            if ((__float_as_uint(the[j]) - S.band_lo_bits) < S.band_w) {
+                                const float z0 = patch_eval(P[j], 0, le.w, li.w), z1 = patch_eval(P[j], 1, le.w, li.w), z2 = patch_eval(P[j], 2, le.w, li.w);
+                                const float qbr = ex2_approx(fminf(z0 + kk, 100.f)), qsy = ex2_approx(fminf((z1 + kk) + z2, 100.f));
+                                const float qthin = qbr + qsy;
+                                const float nm = fmaf(S.ae, the[j], S.ai * thi[j]), dn = fmaf(S.be, the[j], fmaf(S.bi, thi[j], 1.f));
+                                const float qcs = rho[j] * (nm * rsqrt_approx(nm * dn));
+                                const float tabs = qthin * (S.inv_kB * qcs) * rcp_approx(fmaxf(the[j] * the[j] * the[j], 1e-30f));
+                                float q = qthin * rcp_approx(fmaf(tabs, fmaf(1.5f, tabs + S.ksca * qcs, 1.7320508f), 1.f));
+                                if (use_floor && (the[j] + thi[j]) * S.mr < tfloor[j]) q = 0.f;
+                                if ((__float_as_uint(q) - S.rmin_bits) < S.r_w) { bad[j] = true; any_bad = true; nanq[j] = -0.f; }
+                            }
+                        }
+                    }
                     y0 = patch_eval(P[j], 0, le.w, li.w); y1 = patch_eval(P[j], 1, le.w, li.w);
                     y2 = patch_eval(P[j], 2, le.w, li.w); yc = patch_eval(P[j], 3, le.w, li.w);
                 }
@@ -541,8 +588,16 @@ __device__ __forceinline__ void step_cells_f32(const Ctx32 &X, const Fetch &F, c
                 if ((the[j] + thi[j]) * S.mr < tfloor[j]) { rrad = 0.f; floored[j] = true; }
             }
             // inside the steep band of the table, radiating a fraction that is neither negligible nor certainly limited: left to
-            // the precise pass (cool_internal.h); the band is empty when no precise pass follows
-            if (((__float_as_uint(the[j]) - S.band_lo_bits) < S.band_w) & ((__float_as_uint(rrad) - S.rmin_bits) < S.r_w)) fm |= 1u << j;
+            // the precise pass, passed through here like a cell without matter (the band is empty when no precise pass follows)
+            if constexpr (FIXT && MODE == 3) {
+                if (((__float_as_uint(the[j]) - S.band_lo_bits) < S.band_w) & ((__float_as_uint(rrad) - S.rmin_bits) < S.r_w)) {
+                    if constexpr (NSUB1 && !Fetch::kHw) {          // a single update: the precise rate, in place
+                        rrad = precise_rate3(T.f1, T.s_rho, T.s_the, T.ax[CAX_THE].n, T.ax[CAX_THE].lo10, T.ax[CAX_THE].inv10,
+                                             loc_bits(lr[j]) - (int)kMagicBits, loc_bits(lb[j]) - (int)kMagicBits, lr[j].w, lb[j].w, the[j], kcell[j]);
+                        if (use_floor && floored[j]) rrad = 0.f;
+                    } else { bad[j] = true; any_bad = true; nanq[j] = -0.f; }          // sub-steps: the precise pass
+                }
+            }
             if constexpr (DIAG) limited[j] |= (rrad > S.f_limit);
             rrad = fminf(rrad, S.f_limit);
             // Coulomb exchange (eq 15), capped by f_limit of the donor and by the equalising transfer
@@ -563,7 +618,7 @@ __device__ __forceinline__ void step_cells_f32(const Ctx32 &X, const Fetch &F, c
                         C = coulomb_C32<CM, coul_quads<Fetch, CM>()>(T.cax[1].n, T.coulq_stride, T.fcoul, X.coul_s, ca, cb);
                     }
                 } else {
-                    C = (D != 0.f && !((badm >> j) & 1u)) ? (float)coolphys::coulomb_C((double)the[j], (double)thi[j] / S.ion_ratio) : 0.f;
+                    C = (D != 0.f && !bad[j]) ? (float)coolphys::coulomb_C((double)the[j], (double)thi[j] / S.ion_ratio) : 0.f;
                 }
                 const float raw = coul_kr[j] * C * fabsf(D);
                 const float cap1 = (D > 0.f) ? S.cap1i * thi[j] : S.cap1e * the[j];
@@ -604,23 +659,14 @@ __device__ __forceinline__ void step_cells_f32(const Ctx32 &X, const Fetch &F, c
         }
     }
     flagword = 0u;
-    if (fm != 0u) {                      // rare: cells of the precise pass pass through here (the outputs may alias the inputs), unsummed and uncounted
+    if (any_bad) {                       // rare: rho <= 0 and cells of the precise pass pass through, NaN inputs give NaN
 #pragma unroll
         for (int j = 0; j < NV; ++j)
-            if ((fm >> j) & 1u) {
-                if ((badm >> j) & 1u) { fm &= ~(1u << j); continue; }
-                the[j] = in_e[j]; thi[j] = in_i[j];
-                lsum[j][0] = lsum[j][1] = lsum[j][2] = lsum[j][3] = 0.f;
-                limited[j] = floored[j] = clamped[j] = false;
-            }
-    }
-    fixmask = fm;
-    if (badm != 0u) {                    // rare: rho <= 0 passes through, NaN inputs give NaN
-#pragma unroll
-        for (int j = 0; j < NV; ++j)
-            if ((badm >> j) & 1u) {
+            if (bad[j]) {
                 const float z = __fsub_rn(nanq[j], nanq[j]);          // 0, or NaN
                 the[j] = in_e[j] + z; thi[j] = in_i[j] + z;
+                // a cell of the precise pass carries -0 in nanq (the sum of a valid cell's inputs is positive): flag bit 3
+                if (__float_as_uint(nanq[j]) == 0x80000000u) flagword |= 8u << (8 * j);
             }
     }
     if constexpr (DIAG) {
@@ -629,15 +675,19 @@ __device__ __forceinline__ void step_cells_f32(const Ctx32 &X, const Fetch &F, c
 #pragma unroll
         for (int j = 0; j < NV; ++j) {
             const float wgt = rho[j] * vol[j];                  // bad cells (possibly NaN) contribute an exact 0
-            const bool bad = (badm >> j) & 1u;
-            part[0] += bad ? 0.f : lsum[j][0] * wgt;
+            part[0] += bad[j] ? 0.f : lsum[j][0] * wgt;
             if constexpr (MODE == 4) {
 #pragma unroll
-                for (int k = 1; k < 4; ++k) part[k] += bad ? 0.f : lsum[j][k] * wgt;
+                for (int k = 1; k < 4; ++k) part[k] += bad[j] ? 0.f : lsum[j][k] * wgt;
             }
-            if (limited[j] && !bad) { ++acc.lim; flagword |= 1u << (8 * j); }      // predicated: the flags stay predicates
-            if (floored[j] && !bad) { ++acc.flo; flagword |= 2u << (8 * j); }
-            if (clamped[j] && !bad) { ++acc.cla; flagword |= 4u << (8 * j); }
+            if (limited[j] && !bad[j]) ++acc.lim;               // predicated increments: the flags stay predicates
+            if (floored[j] && !bad[j]) ++acc.flo;
+            if (clamped[j] && !bad[j]) ++acc.cla;
+        }
+        if (X.want_flags) {                                     // per-cell event flags (cool_cells::flags): tests and callers that ask
+#pragma unroll
+            for (int j = 0; j < NV; ++j)
+                if (!bad[j]) flagword |= ((limited[j] ? 1u : 0u) | (floored[j] ? 2u : 0u) | (clamped[j] ? 4u : 0u)) << (8 * j);
         }
         acc.lum[0] += (double)part[0];
         if constexpr (MODE == 4) {
@@ -661,14 +711,15 @@ __device__ __forceinline__ void step_cells_f32(const Ctx32 &X, const Fetch &F, c
 constexpr int kF32CellsPerThread = 4;
 constexpr int kWarpTile = 32 * kF32CellsPerThread;          // cells per warp tile
 constexpr unsigned kWarpArrBytes = kWarpTile * 4u;          // 512 B per array per stage
-constexpr unsigned kF32BarBytes = 1024;                     // room for 32 warps x 4 stages of 8-byte mbarriers
+constexpr unsigned kF32BarBytes = 1024;                     // room for 32 warps x 2 stages of 8-byte mbarriers, 32 list counters, the Coulomb barrier
+constexpr unsigned kF32FixCntOff = 768;                     // per-warp count of tiles listed for the precise pass (32 x 4 bytes)
 
 template <int MODE, class Fetch, bool DIAG, int CM, bool NSUB1, int THREADS, int NST>
 __global__ void __launch_bounds__(THREADS, 1)
 cool_f32_kernel(const DevTable T, const F32Const S, const CellPtrs C, double *partials, unsigned *ticket, cool_diag *d_diag)
 {
     constexpr int NW = THREADS / 32;
-    static_assert(NW * NST * 8 <= (int)kF32BarBytes - 8, "mbarrier area too small");
+    static_assert(NW * NST * 8 <= (int)kF32FixCntOff && NW * 4 <= (int)(kF32BarBytes - 8 - kF32FixCntOff), "mbarrier area too small");
     extern __shared__ __align__(128) unsigned char smem_f32[];
     const int tid = threadIdx.x, lane = tid & 31;
     const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);           // warp-uniform by construction: TMA operands stay in uniform registers
@@ -697,6 +748,7 @@ cool_f32_kernel(const DevTable T, const F32Const S, const CellPtrs C, double *pa
     const unsigned bar_w = smem_u32(smem_f32) + (unsigned)(warp * NST) * 8u;              // this warp's mbarriers
     const unsigned stg_w = smem_u32(smem_f32 + S.stage_off) + (unsigned)(warp * NST) * S.wstage_bytes;   // this warp's stages
     if (lane == 0) {
+        *((unsigned *)(smem_f32 + kF32FixCntOff) + warp) = 0u;
 #pragma unroll
         for (int s = 0; s < NST; ++s) mbar_init(bar_w + 8u * s, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -704,7 +756,7 @@ cool_f32_kernel(const DevTable T, const F32Const S, const CellPtrs C, double *pa
     }
     __syncthreads();
     const Fetch F(T, smem_f32 + S.table_off);
-    const Ctx32 X{T, S, smem_u32(smem_f32 + S.coul_off)};
+    const Ctx32 X{T, S, smem_u32(smem_f32 + S.coul_off), DIAG && C.flags != nullptr};
 
     const long long ncell = C.ncell;
     const long long ntiles = (ncell + kWarpTile - 1) / kWarpTile;
@@ -738,7 +790,6 @@ cool_f32_kernel(const DevTable T, const F32Const S, const CellPtrs C, double *pa
     if (CM >= 1 && S.coul_smem) mbar_wait(cbar, 0);
     DiagAcc acc;
     int s = 0; unsigned phase = 0;
-    unsigned fixcnt = 0;                                      // tiles this warp has listed for the precise pass (warp-uniform)
     for (; tile < ntiles; tile += GW) {
         const long long c = tile * kWarpTile + (long long)lane * kF32CellsPerThread;
         float4 rho, bsq, the, thi;
@@ -766,16 +817,16 @@ cool_f32_kernel(const DevTable T, const F32Const S, const CellPtrs C, double *pa
             }
         }
         float tp[4] = {0.f, 0.f, 0.f, 0.f};                 // this thread's luminosity terms of the tile (DIAG)
-        unsigned fixmask = 0u, flagword = 0u;               // bit j / byte j: cell j of this lane
+        unsigned flagword = 0u;                             // byte j: flags of cell j of this lane (bit 3: left to the precise pass)
         if constexpr (MODE == 4) {
             // the 16-register patch allows one cell at a time: one copy of the cell code, run four times with the
             // vectors rotated (a quarter of the instruction footprint of the unrolled form)
             auto rot = [](float4 &v) { const float t = v.x; v.x = v.y; v.y = v.z; v.z = v.w; v.w = t; };
 #pragma unroll 1
             for (int j = 0; j < kF32CellsPerThread; ++j) {
-                unsigned fm1, fw1;
-                step_cells_f32<MODE, Fetch, DIAG, CM, NSUB1, 1>(X, F, &rho.x, &bsq.x, &the.x, &thi.x, &rr.x, &vv.x, acc, tp, (unsigned)tile, fm1, fw1);
-                fixmask |= fm1 << j; flagword |= fw1 << (8 * j);
+                unsigned fw1;
+                step_cells_f32<MODE, Fetch, DIAG, CM, NSUB1, 1, true>(X, F, &rho.x, &bsq.x, &the.x, &thi.x, &rr.x, &vv.x, acc, tp, (unsigned)tile, fw1);
+                if (fw1) flagword |= fw1 << (8 * j);        // rare
                 // a finished cell's rho, bsq, vol and r slots are dead: they carry its four luminosity terms to the end of the tile
                 if constexpr (DIAG) { rho.x = tp[0]; bsq.x = tp[1]; vv.x = tp[2]; rr.x = tp[3]; }
                 rot(rho); rot(bsq); rot(the); rot(thi); rot(rr); rot(vv);
@@ -785,7 +836,20 @@ cool_f32_kernel(const DevTable T, const F32Const S, const CellPtrs C, double *pa
                 tp[2] = (vv.x + vv.y) + (vv.z + vv.w); tp[3] = (rr.x + rr.y) + (rr.z + rr.w);
             }
         } else {
-            step_cells_f32<MODE, Fetch, DIAG, CM, NSUB1, kF32CellsPerThread>(X, F, &rho.x, &bsq.x, &the.x, &thi.x, &rr.x, &vv.x, acc, tp, (unsigned)tile, fixmask, flagword);
+            // Precise pass: a single update can only put a cell there if its INPUT Theta_e lies in the steep band, so one
+            // warp-uniform look at the tile's inputs picks the step without any test (nearly every tile of a coherent field) or
+            // the step that tests every cell.  Sub-stepped launches always test (a cell can cool into the band).
+            bool tested = !NSUB1;
+            if constexpr (NSUB1) {
+                const bool inb = ((__float_as_uint(the.x) - S.band_lo_bits) < S.band_w) | ((__float_as_uint(the.y) - S.band_lo_bits) < S.band_w) |
+                                 ((__float_as_uint(the.z) - S.band_lo_bits) < S.band_w) | ((__float_as_uint(the.w) - S.band_lo_bits) < S.band_w);
+                tested = __any_sync(0xffffffffu, inb);
+            }
+            if (tested) step_cells_f32<MODE, Fetch, DIAG, CM, NSUB1, kF32CellsPerThread, true>(X, F, &rho.x, &bsq.x, &the.x, &thi.x, &rr.x, &vv.x, acc, tp, (unsigned)tile, flagword);
+            else step_cells_f32<MODE, Fetch, DIAG, CM, NSUB1, kF32CellsPerThread, false>(X, F, &rho.x, &bsq.x, &the.x, &thi.x, &rr.x, &vv.x, acc, tp, (unsigned)tile, flagword);
+        }
+        if constexpr (DIAG && MODE == 4) {
+            if (S.lum_shell) shell_flush<MODE>(S, tp, (unsigned)tile);
         }
         if (full) {
             st_stream((float4 *)C.the_out + (c >> 2), the);
@@ -812,22 +876,22 @@ cool_f32_kernel(const DevTable T, const F32Const S, const CellPtrs C, double *pa
                 }
         }
         if (S.fixmap) {                                     // cells left to the precise pass: list the tile
-            if (__any_sync(0xffffffffu, fixmask != 0u)) {
-                const unsigned w0 = __ballot_sync(0xffffffffu, fixmask & 1u), w1 = __ballot_sync(0xffffffffu, fixmask & 2u);
-                const unsigned w2 = __ballot_sync(0xffffffffu, fixmask & 4u), w3 = __ballot_sync(0xffffffffu, fixmask & 8u);
+            if (__any_sync(0xffffffffu, (flagword & 0x08080808u) != 0u)) {
+                const unsigned w0 = __ballot_sync(0xffffffffu, flagword & 0x8u), w1 = __ballot_sync(0xffffffffu, flagword & 0x800u);
+                const unsigned w2 = __ballot_sync(0xffffffffu, flagword & 0x80000u), w3 = __ballot_sync(0xffffffffu, flagword & 0x8000000u);
                 if (lane == 0) {
-                    const size_t slot = (size_t)(blockIdx.x * NW + warp) * S.fix.cap + fixcnt;
+                    // this warp's count of listed tiles lives in shared memory (rarely touched; registers are scarce)
+                    unsigned *cnt = (unsigned *)(smem_f32 + kF32FixCntOff) + warp;
+                    const unsigned k = *cnt;
+                    *cnt = k + 1u;
+                    const size_t slot = (size_t)(blockIdx.x * NW + warp) * S.fix.cap + k;
                     S.fix.tile[slot] = (unsigned)tile;
                     S.fix.words[slot] = make_uint4(w0, w1, w2, w3);
                 }
-                ++fixcnt;
             }
         }
-        if constexpr (DIAG && MODE == 4) {
-            if (S.lum_shell) shell_flush<MODE>(S, tp, (unsigned)tile);
-        }
     }
-    if (S.fixmap && lane == 0) S.fix.count[blockIdx.x * NW + warp] = fixcnt;      // every warp, every launch: no memset needed
+    if (S.fixmap && lane == 0) S.fix.count[blockIdx.x * NW + warp] = *((unsigned *)(smem_f32 + kF32FixCntOff) + warp);      // every warp, every launch: no memset needed
     if constexpr (DIAG) reduce_diag(acc, S.lum_k, partials, ticket, d_diag);
 }
 

@@ -15,22 +15,19 @@
 //
 // Work distribution.  Every warp of the fp32 launch has listed its tiles with marked cells (tile index + four 32-bit words,
 // cool_internal.h fix_layout); tiles go round-robin over the fp32 warps, so a contiguous block of marked cells (a shell of
-// a disc) is already spread over all lists.  kFixSplit warps here share one list (entry i goes to warp i mod kFixSplit); a
-// warp pushes the cell index of every set bit into a 64-entry ring in shared memory and runs the step whenever 32 cells
-// are waiting, so all lanes work whether the marked cells are scattered or dense.  The processing order is fixed by the
-// lists, and the sums go warp -> block -> fixed-order last block: reproducible bit for bit.
+// a disc) is already spread over all lists.  One block here takes one list, one warp one word at a time, one lane one cell.
+// The processing order is fixed by the lists, and the sums go warp -> block -> fixed-order last block: reproducible bit for bit.
 #include "cool_f32.cuh"
 
 namespace cool {
 
-constexpr int kFixThreads = 128, kFixWarps = kFixThreads / 32, kFixSplit = 4;
+constexpr int kFixThreads = 256, kFixWarps = kFixThreads / 32;     // one block per list of the fp32 launch, one warp per word in turn
 
 template <int MODE, bool DIAG>
 __global__ void __launch_bounds__(kFixThreads)
 cool_fix_kernel(const DevTable T, const DevConst K, const StepConst S, const CellPtrs C, const FixLists L, unsigned nlists,
                 double *partials, unsigned *ticket, cool_diag *d_diag)
 {
-    __shared__ long long ring[kFixWarps][64];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const FetchGlobal F(T, nullptr);
     DiagAcc acc;
@@ -49,38 +46,17 @@ cool_fix_kernel(const DevTable T, const DevConst K, const StepConst S, const Cel
         }
     };
 
-    int head = 0, qn = 0;                                       // this warp's ring: warp-uniform
-    const unsigned gw = gridDim.x * kFixWarps;
-    for (unsigned u = blockIdx.x * kFixWarps + warp; u < nlists * kFixSplit; u += gw) {
-        const unsigned v = u / kFixSplit, part = u % kFixSplit;
-        const unsigned cnt = __ldg(L.count + v);
-        const size_t base = (size_t)v * L.cap;
-        for (unsigned i0 = part; i0 < cnt; i0 += 8 * kFixSplit) {
-            // eight list entries at a time (this warp's share: every kFixSplit-th): lane l holds word (l & 3) of entry i0 + kFixSplit (l >> 2)
-            const unsigned e = i0 + kFixSplit * ((unsigned)lane >> 2);
-            unsigned wreg = 0u, treg = 0u;
-            if (e < cnt) {
-                wreg = __ldg((const unsigned *)(L.words + base + e) + (lane & 3));
-                treg = __ldg(L.tile + base + e);
-            }
-#pragma unroll 1
-            for (int k = 0; k < 32; ++k) {                      // word k of the batch: entry k >> 2, cell slot j = k & 3
-                const unsigned w = __shfl_sync(0xffffffffu, wreg, k);
-                if (w == 0u) continue;                          // warp-uniform
-                const long long tile = (long long)__shfl_sync(0xffffffffu, treg, k);
-                const bool has = (w >> lane) & 1u;
-                if (has) ring[warp][(head + qn + __popc(w & ((1u << lane) - 1u))) & 63] = tile * kWarpTile + lane * 4 + (k & 3);
-                qn += __popc(w);
-                __syncwarp();
-                if (qn >= 32) {
-                    process(ring[warp][(head + lane) & 63]);
-                    head = (head + 32) & 63; qn -= 32;
-                    __syncwarp();
-                }
-            }
-        }
+    // One block per list.  A unit of work is one 32-bit word of a listed tile (the cells j of the 32 lanes of the fp32 warp
+    // that listed it): unit u = 4 i + j of list entry i goes to warp u mod kFixWarps, each set bit to its own lane, so a list
+    // of up to two tiles is done in ONE pass of the step whatever it holds.  The step is long (fp64, every sub-step) and the
+    // marked cells are few: what counts is the number of passes a warp makes one after the other, not the idle lanes.
+    const unsigned v = blockIdx.x;
+    const unsigned cnt = __ldg(L.count + v);
+    const size_t base = (size_t)v * L.cap;
+    for (unsigned u = warp; u < 4u * cnt; u += kFixWarps) {
+        const unsigned w = __ldg((const unsigned *)(L.words + base + (u >> 2)) + (u & 3u));
+        if ((w >> lane) & 1u) process((long long)__ldg(L.tile + base + (u >> 2)) * kWarpTile + lane * 4 + (u & 3u));
     }
-    if (lane < qn) process(ring[warp][(head + lane) & 63]);
     __syncwarp();
 
     if constexpr (DIAG) {
@@ -131,8 +107,7 @@ cudaError_t launch_fix(const LaunchCtx &L, int mode, bool diag)
     const unsigned nlists = a.fix_warps;
     if (nlists == 0) return cudaSuccess;
     const FixLists lists = fix_layout(a.fixmap, nlists, (a.ncell + kWarpTile - 1) / kWarpTile);
-    // kFixSplit warps per list of the fp32 launch (<= 24 x SMs lists), within the diagnostics workspace's 32 blocks per SM
-    const int grid = (int)((nlists * kFixSplit + kFixWarps - 1) / kFixWarps);
+    const int grid = (int)nlists;                                    // <= 24 lists per SM, within the diagnostics workspace's 32 blocks per SM
     CellPtrs C{a.rho, a.bsq, a.the_in, a.thi_in, a.r, a.vol, a.the_out, a.thi_out, a.ncell, a.flags};
 #define COOL_FIX_LAUNCH(M, D) cool_fix_kernel<M, D><<<grid, kFixThreads, 0, L.st>>>(L.t->dev, L.t->cst, *L.S, C, lists, nlists, a.partials, a.ticket, a.d_diag)
     if (mode == 3) { if (diag) COOL_FIX_LAUNCH(3, true); else COOL_FIX_LAUNCH(3, false); }

@@ -68,7 +68,8 @@ struct DevTable {
     // the result by more than 1.5e-6, above fix_rmax the 30 % limiter decides whatever the rate.
     int nband;                     // 0: none, 1: band_lo < Theta_e < band_hi
     float band_lo, band_hi;
-    float band_step;               // steepest step of the bands [log2 units per node]
+    float band_step;               // steepest step of the band [log2 units per node]
+    int band_k0, band_k1;          // first and last steep Theta_e interval (0 .. n-2); the whole axis when another axis is steep
 };
 constexpr double kSteepLog2 = 6.0;        // |Delta T'| per Theta_e node above which an interval is steep (precision budget)
 constexpr double kBandMargin = 1.0 / 128; // nodes; far above the distance between the fp32 and the fp64 trajectory of a cell (<= 2e-4 nodes)

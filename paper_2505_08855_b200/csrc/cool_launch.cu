@@ -84,11 +84,14 @@ static F32Const make_f32_const(const cool_table *t, const LaunchArgs &a)
         const DevTable &D0 = t->dev;
         const double dt_nodes = 1e-5 * 1.4426950408889634 / (double)D0.ax[CAX_THE].d2f + 1e-5;
         const double sens = 0.6931471805599453 * (double)D0.band_step * dt_nodes;
-        const bool on = a.fixmap != nullptr && D0.nband != 0;
+        const bool on = D0.nband != 0 && (a.fixmap != nullptr || (D0.mode == 3 && a.nsub == 1));
         auto bits = [](double x) { const float f = (float)x; unsigned u; memcpy(&u, &f, 4); return u; };
         const float hi = std::min(D0.band_hi, 3.0e38f);               // keep the width a finite-float difference
         const unsigned lo_b = bits(D0.band_lo), rmin_b = bits(1.5e-6 / sens), rmax_b = bits(a.f_limit * (1.0 + 2.0 * sens) + 1e-6);
         S.band_lo_bits = lo_b; S.band_w = on ? bits(hi) - lo_b : 0u;
+        // the same band as Theta_e intervals (node-index words of Loc32::tf: 0x4B400000 + i), one neighbour interval each side
+        const int k0 = std::max(D0.band_k0 - 1, 0), k1 = std::min(D0.band_k1 + 1, D0.ax[CAX_THE].n - 2);
+        S.kb_lo = (int)(0x4B400000u + (unsigned)k0); S.kb_n = on ? (unsigned)(k1 - k0 + 1) : 0u;
         S.rmin_bits = rmin_b; S.r_w = (on && rmax_b > rmin_b) ? rmax_b - rmin_b : 0u;
     }
     S.lum_shell = a.lum_shell ? a.shell_rep : nullptr;
@@ -126,7 +129,10 @@ bool variant_supported(const cool_table *t, cool_variant v, cool_dtype, std::str
 // fp64 cells or the analytic variant (already fp64), not the implicit scheme (a root solve is insensitive to the coordinate).
 bool uses_fixmap(const cool_table *t, cool_variant v, cool_dtype dt, const LaunchArgs &a)
 {
-    return t->dev.nband != 0 && dt == COOL_F32 && a.scheme == COOL_SCHEME_EXPLICIT && (v == COOL_V_GLOBAL || v == COOL_V_SMEM || v == COOL_V_TEX_POINT);
+    // (a single update of a 3-D table needs no second kernel: its cells are exact inputs, and the step re-evaluates the rate of
+    // a band cell in place, precise_rate3 of cool_f32.cuh)
+    return t->dev.nband != 0 && dt == COOL_F32 && a.scheme == COOL_SCHEME_EXPLICIT && (v == COOL_V_GLOBAL || v == COOL_V_SMEM || v == COOL_V_TEX_POINT) &&
+           (t->dev.mode == 4 || a.nsub > 1);
 }
 
 cool_status launch_step(const cool_table *t, cool_variant v, cool_dtype dt, const LaunchArgs &a, cudaStream_t st, int *nlaunch)
