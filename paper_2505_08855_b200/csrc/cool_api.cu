@@ -220,6 +220,7 @@ static cool_status check_args(const cool_table *t, const cool_cells *c, const co
     if (!t || !c || !p) { set_error("NULL table, cells or params"); return COOL_EINVAL; }
     if (c->ncell < 0) { set_error("ncell < 0"); return COOL_EINVAL; }
     if (c->dtype != COOL_F32 && c->dtype != COOL_F64) { set_error("unknown dtype"); return COOL_EINVAL; }
+    if (c->ncell >= (1ll << 32)) { set_error("ncell must be below 2^32"); return COOL_EINVAL; }
     if (c->ncell > 0 && (!c->rho || !c->bsq || !c->theta_e_in || !c->theta_i_in || !c->theta_e_out || !c->theta_i_out)) {
         set_error("NULL cell array"); return COOL_EINVAL;
     }

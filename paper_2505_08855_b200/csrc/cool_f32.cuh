@@ -545,12 +545,13 @@ __device__ __forceinline__ void step_cells_f32(const Ctx32 &X, const Fetch &F, c
                     y0 = v.x; y1 = v.y; y2 = v.z; yc = v.w;
                 } else {
                     if (loc_bits(le) != P[j].ke || loc_bits(li) != P[j].ki) {
-                        build_patch(F, lr[j], lb[j], le, li, P[j]);
-                        // Precise pass (F32Const::band_*): a cell whose Theta_e interval is the steep one or a neighbour of it
-                        // keeps its patch invalid, so it comes back here every sub-step, and only here is it tested — the
-                        // sub-step loop itself carries no test.  The radiated fraction is evaluated once more on this rare path.
+                        // Precise pass (F32Const::band_*): the patch of a cell whose Theta_e interval is the steep one or a
+                        // neighbour of it carries the sign bit in its interval word, so the cell comes back here every sub-step
+                        // (rebuilding only when it really changed table cell), and only here is it tested — the sub-step loop
+                        // itself carries no test.  The radiated fraction is evaluated once more on this rare path.
+                        if (loc_bits(le) != (P[j].ke & 0x7fffffff) || loc_bits(li) != P[j].ki) build_patch(F, lr[j], lb[j], le, li, P[j]);
                         if ((unsigned)(loc_bits(le) - S.kb_lo) < S.kb_n) {
-                            P[j].ke = -1;
+                            P[j].ke = loc_bits(le) | (int)0x80000000u;
                             if ((__float_as_uint(the[j]) - S.band_lo_bits) < S.band_w) {
                                 const float z0 = patch_eval(P[j], 0, le.w, li.w), z1 = patch_eval(P[j], 1, le.w, li.w), z2 = patch_eval(P[j], 2, le.w, li.w);
                                 const float qbr = ex2_approx(fminf(z0 + kk, 100.f)), qsy = ex2_approx(fminf((z1 + kk) + z2, 100.f));
@@ -581,7 +582,7 @@ __device__ __forceinline__ void step_cells_f32(const Ctx32 &X, const Fetch &F, c
                 if constexpr (DIAG) {
                     const float inv = rcp_approx(fmaxf(rthin, 1e-37f));
                     const float rs0 = ex2_approx(fminf(esy, 100.f));                               // Q_syn alone
-                    fr[j][0] = rbr * inv; fr[j][1] = rs0 * inv; fr[j][2] = (rsy - rs0) * inv;
+                    fr[j][0] = rbr * inv; fr[j][1] = rs0 * inv; fr[j][2] = (rsy - rs0) * inv;      // shares of Q_thin (reading C-21)
                 }
             }
             if (use_floor) {
@@ -689,16 +690,17 @@ __device__ __forceinline__ void step_cells_f32(const Ctx32 &X, const Fetch &F, c
             for (int j = 0; j < NV; ++j)
                 if (!bad[j]) flagword |= ((limited[j] ? 1u : 0u) | (floored[j] ? 2u : 0u) | (clamped[j] ? 4u : 0u)) << (8 * j);
         }
-        acc.lum[0] += (double)part[0];
-        if constexpr (MODE == 4) {
-#pragma unroll
-            for (int k = 1; k < 4; ++k) acc.lum[k] += (double)part[k];
-        }
         if constexpr (NV == 1) {
-            // one cell of the tile (4-D kernel): the caller gathers the tile's terms and flushes them once
+            // one cell of the tile (4-D kernel): the caller gathers the tile's terms, adds them to the fp64 sums and flushes
+            // them once per tile (four cells summed in fp32 first, as the 3-D kernel does: the fp64 pipe is narrow)
 #pragma unroll
             for (int k = 0; k < 4; ++k) tile_part[k] = part[k];
         } else {
+            acc.lum[0] += (double)part[0];
+            if constexpr (MODE == 4) {
+#pragma unroll
+                for (int k = 1; k < 4; ++k) acc.lum[k] += (double)part[k];
+            }
             if (S.lum_shell) shell_flush<MODE>(S, part, wtile);
         }
     }
@@ -834,6 +836,8 @@ cool_f32_kernel(const DevTable T, const F32Const S, const CellPtrs C, double *pa
             if constexpr (DIAG) {
                 tp[0] = (rho.x + rho.y) + (rho.z + rho.w); tp[1] = (bsq.x + bsq.y) + (bsq.z + bsq.w);
                 tp[2] = (vv.x + vv.y) + (vv.z + vv.w); tp[3] = (rr.x + rr.y) + (rr.z + rr.w);
+#pragma unroll
+                for (int k = 0; k < 4; ++k) acc.lum[k] += (double)tp[k];
             }
         } else {
             // Precise pass: a single update can only put a cell there if its INPUT Theta_e lies in the steep band, so one

@@ -15,13 +15,14 @@
 //
 // Work distribution.  Every warp of the fp32 launch has listed its tiles with marked cells (tile index + four 32-bit words,
 // cool_internal.h fix_layout); tiles go round-robin over the fp32 warps, so a contiguous block of marked cells (a shell of
-// a disc) is already spread over all lists.  One block here takes one list, one warp one word at a time, one lane one cell.
+// a disc) is already spread over all lists.  One small block here takes one list and compacts its cells into a queue (cool_fix_kernel).
 // The processing order is fixed by the lists, and the sums go warp -> block -> fixed-order last block: reproducible bit for bit.
 #include "cool_f32.cuh"
 
 namespace cool {
 
-constexpr int kFixThreads = 256, kFixWarps = kFixThreads / 32;     // one block per list of the fp32 launch, one warp per word in turn
+constexpr int kFixThreads = 64, kFixWarps = kFixThreads / 32;      // one small block per list of the fp32 launch: many blocks per SM
+constexpr int kFixQueue = 1024;                                    // cells compacted per round (8 listed tiles)
 
 template <int MODE, bool DIAG>
 __global__ void __launch_bounds__(kFixThreads)
@@ -46,18 +47,32 @@ cool_fix_kernel(const DevTable T, const DevConst K, const StepConst S, const Cel
         }
     };
 
-    // One block per list.  A unit of work is one 32-bit word of a listed tile (the cells j of the 32 lanes of the fp32 warp
-    // that listed it): unit u = 4 i + j of list entry i goes to warp u mod kFixWarps, each set bit to its own lane, so a list
-    // of up to two tiles is done in ONE pass of the step whatever it holds.  The step is long (fp64, every sub-step) and the
-    // marked cells are few: what counts is the number of passes a warp makes one after the other, not the idle lanes.
+    // One block per list.  The set bits of up to 8 listed tiles (32 words) are compacted, in list order, into a queue of cell
+    // indices in shared memory (one word per lane of warp 0, an exclusive scan of the popcounts), and the block's warps take
+    // the queue 32 cells at a time.  The step is long (fp64, every sub-step) and the marked cells are few, so what counts is
+    // the number of passes a warp makes one after the other and how many blocks fit an SM: full warps, small blocks.
+    __shared__ unsigned queue[kFixQueue];
+    __shared__ unsigned s_total;
     const unsigned v = blockIdx.x;
     const unsigned cnt = __ldg(L.count + v);
     const size_t base = (size_t)v * L.cap;
-    for (unsigned u = warp; u < 4u * cnt; u += kFixWarps) {
-        const unsigned w = __ldg((const unsigned *)(L.words + base + (u >> 2)) + (u & 3u));
-        if ((w >> lane) & 1u) process((long long)__ldg(L.tile + base + (u >> 2)) * kWarpTile + lane * 4 + (u & 3u));
+    for (unsigned u0 = 0; u0 < 4u * cnt; u0 += 32u) {
+        if (warp == 0) {
+            const unsigned u = u0 + lane;
+            unsigned w = 0u, tile = 0u;
+            if (u < 4u * cnt) { w = __ldg((const unsigned *)(L.words + base + (u >> 2)) + (u & 3u)); tile = __ldg(L.tile + base + (u >> 2)); }
+            unsigned pre = __popc(w);                          // inclusive scan over the lanes
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) { const unsigned t = __shfl_up_sync(0xffffffffu, pre, o); if (lane >= o) pre += t; }
+            unsigned pos = pre - __popc(w);
+            while (w) { const int b = __ffs(w) - 1; w &= w - 1u; queue[pos++] = tile * (unsigned)kWarpTile + (unsigned)b * 4u + (u & 3u); }
+            if (lane == 31) s_total = pre;
+        }
+        __syncthreads();
+        const unsigned total = s_total;
+        for (unsigned q = threadIdx.x; q < total; q += kFixThreads) process((long long)queue[q]);
+        __syncthreads();
     }
-    __syncwarp();
 
     if constexpr (DIAG) {
         // warp -> block -> per-block partials -> fixed-order sum by the last block, ADDED to the diagnostics of the fp32 kernel
