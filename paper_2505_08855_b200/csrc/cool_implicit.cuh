@@ -281,10 +281,71 @@ __device__ __forceinline__ float imp32_rate(const F32Const &S, const Imp32 &c, f
     }
 }
 
+// ---- accurate rate inside the bracketing interval -------------------------------------------------------------------------
+// In the strongly cooled limit theta' ~ R/rate carries the full relative error of rate = 2^y, and in fp32 y (|y| up to ~40)
+// is good to 2-4e-6 only: the roundings of the node contraction and of the exponent sum (measured: 4e-6 per sub-step, adding
+// over sub-steps).  The fp32 search over the nodes only has to find the bracketing Theta_e interval; inside it the two node
+// values are contracted once more in fp64 and the exponent y = a + w (b - a) + log2 h + clamp terms is summed in fp64; 2^y
+// then takes the integer part exactly and the fraction (|f| <= 1/2) from MUFU.EX2 (2e-7).  Everything else stays fp32 (the
+// interval weight w is harmless: a weight error moves rate and theta together and cancels to first order in the root).
+__device__ __forceinline__ float imp_exp2_d(double y)
+{
+    y = fmin(fmax(y, -120.0), 120.0);
+    const double yi = rint(y);
+    return __int_as_float(__float_as_int(ex2_approx((float)(y - yi))) + ((int)yi << 23));      // 2^f in [0.70, 1.42] scaled by 2^yi (|yi| <= 120)
+}
+__device__ __forceinline__ double imp_dlerp(float w, float a, float b) { return fma((double)w, (double)b - (double)a, (double)a); }
+__device__ __forceinline__ double imp_dlerp(float w, double a, double b) { return fma((double)w, b - a, a); }
+
+template <int MODE, class Fetch>
+__device__ __forceinline__ void imp_node_d(const Fetch &F, const Loc32 &r, const Loc32 &b, const Loc32 &ii, int ir, int ib, int iii, int i, double (&y)[3])
+{
+    if constexpr (MODE == 3) {
+        y[0] = imp_dlerp(r.w, imp_dlerp(b.w, F.at1(ir, i, ib), F.at1(ir, i, ib + 1)), imp_dlerp(b.w, F.at1(ir + 1, i, ib), F.at1(ir + 1, i, ib + 1)));
+        y[1] = y[2] = 0.0;
+    } else {
+        double v[2][2][3];
+#pragma unroll
+        for (int cr = 0; cr < 2; ++cr)
+#pragma unroll
+            for (int ci = 0; ci < 2; ++ci) {
+                const float4 t0 = F.at4(ir + cr, i, iii + ci, ib), t1 = F.at4(ir + cr, i, iii + ci, ib + 1);
+                v[cr][ci][0] = imp_dlerp(b.w, t0.x, t1.x); v[cr][ci][1] = imp_dlerp(b.w, t0.y, t1.y); v[cr][ci][2] = imp_dlerp(b.w, t0.z, t1.z);
+            }
+#pragma unroll
+        for (int k = 0; k < 3; ++k) y[k] = imp_dlerp(r.w, imp_dlerp(ii.w, v[0][0][k], v[0][1][k]), imp_dlerp(ii.w, v[1][0][k], v[1][1][k]));
+    }
+}
+
+// imp32_rate with the channel exponents y (+ kd = log2 h + rho clamp correction) given in fp64
+template <int MODE>
+__device__ __forceinline__ float imp32_rate_d(const F32Const &S, const Imp32 &c, float thc, const double (&y)[3], double kd, float *frac)
+{
+    if constexpr (MODE == 3) {
+        return imp_exp2_d(y[0] + kd);
+    } else {
+        const float rbr = imp_exp2_d(fmin(y[0] + kd, 100.0));
+        const double esy = y[1] + kd;
+        const float rsy = imp_exp2_d(fmin(esy + y[2], 100.0));                                // eta * Q_syn
+        const float rthin = rbr + rsy;                                                        // eq 10
+        const float num = fmaf(S.ae, thc, S.ai * c.thi0), den = fmaf(S.be, thc, fmaf(S.bi, c.thi0, 1.f));
+        const float rcs = c.rho * (num * rsqrt_approx(num * den));                            // rho c_s   (eqs 13-14)
+        const float th3 = fmaxf(thc * thc * thc, 1e-30f);
+        const float tau_abs = rthin * (S.inv_kB * rcs) * rcp_approx(th3);                     // eq 12
+        const float tau_sca = S.ksca * rcs;
+        if (frac) {
+            const float inv = rcp_approx(fmaxf(rthin, 1e-37f));
+            const float rs0 = imp_exp2_d(fmin(esy, 100.0));
+            frac[0] = rbr * inv; frac[1] = rs0 * inv; frac[2] = (rsy - rs0) * inv;
+        }
+        return rthin * rcp_approx(fmaf(tau_abs, fmaf(1.5f, tau_abs + tau_sca, 1.7320508f), 1.f));   // eq 11
+    }
+}
+
 template <int MODE, class Fetch>
 __device__ void implicit_cell_f32(const DevTable &T, const StepConst &S, const F32Const &S32, const Fetch &F,
                                   float rho, float bsq, float &the, float &thi, float r, float vol, DiagAcc &acc, long long cell,
-                                  unsigned char *flags)
+                                  unsigned char *flags, double k0d)                 // k0d = log2 h in fp64
 {
     if (flags) flags[cell] = 0;
     const float chk = (bsq + the) + (thi + rho);
@@ -319,6 +380,7 @@ __device__ void implicit_cell_f32(const DevTable &T, const StepConst &S, const F
         Imp32 c;
         c.rho = rho; c.thi0 = thi; c.q = a / (1.f + a * g); c.R = fmaf(c.q, thi, the); c.opq = 1.f + c.q;
         c.kc = lr.d * T.ax[CAX_RHO].d2f; c.hf = ex2_approx(S32.k0);
+        const double kd = (double)lr.d * (double)T.ax[CAX_RHO].d2f + k0d;
         if (!(c.R > 0.f)) continue;
         float theta, rate = 0.f, frac[3] = {0.f, 0.f, 0.f};
         if (flo) {
@@ -350,16 +412,22 @@ __device__ void implicit_cell_f32(const DevTable &T, const StepConst &S, const F
                 else if (ilo == n - 1) { ye[0] = ya[0]; ye[1] = ya[1]; ye[2] = ya[2]; }
                 else imp32_node<MODE>(F, lr, lb, li, ir, ib, iii, e, ye);
                 const float te = node_theta(e);
-                rate = imp32_rate<MODE>(S32, c, te, ye, frac);                 // cooling time held outside the range
+                double yed[3];
+                imp_node_d<MODE>(F, lr, lb, li, ir, ib, iii, e, yed);
+                rate = imp32_rate_d<MODE>(S32, c, te, yed, kd, frac);           // cooling time held outside the range
                 theta = c.R / (c.opq + rate);
                 clamped = true;
             } else {
                 if (!have_b) imp32_node<MODE>(F, lr, lb, li, ir, ib, iii, ilo + 1, yb);
                 const float dy[3] = {yb[0] - ya[0], yb[1] - ya[1], yb[2] - ya[2]};
+                double yad[3], ybd[3];                          // the bracketing nodes once more, contracted in fp64
+                imp_node_d<MODE>(F, lr, lb, li, ir, ib, iii, ilo, yad);
+                imp_node_d<MODE>(F, lr, lb, li, ir, ib, iii, ilo + 1, ybd);
+                const double dyd[3] = {ybd[0] - yad[0], ybd[1] - yad[1], ybd[2] - yad[2]};
                 auto Rate = [&](float th, float *fr) {
-                    const float w = fminf(fmaxf(coord32(ax, th, one_bits) - (float)ilo, 0.f), 1.f);
-                    const float y[3] = {fmaf(w, dy[0], ya[0]), fmaf(w, dy[1], ya[1]), fmaf(w, dy[2], ya[2])};
-                    return imp32_rate<MODE>(S32, c, th, y, fr);
+                    const double w = (double)fminf(fmaxf(coord32(ax, th, one_bits) - (float)ilo, 0.f), 1.f);
+                    const double y[3] = {fma(w, dyd[0], yad[0]), fma(w, dyd[1], yad[1]), fma(w, dyd[2], yad[2])};
+                    return imp32_rate_d<MODE>(S32, c, th, y, kd, fr);
                 };
                 float lo = node_theta(ilo), hi = fminf(node_theta(ilo + 1), c.R);
                 const float noise = 1.2e-7f * c.R;              // F is a difference of terms of size R: below ~ulp(R) its sign is
@@ -434,6 +502,7 @@ cool_implicit_f32_kernel(const DevTable T, const StepConst S, const F32Const S32
     const Fetch F(Tp, smem_imp32);
     if (Fetch::kSmem) __syncthreads();
     DiagAcc acc;
+    const double k0d = log2(S.h);
     const long long stride = (long long)gridDim.x * THREADS;
     long long c = (long long)blockIdx.x * THREADS + threadIdx.x;
     // the next cell's values are requested before the current cell is solved: the solve hides the HBM latency
@@ -449,7 +518,7 @@ cool_implicit_f32_kernel(const DevTable T, const StepConst S, const F32Const S32
         float the = n_the, thi = n_thi;
         const float rho = n_rho, bsq = n_bsq, rr = n_rr, vv = n_vv;
         if (c + stride < C.ncell) fetch(c + stride);
-        implicit_cell_f32<MODE, Fetch>(T, S, S32, F, rho, bsq, the, thi, rr, vv, acc, c, d_diag ? C.flags : nullptr);
+        implicit_cell_f32<MODE, Fetch>(T, S, S32, F, rho, bsq, the, thi, rr, vv, acc, c, d_diag ? C.flags : nullptr, k0d);
         __stcs((float *)C.the_out + c, the);
         __stcs((float *)C.thi_out + c, thi);
     }

@@ -188,4 +188,4 @@ def test_implicit_fullsize(oracle):
     _run_workload(oracle, "c5", [api.COOL_V_AUTO], implicit=True, gate=IMPLICIT_GATE)
 
 
-IMPLICIT_GATE = 5e-5
+IMPLICIT_GATE = 1e-5
