@@ -18,6 +18,7 @@ _SRC = os.path.join(_HERE, "cool_oracle.c")
 _LIB = os.path.join(_HERE, "libcool_oracle.so")
 
 AX_LOG_RHO, AX_LOG_THETA_E, AX_LOG_BSQ, AX_LOG_THETA_I = 0, 1, 2, 3
+AX_LOG_HTH, AX_LOG_B, AX_LOG_NE, AX_LOG_TE = 4, 5, 6, 7           # Part D: the paper's parameters in cgs units
 
 
 def build(force: bool = False) -> str:
@@ -47,7 +48,8 @@ class _Table(C.Structure):
     _fields_ = [("ndim", C.c_int), ("axis", C.c_int * 4), ("n", C.c_int * 4),
                 ("lo", C.c_double * 4), ("hi", C.c_double * 4), ("nproc", C.c_int),
                 ("data", C.POINTER(C.c_float) * 3), ("coul", C.POINTER(C.c_float)),
-                ("nc", C.c_int * 2), ("clo", C.c_double * 2), ("chi", C.c_double * 2)]
+                ("nc", C.c_int * 2), ("clo", C.c_double * 2), ("chi", C.c_double * 2),
+                ("cgs", C.c_int), ("coul3", C.POINTER(C.c_float)), ("nc3", C.c_int * 3), ("c3lo", C.c_double * 3), ("c3hi", C.c_double * 3)]
 
 
 class Table:
@@ -55,7 +57,9 @@ class Table:
     (row-major, last axis fastest, log10 values); ``coul`` an optional float32 (nc0, nc1)
     array of log10 C over (log Theta_i, log Theta_e)."""
 
-    def __init__(self, axis, n, lo, hi, data, coul=None, clo=None, chi=None):
+    def __init__(self, axis, n, lo, hi, data, coul=None, clo=None, chi=None, cgs=False, coul3=None, c3lo=None, c3hi=None):
+        """``cgs``: data[0] is the paper's table, log10 Q_total[erg cm^-3 s^-1] over (log H_th, log B, log n_e, log T_e[K]);
+        ``coul3``: optional float32 (n0, n1, n2) array of log10 [Q_cc/(T_i - T_e)] over (log n_e, log T_i[K], log T_e[K])."""
         self.axis = list(axis); self.n = list(n); self.lo = list(lo); self.hi = list(hi)
         self.ndim = len(self.n)
         self.data = [np.ascontiguousarray(d, dtype=np.float32).reshape(self.n) for d in data]
@@ -75,6 +79,13 @@ class Table:
             t.coul = self.coul.ctypes.data_as(C.POINTER(C.c_float))
             t.nc[0], t.nc[1] = self.coul.shape
             t.clo[0], t.clo[1] = self.clo; t.chi[0], t.chi[1] = self.chi
+        t.cgs = int(bool(cgs))
+        self.cgs = bool(cgs)
+        self.coul3 = None if coul3 is None else np.ascontiguousarray(coul3, dtype=np.float32)
+        if self.coul3 is not None:
+            t.coul3 = self.coul3.ctypes.data_as(C.POINTER(C.c_float))
+            for k in range(3):
+                t.nc3[k] = self.coul3.shape[k]; t.c3lo[k] = float(c3lo[k]); t.c3hi[k] = float(c3hi[k])
         self._c = t
 
 
@@ -113,6 +124,8 @@ def lib():
             "orc_fill_total3": (None, [UP, C.POINTER(i), C.POINTER(d), C.POINTER(d), p, i]),
             "orc_fill_coulomb2": (None, [UP, C.POINTER(i), C.POINTER(d), C.POINTER(d), p]),
             "orc_max_threads": (i, []),
+            "orc_fill_total4_cgs": (None, [C.POINTER(i), C.POINTER(d), C.POINTER(d), p, i]),
+            "orc_fill_coulomb3_cgs": (None, [UP, C.POINTER(i), C.POINTER(d), C.POINTER(d), p]),
             "orc_tau_sca_cell": (d, [UP, d, d]),
             "orc_radpress": (None, [UP, C.c_longlong, p, p, p, d, p, C.POINTER(C.c_longlong)]),
         }
@@ -195,6 +208,20 @@ def fill_coulomb2(un, nc, clo, chi):
     return out
 
 
+def fill_total4_cgs(n, lo, hi, nthreads=0):
+    """The paper's table (L124) from Part A: log10 Q_total[cgs] over (log H_th, log B, log n_e, log T_e[K])."""
+    out = np.empty(n, dtype=np.float32)
+    lib().orc_fill_total4_cgs((C.c_int * 4)(*n), (C.c_double * 4)(*lo), (C.c_double * 4)(*hi), out.ctypes.data, nthreads or max_threads())
+    return out
+
+
+def fill_coulomb3_cgs(un, n, lo, hi):
+    """The paper's Coulomb table (L147): log10 [Q_cc/(T_i - T_e)] over (log n_e, log T_i[K], log T_e[K])."""
+    out = np.empty(n, dtype=np.float32)
+    lib().orc_fill_coulomb3_cgs(C.byref(un), (C.c_int * 3)(*n), (C.c_double * 3)(*lo), (C.c_double * 3)(*hi), out.ctypes.data)
+    return out
+
+
 def max_threads():
     n = lib().orc_max_threads()
     try:
@@ -205,7 +232,7 @@ def max_threads():
 
 
 RATE_TABLE, RATE_ANALYTIC = 0, 1
-COULOMB_OFF, COULOMB_TABLE, COULOMB_ANALYTIC = 0, 1, 2
+COULOMB_OFF, COULOMB_TABLE, COULOMB_ANALYTIC, COULOMB_TABLE3 = 0, 1, 2, 3
 
 
 def step(table: Table, un: Units, rho, bsq, theta_e, theta_i, dt, nsub=1, f_limit=0.3,
@@ -217,9 +244,11 @@ def step(table: Table, un: Units, rho, bsq, theta_e, theta_i, dt, nsub=1, f_limi
     rho, bsq, the, thi, r, vol = map(f64, (rho, bsq, theta_e, theta_i, r, vol))
     n = rho.size
     if coulomb_mode is None:
-        coulomb_mode = COULOMB_TABLE if table.coul is not None else COULOMB_ANALYTIC
+        coulomb_mode = COULOMB_TABLE3 if table.coul3 is not None else (COULOMB_TABLE if table.coul is not None else COULOMB_ANALYTIC)
     if coulomb_mode == COULOMB_TABLE:
         assert table.coul is not None
+    if coulomb_mode == COULOMB_TABLE3:
+        assert table.coul3 is not None
     the_o = np.empty(n); thi_o = np.empty(n)
     lam0 = np.empty(n) if want_rates else None
     qcc0 = np.empty(n) if want_rates else None
@@ -249,6 +278,7 @@ def step_implicit(table: Table, un: Units, rho, bsq, theta_e, theta_i, dt, nsub=
     f64 = lambda a: None if a is None else np.ascontiguousarray(a, dtype=np.float64).ravel()
     rho, bsq, the, thi, r, vol = map(f64, (rho, bsq, theta_e, theta_i, r, vol))
     n = rho.size
+    assert not table.cgs, "the implicit scheme is not defined on the paper's cgs table here"
     if coulomb_mode is None:
         coulomb_mode = COULOMB_TABLE if table.coul is not None else COULOMB_ANALYTIC
     the_o = np.empty(n); thi_o = np.empty(n)

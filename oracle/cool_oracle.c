@@ -11,6 +11,9 @@
  *         L181, L185, L197; readings C-1..C-17 of SURVEY.md §8(c) / DESIGN.md)
  * Part B' the implicit scheme (L185 (ii), L369; reading C-18)
  * Part C  the radiation-pressure temperature correction (eq 29; reading C-20)
+ * Part D  the paper's own table (L122-L124): Q(H_th, B, n_e, T_e) in cgs units with H_th per cell from
+ *         eqs 13-14 and the cell's radius (L128-L136), Coulomb table Q_cc(n_e, T_i, T_e) (readings C-22, C-23);
+ *         it is Part B with four more axis kinds, so the same orc_step_cell runs it
  *
  * Pins (tests/test_oracle_*.py): closed-form brems scaling, incomplete-gamma closed
  * form of the synchrotron integral, scipy.special.kve for the Bessel functions,
@@ -346,7 +349,10 @@ double orc_combine_code(const orc_units *u, double rho, double th_e, double th_i
 /* ================================================================================
  * Part B  the step.
  * ============================================================================== */
-enum { ORC_AX_LOG_RHO = 0, ORC_AX_LOG_THETA_E = 1, ORC_AX_LOG_BSQ = 2, ORC_AX_LOG_THETA_I = 3 };
+enum { ORC_AX_LOG_RHO = 0, ORC_AX_LOG_THETA_E = 1, ORC_AX_LOG_BSQ = 2, ORC_AX_LOG_THETA_I = 3,
+       /* Part D, the paper's parameters in cgs units (L122-L124): */
+       ORC_AX_LOG_HTH = 4, ORC_AX_LOG_B = 5, ORC_AX_LOG_NE = 6, ORC_AX_LOG_TE = 7,
+       ORC_AX_LOG_TI = 8 /* Coulomb table only (L147) */ };
 
 typedef struct {
     int ndim;               /* 3 or 4 (any 1..4 works)                              */
@@ -358,6 +364,11 @@ typedef struct {
     const float *coul;      /* optional log10 C over (log Theta_i, log Theta_e)     */
     int nc[2];
     double clo[2], chi[2];
+    /* Part D: */
+    int cgs;                /* 1: data[0] holds log10 Q_total in erg cm^-3 s^-1 (the paper's table) */
+    const float *coul3;     /* optional log10 [Q_cc / (T_i - T_e)] in erg cm^-3 s^-1 K^-1 over (log n_e, log T_i[K], log T_e[K]), T_e fastest (L147, C-23) */
+    int nc3[3];
+    double c3lo[3], c3hi[3];
 } orc_table;
 
 /* B1: coordinate -> (i, w) with edge clamping (C-7).  Returns 1 if clamped. */
@@ -415,9 +426,16 @@ static void orc_step_cell(const orc_table *tab, const orc_units *un,
 
     for (int s = 0; s < nsub; ++s) {
         /* B1/B2: rate lookup */
-        double prim[4];
+        double prim[9];
         prim[ORC_AX_LOG_RHO] = rho; prim[ORC_AX_LOG_THETA_E] = the;
         prim[ORC_AX_LOG_BSQ] = bsq; prim[ORC_AX_LOG_THETA_I] = thi;
+        /* Part D: the paper's parameters of this cell, this sub-step (L181: "the values of H_th, B, n_e and T_e obtained
+         * from the simulation"); H_th = c_s/Omega_K with the cell's own radius (eqs 13-14; r <= 0: r_ref) */
+        prim[ORC_AX_LOG_HTH] = orc_hth_cm(un, the, thi, r > 0.0 ? r : un->r_ref_rg);
+        prim[ORC_AX_LOG_B] = orc_bfield_gauss(un, bsq > 0.0 ? bsq : 0.0);
+        prim[ORC_AX_LOG_NE] = orc_ne_cgs(un, rho);
+        prim[ORC_AX_LOG_TE] = the * ORC_ME * ORC_C * ORC_C / ORC_KB;
+        prim[ORC_AX_LOG_TI] = thi * ORC_ME * ORC_C * ORC_C / ORC_KB;
         double lam, frac[3] = {0, 0, 0};
         if (rate_mode == 0) {
             double x[4]; int cl = 0;
@@ -427,6 +445,7 @@ static void orc_step_cell(const orc_table *tab, const orc_units *un,
             }
             if (tab->nproc == 1) {
                 lam = pow(10.0, orc_interp(tab->ndim, tab->n, tab->lo, tab->hi, tab->data[0], x, &cl));
+                if (tab->cgs) lam *= orc_rate_conv(un);         /* the paper's table is in erg cm^-3 s^-1 */
             } else {
                 double q[3];
                 for (int p = 0; p < 3; ++p)
@@ -437,6 +456,7 @@ static void orc_step_cell(const orc_table *tab, const orc_units *un,
         } else {
             double out[6];
             double H = (tab->ndim == 4) ? orc_hth_cm(un, the, thi, un->r_ref_rg) : un->hth_cm;
+            if (tab->cgs) H = prim[ORC_AX_LOG_HTH];
             orc_cooling_cgs(H, orc_bfield_gauss(un, bsq), orc_ne_cgs(un, rho), the, out);
             lam = out[4] * orc_rate_conv(un);
             frac[0] = out[0] / out[3]; frac[1] = out[1] / out[3]; frac[2] = (out[2] - 1.0) * out[1] / out[3];
@@ -454,6 +474,11 @@ static void orc_step_cell(const orc_table *tab, const orc_units *un,
             qcc = orc_coulomb_pref_cgs(un) * orc_rate_conv(un) * rho * rho * (thi - the) * C;
         } else if (coulomb_mode == 2) {
             qcc = (thi == the) ? 0.0 : orc_coulomb_code(un, rho, the, thi);
+        } else if (coulomb_mode == 3) {     /* Part D: the paper's Q_cc(n_e, T_i, T_e) table (L147), stored per kelvin of T_i - T_e (C-23) */
+            double q3[3] = { prim[ORC_AX_LOG_NE], prim[ORC_AX_LOG_TI], prim[ORC_AX_LOG_TE] }, x3[3];
+            for (int k = 0; k < 3; ++k) x3[k] = (q3[k] > 0.0) ? log10(q3[k]) : -INFINITY;
+            double kq = pow(10.0, orc_interp(3, tab->nc3, tab->c3lo, tab->c3hi, tab->coul3, x3, NULL));
+            qcc = kq * (prim[ORC_AX_LOG_TI] - prim[ORC_AX_LOG_TE]) * orc_rate_conv(un);
         }
         if (s == 0) { if (lam0) *lam0 = lam; if (qcc0) *qcc0 = qcc; }
         /* B5: limited explicit update (L185; readings C-8, C-9) */
@@ -721,6 +746,38 @@ void orc_fill_coulomb2(const orc_units *un, const int *nc, const double *clo, co
             double the = pow(10.0, clo[1] + b * (chi[1] - clo[1]) / (nc[1] - 1));
             out[(size_t)a * nc[1] + b] = (float)log10(orc_coulomb_C(the, thi / un->ion_theta_mass_ratio));
         }
+}
+/* Part D fillers: the paper's table (L124), node by node from Part A.  n, lo, hi over (log10 H_th[cm], log10 B[G],
+ * log10 n_e[cm^-3], log10 T_e[K]), T_e fastest; values log10 Q_total[erg cm^-3 s^-1]. */
+void orc_fill_total4_cgs(const int *n, const double *lo, const double *hi, float *out, int nthreads)
+{
+    long long tot = (long long)n[0] * n[1] * n[2] * n[3];
+#pragma omp parallel for schedule(dynamic, 64) num_threads(nthreads > 0 ? nthreads : 1)
+    for (long long t = 0; t < tot; ++t) {
+        long long rem = t;
+        double x[4];
+        for (int k = 3; k >= 0; --k) { x[k] = lo[k] + (double)(rem % n[k]) * (hi[k] - lo[k]) / (n[k] - 1); rem /= n[k]; }
+        double o6[6];
+        orc_cooling_cgs(pow(10.0, x[0]), pow(10.0, x[1]), pow(10.0, x[2]), pow(10.0, x[3]) * ORC_KB / (ORC_ME * ORC_C * ORC_C), o6);
+        out[t] = (float)log10(o6[4]);
+    }
+}
+/* Coulomb table of L147 over (log10 n_e, log10 T_i[K], log10 T_e[K]), T_e fastest.  Eq 15 with rho/m_p = n_i = n_e (C-14)
+ * is Q_cc = (3/2)(m_e/m_p) n_e^2 lnLambda c k_B sigma_T (T_i - T_e) C(theta_e, theta_i); the table stores
+ * log10 [Q_cc/(T_i - T_e)], which is positive and smooth through T_i = T_e where Q_cc itself changes sign (C-23). */
+void orc_fill_coulomb3_cgs(const orc_units *un, const int *n, const double *lo, const double *hi, float *out)
+{
+    const double k2t = ORC_KB / (ORC_ME * ORC_C * ORC_C);
+    for (int a = 0; a < n[0]; ++a)
+        for (int b = 0; b < n[1]; ++b)
+            for (int c = 0; c < n[2]; ++c) {
+                double ne = pow(10.0, lo[0] + a * (hi[0] - lo[0]) / (n[0] - 1));
+                double ti = pow(10.0, lo[1] + b * (hi[1] - lo[1]) / (n[1] - 1));
+                double te = pow(10.0, lo[2] + c * (hi[2] - lo[2]) / (n[2] - 1));
+                double C = orc_coulomb_C(te * k2t, ti * k2t / un->ion_theta_mass_ratio);
+                double k = 1.5 * (ORC_ME / ORC_MP) * ne * ne * un->ln_lambda * ORC_C * ORC_KB * ORC_SIGT * C;
+                out[((size_t)a * n[1] + b) * n[2] + c] = (float)log10(k);
+            }
 }
 int orc_max_threads(void)
 {
