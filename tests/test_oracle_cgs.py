@@ -148,5 +148,5 @@ def test_cgs_step_conserves_and_limits(oracle):
     assert (o["theta_e"] > 0).all() and (u1 <= u0 * (1 + 1e-14)).all()
     assert o["diag"]["lum_total"] == pytest.approx(float(((u0 - u1) * vol).sum() / 5.0), rel=1e-10)
     assert 0 < o["diag"]["n_limited"] < n
-    far = oracle.step(tab, un, rho[:3] * 1e-9, bsq[:3], the[:3], thi[:3], 1e-3, r=r[:3], coulomb_mode=oracle.COULOMB_OFF)
+    far = oracle.step(tab, un, rho[:3] * 1e-20, bsq[:3], the[:3], thi[:3], 1e-3, r=r[:3], coulomb_mode=oracle.COULOMB_OFF)
     assert far["diag"]["n_clamped"] == 3                         # n_e below 1e2 cm^-3: clamped to the table edge
