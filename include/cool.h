@@ -38,7 +38,10 @@ extern "C" {
 
 typedef enum { COOL_OK = 0, COOL_EINVAL = 1, COOL_ENOMEM = 2, COOL_ECUDA = 3, COOL_EUNSUPPORTED = 4 } cool_status;
 typedef enum { COOL_F32 = 0, COOL_F64 = 1 } cool_dtype;
-typedef enum { COOL_AX_LOG_RHO = 0, COOL_AX_LOG_THETA_E = 1, COOL_AX_LOG_BSQ = 2, COOL_AX_LOG_THETA_I = 3 } cool_axis;
+typedef enum { COOL_AX_LOG_RHO = 0, COOL_AX_LOG_THETA_E = 1, COOL_AX_LOG_BSQ = 2, COOL_AX_LOG_THETA_I = 3,
+               /* the paper's own table parameters, cgs units: disk thermal scale height [cm], magnetic
+                * field strength [G], electron density [cm^-3], electron temperature [K] */
+               COOL_AX_LOG_HTH = 4, COOL_AX_LOG_B = 5, COOL_AX_LOG_NE = 6, COOL_AX_LOG_TE = 7 } cool_axis;
 
 /* Kernel variants (north_star (c)).  All give the same result within the fp tolerance except
  * COOL_V_TEX_HWFILTER, whose hardware filter uses 8-bit fixed-point weights (reported, not
@@ -81,6 +84,15 @@ typedef struct {
  *   ndim = 4, nproc = 3 : axes are a permutation of all four; host_data[0..2] =
  *                         log10 Q_brem_code, log10 Q_syn_code, log10 eta_compton; H_th from
  *                         eqs 13-14 at r_ref with the cell's Theta_e + Theta_i
+ *   ndim = 4, nproc = 1 : THE PAPER'S TABLE (L122-L124, L155-L159): axis[] = {LOG_HTH, LOG_B, LOG_NE, LOG_TE} in this
+ *                         order (T_e fastest, as the paper flattens it); host_data[0] = log10 Q_total[erg cm^-3 s^-1].  The
+ *                         step forms the four parameters of every cell itself (L181): H_th = c_s/Omega_K from eqs 13-14
+ *                         with the cell's own radius cool_cells.r (r_ref_rg when r is NULL), B = sqrt(4 pi bsq rho_scale c^2),
+ *                         n_e = rho rho_scale/m_p, T_e = Theta_e m_e c^2/k_B, and converts the tabulated rate to code units.
+ *                         Optional Coulomb table host_coulomb3 = log10 [Q_cc/(T_i - T_e)] over (log10 n_e, log10 T_i[K],
+ *                         log10 T_e[K]), T_e fastest (L147; per kelvin, so that it is smooth through T_i = T_e).  Variants:
+ *                         GLOBAL, TEX_POINT, TEX_HWFILTER (the paper's scheme: hardware bilinear on (H_th, B), manual
+ *                         interpolation on the flattened (n_e, T_e) axis), ANALYTIC; explicit scheme only.
  * nproc = 0 (no data) is allowed: only COOL_V_ANALYTIC can then be applied.
  * Arrays are row-major with axis[ndim-1] fastest, n[0]*...*n[ndim-1] floats each, node k of
  * axis a at log10-coordinate lo[a] + k (hi[a]-lo[a])/(n[a]-1); n[a] >= 2, hi[a] > lo[a].
@@ -97,6 +109,10 @@ typedef struct {
     int nc[2];
     double clo[2], chi[2];
     cool_units units;
+    /* the paper's Coulomb table (ndim = 4, nproc = 1 tables only; HOST pointer or NULL): nc3[0] x nc3[1] x nc3[2] floats */
+    const float *host_coulomb3;
+    int nc3[3];
+    double c3lo[3], c3hi[3];
 } cool_table_desc;
 
 /* One batch of cells, structure of arrays, ncell contiguous elements of `dtype` each.
@@ -153,7 +169,8 @@ typedef struct cool_table cool_table;      /* opaque */
 /* Host table builder (north_star (a)): tabulates eqs 1-12 (and eq 15's coefficient C when
  * out_coulomb != NULL) on the grid that `shape` describes (its host_data / host_coulomb
  * pointers are ignored).  out[p] must hold prod(n) floats for p < nproc; out_coulomb
- * nc[0]*nc[1] floats.  Runs on `nthreads` host threads (<= 0: all available).  Host only;
+ * nc[0]*nc[1] floats — for the paper's table (axes LOG_HTH, LOG_B, LOG_NE, LOG_TE) nc3[0]*nc3[1]*nc3[2] floats of
+ * log10 [Q_cc/(T_i - T_e)].  Runs on `nthreads` host threads (<= 0: all available).  Host only;
  * needs no GPU.  Errors: COOL_EINVAL for a malformed shape. */
 cool_status cool_table_build_host(const cool_table_desc *shape, float *const out[3], float *out_coulomb, int nthreads);
 

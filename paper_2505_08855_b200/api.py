@@ -20,6 +20,7 @@ LIB_PATH = os.path.join(_HERE, "libcool_b200.so")
 COOL_OK, COOL_EINVAL, COOL_ENOMEM, COOL_ECUDA, COOL_EUNSUPPORTED = range(5)
 COOL_F32, COOL_F64 = 0, 1
 COOL_AX_LOG_RHO, COOL_AX_LOG_THETA_E, COOL_AX_LOG_BSQ, COOL_AX_LOG_THETA_I = range(4)
+COOL_AX_LOG_HTH, COOL_AX_LOG_B, COOL_AX_LOG_NE, COOL_AX_LOG_TE = range(4, 8)          # the paper's table (cgs units)
 COOL_V_AUTO, COOL_V_TEX_POINT, COOL_V_TEX_HWFILTER, COOL_V_SMEM, COOL_V_GLOBAL, COOL_V_ANALYTIC = range(6)
 COOL_COULOMB_AUTO, COOL_COULOMB_OFF, COOL_COULOMB_TABLE, COOL_COULOMB_ANALYTIC = range(4)
 COOL_SCHEME_EXPLICIT, COOL_SCHEME_IMPLICIT = range(2)
@@ -44,7 +45,8 @@ class cool_table_desc(C.Structure):
                 ("lo", C.c_double * 4), ("hi", C.c_double * 4), ("nproc", C.c_int),
                 ("host_data", C.c_void_p * 3), ("host_coulomb", C.c_void_p),
                 ("nc", C.c_int * 2), ("clo", C.c_double * 2), ("chi", C.c_double * 2),
-                ("units", cool_units)]
+                ("units", cool_units),
+                ("host_coulomb3", C.c_void_p), ("nc3", C.c_int * 3), ("c3lo", C.c_double * 3), ("c3hi", C.c_double * 3)]
 
 
 class cool_cells(C.Structure):
@@ -135,7 +137,7 @@ def default_units(**kw) -> cool_units:
     return cool_units(**d)
 
 
-def make_desc(axis, n, lo, hi, nproc, units=None, nc=None, clo=None, chi=None) -> cool_table_desc:
+def make_desc(axis, n, lo, hi, nproc, units=None, nc=None, clo=None, chi=None, nc3=None, c3lo=None, c3hi=None) -> cool_table_desc:
     d = cool_table_desc()
     d.ndim = len(n)
     for k in range(d.ndim):
@@ -145,8 +147,16 @@ def make_desc(axis, n, lo, hi, nproc, units=None, nc=None, clo=None, chi=None) -
         d.nc[0], d.nc[1] = int(nc[0]), int(nc[1])
         d.clo[0], d.clo[1] = float(clo[0]), float(clo[1])
         d.chi[0], d.chi[1] = float(chi[0]), float(chi[1])
+    if nc3 is not None:
+        for k in range(3):
+            d.nc3[k] = int(nc3[k]); d.c3lo[k] = float(c3lo[k]); d.c3hi[k] = float(c3hi[k])
     d.units = units if units is not None else default_units()
     return d
+
+
+def is_cgs(desc: cool_table_desc) -> bool:
+    """The paper's table: axes (log H_th, log B, log n_e, log T_e)."""
+    return desc.ndim == 4 and desc.axis[0] == COOL_AX_LOG_HTH
 
 
 def cool_table_build_host(desc: cool_table_desc, want_coulomb: bool = False, nthreads: int = 0):
@@ -154,7 +164,10 @@ def cool_table_build_host(desc: cool_table_desc, want_coulomb: bool = False, nth
     shape = [desc.n[k] for k in range(desc.ndim)]
     data = [np.empty(shape, dtype=np.float32) for _ in range(desc.nproc)]
     outs = (C.c_void_p * 3)(*[d.ctypes.data for d in data] + [None] * (3 - len(data)))
-    coul = np.empty((desc.nc[0], desc.nc[1]), dtype=np.float32) if want_coulomb else None
+    if want_coulomb and is_cgs(desc):
+        coul = np.empty((desc.nc3[0], desc.nc3[1], desc.nc3[2]), dtype=np.float32)
+    else:
+        coul = np.empty((desc.nc[0], desc.nc[1]), dtype=np.float32) if want_coulomb else None
     _check(lib().cool_table_build_host(C.byref(desc), outs, None if coul is None else coul.ctypes.data, nthreads))
     return data, coul
 
@@ -189,18 +202,24 @@ def cool_table_create(desc: cool_table_desc, data, coulomb=None, device: int = 0
     for p in range(3):
         desc.host_data[p] = keep[p].ctypes.data if p < len(keep) else None
     ck = None
+    desc.host_coulomb = None
+    desc.host_coulomb3 = None
     if coulomb is not None:
         ck = np.ascontiguousarray(coulomb, dtype=np.float32)
-        if ck.shape != (desc.nc[0], desc.nc[1]):
-            raise ValueError("coulomb shape != desc.nc")
-        desc.host_coulomb = ck.ctypes.data
-    else:
-        desc.host_coulomb = None
+        if is_cgs(desc):
+            if ck.shape != (desc.nc3[0], desc.nc3[1], desc.nc3[2]):
+                raise ValueError("coulomb shape != desc.nc3")
+            desc.host_coulomb3 = ck.ctypes.data
+        else:
+            if ck.shape != (desc.nc[0], desc.nc[1]):
+                raise ValueError("coulomb shape != desc.nc")
+            desc.host_coulomb = ck.ctypes.data
     h = C.c_void_p()
     _check(lib().cool_table_create(C.byref(desc), device, C.byref(h)))
     for p in range(3):
         desc.host_data[p] = None
     desc.host_coulomb = None
+    desc.host_coulomb3 = None
     return CoolTable(h, desc)
 
 

@@ -135,6 +135,7 @@ static void free_table(cool_table *t)
     if (t->d_coul) cudaFree(t->d_coul);
     if (t->d_fcoul) cudaFree(t->d_fcoul);
     if (t->d_fcoulq) cudaFree(t->d_fcoulq);
+    if (t->d_coul3) cudaFree(t->d_coul3);
     if (t->d_q3) cudaFree(t->d_q3);
     if (t->d_o3) cudaFree(t->d_o3);
     for (auto &kv : t->diag_ws) { cudaFree(kv.second.partials); cudaFree(kv.second.ticket); if (kv.second.shell_rep) cudaFree(kv.second.shell_rep); if (kv.second.fixmap) cudaFree(kv.second.fixmap); }
@@ -238,15 +239,16 @@ static cool_status check_args(const cool_table *t, const cool_cells *c, const co
     if ((vv == COOL_V_TEX_POINT || vv == COOL_V_TEX_HWFILTER) && !t->dev.tex_pt) { set_error("variant unsupported: table too large for a 3-D texture"); return COOL_EUNSUPPORTED; }
     int cm;
     switch (p->coulomb) {
-        case COOL_COULOMB_AUTO: cm = t->dev.coul ? 1 : 2; break;
+        case COOL_COULOMB_AUTO: cm = (t->dev.coul || t->dev.coul3) ? 1 : 2; break;
         case COOL_COULOMB_OFF: cm = 0; break;
         case COOL_COULOMB_TABLE:
-            if (!t->dev.coul) { set_error("COOL_COULOMB_TABLE but the table has no Coulomb coefficient table"); return COOL_EINVAL; }
+            if (!t->dev.coul && !t->dev.coul3) { set_error("COOL_COULOMB_TABLE but the table has no Coulomb coefficient table"); return COOL_EINVAL; }
             cm = 1; break;
         case COOL_COULOMB_ANALYTIC: cm = 2; break;
         default: set_error("unknown coulomb mode"); return COOL_EINVAL;
     }
     if (p->scheme != COOL_SCHEME_EXPLICIT && p->scheme != COOL_SCHEME_IMPLICIT) { set_error("unknown scheme"); return COOL_EINVAL; }
+    if (p->scheme == COOL_SCHEME_IMPLICIT && desc_is_cgs(&t->desc)) { set_error("variant unsupported: the implicit scheme is not defined on the paper's cgs table"); return COOL_EUNSUPPORTED; }
     if (p->scheme == COOL_SCHEME_IMPLICIT && (vv == COOL_V_TEX_HWFILTER || vv == COOL_V_ANALYTIC)) {
         set_error("variant unsupported: the implicit scheme runs on the GLOBAL, SMEM and TEX_POINT lookups"); return COOL_EUNSUPPORTED;
     }
@@ -275,7 +277,7 @@ extern "C" cool_status cool_table_create(const cool_table_desc *desc, int device
     if (!out) { set_error("cool_table_create: out is NULL"); return COOL_EINVAL; }
     *out = nullptr;
     std::string why;
-    if (!desc_valid(desc, desc && desc->host_coulomb != nullptr, &why)) { set_error("cool_table_create: %s", why.c_str()); return COOL_EINVAL; }
+    if (!desc_valid(desc, desc && (desc->host_coulomb != nullptr || (desc_is_cgs(desc) && desc->host_coulomb3 != nullptr)), &why)) { set_error("cool_table_create: %s", why.c_str()); return COOL_EINVAL; }
     for (int p = 0; p < desc->nproc; ++p)
         if (!desc->host_data[p]) { set_error("cool_table_create: host_data[%d] is NULL", p); return COOL_EINVAL; }
     int ndev = 0;
@@ -309,6 +311,47 @@ extern "C" cool_status cool_table_create(const cool_table_desc *desc, int device
     DevTable &D = t->dev;
     auto fail = [&](cool_status s) { free_table(t); return s; };
     const int nd = desc->ndim;
+    if (desc_is_cgs(desc)) {
+        // ---- the paper's table (mode 5): kept in the caller's order [H_th][B][n_e][T_e]; the 3-D texture flattens (n_e, T_e)
+        // into z and puts (B, H_th) on x, y, which the hardware can filter (L155-L159)
+        D.mode = desc->nproc == 0 ? 0 : 5;
+        for (int k = 0; k < 4; ++k) D.ax[k] = make_axis(desc->n[k], desc->lo[k], desc->hi[k]);
+        const size_t nH = desc->n[0], nB = desc->n[1], nN = desc->n[2], nT = desc->n[3], total = nH * nB * nN * nT;
+        if (desc->nproc > 0) {
+            const size_t bytes = total * sizeof(float);
+            if (bytes > 0xffffffffull) { set_error("table too large"); return fail(COOL_EINVAL); }
+            for (size_t f = 0; f < total; ++f)
+                if (!std::isfinite(desc->host_data[0][f])) { set_error("cool_table_create: non-finite value in host_data[0]"); return fail(COOL_EINVAL); }
+            cudaError_t e = cudaMalloc(&t->d_lin, bytes);
+            if (e == cudaSuccess) e = cudaMemcpy(t->d_lin, desc->host_data[0], bytes, cudaMemcpyHostToDevice);
+            if (e != cudaSuccess) { set_error("table upload: %s", cudaGetErrorString(e)); return fail(e == cudaErrorMemoryAllocation ? COOL_ENOMEM : COOL_ECUDA); }
+            D.lin1 = t->d_lin; D.table_bytes = (unsigned)bytes;
+            if (nB <= 16384 && nH <= 16384 && nN * nT <= 16384) {
+                std::vector<float> tx;
+                try { tx.resize(total); } catch (...) { set_error("out of host memory"); return fail(COOL_ENOMEM); }
+                for (size_t ih = 0; ih < nH; ++ih)
+                    for (size_t ib = 0; ib < nB; ++ib) {
+                        const float *src = desc->host_data[0] + (ih * nB + ib) * nN * nT;
+                        for (size_t z = 0; z < nN * nT; ++z) tx[(z * nH + ih) * nB + ib] = src[z];
+                    }
+                e = make_textures(tx.data(), 1, nB, nH, nN * nT, &t->arr, &D.tex_pt, &D.tex_lin);
+                if (e != cudaSuccess) { set_error("texture setup: %s", cudaGetErrorString(e)); return fail(e == cudaErrorMemoryAllocation ? COOL_ENOMEM : COOL_ECUDA); }
+            }
+        }
+        if (desc->host_coulomb3) {
+            const size_t n3 = (size_t)desc->nc3[0] * desc->nc3[1] * desc->nc3[2];
+            for (size_t k = 0; k < n3; ++k)
+                if (!std::isfinite(desc->host_coulomb3[k])) { set_error("cool_table_create: non-finite value in host_coulomb3"); return fail(COOL_EINVAL); }
+            cudaError_t e = cudaMalloc(&t->d_coul3, n3 * sizeof(float));
+            if (e == cudaSuccess) e = cudaMemcpy(t->d_coul3, desc->host_coulomb3, n3 * sizeof(float), cudaMemcpyHostToDevice);
+            if (e != cudaSuccess) { set_error("Coulomb table upload: %s", cudaGetErrorString(e)); return fail(e == cudaErrorMemoryAllocation ? COOL_ENOMEM : COOL_ECUDA); }
+            D.coul3 = t->d_coul3;
+            for (int k = 0; k < 3; ++k) D.cax3[k] = make_axis(desc->nc3[k], desc->c3lo[k], desc->c3hi[k]);
+        }
+        t->desc.host_coulomb3 = nullptr;
+        *out = t;
+        return COOL_OK;
+    }
     D.mode = desc->nproc == 0 ? 0 : nd;
     int ncan[4] = {1, 1, 1, 1};
     for (int k = 0; k < nd; ++k) {

@@ -10,8 +10,31 @@
 
 namespace cool {
 
+bool desc_is_cgs(const cool_table_desc *d)
+{
+    return d && d->ndim == 4 && d->axis[0] == COOL_AX_LOG_HTH && d->axis[1] == COOL_AX_LOG_B && d->axis[2] == COOL_AX_LOG_NE && d->axis[3] == COOL_AX_LOG_TE;
+}
+
+static bool units_valid(const cool_units &u, std::string *why)
+{
+    if (!(u.rho_scale_cgs > 0 && u.mbh_msun > 0 && u.gamma_e > 1 && u.gamma_i > 1 && u.ln_lambda > 0 &&
+          u.ion_theta_mass_ratio > 0 && u.hth_cm > 0 && u.r_ref_rg > 0 && std::isfinite(u.spin))) {
+        *why = "units: need rho_scale, mbh, ln_lambda, ion_theta_mass_ratio, hth_cm, r_ref > 0 and gamma_e, gamma_i > 1";
+        return false;
+    }
+    return true;
+}
+
 static bool axes_valid(const cool_table_desc *d, std::string *why)
 {
+    if (d->ndim == 4 && d->axis[0] >= COOL_AX_LOG_HTH) {          // the paper's table (L122-L124)
+        if (!desc_is_cgs(d) || !(d->nproc == 1 || d->nproc == 0)) { *why = "the paper's table has axes {LOG_HTH, LOG_B, LOG_NE, LOG_TE} in this order and nproc = 1"; return false; }
+        for (int k = 0; k < 4; ++k) {
+            if (d->n[k] < 2 || d->n[k] > 4096) { *why = "n[k] must be in [2, 4096]"; return false; }
+            if (!(d->hi[k] > d->lo[k]) || !std::isfinite(d->lo[k]) || !std::isfinite(d->hi[k])) { *why = "need finite hi[k] > lo[k]"; return false; }
+        }
+        return units_valid(d->units, why);
+    }
     if (!((d->ndim == 3 && (d->nproc == 1 || d->nproc == 0)) || (d->ndim == 4 && (d->nproc == 3 || d->nproc == 0)))) {
         *why = "supported shapes: ndim=3 with nproc=1, ndim=4 with nproc=3 (nproc=0: analytic only)";
         return false;
@@ -25,18 +48,17 @@ static bool axes_valid(const cool_table_desc *d, std::string *why)
         if (d->n[k] < 2 || d->n[k] > 4096) { *why = "n[k] must be in [2, 4096]"; return false; }
         if (!(d->hi[k] > d->lo[k]) || !std::isfinite(d->lo[k]) || !std::isfinite(d->hi[k])) { *why = "need finite hi[k] > lo[k]"; return false; }
     }
-    const cool_units &u = d->units;
-    if (!(u.rho_scale_cgs > 0 && u.mbh_msun > 0 && u.gamma_e > 1 && u.gamma_i > 1 && u.ln_lambda > 0 &&
-          u.ion_theta_mass_ratio > 0 && u.hth_cm > 0 && u.r_ref_rg > 0 && std::isfinite(u.spin))) {
-        *why = "units: need rho_scale, mbh, ln_lambda, ion_theta_mass_ratio, hth_cm, r_ref > 0 and gamma_e, gamma_i > 1";
-        return false;
-    }
-    return true;
+    return units_valid(d->units, why);
 }
 bool desc_valid(const cool_table_desc *d, bool need_coulomb_shape, std::string *why)
 {
     if (!d) { *why = "NULL descriptor"; return false; }
     if (!axes_valid(d, why)) return false;
+    if (need_coulomb_shape && desc_is_cgs(d)) {
+        for (int k = 0; k < 3; ++k)
+            if (d->nc3[k] < 2 || d->nc3[k] > 4096 || !(d->c3hi[k] > d->c3lo[k])) { *why = "Coulomb table: nc3[k] in [2,4096], c3hi[k] > c3lo[k]"; return false; }
+        return true;
+    }
     if (need_coulomb_shape) {
         for (int k = 0; k < 2; ++k)
             if (d->nc[k] < 2 || d->nc[k] > 4096 || !(d->chi[k] > d->clo[k])) { *why = "Coulomb table: nc[k] in [2,4096], chi[k] > clo[k]"; return false; }
@@ -91,6 +113,33 @@ extern "C" cool_status cool_table_build_host(const cool_table_desc *shape, float
     long long total = 1;
     for (int k = 0; k < nd; ++k) total *= shape->n[k];
 
+    if (desc_is_cgs(shape)) {
+        // the paper's table: log10 Q_total[erg cm^-3 s^-1] at (H_th[cm], B[G], n_e[cm^-3], T_e[K]) nodes, T_e fastest (L124, L157)
+        if (np > 0) {
+            parallel_for(total, nthreads, [&](long long flat) {
+                double x[4];
+                long long rem = flat;
+                for (int k = 3; k >= 0; --k) {
+                    x[k] = pow(10.0, shape->lo[k] + (double)(rem % shape->n[k]) * (shape->hi[k] - shape->lo[k]) / (shape->n[k] - 1));
+                    rem /= shape->n[k];
+                }
+                out[0][flat] = (float)log10(coolphys::cooling_cgs(x[0], x[1], x[2], x[3] / coolphys::kTHETA_TO_K).total);
+            });
+        }
+        if (out_coulomb) {
+            // Q_cc(n_e, T_i, T_e) of L147 per kelvin of T_i - T_e: (3/2)(m_e/m_p) n_e^2 lnLambda c k_B sigma_T C(theta_e, theta_i)
+            const int n0 = shape->nc3[0], n1 = shape->nc3[1], n2 = shape->nc3[2];
+            parallel_for((long long)n0 * n1 * n2, nthreads, [&](long long flat) {
+                const int c = (int)(flat % n2), b = (int)((flat / n2) % n1), a = (int)(flat / ((long long)n1 * n2));
+                const double ne = pow(10.0, shape->c3lo[0] + a * (shape->c3hi[0] - shape->c3lo[0]) / (n0 - 1));
+                const double ti = pow(10.0, shape->c3lo[1] + b * (shape->c3hi[1] - shape->c3lo[1]) / (n1 - 1));
+                const double te = pow(10.0, shape->c3lo[2] + c * (shape->c3hi[2] - shape->c3lo[2]) / (n2 - 1));
+                const double C = coolphys::coulomb_C(te / coolphys::kTHETA_TO_K, ti / coolphys::kTHETA_TO_K / un.ion_theta_mass_ratio);
+                out_coulomb[flat] = (float)log10(1.5 * coolphys::kMR * ne * ne * un.ln_lambda * coolphys::kC * coolphys::kKB * coolphys::kSIGT * C);
+            });
+        }
+        return COOL_OK;
+    }
     if (np > 0) {
         parallel_for(total, nthreads, [&](long long flat) {
             double prim[4] = {0, 0, 0, 0};           // indexed by cool_axis: rho, theta_e, bsq, theta_i

@@ -66,6 +66,11 @@ struct DevTable {
     // sub-step in which it radiates a fraction r of its electron energy with fix_rmin < r < fix_rmax (F32Const) is left to
     // the precise pass (cool_fix.cu: the fp64 step on the canonical log10 tables): below fix_rmin the steep rate cannot move
     // the result by more than 1.5e-6, above fix_rmax the 30 % limiter decides whatever the rate.
+    // mode 5, the paper's table (cool_cgs.cu): lin1 = [H][B][n_e][T_e] float (T_e fastest), ax[0..3] = those axes in this
+    // order; tex_pt / tex_lin: 3-D array x = B, y = H_th, z = i_ne * n_Te + i_Te (the paper's flattening, L155-L159);
+    // coul3 = log10 [Q_cc/(T_i - T_e)] over [n_e][T_i][T_e], axes cax3[0..2]
+    const float *coul3;
+    AxisCoef cax3[3];
     int nband;                     // 0: none, 1: band_lo < Theta_e < band_hi
     float band_lo, band_hi;
     float band_step;               // steepest step of the band [log2 units per node]
@@ -138,7 +143,7 @@ struct cool_table {
     cool::DevConst cst{};
     float *d_lin = nullptr;        // owns lin1 / lin4
     float *d_f32 = nullptr;        // owns f1 / f4
-    float *d_coul = nullptr, *d_fcoul = nullptr, *d_fcoulq = nullptr, *d_q3 = nullptr, *d_o3 = nullptr;
+    float *d_coul = nullptr, *d_fcoul = nullptr, *d_fcoulq = nullptr, *d_q3 = nullptr, *d_o3 = nullptr, *d_coul3 = nullptr;
     cudaArray_t arr = nullptr, arr32 = nullptr;
     int sm_count = 148;
     int max_smem_optin = 0;
@@ -160,6 +165,7 @@ void set_error(const char *fmt, ...);
 void note_launches(int n);           // what cool_last_launch_count() reports for this thread
 void note_kernel(const char *fmt, ...);   // what cool_last_kernel_name() reports for this thread
 bool desc_valid(const cool_table_desc *d, bool need_coulomb_shape, std::string *why);
+bool desc_is_cgs(const cool_table_desc *d);          // the paper's table: axes (log H_th, log B, log n_e, log T_e)
 coolphys::Units to_units(const cool_units &u);
 cool_status launch_step(const cool_table *t, cool_variant v, cool_dtype dt, const LaunchArgs &a, cudaStream_t s, int *nlaunch);
 bool variant_supported(const cool_table *t, cool_variant v, cool_dtype dt, std::string *why);

@@ -25,6 +25,7 @@ struct StepConst {
     double hfloor2, spin;          // floor: (pi/2) h_floor^2 (Omega_K r)^2                     (eq 19)
     double lum_k;                  // lum = sum(dTheta_rad rho vol) * lum_k,  lum_k = mr/(ge1 dt)
     int nsub, coulomb, has_r, has_vol, aligned;
+    int cgs; double omk_ref_inv;   // the paper's table: H_th from the cell's radius; omk_ref_inv = r_ref^1.5 + a
     // radial profile (eq 25): shell = (cell_offset + cell)/shell_cells; sums go to replica (block index & shell_rmask) of lum_shell
     // (this launch's workspace, local shell index); shell_reduce_kernel then adds the replicas into the caller's array
     double *lum_shell; long long shell_cells, cell_offset, shell0; unsigned shell_nloc4, shell_rmask;
@@ -230,22 +231,16 @@ __device__ __forceinline__ double coulomb_C_table64(const DevTable &T, double th
     return exp10(y);
 }
 
-// shared by the fp64 table path and the analytic kernel: floor, Coulomb, limited update (B3-B6)
-__device__ __forceinline__ void update64(const DevTable &T, const DevConst &K, const StepConst &S, double rho, double r,
-                                         double lam, const double frac[3], double &the, double &thi, double de_sum[4],
-                                         int &limited, int &floored)
+// shared by the fp64 table path, the analytic kernel and the paper's-table kernel: floor, limited update (B3-B6);
+// dcoul = raw Coulomb change of Theta_e over h
+__device__ __forceinline__ void update64_core(const StepConst &S, double rho, double r, double lam, const double frac[3], double &the, double &thi,
+                                              double de_sum[4], int &limited, int &floored, double dcoul)
 {
     if (S.hfloor2 > 0.0 && r > 0.0) {
         double ok = r / (r * sqrt(r) + S.spin);            // Omega_K r
         if ((the + thi) * S.mr < S.hfloor2 * ok * ok) { lam = 0.0; floored = 1; }
     }
-    double dcoul = 0.0;                                    // raw Coulomb change of Theta_e over h
     const double D = thi - the;
-    if (S.coulomb != 0 && D != 0.0) {
-        double C = (S.coulomb == 1) ? coulomb_C_table64(T, the, thi)
-                                    : coolphys::coulomb_C(the, thi / K.units.ion_theta_mass_ratio);
-        dcoul = S.coul_kh * rho * C * D;
-    }
     // energies per (rho mr): u_e = the/ge1, u_i = thi/gi1; work directly in Theta
     double dth_rad = lam * S.h * S.ge1 / (rho * S.mr);
     if (dth_rad > S.f_limit * the) { dth_rad = S.f_limit * the; limited = 1; }
@@ -258,6 +253,27 @@ __device__ __forceinline__ void update64(const DevTable &T, const DevConst &K, c
     de_sum[1] += dth_rad * frac[0]; de_sum[2] += dth_rad * frac[1]; de_sum[3] += dth_rad * frac[2];
     the = the - dth_rad + dthe;
     thi = thi - dthe * (S.gi1 / S.ge1);
+}
+__device__ __forceinline__ void update64(const DevTable &T, const DevConst &K, const StepConst &S, double rho, double r,
+                                         double lam, const double frac[3], double &the, double &thi, double de_sum[4],
+                                         int &limited, int &floored)
+{
+    double dcoul = 0.0;
+    const double D = thi - the;
+    if (S.coulomb != 0 && D != 0.0) {
+        double C = (S.coulomb == 1) ? coulomb_C_table64(T, the, thi)
+                                    : coolphys::coulomb_C(the, thi / K.units.ion_theta_mass_ratio);
+        dcoul = S.coul_kh * rho * C * D;
+    }
+    update64_core(S, rho, r, lam, frac, the, thi, de_sum, limited, floored, dcoul);
+}
+// Coulomb term given as Q_cc/(Theta_i - Theta_e) in code units (the paper's Q_cc(n_e, T_i, T_e) table, cool_cgs.cu):
+// dTheta_e = Q_cc h (gamma_e - 1)/(rho m_e/m_p)
+__device__ __forceinline__ void update64_q(const StepConst &S, double rho, double r, double lam, const double frac[3], double &the, double &thi,
+                                           double de_sum[4], int &limited, int &floored, double qcc_per_D)
+{
+    const double D = thi - the;
+    update64_core(S, rho, r, lam, frac, the, thi, de_sum, limited, floored, D != 0.0 ? qcc_per_D * D * S.h * S.ge1 / (rho * S.mr) : 0.0);
 }
 
 template <int MODE, class Fetch, bool DIAG>
@@ -318,6 +334,7 @@ __device__ __noinline__ void step_cell_analytic(const DevTable &T, const DevCons
     for (int s = 0; s < S.nsub; ++s) {
         double H = S.hth_cm;
         if (MODE == 4) H = S.h_per_cs * sqrt((S.ae * the + S.ai * thi) / (1.0 + S.be * the + S.bi * thi));
+        if (MODE == 4 && S.cgs && r > 0.0) H *= (r * sqrt(r) + S.spin) / S.omk_ref_inv;      // the paper's table: H_th at the cell's own radius (eq 13)
         coolphys::Cooling c = coolphys::cooling_cgs(H, B, ne, the);
         double frac[3] = {c.brems / c.thin, c.synch / c.thin, (c.eta - 1.0) * c.synch / c.thin};
         update64(T, K, S, rho, r, c.total * K.der.rate_conv, frac, the, thi, de_sum, limited, floored);
@@ -496,6 +513,7 @@ static cudaError_t launch_one(const LaunchCtx &L, size_t smem)
 // one function per translation unit of instantiations (cool_inst_*.cu)
 cudaError_t launch_f64(const LaunchCtx &L, int mode, cool_variant v, bool diag);
 cudaError_t launch_analytic(const LaunchCtx &L, int mode, cool_dtype dt, bool diag);
+cudaError_t launch_cgs(const LaunchCtx &L, cool_variant v, cool_dtype dt, bool diag);      // the paper's table (cool_cgs.cu)
 
 
 constexpr int kSmemThreads = 512;

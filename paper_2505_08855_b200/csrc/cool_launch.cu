@@ -32,7 +32,8 @@ static StepConst make_step_const(const cool_table *t, cool_dtype dt, const Launc
     S.spin = K.units.spin;
     S.lum_k = K.mr / (K.ge1 * a.dt);
     S.nsub = a.nsub; S.coulomb = a.coulomb;
-    S.has_r = a.r != nullptr && S.hfloor2 > 0.0; S.has_vol = a.vol != nullptr && a.want_diag;      // arrays nobody uses are not read
+    S.cgs = desc_is_cgs(&t->desc); S.omk_ref_inv = pow(K.units.r_ref_rg, 1.5) + K.units.spin;
+    S.has_r = a.r != nullptr && (S.hfloor2 > 0.0 || S.cgs); S.has_vol = a.vol != nullptr && a.want_diag;      // arrays nobody uses are not read
     auto ok = [&](const void *p) { return p == nullptr || ((size_t)p % 16) == 0; };
     S.lum_shell = a.lum_shell ? a.shell_rep : nullptr; S.shell_cells = a.shell_cells > 0 ? a.shell_cells : 1;
     S.cell_offset = a.cell_offset; S.shell0 = a.shell0; S.shell_nloc4 = a.shell_nloc4; S.shell_rmask = a.shell_rmask;
@@ -116,6 +117,7 @@ static F32Const make_f32_const(const cool_table *t, const LaunchArgs &a)
 bool variant_supported(const cool_table *t, cool_variant v, cool_dtype, std::string *why)
 {
     if (v == COOL_V_ANALYTIC) return true;
+    if (t->dev.mode == 5 && v == COOL_V_SMEM) { if (why) *why = "the paper's table runs on the GLOBAL, TEX_POINT, TEX_HWFILTER and ANALYTIC lookups"; return false; }
     if (t->dev.mode == 0) { if (why) *why = "table has no data (nproc = 0): only COOL_V_ANALYTIC applies"; return false; }
     // SMEM variant: table image + the warps' 6-array cell stages + plain Coulomb table + barriers
     if (v == COOL_V_SMEM && (size_t)t->dev.table_bytes + kCoulSmemMax + (size_t)kF32SmemStages * 6 * (size_t)kF32SmemThreads * kF32CellsPerThread * 4 + kF32BarBytes > (size_t)t->max_smem_optin) {
@@ -131,12 +133,16 @@ bool uses_fixmap(const cool_table *t, cool_variant v, cool_dtype dt, const Launc
 {
     // (a single update of a 3-D table needs no second kernel: its cells are exact inputs, and the step re-evaluates the rate of
     // a band cell in place, precise_rate3 of cool_f32.cuh)
-    return t->dev.nband != 0 && dt == COOL_F32 && a.scheme == COOL_SCHEME_EXPLICIT && (v == COOL_V_GLOBAL || v == COOL_V_SMEM || v == COOL_V_TEX_POINT) &&
+    return t->dev.mode != 5 && t->dev.nband != 0 && dt == COOL_F32 && a.scheme == COOL_SCHEME_EXPLICIT && (v == COOL_V_GLOBAL || v == COOL_V_SMEM || v == COOL_V_TEX_POINT) &&
            (t->dev.mode == 4 || a.nsub > 1);
 }
 
-cool_status launch_step(const cool_table *t, cool_variant v, cool_dtype dt, const LaunchArgs &a, cudaStream_t st, int *nlaunch)
+cool_status launch_step(const cool_table *t, cool_variant v, cool_dtype dt, const LaunchArgs &a_in, cudaStream_t st, int *nlaunch)
 {
+    LaunchArgs a_loc = a_in;
+    // the analytic variant has no use for the paper's Coulomb TABLE: eq 15 analytically
+    if (desc_is_cgs(&t->desc) && v == COOL_V_ANALYTIC && a_loc.coulomb == 1) a_loc.coulomb = 2;
+    const LaunchArgs &a = a_loc;
     const StepConst S = make_step_const(t, dt, a);
     const LaunchCtx L{t, &S, &a, st};
     const int mode = t->dev.mode == 0 ? (t->desc.ndim == 4 ? 4 : 3) : t->dev.mode;
@@ -150,6 +156,9 @@ cool_status launch_step(const cool_table *t, cool_variant v, cool_dtype dt, cons
     } else if (v == COOL_V_ANALYTIC) {
         note_kernel("cool_step_kernel<%s,MODE=%d,analytic,DIAG=%d>", dt == COOL_F64 ? "double" : "float", mode, (int)diag);
         e = launch_analytic(L, mode, dt, diag);
+    } else if (t->dev.mode == 5) {
+        note_kernel("cool_cgs_kernel<%s,%s,DIAG=%d>", dt == COOL_F64 ? "double" : "float", vname[v], (int)diag);
+        e = launch_cgs(L, v, dt, diag);
     } else if (dt == COOL_F64) {
         note_kernel("cool_step_kernel<double,MODE=%d,%s,DIAG=%d>", mode, vname[v], (int)diag);
         e = launch_f64(L, mode, v, diag);

@@ -37,7 +37,7 @@ def test_struct_layouts_match_header():
     assert ctypes.sizeof(api.cool_diag) == 7 * 8
     assert ctypes.sizeof(api.cool_params) == 8 + 8 + 8 + 8 + 8 + 8  # dt, nsub(+pad), f_limit, h_floor, variant+coulomb, scheme(+pad)
     assert ctypes.sizeof(api.cool_cells) == 8 + 8 + 8 * 8 + 8 + 8 + 8  # + shell_cells, lum_shell, flags
-    assert ctypes.sizeof(api.cool_table_desc) == 4 + 16 + 16 + 4 + 32 + 32 + 8 + 24 + 8 + 8 + 16 + 16 + 72
+    assert ctypes.sizeof(api.cool_table_desc) == 4 + 16 + 16 + 4 + 32 + 32 + 8 + 24 + 8 + 8 + 16 + 16 + 72 + 8 + 12 + 4 + 24 + 24   # + host_coulomb3, nc3 (+pad), c3lo, c3hi
 
 
 def test_builder_matches_oracle_3d(oracle):

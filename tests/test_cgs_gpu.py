@@ -1,0 +1,140 @@
+"""The cooling step on THE PAPER'S OWN TABLE: Q(H_th, B, n_e, T_e) in cgs units on the paper's ranges
+ with H_th per cell from eqs 13-14 and the cell's radius (L128-L136), the Coulomb table
+Q_cc(n_e, T_i, T_e) (L147) and the paper's flattened texture layout (L155-L159), against oracle Part D.
+fp32 cells <= 1e-5, fp64 cells <= 1e-12; the hardware-filtered texture (the paper's own scheme) is reported, not gated."""
+import numpy as np
+import pytest
+
+import common as cm
+from paper_2505_08855_b200 import api, synth
+
+AX = [api.COOL_AX_LOG_HTH, api.COOL_AX_LOG_B, api.COOL_AX_LOG_NE, api.COOL_AX_LOG_TE]
+LO, HI = [3.0, 0.0, 2.0, 2.0], [12.0, 10.0, 25.0, 15.0]          # the paper's ranges (L124)
+C3LO, C3HI = [2.0, 2.0, 2.0], [25.0, 15.0, 15.0]                  # (L147)
+TOL = {np.float32: 1e-5, np.float64: 1e-12}
+_cache = {}
+
+
+def cgs_tables(n=(24, 24, 24, 24), nc3=(16, 20, 20)):
+    key = (tuple(n), tuple(nc3))
+    if key not in _cache:
+        desc = api.make_desc(AX, list(n), LO, HI, 1, nc3=list(nc3), c3lo=C3LO, c3hi=C3HI)
+        data, coul3 = api.cool_table_build_host(desc, want_coulomb=True)
+        _cache[key] = (desc, data, coul3)
+    return _cache[key]
+
+
+def oracle_cgs_table(oracle, desc, data, coul3):
+    return oracle.Table(list(AX), [desc.n[k] for k in range(4)], LO, HI, data, cgs=True, coul3=coul3, c3lo=C3LO, c3hi=C3HI)
+
+
+def test_builder_matches_oracle_on_the_papers_table(oracle):
+    """The product's host builder (Newton + incomplete-gamma closed forms) against oracle Part D (bisection + quadrature) at
+    nodes of the paper's table and of its Coulomb table.  CPU only."""
+    desc, data, coul3 = cgs_tables()
+    T = data[0]
+    assert T.shape == (24, 24, 24, 24) and np.isfinite(T).all() and np.isfinite(coul3).all()
+    un = cm.oracle_units(oracle, desc)
+    ax = [np.linspace(LO[k], HI[k], 24) for k in range(4)]
+    rng = np.random.default_rng(0)
+    bad = 0
+    for i, j, k, l in rng.integers(0, 24, size=(600, 4)):
+        ref = np.log10(oracle.cooling_cgs(10 ** ax[0][i], 10 ** ax[1][j], 10 ** ax[2][k], 10 ** ax[3][l] * 1.380649e-16 / (9.1093837015e-28 * 2.99792458e10 ** 2))["total"])
+        assert abs(T[i, j, k, l] - ref) <= 1e-6 * max(1.0, abs(ref)) + 4e-6
+        bad += np.float32(ref) != T[i, j, k, l]
+    assert bad <= 12
+    K3 = oracle.fill_coulomb3_cgs(un, [16, 20, 20], C3LO, C3HI)
+    assert np.abs(coul3 - K3).max() <= 2e-5                     # log10 of values up to 1e40: fp32 ulp 4e-6
+
+
+pytestmark_gpu = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def tab(oracle):
+    desc, data, coul3 = cgs_tables()
+    t = api.cool_table_create(desc, data, coul3)
+    yield t, oracle_cgs_table(oracle, desc, data, coul3), cm.oracle_units(oracle, desc)
+    t.destroy()
+
+
+def _fields(dtype, n=40003, seed=3):
+    f = synth.log_uniform_cells(n, dtype=dtype, config=7, outlier_frac=0.0)
+    rng = np.random.default_rng(seed)
+    f["r"] = (10 ** rng.uniform(0.2, 2.8, n)).astype(dtype)
+    f["vol"] = rng.uniform(0.5, 2.0, n).astype(dtype)
+    f["rho"][:50] *= dtype(1e-17)                                # n_e below the table: clamped
+    return f
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+@pytest.mark.parametrize("dt,nsub", [(1e-3, 1), (5.0, 4)])
+def test_papers_table_global_and_point_texture(oracle, tab, dtype, dt, nsub):
+    table, otab, un = tab
+    f = _fields(dtype)
+    ref = cm.oracle_step(oracle, otab, un, f, dt, nsub=nsub, use_r=True, use_vol=True)
+    base = None
+    for v in (api.COOL_V_GLOBAL, api.COOL_V_TEX_POINT, api.COOL_V_AUTO):
+        got = cm.gpu_step(table, f, dtype, dt, nsub=nsub, variant=v, use_r=True, use_vol=True)
+        ee, ei = cm.rel_err(got["theta_e"], ref["theta_e"]).max(), cm.rel_err(got["theta_i"], ref["theta_i"]).max()
+        print(f"\npaper's table {np.dtype(dtype).name} dt={dt} nsub={nsub} {api.VARIANT_NAMES[v]}: max rel err e={ee:.2e} i={ei:.2e}, kernel {got['kernel']}")
+        assert ee <= TOL[dtype] and ei <= TOL[dtype]
+        d, r = got["diag"], ref["diag"]
+        assert d["lum_total"] == pytest.approx(r["lum_total"], rel=2e-6 if dtype == np.float32 else 1e-10)
+        assert abs(d["n_limited"] - r["n_limited"]) <= (2 if dtype == np.float32 else 0) and abs(d["n_clamped"] - r["n_clamped"]) <= (2 if dtype == np.float32 else 0)
+        assert r["n_clamped"] >= 50 and got["launches"] == 1
+        if base is None:
+            base = got
+        else:
+            assert np.array_equal(base["theta_e"], got["theta_e"]) and np.array_equal(base["theta_i"], got["theta_i"])
+    ce, nact = cm.change_err(got["theta_e"], ref["theta_e"], f["theta_e"].astype(np.float64))
+    assert nact > 3000 and ce < 1e-4                             # not a vacuous comparison
+
+
+@pytest.mark.gpu
+def test_papers_scheme_hardware_filter_is_reported(oracle, tab):
+    """The paper's own lookup (L155-L159): hardware bilinear filtering on (H_th, B), manual interpolation on the flattened
+    (n_e, T_e) axis.  The filter's weights have 8 fractional bits, so the error is ~1e-3: printed, loosely bounded."""
+    table, otab, un = tab
+    f = _fields(np.float32)
+    ref = cm.oracle_step(oracle, otab, un, f, 1e-3, use_r=True)
+    got = cm.gpu_step(table, f, np.float32, 1e-3, variant=api.COOL_V_TEX_HWFILTER, use_r=True)
+    err = cm.rel_err(got["theta_e"], ref["theta_e"])
+    print(f"\npaper's scheme (hw filter on H_th, B): max rel err {err.max():.3e}, median {np.median(err):.3e}")
+    assert 1e-6 < err.max() < 0.3 and np.median(err) < 1e-5
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("dtype,tol", [(np.float64, 1e-9), (np.float32, 2e-7)])
+def test_papers_table_analytic_variant_uses_the_cells_radius(oracle, tab, dtype, tol):
+    table, otab, un = tab
+    f = _fields(dtype, n=3001)
+    ref = cm.oracle_step(oracle, otab, un, f, 1.0, nsub=2, use_r=True, rate_mode=oracle.RATE_ANALYTIC, coulomb_mode=oracle.COULOMB_ANALYTIC)
+    got = cm.gpu_step(table, f, dtype, 1.0, nsub=2, variant=api.COOL_V_ANALYTIC, use_r=True)
+    assert cm.rel_err(got["theta_e"], ref["theta_e"]).max() <= tol and cm.rel_err(got["theta_i"], ref["theta_i"]).max() <= tol
+
+
+@pytest.mark.gpu
+def test_papers_table_mad_field_floor_edge_cases_and_errors(oracle, tab):
+    table, otab, un = tab
+    f = synth.mad_like_cells(36, 24, 20, dtype=np.float32)
+    ref = cm.oracle_step(oracle, otab, un, f, 50.0, nsub=2, h_floor=0.117, use_r=True, use_vol=True)
+    got = cm.gpu_step(table, f, np.float32, 50.0, nsub=2, h_floor=0.117, use_r=True, use_vol=True, variant=api.COOL_V_GLOBAL, want_flags=True)
+    assert cm.rel_err(got["theta_e"], ref["theta_e"]).max() <= 1e-5 and cm.rel_err(got["theta_i"], ref["theta_i"]).max() <= 1e-5
+    assert got["diag"]["n_floored"] == pytest.approx(ref["diag"]["n_floored"], abs=3) and ref["diag"]["n_floored"] > 100
+    assert int(((got["flags"] & 2) != 0).sum()) == got["diag"]["n_floored"]
+    # without a radius array: H_th at r_ref (C-6); ragged, misaligned, in place; rho <= 0 and NaN cells
+    g = {k: v[:1003].copy() for k, v in f.items() if isinstance(v, np.ndarray)}
+    g["rho"][1] = 0.0; g["theta_i"][3] = np.nan
+    ref = cm.oracle_step(oracle, otab, un, g, 5.0)
+    for kw in (dict(), dict(offset=1), dict(inplace=True)):
+        got = cm.gpu_step(table, g, np.float32, 5.0, variant=api.COOL_V_GLOBAL, **kw)
+        ok = np.ones(1003, bool); ok[3] = False
+        assert cm.rel_err(got["theta_e"][ok], ref["theta_e"][ok]).max() <= 1e-5
+        assert got["theta_e"][1] == g["theta_e"][1] and np.isnan(got["theta_e"][3])
+    for bad in (dict(variant=api.COOL_V_SMEM), dict(scheme=api.COOL_SCHEME_IMPLICIT)):
+        with pytest.raises(api.CoolError) as e:
+            cm.gpu_step(table, g, np.float32, 5.0, **bad)
+        assert e.value.status == api.COOL_EUNSUPPORTED
+    assert table.auto_variant() == api.COOL_V_GLOBAL
