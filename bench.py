@@ -350,6 +350,118 @@ def run_radpress(args, rank, local_rank, world):
     return 0
 
 
+# ------------------------------------------------------------------------------------------------
+# the paper's own table: --workload p100 and the App. A replay --workload appA-<N>
+# ------------------------------------------------------------------------------------------------
+CGS_AX = [4, 5, 6, 7]                                  # log H_th[cm], log B[G], log n_e[cm^-3], log T_e[K]
+CGS_LO, CGS_HI = [3.0, 0.0, 2.0, 2.0], [12.0, 10.0, 25.0, 15.0]
+CGS_C3LO, CGS_C3HI = [2.0, 2.0, 2.0], [25.0, 15.0, 15.0]
+
+
+def run_cgs(args, rank, local_rank, world):
+    """p100: one cooling step of 2^26 log-uniform cells (random radii) on the paper's 100^4 table (400 MB: beyond L2) and its
+    100^3 Coulomb table.  appA-<N>: the paper's stand-alone test: N^4 lookups on a regular grid of
+    (H_th, B, n_e, T_e), hardware-filtered texture (the paper's scheme) | point texture | global memory | analytic, as one
+    cooling step per query cell (Coulomb off, dt -> 0: the lookup is all that differs between the variants)."""
+    import torch
+    from paper_2505_08855_b200 import api
+    if args.impl == "reference":
+        if rank == 0:
+            print(json.dumps(dict(impl="reference", unavailable="the oracle leg for the paper's 100^4 table lives in tests/test_cgs_gpu.py (sampled cells); no timed CPU arm for this workload")))
+        return 0
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    ntab = args.table_n
+    desc = api.make_desc(CGS_AX, [ntab] * 4, CGS_LO, CGS_HI, 1, nc3=[ntab] * 3, c3lo=CGS_C3LO, c3hi=CGS_C3HI)
+    t0 = time.perf_counter()
+    data = api.cool_table_build_device(desc, device=local_rank)
+    t_build = time.perf_counter() - t0
+    _, coul3 = api.cool_table_build_host(api.make_desc(CGS_AX, [2] * 4, CGS_LO, CGS_HI, 0, nc3=[ntab] * 3, c3lo=CGS_C3LO, c3hi=CGS_C3HI), want_coulomb=True)
+    table = api.cool_table_create(desc, data, coul3, device=local_rank)
+    app = args.workload.startswith("appA-")
+    g = torch.Generator(device=dev); g.manual_seed(20250508 + rank)
+    MP, C, KB, ME = 1.67262192369e-24, 2.99792458e10, 1.380649e-16, 9.1093837015e-28
+    rg, rs = 1.32712440018e26 * 10.0 / C ** 2, 3e-7
+    if app:
+        N = int(args.workload[5:])
+        ncell = N ** 4
+        idx = torch.arange(ncell, device=dev, dtype=torch.int64)
+        frac = lambda k: ((idx // (N ** k)) % N).to(torch.float64) / (N - 1)            # k = 0: T_e fastest (the paper's flattening)
+        Te = 10.0 ** (7.0 + 4.0 * frac(0)); ne = 10.0 ** (8.0 + 12.0 * frac(1)); B = 10.0 ** (1.0 + 7.0 * frac(2)); H = 10.0 ** (7.0 + 4.0 * frac(3))
+        the = Te * KB / (ME * C * C); thi = the
+        p = (the + thi) * (ME / MP)
+        cs = torch.sqrt((5.0 / 3.0) * p / (1.0 + 2.5 * p))
+        r = torch.clamp(H / (rg * cs) - 0.9375, min=1.0) ** (2.0 / 3.0)
+        d = dict(rho=(ne * MP / rs), bsq=(B * B / (4.0 * np.pi * rs * C * C)), theta_e=the, theta_i=thi, r=r)
+        d = {k: v.to(torch.float32) for k, v in d.items()}
+        del idx, Te, ne, B, H, the, thi, p, cs, r
+        label = f"App. A replay: {N}^4 = {ncell} lookups on a regular (H_th, B, n_e, T_e) grid, table {ntab}^4, one cooling step per query (Coulomb off)"
+        dt, coul = 1e-6, api.COOL_COULOMB_OFF
+    else:
+        ncell = 1 << 26
+        u = lambda lo, hi: 10.0 ** (lo + (hi - lo) * torch.rand(ncell, device=dev, generator=g, dtype=torch.float32))
+        d = dict(rho=u(-6.0, 0.0), bsq=u(-8.0, 0.0), theta_e=u(-3.0, 1.5), theta_i=u(-3.0, 1.5), r=u(0.2, 2.8))
+        label = f"2^26 fp32 log-uniform cells with log-uniform radii, the paper's {ntab}^4 table ({4 * ntab ** 4 / 1e6:.0f} MB) + {ntab}^3 Coulomb table, single update"
+        dt, coul = 1e-3, api.COOL_COULOMB_TABLE
+    the_o = torch.empty(ncell, dtype=torch.float32, device=dev); thi_o = torch.empty_like(the_o)
+    stream = torch.cuda.current_stream().cuda_stream
+    names = ["tex_hwfilter", "tex_point", "global"] + (["analytic"] if app and args.with_analytic else []) if (app or args.variant == "auto") else [args.variant]
+    res = {}
+    mon = ClocksMonitor(torch.cuda.get_device_properties(dev).uuid)
+    mon.start(local_rank)
+    for nm in names:
+        params = api.make_params(dt, 1, 0.3, 0.0, api.VARIANTS[nm], coul)
+        step = lambda: api.cool_apply(table, ncell, api.COOL_F32, d["rho"], d["bsq"], d["theta_e"], d["theta_i"], the_o, thi_o, params, r=d["r"], stream=stream)
+        steps = args.steps if nm != "analytic" else max(1, min(args.steps, 2))
+        for _ in range(args.warmup if nm != "analytic" else 1):
+            step()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(steps):
+            step()
+        e1.record(); torch.cuda.synchronize()
+        res[nm] = dict(ms_per_step=float(e0.elapsed_time(e1)) / steps, kernel=api.cool_last_kernel_name())
+    clocks = mon.stop()
+    peak, peak_src = peaks()
+    best = "global" if "global" in res else names[0]
+    ms = res[best]["ms_per_step"]
+    bpc = 28                                                     # rho, bsq, Theta_e, Theta_i, r read; Theta_e', Theta_i' written
+    ach = bpc * ncell / (ms * 1e-3) / 1e9
+    line = dict(metric=METRIC, value=ncell / (ms * 1e-3) / 1e9, unit=UNIT, n_gpus=1, steps=args.steps, warmup=args.warmup, ms_per_step=ms,
+                higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f64", data="synthetic",
+                config=dict(workload=args.workload, description=label, cells_per_gpu=ncell, variant=best, table_build_s_on_device=t_build,
+                            l2="inputs (%.2f GB per step) and the table larger than L2" % (bpc * ncell / 1e9)),
+                variants=res, clocks=clocks, gpu_launches=args.steps,
+                roofline=dict(bound="hbm", achieved=ach, peak=peak, unit="GB/s", frac=ach / peak, traffic=ncu_value(args.workload, best, "dram_bytes"),
+                              kernel=res[best]["kernel"], bytes_per_cell=bpc, algorithmic_bytes_per_launch=bpc * ncell, peak_source=peak_src,
+                              note="algorithmic bytes are the cell stream; the 16 table corners of a cell are 16 scattered 32-byte sectors when the "
+                                   "table does not fit L2 (see traffic)"))
+    if "tex_hwfilter" in res and "global" in res:
+        line["texture_over_global_time"] = res["tex_hwfilter"]["ms_per_step"] / res["global"]["ms_per_step"]
+    if "analytic" in res:
+        line["analytic_over_texture_time"] = res["analytic"]["ms_per_step"] / res["tex_hwfilter"]["ms_per_step"]
+    print(json.dumps(line))
+    table.destroy()
+    return 0
+
+
+def ncu_value(workload, variant, column):
+    """Per-launch counters of the dominant kernel from the ncu captures summarised in profiles/r02_ncu_per_launch.csv
+    (workload,variant,kernel,dram_bytes,warp_inst,source); None when that (workload, variant) was not captured."""
+    path = os.path.join(ROOT, "profiles", "r02_ncu_per_launch.csv")
+    if not os.path.exists(path):
+        return None
+    import csv
+    with open(path) as fh:
+        for row in csv.DictReader(fh):
+            if row["workload"] == workload and row["variant"] == variant and row.get(column):
+                return float(row[column])
+    return None
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -364,6 +476,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-also", action="store_true", help="skip the companion s512 measurement of the default workload")
     ap.add_argument("--cpu-sample", type=int, default=1 << 27)
+    ap.add_argument("--table-n", type=int, default=100, help="points per axis of the paper's table (p100, appA-<N>); the paper uses 100")
+    ap.add_argument("--with-analytic", action="store_true", help="appA-<N>: also time the analytic variant (slow)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3                                       # timing rule: W >= 3
@@ -373,6 +487,8 @@ def main():
     world = int(os.environ.get("WORLD_SIZE", "1"))
     if args.workload == "rp512":
         return run_radpress(args, rank, local_rank, world)
+    if args.workload == "p100" or args.workload.startswith("appA-"):
+        return run_cgs(args, rank, local_rank, world)
     spec = workload_spec(args.workload)
     axis, lo, hi = table_ranges(spec["n"])
 

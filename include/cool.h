@@ -174,6 +174,12 @@ typedef struct cool_table cool_table;      /* opaque */
  * needs no GPU.  Errors: COOL_EINVAL for a malformed shape. */
 cool_status cool_table_build_host(const cool_table_desc *shape, float *const out[3], float *out_coulomb, int nthreads);
 
+/* The same tabulation on a CUDA device, for the paper's table only (axes LOG_HTH, LOG_B, LOG_NE, LOG_TE; nproc = 1):
+ * 100^4 nodes (L124) take the host builder minutes and the device a second.  host_out: HOST array of prod(n) floats
+ * (log10 Q_total[erg cm^-3 s^-1]).  Synchronous.  Errors: COOL_EINVAL, COOL_EUNSUPPORTED (another shape), COOL_ENOMEM,
+ * COOL_ECUDA (no usable device). */
+cool_status cool_table_build_device(const cool_table_desc *shape, int device, float *host_out);
+
 /* Uploads a table to `device` and prepares every device representation (linear arrays,
  * cudaArray + texture objects, the shared-memory image).  Host arrays are copied; the
  * caller may free them on return.  *out is owned by the library until cool_table_destroy.

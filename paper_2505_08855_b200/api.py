@@ -75,7 +75,7 @@ class cool_diag(C.Structure):
 DIAG_BYTES = C.sizeof(cool_diag)
 EXPORTS = ("cool_table_build_host", "cool_table_create", "cool_apply", "cool_apply_host",
            "cool_table_auto_variant", "cool_last_launch_count", "cool_table_destroy",
-           "cool_last_error", "cool_version", "cool_radpress_correct", "cool_last_kernel_name")
+           "cool_last_error", "cool_version", "cool_radpress_correct", "cool_last_kernel_name", "cool_table_build_device")
 
 _lib = None
 
@@ -90,6 +90,8 @@ def lib():
         L = C.CDLL(LIB_PATH)
         L.cool_table_build_host.restype = C.c_int
         L.cool_table_build_host.argtypes = [C.POINTER(cool_table_desc), C.POINTER(C.c_void_p), C.c_void_p, C.c_int]
+        L.cool_table_build_device.restype = C.c_int
+        L.cool_table_build_device.argtypes = [C.POINTER(cool_table_desc), C.c_int, C.c_void_p]
         L.cool_table_create.restype = C.c_int
         L.cool_table_create.argtypes = [C.POINTER(cool_table_desc), C.c_int, C.POINTER(C.c_void_p)]
         L.cool_apply.restype = C.c_int
@@ -170,6 +172,13 @@ def cool_table_build_host(desc: cool_table_desc, want_coulomb: bool = False, nth
         coul = np.empty((desc.nc[0], desc.nc[1]), dtype=np.float32) if want_coulomb else None
     _check(lib().cool_table_build_host(C.byref(desc), outs, None if coul is None else coul.ctypes.data, nthreads))
     return data, coul
+
+
+def cool_table_build_device(desc: cool_table_desc, device: int = 0):
+    """The paper's table tabulated on the GPU (see include/cool.h).  Returns [float32 array of shape n]."""
+    out = np.empty([desc.n[k] for k in range(desc.ndim)], dtype=np.float32)
+    _check(lib().cool_table_build_device(C.byref(desc), device, out.ctypes.data))
+    return [out]
 
 
 class CoolTable:

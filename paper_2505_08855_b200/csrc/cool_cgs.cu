@@ -167,4 +167,49 @@ cudaError_t launch_cgs(const LaunchCtx &L, cool_variant v, cool_dtype dt, bool d
 #undef COOL_CGS_GO
 }
 
+// ---- device table builder for the paper's table ---------------------------------------------------------------------------
+// 100^4 nodes take the host builder minutes; the same cool_physics.cuh code on the device takes a second.
+__global__ void __launch_bounds__(128) cgs_build_kernel(int n0, int n1, int n2, int n3, double lo0, double lo1, double lo2, double lo3,
+                                                        double d0, double d1, double d2, double d3, float *out, long long total)
+{
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long f = (long long)blockIdx.x * blockDim.x + threadIdx.x; f < total; f += stride) {
+        long long rem = f;
+        const int i3 = (int)(rem % n3); rem /= n3;
+        const int i2 = (int)(rem % n2); rem /= n2;
+        const int i1 = (int)(rem % n1); const int i0 = (int)(rem / n1);
+        (void)n0;
+        const coolphys::Cooling c = coolphys::cooling_cgs(pow(10.0, lo0 + i0 * d0), pow(10.0, lo1 + i1 * d1), pow(10.0, lo2 + i2 * d2),
+                                                          pow(10.0, lo3 + i3 * d3) / coolphys::kTHETA_TO_K);
+        out[f] = (float)log10(c.total);
+    }
+}
+
 }  // namespace cool
+
+extern "C" cool_status cool_table_build_device(const cool_table_desc *shape, int device, float *host_out)
+{
+    using namespace cool;
+    std::string why;
+    if (!desc_valid(shape, false, &why)) { set_error("cool_table_build_device: %s", why.c_str()); return COOL_EINVAL; }
+    if (!desc_is_cgs(shape) || shape->nproc != 1) { set_error("cool_table_build_device: only the paper's table (axes LOG_HTH, LOG_B, LOG_NE, LOG_TE; nproc = 1)"); return COOL_EUNSUPPORTED; }
+    if (!host_out) { set_error("cool_table_build_device: host_out is NULL"); return COOL_EINVAL; }
+    int prev = -1;
+    if (cudaGetDevice(&prev) != cudaSuccess || cudaSetDevice(device) != cudaSuccess) { set_error("cool_table_build_device: no usable CUDA device %d", device); return COOL_ECUDA; }
+    const long long total = (long long)shape->n[0] * shape->n[1] * shape->n[2] * shape->n[3];
+    float *d = nullptr;
+    cudaError_t e = cudaMalloc(&d, (size_t)total * sizeof(float));
+    if (e == cudaSuccess) {
+        double dd[4];
+        for (int k = 0; k < 4; ++k) dd[k] = (shape->hi[k] - shape->lo[k]) / (shape->n[k] - 1);
+        const long long blocks = (total + 127) / 128;
+        cgs_build_kernel<<<(int)(blocks < 148 * 64 ? blocks : 148 * 64), 128>>>(shape->n[0], shape->n[1], shape->n[2], shape->n[3], shape->lo[0], shape->lo[1],
+                                                                               shape->lo[2], shape->lo[3], dd[0], dd[1], dd[2], dd[3], d, total);
+        e = cudaGetLastError();
+        if (e == cudaSuccess) e = cudaMemcpy(host_out, d, (size_t)total * sizeof(float), cudaMemcpyDeviceToHost);
+    }
+    if (d) cudaFree(d);
+    if (prev >= 0) cudaSetDevice(prev);
+    if (e != cudaSuccess) { set_error("cool_table_build_device: %s", cudaGetErrorString(e)); return e == cudaErrorMemoryAllocation ? COOL_ENOMEM : COOL_ECUDA; }
+    return COOL_OK;
+}

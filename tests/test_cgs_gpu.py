@@ -138,3 +138,32 @@ def test_papers_table_mad_field_floor_edge_cases_and_errors(oracle, tab):
             cm.gpu_step(table, g, np.float32, 5.0, **bad)
         assert e.value.status == api.COOL_EUNSUPPORTED
     assert table.auto_variant() == api.COOL_V_GLOBAL
+
+
+@pytest.mark.gpu
+def test_device_builder_and_the_full_100_4_table(oracle):
+    """cool_table_build_device against the host builder (same cool_physics.cuh code: node values agree to fp32 rounding), and
+    the paper's full-size table — 100^4 nodes, 400 MB, beyond L2, as bench.py --workload p100 runs it — on 2^22 log-uniform
+    cells, 20 000 of them sampled against the oracle on the same table values, every lookup variant."""
+    import torch
+    small = api.make_desc(AX, [12, 11, 13, 14], LO, HI, 1)
+    host, _ = api.cool_table_build_host(small)
+    devb = api.cool_table_build_device(small)
+    assert np.abs(devb[0] - host[0]).max() <= 8e-6 and (devb[0] != host[0]).mean() < 0.02      # libm vs CUDA math: a last-bit tie here and there
+    desc = api.make_desc(AX, [100] * 4, LO, HI, 1, nc3=[32, 32, 32], c3lo=C3LO, c3hi=C3HI)
+    data = api.cool_table_build_device(desc)
+    assert np.isfinite(data[0]).all()
+    _, coul3 = api.cool_table_build_host(api.make_desc(AX, [2] * 4, LO, HI, 0, nc3=[32, 32, 32], c3lo=C3LO, c3hi=C3HI), want_coulomb=True)
+    table = api.cool_table_create(desc, data, coul3)
+    otab, un = oracle_cgs_table(oracle, desc, data, coul3), cm.oracle_units(oracle, desc)
+    n = 1 << 22
+    f = _fields(np.float32, n=n)
+    idx = np.sort(np.random.default_rng(5).choice(n, 20000, replace=False))
+    sub = {k: v[idx] for k, v in f.items()}
+    ref = cm.oracle_step(oracle, otab, un, sub, 1e-3, use_r=True)
+    for v in (api.COOL_V_GLOBAL, api.COOL_V_TEX_POINT, api.COOL_V_TEX_HWFILTER):
+        got = cm.gpu_step(table, f, np.float32, 1e-3, variant=v, use_r=True, want_diag=False)
+        err = max(cm.rel_err(got["theta_e"][idx], ref["theta_e"]).max(), cm.rel_err(got["theta_i"][idx], ref["theta_i"]).max())
+        print(f"\n100^4 table, {api.VARIANT_NAMES[v]}: sampled max rel err {err:.2e}")
+        assert err <= (1e-5 if v != api.COOL_V_TEX_HWFILTER else 0.3)
+    table.destroy()
