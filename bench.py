@@ -34,14 +34,11 @@ METRIC = "Gcell-updates/s of the cooling step"
 UNIT = "Gcell-updates/s"
 SPEC_HBM_GBS = 8000.0                     # BASELINE.json: "vs 8 TB/s"
 FALLBACK_HBM_GBS = 6650.0                 # B200_PROFILING.md fallback
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from one `ncu --set full` capture each
-# (profiles/r01e_<workload>_global_full.txt, rp512: r01e_rp512_radpress_full.txt, c2: r01c; line "traffic ="); null for workloads that were not captured
-NCU_TRAFFIC_GB = {"c5": 3.7339, "s512": 3.1948, "s512f": 4.2766, "c2": 0.4301, "c3": 0.2358, "rp512": 2.1180}   # rp512: profiles/r01e_rp512_radpress_full.txt
 # issue-slot ceiling of the SMs (the bound that actually limits the sub-stepped 4-D step): 148 SMs x 4 schedulers x
 # 1 warp instruction per clock at clocks.max.sm 1965 MHz (B200_PROFILING.md unit counts) = 1163 G warp-instructions/s
 ISSUE_PEAK_GWINST = 148 * 4 * 1.965
-# warp instructions per launch (smsp__inst_executed.sum of the same captures)
-NCU_WARP_INST = {"c5": 3322223572, "s512": 613040600, "s512f": 780244894, "c3": 48924970}
+# dram__bytes and smsp__inst_executed per launch of the dominant kernel are read from profiles/r02_ncu_per_launch.csv
+# (ncu_value below), the summary of the ncu captures kept under profiles/
 
 
 # ------------------------------------------------------------------------------------------------
@@ -105,7 +102,7 @@ def peaks():
 # ------------------------------------------------------------------------------------------------
 # oracle legs (cpu_baseline and --impl reference): the only places bench.py touches oracle/
 # ------------------------------------------------------------------------------------------------
-def oracle_leg(spec, desc, data, coul, fields, sample_cells, steps=1, scheme="explicit"):
+def oracle_leg(spec, desc, data, coul, fields, sample_cells, steps=1, scheme="explicit", nthreads=0):
     import oracle as O
     O.build()
     nd = desc.ndim
@@ -113,11 +110,11 @@ def oracle_leg(spec, desc, data, coul, fields, sample_cells, steps=1, scheme="ex
                    [desc.hi[k] for k in range(nd)], data, coul=coul, clo=[desc.clo[0], desc.clo[1]], chi=[desc.chi[0], desc.chi[1]])
     u = desc.units
     un = O.Units(u.rho_scale_cgs, u.mbh_msun, u.gamma_e, u.gamma_i, u.ln_lambda, u.ion_theta_mass_ratio, u.hth_cm, u.r_ref_rg, u.spin)
+    cores = nthreads or O.max_threads()
     ncell = fields["rho"].size
     m = min(sample_cells, ncell)
     lo = (ncell - m) // 2                     # contiguous sample from the middle of the field
     sl = slice(lo, lo + m)
-    cores = O.max_threads()
     times = []
     for _ in range(steps):
         t0 = time.perf_counter()
@@ -334,7 +331,7 @@ def run_radpress(args, rank, local_rank, world):
                 e2e=dict(value=ncell * world * e2e_steps / dt_e2e / 1e9, unit=unit, h2d_bytes_per_step=12 * ncell, d2h_bytes_per_step=4 * ncell + 8,
                          steps=e2e_steps, api="cool_radpress_correct after 3 pinned host->device copies, device->host copy of the result"),
                 roofline=dict(bound="hbm", achieved=achieved, peak=peak, unit="GB/s", frac=achieved / peak,
-                              traffic=NCU_TRAFFIC_GB["rp512"] * 1e9 if "rp512" in NCU_TRAFFIC_GB else None,
+                              traffic=ncu_value("rp512", "radpress", "dram_bytes"),
                               kernel="cool_radpress_kernel<float, VEC=1, COUNT=1>", bytes_per_cell=16, algorithmic_bytes_per_launch=16 * ncell,
                               peak_source=peak_src, ms_per_launch_median=float(np.median(per_step_ms)), ms_per_launch_best=float(per_step_ms.min())))
     if not args.no_cpu_baseline:
@@ -496,10 +493,21 @@ def main():
     if args.impl == "reference":
         if rank != 0:
             return 0
-        from paper_2505_08855_b200 import api
-        desc = api.make_desc(axis, spec["n"], lo, hi, 1 if len(spec["n"]) == 3 else 3, nc=spec["nc"],
-                             clo=[synth.LOG_THETA[0]] * 2, chi=[synth.LOG_THETA[1]] * 2)
-        data, coul = api.cool_table_build_host(desc, want_coulomb=True)      # host builder: tables are data
+        # tables from the oracle's own fillers: this arm loads nothing of the product
+        import oracle as O
+        O.build()
+        un0 = O.Units()
+        if len(spec["n"]) == 3:
+            data = [O.fill_total3(un0, spec["n"], lo, hi)]
+        else:
+            data = O.fill_proc4(un0, spec["n"], lo, hi)
+        coul = O.fill_coulomb2(un0, spec["nc"], [synth.LOG_THETA[0]] * 2, [synth.LOG_THETA[1]] * 2)
+
+        class _Desc:                                   # what oracle_leg reads of a table descriptor
+            pass
+        desc = _Desc()
+        desc.ndim = len(spec["n"]); desc.axis = axis; desc.n = spec["n"]; desc.lo = lo; desc.hi = hi
+        desc.clo = [synth.LOG_THETA[0]] * 2; desc.chi = [synth.LOG_THETA[1]] * 2; desc.units = un0
         small = dict(spec); f = spec["field"]
         if f[0] == "mad":
             small["field"] = ("mad", f[1], f[2], max(1, (1 << 22) // (f[1] * f[2])))   # a phi-slab of the same field
@@ -570,6 +578,7 @@ def main():
     for _ in range(args.warmup):
         step()
     launches_per_step = api.cool_last_launch_count()
+    kernel_name = api.cool_last_kernel_name()         # the dispatcher's own choice, reported by the library
     barrier()
     mon = ClocksMonitor(torch.cuda.get_device_properties(dev).uuid) if rank == 0 else None
     ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
@@ -598,40 +607,81 @@ def main():
             dd["lum_total"], dd["lum_brems"], dd["lum_synch"], dd["lum_compton"] = [float(x) for x in t.tolist()]
         diag_out = dd
 
-    # ---- companion line: the single-update 3-D step (table 128^3) on the same 512^3 field, same timing protocol ----
+    # ---- executed sub-steps (outside the timed region).  A cell stops sub-stepping as soon as a sub-step changes no bit of its
+    # state (exact: every later sub-step would be the same identity).  Measured through the public call: chain nsub single
+    # sub-step updates with h = dt/nsub and count, stage by stage, the cells every earlier stage has changed. ----
+    substeps_executed = None
+    if spec["nsub"] > 1 and args.scheme == "explicit" and not args.shells:
+        p1 = api.make_params(spec["dt"] / spec["nsub"], 1, 0.3, spec.get("floor", 0.0), variant, api.COOL_COULOMB_TABLE, scheme)
+        cur_e, cur_i = d["theta_e"].clone(), d["theta_i"].clone()
+        nxt_e, nxt_i = torch.empty_like(cur_e), torch.empty_like(cur_i)
+        active = torch.ones(ncell, dtype=torch.bool, device=dev)
+        executed = 0
+        for _ in range(spec["nsub"]):
+            executed += int(active.sum().item())
+            api.cool_apply(table, ncell, api.COOL_F32, d["rho"], d["bsq"], cur_e, cur_i, nxt_e, nxt_i, p1, r=d.get("r"), vol=d.get("vol"), stream=stream)
+            torch.cuda.synchronize()
+            active &= (nxt_e.view(torch.int32) != cur_e.view(torch.int32)) | (nxt_i.view(torch.int32) != cur_i.view(torch.int32))
+            cur_e, nxt_e = nxt_e, cur_e
+            cur_i, nxt_i = nxt_i, cur_i
+        substeps_executed = executed / ncell
+        del cur_e, cur_i, nxt_e, nxt_i, active
+        step()
+        torch.cuda.synchronize()
+
+    # ---- companion lines of the default workload, same timing protocol: (1) the single-update 3-D step (table 128^3) on the
+    # same 512^3 field, which is what north_star's 70 % bar is about; (2) configs[4] on log-uniform cells (worst locality),
+    # "run both" ----
     also = None
     if args.workload == "c5" and args.variant == "auto" and not args.no_also and args.scheme == "explicit":
+        also = []
+        peak2, _ = peaks()
+
+        def timed(fn):
+            for _ in range(args.warmup):
+                fn()
+            barrier()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(args.steps):
+                fn()
+            e1.record()
+            barrier()
+            ms = float(e0.elapsed_time(e1)) / args.steps
+            if world > 1:
+                t = torch.tensor([ms], dtype=torch.float64, device=dev)
+                dist.all_reduce(t, op=dist.ReduceOp.MAX)
+                ms = float(t.item())
+            return ms
         spec2 = workload_spec("s512")
         axis2, lo2, hi2 = table_ranges(spec2["n"])
         desc2 = api.make_desc(axis2, spec2["n"], lo2, hi2, 1, nc=spec2["nc"], clo=[synth.LOG_THETA[0]] * 2, chi=[synth.LOG_THETA[1]] * 2)
         data2, coul2 = api.cool_table_build_host(desc2, want_coulomb=True)
         table2 = api.cool_table_create(desc2, data2, coul2, device=local_rank)
         params2 = api.make_params(spec2["dt"], 1, 0.3, 0.0, api.COOL_V_AUTO, api.COOL_COULOMB_TABLE)
-
-        def step2():
-            api.cool_apply(table2, ncell, api.COOL_F32, d["rho"], d["bsq"], d["theta_e"], d["theta_i"], the_o, thi_o, params2, stream=stream)
-        for _ in range(args.warmup):
-            step2()
-        barrier()
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record()
-        for _ in range(args.steps):
-            step2()
-        e1.record()
-        barrier()
-        ms2 = float(e0.elapsed_time(e1)) / args.steps
-        if world > 1:
-            t = torch.tensor([ms2], dtype=torch.float64, device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms2 = float(t.item())
-        peak2, _ = peaks()
+        ms2 = timed(lambda: api.cool_apply(table2, ncell, api.COOL_F32, d["rho"], d["bsq"], d["theta_e"], d["theta_i"], the_o, thi_o, params2, stream=stream))
         ach2 = 24 * ncell / (ms2 * 1e-3) / 1e9
-        also = dict(workload="s512", description=spec2["label"], ms_per_step=ms2, value=ncell * world / (ms2 * 1e-3) / 1e9, unit=UNIT,
-                    roofline=dict(bound="hbm", achieved=ach2, peak=peak2, unit="GB/s", frac=ach2 / peak2, traffic=NCU_TRAFFIC_GB["s512"] * 1e9,
-                                  kernel="cool_f32_kernel<MODE=3, F32GlobalQ, DIAG=0, CM=1, NSUB1=1, 768 threads, 2 stages>", bytes_per_cell=24),
-                    frac_of_8TBs=ach2 / SPEC_HBM_GBS)
+        also.append(dict(workload="s512", description=spec2["label"], ms_per_step=ms2, value=ncell * world / (ms2 * 1e-3) / 1e9, unit=UNIT,
+                         gpu_launches_per_step=api.cool_last_launch_count(),
+                         roofline=dict(bound="hbm", achieved=ach2, peak=peak2, unit="GB/s", frac=ach2 / peak2, traffic=ncu_value("s512", "global", "dram_bytes"),
+                                       kernel=api.cool_last_kernel_name(), bytes_per_cell=24),
+                         frac_of_8TBs=ach2 / SPEC_HBM_GBS))
         table2.destroy()
-        step()                                       # leave the_o / thi_o holding the main workload's result for the e2e check below
+        spec3 = workload_spec("c5u")
+        f3 = make_fields(spec3, rank)
+        d3 = {k: torch.from_numpy(f3[k]).to(dev) for k in ("rho", "bsq", "theta_e", "theta_i")}
+        del f3
+        params3 = api.make_params(spec3["dt"], spec3["nsub"], 0.3, 0.0, api.COOL_V_AUTO, api.COOL_COULOMB_TABLE)
+        ms3 = timed(lambda: api.cool_apply(table, ncell, api.COOL_F32, d3["rho"], d3["bsq"], d3["theta_e"], d3["theta_i"], the_o, thi_o, params3,
+                                           d_diag=d_diag, stream=stream))
+        ach3 = 24 * ncell / (ms3 * 1e-3) / 1e9
+        also.append(dict(workload="c5u", description=spec3["label"], ms_per_step=ms3, value=ncell * world / (ms3 * 1e-3) / 1e9, unit=UNIT,
+                         gpu_launches_per_step=api.cool_last_launch_count(),
+                         roofline=dict(bound="hbm", achieved=ach3, peak=peak2, unit="GB/s", frac=ach3 / peak2, traffic=ncu_value("c5u", "global", "dram_bytes"),
+                                       kernel=api.cool_last_kernel_name(), bytes_per_cell=24),
+                         note="uncorrelated cells: bound by L2 -> L1 gather traffic and instruction issue, not by HBM"))
+        del d3
+        step()                                       # leave the_o / thi_o and d_diag holding the main workload's result for the e2e check below
         torch.cuda.synchronize()
 
     # ---- end to end: host buffers, copies inside the timed region (rank-local, max over ranks) ----
@@ -669,41 +719,39 @@ def main():
 
     peak, peak_src = peaks()
     bpc = bytes_per_cell(spec)
-    kern_ms = float(np.mean(per_step_ms))                     # one kernel per step: step time == kernel time
+    kern_ms = float(np.mean(per_step_ms))                     # the step's kernels back to back (fp32 kernel + the precise pass where one runs)
     achieved = bpc * ncell / (kern_ms * 1e-3) / 1e9
-    mode = len(spec["n"])
-    single = mode == 3 and spec["nsub"] == 1
-    fetch = {"global": ("F32GlobalO" if np.prod(spec["n"]) * 32 <= (16 << 20) else "F32GlobalQ" if np.prod(spec["n"]) * 16 <= (64 << 20) else "F32Global") if mode == 3 else "F32Global",
-             "smem": "F32Smem",
-             "tex_point": "F32TexPoint", "tex_hwfilter": "F32TexHw"}.get(api.VARIANT_NAMES[resolved], api.VARIANT_NAMES[resolved])
     explicit = args.scheme == "explicit"
-    kernel_name = ("cool_implicit_f32_kernel<MODE=%d, %s>" % (mode, api.VARIANT_NAMES[resolved])) if not explicit else "cool_f32_kernel<MODE=%d, %s, DIAG=%d, CM=%d, NSUB1=%d, %s>" % (
-        mode, fetch, int(bool(spec["diag"])), 2 if (mode == 3 and spec["diag"] and fetch != "F32Smem" and (ncell < (1 << 25) or not spec.get("floor"))) else 1, int(spec["nsub"] == 1),
-        "384 threads, 2 stages" if fetch == "F32Smem" else ("768 threads, 2 stages" if single else "512 threads, 2 stages"))
+    vname = api.VARIANT_NAMES[resolved]
     line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=args.warmup,
                 ms_per_step=total_ms / args.steps, higher_is_better=True, scaling="weak", vs_baseline=None,
                 dtype="f32", data="synthetic",
                 config=dict(workload=args.workload, description=spec["label"], cells_per_gpu=ncell, nsub=spec["nsub"],
                             variant=api.VARIANT_NAMES[resolved], scheme=args.scheme, radial_profile=bool(args.shells), l2="inputs (%.2f GB per step) larger than L2" % (bpc * ncell / 1e9),
-                            cell_substeps_per_s=value * spec["nsub"] * 1e9),
+                            cell_substeps_executed_per_update=substeps_executed,
+                            substeps_note="nsub sub-steps per update are requested; a cell whose sub-step changes no bit stops early (exact); the executed count is measured by chaining single sub-step calls"),
                 hbm_gbs=achieved * world, frac_of_8TBs=achieved / SPEC_HBM_GBS,
                 clocks=clocks, e2e=e2e, gpu_launches=launches_per_step * args.steps,
                 roofline=dict(bound="hbm", achieved=achieved, peak=peak, unit="GB/s", frac=achieved / peak,
-                              traffic=(NCU_TRAFFIC_GB[args.workload] * 1e9 if args.workload in NCU_TRAFFIC_GB and args.variant == "auto" and explicit and not args.shells else None),
+                              traffic=(ncu_value(args.workload, vname, "dram_bytes") if explicit and not args.shells else None),
                               kernel=kernel_name, bytes_per_cell=bpc, algorithmic_bytes_per_launch=bpc * ncell, peak_source=peak_src,
                               ms_per_launch_median=float(np.median(per_step_ms)), ms_per_launch_best=float(per_step_ms.min())),
                 diag=diag_out)
-    if args.workload in NCU_WARP_INST and args.variant == "auto" and explicit:
-        gw = NCU_WARP_INST[args.workload] / (kern_ms * 1e-3) / 1e9
+    winst = ncu_value(args.workload, vname, "warp_inst") if explicit and not args.shells else None
+    if winst:
+        gw = winst / (kern_ms * 1e-3) / 1e9
         line["issue_roofline"] = dict(bound="alu", achieved=gw, peak=ISSUE_PEAK_GWINST, unit="G warp-instructions/s", frac=gw / ISSUE_PEAK_GWINST,
-                                      warp_inst_per_launch=NCU_WARP_INST[args.workload],
-                                      note="instruction-issue ceiling (148 SMs x 4 schedulers x 1965 MHz); instruction count from the ncu capture in profiles/")
+                                      warp_inst_per_launch=winst,
+                                      note="instruction-issue ceiling (148 SMs x 4 schedulers x 1965 MHz); instruction count of all kernels of a step from profiles/r02_ncu_per_launch.csv")
     if also is not None:
         line["also"] = also
     if not args.no_cpu_baseline:
         m, cores, times = oracle_leg(spec, desc, data, coul, fields, args.cpu_sample if explicit else min(args.cpu_sample, 1 << 23), 1, args.scheme)
         line["cpu_baseline"] = dict(value=m / times[0] / 1e9, unit=UNIT, cores=cores, kind="oracle",
                                     sample=f"{m} contiguous cells from the middle of the workload, one pass, {times[0]:.1f} s")
+        m1, _, t1 = oracle_leg(spec, desc, data, coul, fields, min(args.cpu_sample, 1 << 22) if explicit else 1 << 19, 1, args.scheme, nthreads=1)
+        line["cpu_baseline"]["single_thread"] = dict(value=m1 / t1[0] / 1e9, unit=UNIT, cores=1,
+                                                     sample=f"{m1} contiguous cells from the middle of the workload, one pass, {t1[0]:.1f} s")
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()

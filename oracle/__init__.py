@@ -123,6 +123,7 @@ def lib():
             "orc_implicit_residual": (d, [C.POINTER(_Table), UP, d, d, d, d, d, d, i, d, i, d]),
             "orc_fill_total3": (None, [UP, C.POINTER(i), C.POINTER(d), C.POINTER(d), p, i]),
             "orc_fill_coulomb2": (None, [UP, C.POINTER(i), C.POINTER(d), C.POINTER(d), p]),
+            "orc_fill_proc4": (None, [UP, C.POINTER(i), C.POINTER(d), C.POINTER(d), p, p, p, i]),
             "orc_max_threads": (i, []),
             "orc_fill_total4_cgs": (None, [C.POINTER(i), C.POINTER(d), C.POINTER(d), p, i]),
             "orc_fill_coulomb3_cgs": (None, [UP, C.POINTER(i), C.POINTER(d), C.POINTER(d), p]),
@@ -199,6 +200,14 @@ def fill_total3(un, n, lo, hi, nthreads=0):
     lib().orc_fill_total3(C.byref(un), (C.c_int * 3)(*n), (C.c_double * 3)(*lo), (C.c_double * 3)(*hi),
                           out.ctypes.data, nthreads or max_threads())
     return out
+
+
+def fill_proc4(un, n, lo, hi, nthreads=0):
+    """[log10 Q_brem, log10 Q_syn, log10 eta] over (log rho, log Theta_e, log bsq, log Theta_i) from Part A."""
+    outs = [np.empty(n, dtype=np.float32) for _ in range(3)]
+    lib().orc_fill_proc4(C.byref(un), (C.c_int * 4)(*n), (C.c_double * 4)(*lo), (C.c_double * 4)(*hi),
+                         outs[0].ctypes.data, outs[1].ctypes.data, outs[2].ctypes.data, nthreads or max_threads())
+    return outs
 
 
 def fill_coulomb2(un, nc, clo, chi):

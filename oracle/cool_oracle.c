@@ -738,6 +738,20 @@ void orc_fill_total3(const orc_units *un, const int *n, const double *lo, const 
         out[t] = (float)orc_node_total_log10(un, rho, the, bsq);
     }
 }
+/* 4-D process tables over (log rho, log Theta_e, log bsq, log Theta_i), Theta_i fastest: log10 Q_brem, log10 Q_syn (code
+ * units) and log10 eta at every node, from orc_node_proc_log10 (used where a run must not load the product's builder). */
+void orc_fill_proc4(const orc_units *un, const int *n, const double *lo, const double *hi, float *out0, float *out1, float *out2, int nthreads)
+{
+    long long tot = (long long)n[0] * n[1] * n[2] * n[3];
+#pragma omp parallel for schedule(dynamic, 64) num_threads(nthreads > 0 ? nthreads : 1)
+    for (long long t = 0; t < tot; ++t) {
+        long long rem = t;
+        double x[4], o3[3];
+        for (int k = 3; k >= 0; --k) { x[k] = pow(10.0, lo[k] + (double)(rem % n[k]) * (hi[k] - lo[k]) / (n[k] - 1)); rem /= n[k]; }
+        orc_node_proc_log10(un, x[0], x[1], x[2], x[3], o3);
+        out0[t] = (float)o3[0]; out1[t] = (float)o3[1]; out2[t] = (float)o3[2];
+    }
+}
 void orc_fill_coulomb2(const orc_units *un, const int *nc, const double *clo, const double *chi, float *out)
 {
     for (int a = 0; a < nc[0]; ++a)
