@@ -550,6 +550,7 @@ __device__ __forceinline__ void step_cells_f32(const Ctx32 &X, const Fetch &F, c
                         // (rebuilding only when it really changed table cell), and only here is it tested — the sub-step loop
                         // itself carries no test.  The radiated fraction is evaluated once more on this rare path.
                         if (loc_bits(le) != (P[j].ke & 0x7fffffff) || loc_bits(li) != P[j].ki) build_patch(F, lr[j], lb[j], le, li, P[j]);
+#ifndef COOL_EXP_NOBAND4
                         if ((unsigned)(loc_bits(le) - S.kb_lo) < S.kb_n) {
                             P[j].ke = loc_bits(le) | (int)0x80000000u;
                             if ((__float_as_uint(the[j]) - S.band_lo_bits) < S.band_w) {
@@ -564,6 +565,7 @@ __device__ __forceinline__ void step_cells_f32(const Ctx32 &X, const Fetch &F, c
                                 if ((__float_as_uint(q) - S.rmin_bits) < S.r_w) { bad[j] = true; any_bad = true; nanq[j] = -0.f; }
                             }
                         }
+#endif
                     }
                     y0 = patch_eval(P[j], 0, le.w, li.w); y1 = patch_eval(P[j], 1, le.w, li.w);
                     y2 = patch_eval(P[j], 2, le.w, li.w); yc = patch_eval(P[j], 3, le.w, li.w);
@@ -781,6 +783,7 @@ cool_f32_kernel(const DevTable T, const F32Const S, const CellPtrs C, double *pa
         if (S.has_r) tma_load_1d(dst + k * kWarpArrBytes, (const char *)C.r + goff, kWarpArrBytes, bar);
     };
 
+    constexpr bool kLists = !(MODE == 3 && NSUB1);          // a single 3-D update recomputes its precise cells in place: no lists
     long long tile = (long long)blockIdx.x * NW + warp;
     if (lane == 0) {
 #pragma unroll
@@ -848,6 +851,9 @@ cool_f32_kernel(const DevTable T, const F32Const S, const CellPtrs C, double *pa
                 const bool inb = ((__float_as_uint(the.x) - S.band_lo_bits) < S.band_w) | ((__float_as_uint(the.y) - S.band_lo_bits) < S.band_w) |
                                  ((__float_as_uint(the.z) - S.band_lo_bits) < S.band_w) | ((__float_as_uint(the.w) - S.band_lo_bits) < S.band_w);
                 tested = __any_sync(0xffffffffu, inb);
+#ifdef COOL_EXP_NOPRE
+                tested = false;
+#endif
             }
             if (tested) step_cells_f32<MODE, Fetch, DIAG, CM, NSUB1, kF32CellsPerThread, true>(X, F, &rho.x, &bsq.x, &the.x, &thi.x, &rr.x, &vv.x, acc, tp, (unsigned)tile, flagword);
             else step_cells_f32<MODE, Fetch, DIAG, CM, NSUB1, kF32CellsPerThread, false>(X, F, &rho.x, &bsq.x, &the.x, &thi.x, &rr.x, &vv.x, acc, tp, (unsigned)tile, flagword);
@@ -879,7 +885,7 @@ cool_f32_kernel(const DevTable T, const F32Const S, const CellPtrs C, double *pa
                     }
                 }
         }
-        if (S.fixmap) {                                     // cells left to the precise pass: list the tile
+        if constexpr (kLists) if (S.fixmap) {               // cells left to the precise pass: list the tile
             if (__any_sync(0xffffffffu, (flagword & 0x08080808u) != 0u)) {
                 const unsigned w0 = __ballot_sync(0xffffffffu, flagword & 0x8u), w1 = __ballot_sync(0xffffffffu, flagword & 0x800u);
                 const unsigned w2 = __ballot_sync(0xffffffffu, flagword & 0x80000u), w3 = __ballot_sync(0xffffffffu, flagword & 0x8000000u);
@@ -895,7 +901,7 @@ cool_f32_kernel(const DevTable T, const F32Const S, const CellPtrs C, double *pa
             }
         }
     }
-    if (S.fixmap && lane == 0) S.fix.count[blockIdx.x * NW + warp] = *((unsigned *)(smem_f32 + kF32FixCntOff) + warp);      // every warp, every launch: no memset needed
+    if constexpr (kLists) if (S.fixmap && lane == 0) S.fix.count[blockIdx.x * NW + warp] = *((unsigned *)(smem_f32 + kF32FixCntOff) + warp);      // every warp, every launch: no memset needed
     if constexpr (DIAG) reduce_diag(acc, S.lum_k, partials, ticket, d_diag);
 }
 

@@ -342,6 +342,8 @@ __device__ __forceinline__ float imp32_rate_d(const F32Const &S, const Imp32 &c,
     }
 }
 
+constexpr float kImpF32Rate = 0.03f;      // radiated fraction h Lambda/u_e below which the fp32 rate is accurate enough for the implicit root
+
 template <int MODE, class Fetch>
 __device__ void implicit_cell_f32(const DevTable &T, const StepConst &S, const F32Const &S32, const Fetch &F,
                                   float rho, float bsq, float &the, float &thi, float r, float vol, DiagAcc &acc, long long cell,
@@ -420,16 +422,29 @@ __device__ void implicit_cell_f32(const DevTable &T, const StepConst &S, const F
             } else {
                 if (!have_b) imp32_node<MODE>(F, lr, lb, li, ir, ib, iii, ilo + 1, yb);
                 const float dy[3] = {yb[0] - ya[0], yb[1] - ya[1], yb[2] - ya[2]};
-                double yad[3], ybd[3];                          // the bracketing nodes once more, contracted in fp64
-                imp_node_d<MODE>(F, lr, lb, li, ir, ib, iii, ilo, yad);
-                imp_node_d<MODE>(F, lr, lb, li, ir, ib, iii, ilo + 1, ybd);
-                const double dyd[3] = {ybd[0] - yad[0], ybd[1] - yad[1], ybd[2] - yad[2]};
+                float lo = node_theta(ilo), hi = fminf(node_theta(ilo + 1), c.R);
+                // The root moves with the rate by d ln(theta) = -[rate/(opq + rate)] d ln(rate), and fp32 exponents give the rate to
+                // <= 1e-4 even in the steepest interval (5e-6 nodes x 16 log2 units), so where the radiated fraction is below
+                // kImpF32Rate over the whole interval the fp32 rate holds 1e-5 with a wide margin; elsewhere the bracketing
+                // nodes are contracted once more in fp64 and the exponent is summed in fp64.
+                const bool f32ok = fmaxf(imp32_rate<MODE>(S32, c, lo, ya, nullptr), imp32_rate<MODE>(S32, c, node_theta(ilo + 1), yb, nullptr)) < kImpF32Rate;
+                double yad[3] = {0.0, 0.0, 0.0}, dyd[3] = {0.0, 0.0, 0.0};
+                if (!f32ok) {
+                    double ybd[3];
+                    imp_node_d<MODE>(F, lr, lb, li, ir, ib, iii, ilo, yad);
+                    imp_node_d<MODE>(F, lr, lb, li, ir, ib, iii, ilo + 1, ybd);
+                    dyd[0] = ybd[0] - yad[0]; dyd[1] = ybd[1] - yad[1]; dyd[2] = ybd[2] - yad[2];
+                }
                 auto Rate = [&](float th, float *fr) {
-                    const double w = (double)fminf(fmaxf(coord32(ax, th, one_bits) - (float)ilo, 0.f), 1.f);
+                    const float w32 = fminf(fmaxf(coord32(ax, th, one_bits) - (float)ilo, 0.f), 1.f);
+                    if (f32ok) {
+                        const float y32[3] = {fmaf(w32, dy[0], ya[0]), fmaf(w32, dy[1], ya[1]), fmaf(w32, dy[2], ya[2])};
+                        return imp32_rate<MODE>(S32, c, th, y32, fr);
+                    }
+                    const double w = (double)w32;
                     const double y[3] = {fma(w, dyd[0], yad[0]), fma(w, dyd[1], yad[1]), fma(w, dyd[2], yad[2])};
                     return imp32_rate_d<MODE>(S32, c, th, y, kd, fr);
                 };
-                float lo = node_theta(ilo), hi = fminf(node_theta(ilo + 1), c.R);
                 const float noise = 1.2e-7f * c.R;              // F is a difference of terms of size R: below ~ulp(R) its sign is
                                                                 // rounding noise and the point is as good a root as fp32 can tell
                                                                 // (F' >= opq + rate where the rate does not fall with Theta_e, so
