@@ -67,8 +67,8 @@ template <typename Real, typename V> __device__ __forceinline__ V rp_vec(V r, V 
 // VEC: all four arrays 16-byte aligned -> 128-bit streaming loads/stores, two vectors per thread in flight.
 template <typename Real, bool VEC, bool COUNT>
 __global__ void __launch_bounds__(kRpThreads)
-cool_radpress_kernel(const Real *__restrict__ rho, const Real *__restrict__ the, const Real *__restrict__ hs,
-                     Real *__restrict__ out, long long ncell, RpConst K, unsigned long long *__restrict__ ncorrected)
+cool_radpress_kernel(const Real *__restrict__ rho, const Real *the, const Real *__restrict__ hs,
+                     Real *out, long long ncell, RpConst K, unsigned long long *__restrict__ ncorrected)
 {
     const Real ct = (Real)K.c_tau, cb = (Real)K.c_beta, tc = (Real)K.tau_crit;
     int cnt = 0;
