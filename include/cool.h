@@ -203,6 +203,23 @@ cool_status cool_apply(const cool_table *table, const cool_cells *cells, const c
 cool_status cool_apply_host(const cool_table *table, const cool_cells *host_cells, const cool_params *params,
                             cool_diag *h_diag);
 
+/* cool_apply for callers that cannot allocate (CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc).
+ * Same arguments, same kernels, same results as cool_apply (DEVICE arrays, asynchronous on `cuda_stream`), but the scratch
+ * memory the step needs — the per-block partial sums and the ticket of the luminosity diagnostic (eq 22), and the work lists
+ * of the precise pass — lives in ONE file-scope device array of COOL_NOALLOC_SCRATCH_BYTES that every GPU which loads the
+ * library holds until the process exits.  The call runs no cudaMalloc, cudaFree or allocating library routine.
+ * Limits: cells->ncell <= COOL_NOALLOC_MAX_CELLS and no radial profile (cells->lum_shell must be NULL); beyond them the call
+ * returns COOL_EINVAL / COOL_EUNSUPPORTED with a message in cool_last_error() and launches nothing.
+ * Sharing: every call on a device uses the same array, whatever the table or the stream, and the array keeps the last call's
+ * contents (the call clears what must start at zero, on `cuda_stream`).  Calls that overlap on the GPU — different streams
+ * without an ordering between them — RACE on it: order them (one stream, or events), or use cool_apply.
+ * The first call on a device resolves the array's device address (cudaGetSymbolAddress); make that call — ncell = 0 will
+ * do — before starting a graph capture. */
+#define COOL_NOALLOC_MAX_CELLS (1ll << 24)
+#define COOL_NOALLOC_SCRATCH_BYTES (4u << 20)
+cool_status cool_apply_noalloc(const cool_table *table, const cool_cells *cells, const cool_params *params,
+                               cool_diag *d_diag, void *cuda_stream);
+
 /* Which variant COOL_V_AUTO resolves to for this table (always a concrete variant). */
 cool_variant cool_table_auto_variant(const cool_table *table);
 

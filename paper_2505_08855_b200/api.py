@@ -75,7 +75,8 @@ class cool_diag(C.Structure):
 DIAG_BYTES = C.sizeof(cool_diag)
 EXPORTS = ("cool_table_build_host", "cool_table_create", "cool_apply", "cool_apply_host",
            "cool_table_auto_variant", "cool_last_launch_count", "cool_table_destroy",
-           "cool_last_error", "cool_version", "cool_radpress_correct", "cool_last_kernel_name", "cool_table_build_device")
+           "cool_last_error", "cool_version", "cool_radpress_correct", "cool_last_kernel_name", "cool_table_build_device",
+           "cool_apply_noalloc")
 
 _lib = None
 
@@ -96,6 +97,8 @@ def lib():
         L.cool_table_create.argtypes = [C.POINTER(cool_table_desc), C.c_int, C.POINTER(C.c_void_p)]
         L.cool_apply.restype = C.c_int
         L.cool_apply.argtypes = [C.c_void_p, C.POINTER(cool_cells), C.POINTER(cool_params), C.c_void_p, C.c_void_p]
+        L.cool_apply_noalloc.restype = C.c_int
+        L.cool_apply_noalloc.argtypes = [C.c_void_p, C.POINTER(cool_cells), C.POINTER(cool_params), C.c_void_p, C.c_void_p]
         L.cool_apply_host.restype = C.c_int
         L.cool_apply_host.argtypes = [C.c_void_p, C.POINTER(cool_cells), C.POINTER(cool_params), C.POINTER(cool_diag)]
         L.cool_table_auto_variant.restype = C.c_int
@@ -255,6 +258,18 @@ def cool_apply(table: CoolTable, ncell, dtype, rho, bsq, theta_e_in, theta_i_in,
     ``flags``: optional device uint8 array of ncell per-cell event flags (see include/cool.h)."""
     c = _cells(ncell, dtype, rho, bsq, theta_e_in, theta_i_in, theta_e_out, theta_i_out, r, vol, shell_cells, lum_shell, flags)
     _check(lib().cool_apply(table.handle, C.byref(c), C.byref(params), _ptr(d_diag), stream))
+
+
+COOL_NOALLOC_MAX_CELLS = 1 << 24
+COOL_NOALLOC_SCRATCH_BYTES = 4 << 20
+
+
+def cool_apply_noalloc(table: CoolTable, ncell, dtype, rho, bsq, theta_e_in, theta_i_in, theta_e_out, theta_i_out,
+                       params: cool_params, r=None, vol=None, d_diag=None, stream=None, flags=None):
+    """``cool_apply`` with the step's scratch in a static device array: no allocation inside the call (include/cool.h).
+    At most COOL_NOALLOC_MAX_CELLS cells, no radial profile; calls that overlap on the GPU race on the shared scratch."""
+    c = _cells(ncell, dtype, rho, bsq, theta_e_in, theta_i_in, theta_e_out, theta_i_out, r, vol, 0, None, flags)
+    _check(lib().cool_apply_noalloc(table.handle, C.byref(c), C.byref(params), _ptr(d_diag), stream))
 
 
 def cool_apply_host(table: CoolTable, ncell, dtype, rho, bsq, theta_e_in, theta_i_in, theta_e_out, theta_i_out,

@@ -635,6 +635,81 @@ extern "C" cool_status cool_apply(const cool_table *t, const cool_cells *c, cons
     return launch_step(t, v, c->dtype, a, st, &g_launches);
 }
 
+// ------------------------------------------------------------------------------------------
+// cool_apply_noalloc (include/cool.h): the step with its scratch in a file-scope device array instead of the per-stream
+// workspace get_diag_ws() allocates.  Layout: [0, 256) the ticket | per-block partial sums | precise-pass lists.
+// In host code `g_noalloc_scratch` is only a stand-in for the symbol: its device address comes from cudaGetSymbolAddress,
+// once per device, with that device current.
+// ------------------------------------------------------------------------------------------
+static __device__ __align__(256) unsigned char g_noalloc_scratch[COOL_NOALLOC_SCRATCH_BYTES];
+
+namespace cool {
+constexpr int kNoAllocMaxDevices = 64;
+static std::mutex g_noalloc_mu;
+static unsigned char *g_noalloc_ptr[kNoAllocMaxDevices] = {};
+
+// device address of the scratch array on the CURRENT device (`device`)
+static cool_status noalloc_scratch(int device, unsigned char **out)
+{
+    if (device < 0 || device >= kNoAllocMaxDevices) { set_error("cool_apply_noalloc: device index %d out of range", device); return COOL_EINVAL; }
+    std::lock_guard<std::mutex> lk(g_noalloc_mu);
+    if (!g_noalloc_ptr[device]) {
+        void *ptr = nullptr;
+        cudaError_t e = cudaGetSymbolAddress(&ptr, g_noalloc_scratch);
+        if (e != cudaSuccess || !ptr) { set_error("cudaGetSymbolAddress(no-alloc scratch): %s", cudaGetErrorString(e)); return COOL_ECUDA; }
+        g_noalloc_ptr[device] = (unsigned char *)ptr;
+    }
+    *out = g_noalloc_ptr[device];
+    return COOL_OK;
+}
+}  // namespace cool
+
+extern "C" cool_status cool_apply_noalloc(const cool_table *t, const cool_cells *c, const cool_params *p, cool_diag *d_diag, void *stream)
+{
+    g_launches = 0;
+    cool_variant v; int coul;
+    cool_status s = check_args(t, c, p, &v, &coul);
+    if (s != COOL_OK) return s;
+    if (c->ncell > COOL_NOALLOC_MAX_CELLS) {
+        set_error("cool_apply_noalloc: ncell = %lld exceeds COOL_NOALLOC_MAX_CELLS = %lld (split the batch or use cool_apply)", c->ncell, (long long)COOL_NOALLOC_MAX_CELLS);
+        return COOL_EINVAL;
+    }
+    if (c->lum_shell) { set_error("cool_apply_noalloc: the radial profile (lum_shell) needs a workspace that grows with the shells; use cool_apply"); return COOL_EUNSUPPORTED; }
+    if (c->flags && !d_diag) { set_error("flags needs d_diag"); return COOL_EINVAL; }
+    DeviceGuard dg;
+    CUDA_TRY(dg.enter(t->device), "cudaSetDevice");
+    unsigned char *scratch = nullptr;
+    s = noalloc_scratch(t->device, &scratch);
+    if (s != COOL_OK) return s;
+    cudaStream_t st = (cudaStream_t)stream;
+    LaunchArgs a{};
+    a.ncell = c->ncell; a.rho = c->rho; a.bsq = c->bsq; a.the_in = c->theta_e_in; a.thi_in = c->theta_i_in;
+    a.r = c->r; a.vol = c->vol; a.the_out = c->theta_e_out; a.thi_out = c->theta_i_out;
+    a.dt = p->dt; a.nsub = p->nsub; a.f_limit = p->f_limit; a.h_floor = p->h_floor; a.coulomb = coul; a.scheme = p->scheme;
+    a.want_diag = d_diag != nullptr; a.d_diag = d_diag;
+    a.flags = c->flags;
+    if (c->ncell == 0) {
+        if (d_diag) CUDA_TRY(cudaMemsetAsync(d_diag, 0, sizeof(cool_diag), st), "cudaMemsetAsync(diag)");
+        return COOL_OK;
+    }
+    const bool fix = uses_fixmap(t, v, c->dtype, a);
+    const size_t part_off = 256, part_bytes = sizeof(double) * 8 * (size_t)t->sm_count * 32;      // as get_diag_ws sizes them
+    const size_t fix_off = (part_off + part_bytes + 255) & ~(size_t)255;
+    const size_t need = fix_off + (fix ? fixmap_bytes(t, c->ncell) : 0);
+    if (need > (size_t)COOL_NOALLOC_SCRATCH_BYTES) {
+        set_error("cool_apply_noalloc: this launch needs %zu bytes of scratch, the static array holds %u", need, (unsigned)COOL_NOALLOC_SCRATCH_BYTES);
+        return COOL_EINVAL;
+    }
+    if (d_diag || fix) {
+        a.ticket = (unsigned *)scratch; a.partials = (double *)(scratch + part_off);
+        // the array keeps the last call's contents: the ticket must start at zero (the kernels leave it at zero, but a
+        // launch that failed half way would not have)
+        CUDA_TRY(cudaMemsetAsync(a.ticket, 0, sizeof(unsigned), st), "cudaMemsetAsync(no-alloc ticket)");
+    }
+    if (fix) a.fixmap = (unsigned *)(scratch + fix_off);       // every list counter is written by every launch: nothing to clear
+    return launch_step(t, v, c->dtype, a, st, &g_launches);
+}
+
 extern "C" cool_status cool_apply_host(const cool_table *t, const cool_cells *c, const cool_params *p, cool_diag *h_diag)
 {
     g_launches = 0;
