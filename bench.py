@@ -396,6 +396,19 @@ def run_cgs(args, rank, local_rank, world):
         del idx, Te, ne, B, H, the, thi, p, cs, r
         label = f"App. A replay: {N}^4 = {ncell} lookups on a regular (H_th, B, n_e, T_e) grid, table {ntab}^4, one cooling step per query (Coulomb off)"
         dt, coul = 1e-6, api.COOL_COULOMB_OFF
+    elif args.workload == "p100w":
+        # queries spread over the WHOLE table (log-uniform in B, n_e, T_e over the paper's ranges, radii over four decades so
+        # that H_th = c_s/Omega_K spreads too): unphysical as a simulation state, but the one workload whose table reads
+        # do not stay inside an L2-resident corner of the 400 MB table
+        ncell = 1 << 26
+        u64 = lambda lo, hi: 10.0 ** (lo + (hi - lo) * torch.rand(ncell, device=dev, generator=g, dtype=torch.float64))
+        ne, B, Te = u64(CGS_LO[2], CGS_HI[2]), u64(CGS_LO[1], CGS_HI[1]), u64(CGS_LO[3], CGS_HI[3])
+        the = Te * KB / (ME * C * C)
+        d = dict(rho=ne * MP / rs, bsq=B * B / (4.0 * np.pi * rs * C * C), theta_e=the, theta_i=the, r=u64(0.0, 4.0))
+        d = {k: v.to(torch.float32) for k, v in d.items()}
+        del ne, B, Te, the
+        label = f"2^26 fp32 cells log-uniform over the WHOLE (B, n_e, T_e) range of the paper's {ntab}^4 table ({4 * ntab ** 4 / 1e6:.0f} MB), radii 1-10^4 r_g, single update"
+        dt, coul = 1e-3, api.COOL_COULOMB_TABLE
     else:
         ncell = 1 << 26
         u = lambda lo, hi: 10.0 ** (lo + (hi - lo) * torch.rand(ncell, device=dev, generator=g, dtype=torch.float32))
@@ -484,7 +497,7 @@ def main():
     world = int(os.environ.get("WORLD_SIZE", "1"))
     if args.workload == "rp512":
         return run_radpress(args, rank, local_rank, world)
-    if args.workload == "p100" or args.workload.startswith("appA-"):
+    if args.workload in ("p100", "p100w") or args.workload.startswith("appA-"):
         return run_cgs(args, rank, local_rank, world)
     spec = workload_spec(args.workload)
     axis, lo, hi = table_ranges(spec["n"])
