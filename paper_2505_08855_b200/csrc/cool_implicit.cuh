@@ -347,12 +347,14 @@ constexpr float kImpF32Rate = 0.03f;      // radiated fraction h Lambda/u_e belo
 template <int MODE, class Fetch>
 __device__ void implicit_cell_f32(const DevTable &T, const StepConst &S, const F32Const &S32, const Fetch &F,
                                   float rho, float bsq, float &the, float &thi, float r, float vol, DiagAcc &acc, long long cell,
-                                  unsigned char *flags, double k0d)                 // k0d = log2 h in fp64
+                                  unsigned char *flags, double k0d, bool want_diag)   // k0d = log2 h in fp64
 {
-    if (flags) flags[cell] = 0;
     const float chk = (bsq + the) + (thi + rho);
-    if (chk != chk) { the = thi = __int_as_float(0x7fc00000); return; }
-    if (!(rho > 0.f)) return;
+    if (chk != chk || !(rho > 0.f)) {                // NaN in -> NaN out, no matter -> unchanged; no events
+        if (chk != chk) the = thi = __int_as_float(0x7fc00000);
+        if (flags) flags[cell] = 0;
+        return;
+    }
     const int one_bits = 0x3f800000;
     const AxisCoef &ax = T.ax[CAX_THE];
     const int n = ax.n;
@@ -382,7 +384,7 @@ __device__ void implicit_cell_f32(const DevTable &T, const StepConst &S, const F
         Imp32 c;
         c.rho = rho; c.thi0 = thi; c.q = a / (1.f + a * g); c.R = fmaf(c.q, thi, the); c.opq = 1.f + c.q;
         c.kc = lr.d * T.ax[CAX_RHO].d2f; c.hf = ex2_approx(S32.k0);
-        const double kd = (double)lr.d * (double)T.ax[CAX_RHO].d2f + k0d;
+        auto kd_of = [&]() { return (double)lr.d * (double)T.ax[CAX_RHO].d2f + k0d; };     // log2 h + clamp term, fp64: only the fp64-exponent paths form it
         if (!(c.R > 0.f)) continue;
         float theta, rate = 0.f, frac[3] = {0.f, 0.f, 0.f};
         if (flo) {
@@ -392,13 +394,15 @@ __device__ void implicit_cell_f32(const DevTable &T, const StepConst &S, const F
             const int imax = tR >= (float)(n - 1) ? n - 1 : (tR < 0.f ? -1 : (int)tR);
             int ilo = -1, ihi = imax + 1;
             float ya[3] = {0.f, 0.f, 0.f}, yb[3] = {0.f, 0.f, 0.f};
+            float ra = 0.f, ta = 0.f;                        // rate and Theta_e at node ilo, as the probe that set ilo computed them
             bool have_b = false;
             auto probe = [&](int m) {                        // F at node m; narrows [ilo, ihi]; true when F < 0 there
                 float ym[3];
                 imp32_node<MODE>(F, lr, lb, li, ir, ib, iii, m, ym);
                 const float tm = node_theta(m);
-                const float fm = fmaf(tm, c.opq, -c.R) + tm * imp32_rate<MODE>(S32, c, tm, ym, nullptr);
-                if (fm < 0.f) { ilo = m; ya[0] = ym[0]; ya[1] = ym[1]; ya[2] = ym[2]; return true; }
+                const float rm = imp32_rate<MODE>(S32, c, tm, ym, nullptr);
+                const float fm = fmaf(tm, c.opq, -c.R) + tm * rm;
+                if (fm < 0.f) { ilo = m; ya[0] = ym[0]; ya[1] = ym[1]; ya[2] = ym[2]; ra = rm; ta = tm; return true; }
                 ihi = m; yb[0] = ym[0]; yb[1] = ym[1]; yb[2] = ym[2]; have_b = true;
                 return false;
             };
@@ -416,25 +420,22 @@ __device__ void implicit_cell_f32(const DevTable &T, const StepConst &S, const F
                 const float te = node_theta(e);
                 double yed[3];
                 imp_node_d<MODE>(F, lr, lb, li, ir, ib, iii, e, yed);
-                rate = imp32_rate_d<MODE>(S32, c, te, yed, kd, frac);           // cooling time held outside the range
+                rate = imp32_rate_d<MODE>(S32, c, te, yed, kd_of(), frac);           // cooling time held outside the range
                 theta = c.R / (c.opq + rate);
                 clamped = true;
             } else {
                 if (!have_b) imp32_node<MODE>(F, lr, lb, li, ir, ib, iii, ilo + 1, yb);
                 const float dy[3] = {yb[0] - ya[0], yb[1] - ya[1], yb[2] - ya[2]};
-                float lo = node_theta(ilo), hi = fminf(node_theta(ilo + 1), c.R);
+                float lo = ta, hi = fminf(node_theta(ilo + 1), c.R);
                 // The root moves with the rate by d ln(theta) = -[rate/(opq + rate)] d ln(rate), and fp32 exponents give the rate to
                 // <= 1e-4 even in the steepest interval (5e-6 nodes x 16 log2 units), so where the radiated fraction is below
-                // kImpF32Rate over the whole interval the fp32 rate holds 1e-5 with a wide margin; elsewhere the bracketing
-                // nodes are contracted once more in fp64 and the exponent is summed in fp64.
-                const bool f32ok = fmaxf(imp32_rate<MODE>(S32, c, lo, ya, nullptr), imp32_rate<MODE>(S32, c, node_theta(ilo + 1), yb, nullptr)) < kImpF32Rate;
-                double yad[3] = {0.0, 0.0, 0.0}, dyd[3] = {0.0, 0.0, 0.0};
-                if (!f32ok) {
-                    double ybd[3];
-                    imp_node_d<MODE>(F, lr, lb, li, ir, ib, iii, ilo, yad);
-                    imp_node_d<MODE>(F, lr, lb, li, ir, ib, iii, ilo + 1, ybd);
-                    dyd[0] = ybd[0] - yad[0]; dyd[1] = ybd[1] - yad[1]; dyd[2] = ybd[2] - yad[2];
-                }
+                // kImpF32Rate over the bracket [lo, hi] the fp32 rate holds 1e-5 with a wide margin; elsewhere the bracketing
+                // nodes are contracted once more in fp64 and the exponent is summed in fp64.  Inside a table interval every process
+                // is a power law of Theta_e, so the bracket's two ends bound the rate (the bridged sum of a 4-D table can exceed both
+                // only marginally; the threshold leaves a factor 3): the lower end is what the probe of node ilo computed, the
+                // upper end is the first evaluation of the iteration anyway.
+                bool f32ok = true;
+                double yad[3] = {0.0, 0.0, 0.0}, dyd[3] = {0.0, 0.0, 0.0}, kd = 0.0;
                 auto Rate = [&](float th, float *fr) {
                     const float w32 = fminf(fmaxf(coord32(ax, th, one_bits) - (float)ilo, 0.f), 1.f);
                     if (f32ok) {
@@ -450,10 +451,20 @@ __device__ void implicit_cell_f32(const DevTable &T, const StepConst &S, const F
                                                                 // (F' >= opq + rate where the rate does not fall with Theta_e, so
                                                                 // the error in theta is <= ulp(theta))
                 float rhi = Rate(hi, nullptr);
+                float flo0 = fmaf(lo, c.opq, -c.R) + lo * ra;                  // < 0: that is how the probe chose ilo
+                if (!(fmaxf(ra, rhi) < kImpF32Rate)) {
+                    double ybd[3];
+                    imp_node_d<MODE>(F, lr, lb, li, ir, ib, iii, ilo, yad);
+                    imp_node_d<MODE>(F, lr, lb, li, ir, ib, iii, ilo + 1, ybd);
+                    dyd[0] = ybd[0] - yad[0]; dyd[1] = ybd[1] - yad[1]; dyd[2] = ybd[2] - yad[2];
+                    f32ok = false; kd = kd_of();
+                    rhi = Rate(hi, nullptr);
+                    flo0 = fmaf(lo, c.opq, -c.R) + lo * Rate(lo, nullptr);
+                }
                 float fhi = fmaf(hi, c.opq, -c.R) + hi * rhi;
+                float rate_hi = rhi;                            // the rate at `hi` wherever the iteration leaves it (3-D tables)
                 if (fhi > noise) {
-                    const float flo0 = fmaf(lo, c.opq, -c.R) + lo * Rate(lo, nullptr);
-                    if (!(flo0 < 0.f)) { hi = lo; fhi = 0.f; }                  // rounding at the lower node: it is the root
+                    if (!(flo0 < 0.f)) { hi = lo; fhi = 0.f; rhi = f32ok ? ra : Rate(lo, nullptr); rate_hi = rhi; }   // rounding at the lower node: it is the root
                     if constexpr (MODE == 3) {
                         // inside the interval the rate is an exact power law, rate ~ theta^p with p = dy invf, so
                         // F' = opq + rate (1 + p): Newton steps, kept inside the bracket
@@ -470,7 +481,7 @@ __device__ void implicit_cell_f32(const DevTable &T, const StepConst &S, const F
                             x = m; fx = fm; rx = rm;
                             if (done) break;
                         }
-                        hi = x;
+                        hi = x; rate_hi = rx;
                     } else {
                         float flo_ = flo0;
                         int side = 0, stall = 0;
@@ -489,7 +500,8 @@ __device__ void implicit_cell_f32(const DevTable &T, const StepConst &S, const F
                     }
                 }
                 theta = hi;
-                rate = Rate(theta, frac);
+                if constexpr (MODE == 3) rate = rate_hi;        // no process split on a 3-D table: the last evaluation is the rate at theta
+                else rate = Rate(theta, frac);
             }
         }
         const float de = theta * rate;
@@ -498,17 +510,24 @@ __device__ void implicit_cell_f32(const DevTable &T, const StepConst &S, const F
         thi = fmaf(g * a, theta, thi) / fmaf(a, g, 1.f);
         the = theta;
     }
+    if (!want_diag) return;                          // kernel argument: warp-uniform
     const double wgt = (double)rho * (double)vol;
     const double ds[4] = {(double)de_sum[0], (double)de_sum[1], (double)de_sum[2], (double)de_sum[3]};
 #pragma unroll
-    for (int k = 0; k < 4; ++k) acc.lum[k] += ds[k] * wgt;
+    for (int k = 0; k < (MODE == 4 ? 4 : 1); ++k) acc.lum[k] += ds[k] * wgt;      // no process split on a 3-D table
     acc.flo += floored; acc.cla += clamped ? 1 : 0;
     shell_add(S, cell, ds, wgt, MODE == 4);
     if (flags) flags[cell] = (unsigned char)((floored << 1) | (clamped ? 4 : 0));
 }
 
+#ifndef COOL_IMP_MINB3
+#define COOL_IMP_MINB3 3
+#endif
+#ifndef COOL_IMP_MINB4
+#define COOL_IMP_MINB4 2
+#endif
 template <int MODE, class Fetch, int THREADS>
-__global__ void __launch_bounds__(THREADS)
+__global__ void __launch_bounds__(THREADS, MODE == 3 ? COOL_IMP_MINB3 : COOL_IMP_MINB4)
 cool_implicit_f32_kernel(const DevTable T, const StepConst S, const F32Const S32, const CellPtrs C, double *partials, unsigned *ticket, cool_diag *d_diag)
 {
     extern __shared__ __align__(16) unsigned char smem_imp32[];
@@ -533,7 +552,7 @@ cool_implicit_f32_kernel(const DevTable T, const StepConst S, const F32Const S32
         float the = n_the, thi = n_thi;
         const float rho = n_rho, bsq = n_bsq, rr = n_rr, vv = n_vv;
         if (c + stride < C.ncell) fetch(c + stride);
-        implicit_cell_f32<MODE, Fetch>(T, S, S32, F, rho, bsq, the, thi, rr, vv, acc, c, d_diag ? C.flags : nullptr, k0d);
+        implicit_cell_f32<MODE, Fetch>(T, S, S32, F, rho, bsq, the, thi, rr, vv, acc, c, d_diag ? C.flags : nullptr, k0d, d_diag != nullptr);
         __stcs((float *)C.the_out + c, the);
         __stcs((float *)C.thi_out + c, thi);
     }
