@@ -254,6 +254,19 @@ __device__ __forceinline__ void imp32_node(const Fetch &F, const Loc32 &r, const
     }
 }
 
+// 3-D tables in global memory with the quad layout (cool_internal.h: q3[r][e][b] = {T'(r,e,b), T'(r,e,b+1), T'(r,e+1,b),
+// T'(r,e+1,b+1)}, edges duplicated): the column values at Theta_e nodes i AND i+1 from two 128-bit loads — a probe of node
+// i brings the other end of its interval along, which is the whole bracket when the root lies in the interval below R.
+__device__ __forceinline__ void imp32_pair3(const float4 *q3, int sr, int se, const Loc32 &r, const Loc32 &b, int ir, int ib, int i, float &y_i, float &y_i1)
+{
+    const float4 *p = q3 + (unsigned)(ir * sr + i * se + ib);
+    const float4 q0 = ldg_f4(p), q1 = ldg_f4(p + sr);
+    y_i = lerp(r.w, lerp(b.w, q0.x, q0.y), lerp(b.w, q1.x, q1.y));
+    y_i1 = lerp(r.w, lerp(b.w, q0.z, q0.w), lerp(b.w, q1.z, q1.w));
+}
+template <int MODE, class Fetch> struct ImpPairFetch { static constexpr bool value = false; };
+template <> struct ImpPairFetch<3, FetchGlobal> { static constexpr bool value = true; };
+
 // loss(th)/th = h Lambda(th_c)/u_e(th_c) from the channel values y at th_c; optional process shares
 template <int MODE>
 __device__ __forceinline__ float imp32_rate(const F32Const &S, const Imp32 &c, float thc, const float (&y)[3], float *frac)
@@ -396,9 +409,12 @@ __device__ void implicit_cell_f32(const DevTable &T, const StepConst &S, const F
             float ya[3] = {0.f, 0.f, 0.f}, yb[3] = {0.f, 0.f, 0.f};
             float ra = 0.f, ta = 0.f;                        // rate and Theta_e at node ilo, as the probe that set ilo computed them
             bool have_b = false;
+            const bool pair = ImpPairFetch<MODE, Fetch>::value && T.q3 != nullptr;       // warp-uniform
+            int pa_idx = -2; float pa_lo = 0.f, pa_hi = 0.f;                            // the last pair loaded: nodes pa_idx, pa_idx + 1
             auto probe = [&](int m) {                        // F at node m; narrows [ilo, ihi]; true when F < 0 there
                 float ym[3];
-                imp32_node<MODE>(F, lr, lb, li, ir, ib, iii, m, ym);
+                if (pair) { imp32_pair3(T.q3, T.s_rho, T.s_the, lr, lb, ir, ib, m, pa_lo, pa_hi); pa_idx = m; ym[0] = pa_lo; ym[1] = ym[2] = 0.f; }
+                else imp32_node<MODE>(F, lr, lb, li, ir, ib, iii, m, ym);
                 const float tm = node_theta(m);
                 const float rm = imp32_rate<MODE>(S32, c, tm, ym, nullptr);
                 const float fm = fmaf(tm, c.opq, -c.R) + tm * rm;
@@ -424,7 +440,10 @@ __device__ void implicit_cell_f32(const DevTable &T, const StepConst &S, const F
                 theta = c.R / (c.opq + rate);
                 clamped = true;
             } else {
-                if (!have_b) imp32_node<MODE>(F, lr, lb, li, ir, ib, iii, ilo + 1, yb);
+                if (pair) {
+                    if (pa_idx != ilo) imp32_pair3(T.q3, T.s_rho, T.s_the, lr, lb, ir, ib, ilo, pa_lo, pa_hi);
+                    ya[0] = pa_lo; yb[0] = pa_hi;
+                } else if (!have_b) imp32_node<MODE>(F, lr, lb, li, ir, ib, iii, ilo + 1, yb);
                 const float dy[3] = {yb[0] - ya[0], yb[1] - ya[1], yb[2] - ya[2]};
                 float lo = ta, hi = fminf(node_theta(ilo + 1), c.R);
                 // The root moves with the rate by d ln(theta) = -[rate/(opq + rate)] d ln(rate), and fp32 exponents give the rate to
