@@ -15,7 +15,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJDIR = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libcool_b200.so")
-SOURCES = ["cool_api.cu", "cool_builder.cu", "cool_launch.cu", "cool_inst_f32_m3.cu", "cool_inst_f32_m4.cu",
+SOURCES = ["cool_api.cu", "cool_builder.cu", "cool_launch.cu", "cool_inst_f32_m3.cu", "cool_inst_f32_m3f.cu", "cool_inst_f32_m4.cu", "cool_inst_f32_m4f.cu",
            "cool_inst_f64.cu", "cool_inst_analytic.cu", "cool_inst_implicit.cu", "cool_radpress.cu", "cool_fix.cu", "cool_cgs.cu"]
 HEADERS = ["cool_internal.h", "cool_physics.cuh", "cool_kernels.cuh", "cool_f32.cuh", "cool_implicit.cuh", os.path.join("..", "..", "include", "cool.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",

@@ -445,7 +445,7 @@ __device__ __forceinline__ void shell_flush(const F32Const &S, const float (&par
 template <class Fetch, int CM>
 __host__ __device__ constexpr bool coul_quads() { return CM == 1 && !Fetch::kSmem; }
 
-struct Ctx32 { const DevTable &T; const F32Const &S; unsigned coul_s; bool want_flags; };      // coul_s: shared-memory address of the staged Coulomb quads
+struct Ctx32 { const DevTable &T; const F32Const &S; unsigned coul_s; };      // coul_s: shared-memory address of the staged Coulomb quads
 
 // ------------------------------------------------------------------------------------------
 // NV cells of one thread through all sub-steps, straight-line (no per-cell branches except the
@@ -482,7 +482,10 @@ static __device__ __noinline__ float precise_rate3(const float *f1, int s_rho, i
 // FIXT: test every cell at every sub-step for the precise pass (F32Const::band_*).  MODE 3 only; the 4-D step tests inside its
 // patch-rebuild branch instead (cells in or next to the steep interval rebuild their patch every sub-step), which costs the
 // sub-step loop nothing.
-template <int MODE, class Fetch, bool DIAG, int CM, bool NSUB1, int NV, bool FIXT>
+// WF: also form the per-cell event flags (cool_cells::flags).  Compile time, because keeping the three event predicates of
+// every cell alive to the end of the step costs the diagnostics kernels registers they do not have (s512f: 11 % with the
+// flags merely possible); only tests and callers that pass a flags array get the WF instantiations.
+template <int MODE, class Fetch, bool DIAG, int CM, bool NSUB1, int NV, bool FIXT, bool WF>
 __device__ __forceinline__ void step_cells_f32(const Ctx32 &X, const Fetch &F, const float *rho, const float *bsq, float *the, float *thi,
                                                const float *rr, const float *vol, DiagAcc &acc, float (&tile_part)[4], unsigned wtile,
                                                unsigned &flagword)   // byte j: event flags of cell j (include/cool.h); bit 3 = left to the precise pass
@@ -687,24 +690,15 @@ __device__ __forceinline__ void step_cells_f32(const Ctx32 &X, const Fetch &F, c
             if (floored[j] && !bad[j]) ++acc.flo;
             if (clamped[j] && !bad[j]) ++acc.cla;
         }
-        if (X.want_flags) {                                     // per-cell event flags (cool_cells::flags): tests and callers that ask
+        if constexpr (WF) {                                     // per-cell event flags (cool_cells::flags): tests and callers that ask
 #pragma unroll
             for (int j = 0; j < NV; ++j)
                 if (!bad[j]) flagword |= ((limited[j] ? 1u : 0u) | (floored[j] ? 2u : 0u) | (clamped[j] ? 4u : 0u)) << (8 * j);
         }
-        if constexpr (NV == 1) {
-            // one cell of the tile (4-D kernel): the caller gathers the tile's terms, adds them to the fp64 sums and flushes
-            // them once per tile (four cells summed in fp32 first, as the 3-D kernel does: the fp64 pipe is narrow)
+        // the caller adds the tile's terms (the NV cells summed in fp32 first: the fp64 pipe is narrow) to its fp64 sums and
+        // flushes them to the radial profile once per tile
 #pragma unroll
-            for (int k = 0; k < 4; ++k) tile_part[k] = part[k];
-        } else {
-            acc.lum[0] += (double)part[0];
-            if constexpr (MODE == 4) {
-#pragma unroll
-                for (int k = 1; k < 4; ++k) acc.lum[k] += (double)part[k];
-            }
-            if (S.lum_shell) shell_flush<MODE>(S, part, wtile);
-        }
+        for (int k = 0; k < 4; ++k) tile_part[k] = part[k];
     }
 }
 
@@ -718,7 +712,7 @@ constexpr unsigned kWarpArrBytes = kWarpTile * 4u;          // 512 B per array p
 constexpr unsigned kF32BarBytes = 1024;                     // room for 32 warps x 2 stages of 8-byte mbarriers, 32 list counters, the Coulomb barrier
 constexpr unsigned kF32FixCntOff = 768;                     // per-warp count of tiles listed for the precise pass (32 x 4 bytes)
 
-template <int MODE, class Fetch, bool DIAG, int CM, bool NSUB1, int THREADS, int NST>
+template <int MODE, class Fetch, bool DIAG, int CM, bool NSUB1, int THREADS, int NST, bool WF>
 __global__ void __launch_bounds__(THREADS, 1)
 cool_f32_kernel(const DevTable T, const F32Const S, const CellPtrs C, double *partials, unsigned *ticket, cool_diag *d_diag)
 {
@@ -760,7 +754,8 @@ cool_f32_kernel(const DevTable T, const F32Const S, const CellPtrs C, double *pa
     }
     __syncthreads();
     const Fetch F(T, smem_f32 + S.table_off);
-    const Ctx32 X{T, S, smem_u32(smem_f32 + S.coul_off), DIAG && C.flags != nullptr};
+    static_assert(DIAG || !WF, "per-cell flags come with the diagnostics");
+    const Ctx32 X{T, S, smem_u32(smem_f32 + S.coul_off)};
 
     const long long ncell = C.ncell;
     const long long ntiles = (ncell + kWarpTile - 1) / kWarpTile;
@@ -794,6 +789,13 @@ cool_f32_kernel(const DevTable T, const F32Const S, const CellPtrs C, double *pa
 
     if (CM >= 1 && S.coul_smem) mbar_wait(cbar, 0);
     DiagAcc acc;
+    // The fp64 luminosity sums are touched once per tile: they live in local memory (L1), not in registers, on purpose.  The
+    // diagnostics kernels sit at their register caps, and left to itself the compiler spills either these (harmless) or a
+    // value inside the step (s512d: 0.81 vs 0.93 ms), depending on unrelated details of the source.
+    constexpr int NLUM = MODE == 4 ? 4 : 1;                 // a 3-D table has no process split
+    volatile double lumv[NLUM];
+#pragma unroll
+    for (int k = 0; k < NLUM; ++k) lumv[k] = 0.0;
     int s = 0; unsigned phase = 0;
     for (; tile < ntiles; tile += GW) {
         const long long c = tile * kWarpTile + (long long)lane * kF32CellsPerThread;
@@ -830,7 +832,7 @@ cool_f32_kernel(const DevTable T, const F32Const S, const CellPtrs C, double *pa
 #pragma unroll 1
             for (int j = 0; j < kF32CellsPerThread; ++j) {
                 unsigned fw1;
-                step_cells_f32<MODE, Fetch, DIAG, CM, NSUB1, 1, true>(X, F, &rho.x, &bsq.x, &the.x, &thi.x, &rr.x, &vv.x, acc, tp, (unsigned)tile, fw1);
+                step_cells_f32<MODE, Fetch, DIAG, CM, NSUB1, 1, true, WF>(X, F, &rho.x, &bsq.x, &the.x, &thi.x, &rr.x, &vv.x, acc, tp, (unsigned)tile, fw1);
                 if (fw1) flagword |= fw1 << (8 * j);        // rare
                 // a finished cell's rho, bsq, vol and r slots are dead: they carry its four luminosity terms to the end of the tile
                 if constexpr (DIAG) { rho.x = tp[0]; bsq.x = tp[1]; vv.x = tp[2]; rr.x = tp[3]; }
@@ -839,8 +841,6 @@ cool_f32_kernel(const DevTable T, const F32Const S, const CellPtrs C, double *pa
             if constexpr (DIAG) {
                 tp[0] = (rho.x + rho.y) + (rho.z + rho.w); tp[1] = (bsq.x + bsq.y) + (bsq.z + bsq.w);
                 tp[2] = (vv.x + vv.y) + (vv.z + vv.w); tp[3] = (rr.x + rr.y) + (rr.z + rr.w);
-#pragma unroll
-                for (int k = 0; k < 4; ++k) acc.lum[k] += (double)tp[k];
             }
         } else {
             // Precise pass: a single update can only put a cell there if its INPUT Theta_e lies in the steep band, so one
@@ -855,18 +855,18 @@ cool_f32_kernel(const DevTable T, const F32Const S, const CellPtrs C, double *pa
                 tested = false;
 #endif
             }
-            if (tested) step_cells_f32<MODE, Fetch, DIAG, CM, NSUB1, kF32CellsPerThread, true>(X, F, &rho.x, &bsq.x, &the.x, &thi.x, &rr.x, &vv.x, acc, tp, (unsigned)tile, flagword);
-            else step_cells_f32<MODE, Fetch, DIAG, CM, NSUB1, kF32CellsPerThread, false>(X, F, &rho.x, &bsq.x, &the.x, &thi.x, &rr.x, &vv.x, acc, tp, (unsigned)tile, flagword);
+            if (tested) step_cells_f32<MODE, Fetch, DIAG, CM, NSUB1, kF32CellsPerThread, true, WF>(X, F, &rho.x, &bsq.x, &the.x, &thi.x, &rr.x, &vv.x, acc, tp, (unsigned)tile, flagword);
+            else step_cells_f32<MODE, Fetch, DIAG, CM, NSUB1, kF32CellsPerThread, false, WF>(X, F, &rho.x, &bsq.x, &the.x, &thi.x, &rr.x, &vv.x, acc, tp, (unsigned)tile, flagword);
         }
-        if constexpr (DIAG && MODE == 4) {
+        if constexpr (DIAG) {
+#pragma unroll
+            for (int k = 0; k < NLUM; ++k) lumv[k] = lumv[k] + (double)tp[k];
             if (S.lum_shell) shell_flush<MODE>(S, tp, (unsigned)tile);
         }
         if (full) {
             st_stream((float4 *)C.the_out + (c >> 2), the);
             st_stream((float4 *)C.thi_out + (c >> 2), thi);
-            if constexpr (DIAG) {
-                if (C.flags) *((unsigned *)(C.flags + c)) = flagword;
-            }
+            if constexpr (WF) *((unsigned *)(C.flags + c)) = flagword;
             // Re-arm the stage only now: the stores above depend on every value this warp read from it, so its
             // LDS have all returned (read-before-overwrite across the generic and async proxies).  With NST
             // stages the refill is still NST-1 tiles ahead of its use.
@@ -880,9 +880,7 @@ cool_f32_kernel(const DevTable T, const F32Const S, const CellPtrs C, double *pa
             for (int j = 0; j < kF32CellsPerThread; ++j)
                 if (c + j < ncell) {
                     ((float *)C.the_out)[c + j] = (&the.x)[j]; ((float *)C.thi_out)[c + j] = (&thi.x)[j];
-                    if constexpr (DIAG) {
-                        if (C.flags) C.flags[c + j] = (unsigned char)(flagword >> (8 * j));
-                    }
+                    if constexpr (WF) C.flags[c + j] = (unsigned char)(flagword >> (8 * j));
                 }
         }
         if constexpr (kLists) if (S.fixmap) {               // cells left to the precise pass: list the tile
@@ -902,7 +900,11 @@ cool_f32_kernel(const DevTable T, const F32Const S, const CellPtrs C, double *pa
         }
     }
     if constexpr (kLists) if (S.fixmap && lane == 0) S.fix.count[blockIdx.x * NW + warp] = *((unsigned *)(smem_f32 + kF32FixCntOff) + warp);      // every warp, every launch: no memset needed
-    if constexpr (DIAG) reduce_diag(acc, S.lum_k, partials, ticket, d_diag);
+    if constexpr (DIAG) {
+#pragma unroll
+        for (int k = 0; k < NLUM; ++k) acc.lum[k] = lumv[k];
+        reduce_diag(acc, S.lum_k, partials, ticket, d_diag);
+    }
 }
 
 // ------------------------------------------------------------------------------------------
@@ -928,12 +930,12 @@ inline size_t f32_smem_layout(F32Const &S, int threads, int nst, bool table_in_s
     return off;
 }
 
-template <int MODE, class Fetch, bool DIAG, int CM, bool NSUB1, int THREADS, int NST>
+template <int MODE, class Fetch, bool DIAG, int CM, bool NSUB1, int THREADS, int NST, bool WF>
 static cudaError_t launch_f32_one(const LaunchCtx32 &L)
 {
     F32Const S = L.S;
     const size_t smem = f32_smem_layout(S, THREADS, NST, Fetch::kSmem, coul_quads<Fetch, CM>(), L.t);
-    auto kern = cool_f32_kernel<MODE, Fetch, DIAG, CM, NSUB1, THREADS, NST>;
+    auto kern = cool_f32_kernel<MODE, Fetch, DIAG, CM, NSUB1, THREADS, NST, WF>;
     if (smem > 48 * 1024) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
@@ -948,13 +950,13 @@ static cudaError_t launch_f32_one(const LaunchCtx32 &L)
         a.fix_warps = warps; a.fix_cap = S.fix.cap;
     }
     CellPtrs C{a.rho, a.bsq, a.the_in, a.thi_in, a.r, a.vol, a.the_out, a.thi_out, a.ncell, a.flags};
-    note_kernel("cool_f32_kernel<MODE=%d,%s,DIAG=%d,CM=%d,NSUB1=%d,%dx%d>", MODE, Fetch::name(), (int)DIAG, CM, (int)NSUB1, THREADS, NST);
+    note_kernel("cool_f32_kernel<MODE=%d,%s,DIAG=%d,CM=%d,NSUB1=%d,%dx%d%s>", MODE, Fetch::name(), (int)DIAG, CM, (int)NSUB1, THREADS, NST, WF ? ",flags" : "");
     kern<<<grid, THREADS, smem, L.st>>>(L.t->dev, S, C, a.partials, a.ticket, a.d_diag);
     return cudaGetLastError();
 }
 
 // dispatch over the table variants for fixed <MODE, DIAG, CM, NSUB1>
-template <int MODE, bool DIAG, int CM, bool NSUB1>
+template <int MODE, bool DIAG, int CM, bool NSUB1, bool WF>
 static cudaError_t launch_f32_by_variant(const LaunchCtx32 &L, cool_variant v)
 {
     // The single-update 3-D step fits 80 registers: 24 warps per SM hide the gather latency (measured best on B200:
@@ -965,13 +967,13 @@ static cudaError_t launch_f32_by_variant(const LaunchCtx32 &L, cool_variant v)
     switch (v) {
         case COOL_V_GLOBAL:
             if constexpr (MODE == 3) {
-                if (L.t->dev.o3) return launch_f32_one<MODE, F32GlobalO, DIAG, CM, NSUB1, TH, NS>(L);
-                if (L.t->dev.q3) return launch_f32_one<MODE, F32GlobalQ, DIAG, CM, NSUB1, TH, NS>(L);
+                if (L.t->dev.o3) return launch_f32_one<MODE, F32GlobalO, DIAG, CM, NSUB1, TH, NS, WF>(L);
+                if (L.t->dev.q3) return launch_f32_one<MODE, F32GlobalQ, DIAG, CM, NSUB1, TH, NS, WF>(L);
             }
-            return launch_f32_one<MODE, F32Global, DIAG, CM, NSUB1, TH, NS>(L);
-        case COOL_V_TEX_POINT: return launch_f32_one<MODE, F32TexPoint, DIAG, CM, NSUB1, TH, NS>(L);
-        case COOL_V_TEX_HWFILTER: return launch_f32_one<MODE, F32TexHw, DIAG, CM, NSUB1, TH, NS>(L);
-        case COOL_V_SMEM: return launch_f32_one<MODE, F32Smem, DIAG, CM, NSUB1, kF32SmemThreads, kF32SmemStages>(L);
+            return launch_f32_one<MODE, F32Global, DIAG, CM, NSUB1, TH, NS, WF>(L);
+        case COOL_V_TEX_POINT: return launch_f32_one<MODE, F32TexPoint, DIAG, CM, NSUB1, TH, NS, WF>(L);
+        case COOL_V_TEX_HWFILTER: return launch_f32_one<MODE, F32TexHw, DIAG, CM, NSUB1, TH, NS, WF>(L);
+        case COOL_V_SMEM: return launch_f32_one<MODE, F32Smem, DIAG, CM, NSUB1, kF32SmemThreads, kF32SmemStages, WF>(L);
         default: return cudaErrorInvalidValue;
     }
 }
@@ -979,6 +981,9 @@ static cudaError_t launch_f32_by_variant(const LaunchCtx32 &L, cool_variant v)
 // one function per translation unit of instantiations (cool_inst_f32_*.cu)
 cudaError_t launch_f32_m3(const LaunchCtx32 &L, cool_variant v, bool diag, int cm, bool nsub1);
 cudaError_t launch_f32_m4(const LaunchCtx32 &L, cool_variant v, bool diag, int cm);
+// the same with per-cell event flags (diagnostics on, LaunchArgs::flags set): translation units of their own
+cudaError_t launch_f32_m3_flags(const LaunchCtx32 &L, cool_variant v, int cm, bool nsub1);
+cudaError_t launch_f32_m4_flags(const LaunchCtx32 &L, cool_variant v, int cm);
 // precise pass over the cells the fp32 launch listed in LaunchArgs::fixmap (cool_fix.cu)
 cudaError_t launch_fix(const LaunchCtx &L, int mode, bool diag);
 

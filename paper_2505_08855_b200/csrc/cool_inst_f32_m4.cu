@@ -3,7 +3,8 @@
 namespace cool {
 cudaError_t launch_f32_m4(const LaunchCtx32 &L, cool_variant v, bool diag, int cm)
 {
-    if (diag) return cm == 2 ? launch_f32_by_variant<4, true, 2, false>(L, v) : cm ? launch_f32_by_variant<4, true, 1, false>(L, v) : launch_f32_by_variant<4, true, 0, false>(L, v);
-    return cm ? launch_f32_by_variant<4, false, 1, false>(L, v) : launch_f32_by_variant<4, false, 0, false>(L, v);
+    if (diag && L.a->flags) return launch_f32_m4_flags(L, v, cm);
+    if (diag) return cm == 2 ? launch_f32_by_variant<4, true, 2, false, false>(L, v) : cm ? launch_f32_by_variant<4, true, 1, false, false>(L, v) : launch_f32_by_variant<4, true, 0, false, false>(L, v);
+    return cm ? launch_f32_by_variant<4, false, 1, false, false>(L, v) : launch_f32_by_variant<4, false, 0, false, false>(L, v);
 }
 }  // namespace cool
