@@ -57,7 +57,6 @@ struct F32Const {
     // NaN x; width 0 = empty (no precise pass).  Such a cell is treated like a cell with rho <= 0 here (passed through,
     // neither summed nor counted) and its tile is listed for the precise pass (cool_internal.h, fix_layout).
     unsigned band_lo_bits, band_w, rmin_bits, r_w;
-    int kb_lo; unsigned kb_n;         // the band's Theta_e intervals and one neighbour each side, as node-index words (Loc32::tf bits): (bits - kb_lo) < kb_n
     unsigned *fixmap;                 // NULL: no precise pass
     FixLists fix;
 };
@@ -479,9 +478,9 @@ static __device__ __noinline__ float precise_rate3(const float *f1, int s_rho, i
     return (float)scalbn((double)ex2_approx((float)(y - yi)), (int)yi);
 }
 
-// FIXT: test every cell at every sub-step for the precise pass (F32Const::band_*).  MODE 3 only; the 4-D step tests inside its
-// patch-rebuild branch instead (cells in or next to the steep interval rebuild their patch every sub-step), which costs the
-// sub-step loop nothing.
+// FIXT: test every cell at every sub-step for the precise pass (F32Const::band_*): two integer subtractions and two unsigned
+// compares on values that are live anyway.  (The 4-D step used to test inside its patch-rebuild branch only, with the cells in
+// or next to the steep interval re-entering that branch every sub-step: measured 1.5 % slower than the plain test.)
 // WF: also form the per-cell event flags (cool_cells::flags).  Compile time, because keeping the three event predicates of
 // every cell alive to the end of the step costs the diagnostics kernels registers they do not have (s512f: 11 % with the
 // flags merely possible); only tests and callers that pass a flags array get the WF instantiations.
@@ -547,29 +546,7 @@ __device__ __forceinline__ void step_cells_f32(const Ctx32 &X, const Fetch &F, c
                     const float4 v = F.hw4(lr[j], le, li, lb[j]);
                     y0 = v.x; y1 = v.y; y2 = v.z; yc = v.w;
                 } else {
-                    if (loc_bits(le) != P[j].ke || loc_bits(li) != P[j].ki) {
-                        // Precise pass (F32Const::band_*): the patch of a cell whose Theta_e interval is the steep one or a
-                        // neighbour of it carries the sign bit in its interval word, so the cell comes back here every sub-step
-                        // (rebuilding only when it really changed table cell), and only here is it tested — the sub-step loop
-                        // itself carries no test.  The radiated fraction is evaluated once more on this rare path.
-                        if (loc_bits(le) != (P[j].ke & 0x7fffffff) || loc_bits(li) != P[j].ki) build_patch(F, lr[j], lb[j], le, li, P[j]);
-#ifndef COOL_EXP_NOBAND4
-                        if ((unsigned)(loc_bits(le) - S.kb_lo) < S.kb_n) {
-                            P[j].ke = loc_bits(le) | (int)0x80000000u;
-                            if ((__float_as_uint(the[j]) - S.band_lo_bits) < S.band_w) {
-                                const float z0 = patch_eval(P[j], 0, le.w, li.w), z1 = patch_eval(P[j], 1, le.w, li.w), z2 = patch_eval(P[j], 2, le.w, li.w);
-                                const float qbr = ex2_approx(fminf(z0 + kk, 100.f)), qsy = ex2_approx(fminf((z1 + kk) + z2, 100.f));
-                                const float qthin = qbr + qsy;
-                                const float nm = fmaf(S.ae, the[j], S.ai * thi[j]), dn = fmaf(S.be, the[j], fmaf(S.bi, thi[j], 1.f));
-                                const float qcs = rho[j] * (nm * rsqrt_approx(nm * dn));
-                                const float tabs = qthin * (S.inv_kB * qcs) * rcp_approx(fmaxf(the[j] * the[j] * the[j], 1e-30f));
-                                float q = qthin * rcp_approx(fmaf(tabs, fmaf(1.5f, tabs + S.ksca * qcs, 1.7320508f), 1.f));
-                                if (use_floor && (the[j] + thi[j]) * S.mr < tfloor[j]) q = 0.f;
-                                if ((__float_as_uint(q) - S.rmin_bits) < S.r_w) { bad[j] = true; any_bad = true; nanq[j] = -0.f; }
-                            }
-                        }
-#endif
-                    }
+                    if (loc_bits(le) != P[j].ke || loc_bits(li) != P[j].ki) build_patch(F, lr[j], lb[j], le, li, P[j]);
                     y0 = patch_eval(P[j], 0, le.w, li.w); y1 = patch_eval(P[j], 1, le.w, li.w);
                     y2 = patch_eval(P[j], 2, le.w, li.w); yc = patch_eval(P[j], 3, le.w, li.w);
                 }
@@ -595,7 +572,7 @@ __device__ __forceinline__ void step_cells_f32(const Ctx32 &X, const Fetch &F, c
             }
             // inside the steep band of the table, radiating a fraction that is neither negligible nor certainly limited: left to
             // the precise pass, passed through here like a cell without matter (the band is empty when no precise pass follows)
-            if constexpr (FIXT && MODE == 3) {
+            if constexpr (FIXT) {
                 if (((__float_as_uint(the[j]) - S.band_lo_bits) < S.band_w) & ((__float_as_uint(rrad) - S.rmin_bits) < S.r_w)) {
                     if constexpr (NSUB1 && !Fetch::kHw) {          // a single update: the precise rate, in place
                         rrad = precise_rate3(T.f1, T.s_rho, T.s_the, T.ax[CAX_THE].n, T.ax[CAX_THE].lo10, T.ax[CAX_THE].inv10,

@@ -90,9 +90,6 @@ static F32Const make_f32_const(const cool_table *t, const LaunchArgs &a)
         const float hi = std::min(D0.band_hi, 3.0e38f);               // keep the width a finite-float difference
         const unsigned lo_b = bits(D0.band_lo), rmin_b = bits(1.5e-6 / sens), rmax_b = bits(a.f_limit * (1.0 + 2.0 * sens) + 1e-6);
         S.band_lo_bits = lo_b; S.band_w = on ? bits(hi) - lo_b : 0u;
-        // the same band as Theta_e intervals (node-index words of Loc32::tf: 0x4B400000 + i), one neighbour interval each side
-        const int k0 = std::max(D0.band_k0 - 1, 0), k1 = std::min(D0.band_k1 + 1, D0.ax[CAX_THE].n - 2);
-        S.kb_lo = (int)(0x4B400000u + (unsigned)k0); S.kb_n = on ? (unsigned)(k1 - k0 + 1) : 0u;
         S.rmin_bits = rmin_b; S.r_w = (on && rmax_b > rmin_b) ? rmax_b - rmin_b : 0u;
     }
     S.lum_shell = a.lum_shell ? a.shell_rep : nullptr;
