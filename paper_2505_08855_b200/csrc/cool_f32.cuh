@@ -890,6 +890,10 @@ cool_f32_kernel(const DevTable T, const F32Const S, const CellPtrs C, double *pa
 struct LaunchCtx32 { const cool_table *t; F32Const S; const LaunchArgs *a; cudaStream_t st; };
 
 constexpr int kF32Threads3 = 768, kF32Stages3 = 2;          // GLOBAL / texture variants, single-update 3-D step: 24 warps, 2 stages each
+// ... with diagnostics: 20 warps x 96 registers.  At 80 registers the luminosity terms and event counters spill inside the step
+// (s512d 0.88 -> 0.79 ms, s512f 0.91 -> 0.89 ms).  Thread counts are multiples of 128 so that the four schedulers of an SM hold
+// the same number of warps: 608, 672 and 704 threads all measure 4-15 % slower than 640.
+constexpr int kF32Threads3Diag = 640;
 constexpr int kF32Threads4 = 512, kF32Stages4 = 2;          // GLOBAL / texture variants, sub-stepped or 4-D: 16 warps, 2 stages each
 constexpr int kF32SmemThreads = 384, kF32SmemStages = 2;    // SMEM variant: the table image takes most of the shared memory
 constexpr int kCoulQuadSmemMax = 73728;                     // Coulomb quads up to 64 x (64 + 2 skew) x 16 B (and a little more) are staged in shared memory
@@ -940,7 +944,7 @@ static cudaError_t launch_f32_by_variant(const LaunchCtx32 &L, cool_variant v)
     // 768 threads, 2 stages).  Sub-stepping loops and MODE 4 (a 16-register patch per cell) need 128 registers:
     // 16 warps, 2 stages (3 stages measure 1-4 % slower: less L1 under the gathers).
     constexpr bool kWide = MODE == 3 && NSUB1;
-    constexpr int TH = kWide ? kF32Threads3 : kF32Threads4, NS = kWide ? kF32Stages3 : kF32Stages4;
+    constexpr int TH = kWide ? (DIAG ? kF32Threads3Diag : kF32Threads3) : kF32Threads4, NS = kWide ? kF32Stages3 : kF32Stages4;
     switch (v) {
         case COOL_V_GLOBAL:
             if constexpr (MODE == 3) {
