@@ -484,7 +484,10 @@ static __device__ __noinline__ float precise_rate3(const float *f1, int s_rho, i
 // WF: also form the per-cell event flags (cool_cells::flags).  Compile time, because keeping the three event predicates of
 // every cell alive to the end of the step costs the diagnostics kernels registers they do not have (s512f: 11 % with the
 // flags merely possible); only tests and callers that pass a flags array get the WF instantiations.
-template <int MODE, class Fetch, bool DIAG, int CM, bool NSUB1, int NV, bool FIXT, bool WF>
+// FLM: 1 = the temperature floor is a run-time switch (S.hfloor2 > 0), 0 = compiled out.  The floor test sits in the sub-step loop
+// (the compiler predicates it rather than branching around it: 8 issue slots per sub-step when the floor is off), so the 4-D
+// kernels, where the sub-step loop is nearly everything, exist in both forms.
+template <int MODE, class Fetch, bool DIAG, int CM, bool NSUB1, int NV, bool FIXT, bool WF, int FLM>
 __device__ __forceinline__ void step_cells_f32(const Ctx32 &X, const Fetch &F, const float *rho, const float *bsq, float *the, float *thi,
                                                const float *rr, const float *vol, DiagAcc &acc, float (&tile_part)[4], unsigned wtile,
                                                unsigned &flagword)   // byte j: event flags of cell j (include/cool.h); bit 3 = left to the precise pass
@@ -492,12 +495,17 @@ __device__ __forceinline__ void step_cells_f32(const Ctx32 &X, const Fetch &F, c
     const DevTable &T = X.T; const F32Const &S = X.S;
     const int coulomb = (CM >= 1) ? 1 : S.coulomb;
     const int one_bits = opaque_const(0x3f800000);
-    const bool use_floor = S.hfloor2 > 0.f;                 // warp-uniform
+    const bool use_floor = FLM != 0 && S.hfloor2 > 0.f;     // warp-uniform
     bool bad[NV], any_bad = false;
     float in_e[NV], in_i[NV], nanq[NV];
     Loc32 lr[NV], lb[NV];
     float kcell[NV], coul_kr[NV], tfloor[NV], lsum[NV][4];
     bool clamped[NV], limited[NV], floored[NV];
+    // events of the sub-step loop as running maxima (one instruction each per sub-step, decided once at the end) instead of
+    // or-ed predicates, which the compiler keeps as bytes packed into registers: rlim = largest radiated fraction; cmax_* =
+    // largest node-coordinate bit pattern of the Theta_e / Theta_i axis (unsigned: negative and too-large t both sort above n-1)
+    float rlim[NV]; unsigned cmax_e[NV], cmax_i[NV];
+    constexpr bool kMaxEv = DIAG && !NSUB1 && NV == 1;
     Patch4 P[(MODE == 4 && !Fetch::kHw) ? NV : 1];
 #pragma unroll
     for (int j = 0; j < NV; ++j) {
@@ -507,6 +515,7 @@ __device__ __forceinline__ void step_cells_f32(const Ctx32 &X, const Fetch &F, c
         any_bad |= bad[j];
         in_e[j] = the[j]; in_i[j] = thi[j];
         clamped[j] = limited[j] = floored[j] = false;
+        rlim[j] = 0.f; cmax_e[j] = cmax_i[j] = 0u;
         lr[j] = locate32<DIAG>(T.ax[CAX_RHO], rho[j], clamped[j], one_bits);
         lb[j] = locate32<DIAG>(T.ax[CAX_BSQ], bsq[j], clamped[j], one_bits);
         tfloor[j] = 0.f;
@@ -531,7 +540,9 @@ __device__ __forceinline__ void step_cells_f32(const Ctx32 &X, const Fetch &F, c
 #pragma unroll
         for (int j = 0; j < NV; ++j) {
             const float te = coord32(T.ax[CAX_THE], the[j], one_bits);
-            const Loc32 le = split32<DIAG>(T.ax[CAX_THE], te, clamped[j]);
+            bool cdummy = false;
+            const Loc32 le = split32<DIAG && !kMaxEv>(T.ax[CAX_THE], te, kMaxEv ? cdummy : clamped[j]);
+            if constexpr (kMaxEv) cmax_e[j] = max(cmax_e[j], __float_as_uint(te));
             const float kk = fmaf(le.d, T.ax[CAX_THE].d2f, kcell[j]);
             float rrad, yc = 0.f, ti = 0.f;
             fr[j][0] = fr[j][1] = fr[j][2] = 0.f;
@@ -540,7 +551,8 @@ __device__ __forceinline__ void step_cells_f32(const Ctx32 &X, const Fetch &F, c
                 rrad = ex2_approx(interp3_f32(F, lr[j], le, lb[j]) + kk);
             } else {
                 ti = coord32(T.ax[CAX_THI], thi[j], one_bits);
-                li = split32<DIAG>(T.ax[CAX_THI], ti, clamped[j]);
+                li = split32<DIAG && !kMaxEv>(T.ax[CAX_THI], ti, kMaxEv ? cdummy : clamped[j]);
+                if constexpr (kMaxEv) cmax_i[j] = max(cmax_i[j], __float_as_uint(ti));
                 float y0, y1, y2;
                 if constexpr (Fetch::kHw) {
                     const float4 v = F.hw4(lr[j], le, li, lb[j]);
@@ -581,7 +593,10 @@ __device__ __forceinline__ void step_cells_f32(const Ctx32 &X, const Fetch &F, c
                     } else { bad[j] = true; any_bad = true; nanq[j] = -0.f; }          // sub-steps: the precise pass
                 }
             }
-            if constexpr (DIAG) limited[j] |= (rrad > S.f_limit);
+            if constexpr (DIAG) {
+                if constexpr (NSUB1) limited[j] = rrad > S.f_limit;
+                else rlim[j] = fmaxf(rlim[j], rrad);            // one FMNMX per sub-step; compared once at the end (NaN: no event, as before)
+            }
             rrad = fminf(rrad, S.f_limit);
             // Coulomb exchange (eq 15), capped by f_limit of the donor and by the equalising transfer
             float dthe = 0.f;
@@ -663,6 +678,8 @@ __device__ __forceinline__ void step_cells_f32(const Ctx32 &X, const Fetch &F, c
 #pragma unroll
                 for (int k = 1; k < 4; ++k) part[k] += bad[j] ? 0.f : lsum[j][k] * wgt;
             }
+            if constexpr (!NSUB1) limited[j] = rlim[j] > S.f_limit;
+            if constexpr (kMaxEv) clamped[j] |= (cmax_e[j] > __float_as_uint(T.ax[CAX_THE].nm1f)) | (MODE == 4 && cmax_i[j] > __float_as_uint(T.ax[CAX_THI].nm1f));
             if (limited[j] && !bad[j]) ++acc.lim;               // predicated increments: the flags stay predicates
             if (floored[j] && !bad[j]) ++acc.flo;
             if (clamped[j] && !bad[j]) ++acc.cla;
@@ -689,7 +706,7 @@ constexpr unsigned kWarpArrBytes = kWarpTile * 4u;          // 512 B per array p
 constexpr unsigned kF32BarBytes = 1024;                     // room for 32 warps x 2 stages of 8-byte mbarriers, 32 list counters, the Coulomb barrier
 constexpr unsigned kF32FixCntOff = 768;                     // per-warp count of tiles listed for the precise pass (32 x 4 bytes)
 
-template <int MODE, class Fetch, bool DIAG, int CM, bool NSUB1, int THREADS, int NST, bool WF>
+template <int MODE, class Fetch, bool DIAG, int CM, bool NSUB1, int THREADS, int NST, bool WF, int FLM>
 __global__ void __launch_bounds__(THREADS, 1)
 cool_f32_kernel(const DevTable T, const F32Const S, const CellPtrs C, double *partials, unsigned *ticket, cool_diag *d_diag)
 {
@@ -809,7 +826,7 @@ cool_f32_kernel(const DevTable T, const F32Const S, const CellPtrs C, double *pa
 #pragma unroll 1
             for (int j = 0; j < kF32CellsPerThread; ++j) {
                 unsigned fw1;
-                step_cells_f32<MODE, Fetch, DIAG, CM, NSUB1, 1, true, WF>(X, F, &rho.x, &bsq.x, &the.x, &thi.x, &rr.x, &vv.x, acc, tp, (unsigned)tile, fw1);
+                step_cells_f32<MODE, Fetch, DIAG, CM, NSUB1, 1, true, WF, FLM>(X, F, &rho.x, &bsq.x, &the.x, &thi.x, &rr.x, &vv.x, acc, tp, (unsigned)tile, fw1);
                 if (fw1) flagword |= fw1 << (8 * j);        // rare
                 // a finished cell's rho, bsq, vol and r slots are dead: they carry its four luminosity terms to the end of the tile
                 if constexpr (DIAG) { rho.x = tp[0]; bsq.x = tp[1]; vv.x = tp[2]; rr.x = tp[3]; }
@@ -832,8 +849,8 @@ cool_f32_kernel(const DevTable T, const F32Const S, const CellPtrs C, double *pa
                 tested = false;
 #endif
             }
-            if (tested) step_cells_f32<MODE, Fetch, DIAG, CM, NSUB1, kF32CellsPerThread, true, WF>(X, F, &rho.x, &bsq.x, &the.x, &thi.x, &rr.x, &vv.x, acc, tp, (unsigned)tile, flagword);
-            else step_cells_f32<MODE, Fetch, DIAG, CM, NSUB1, kF32CellsPerThread, false, WF>(X, F, &rho.x, &bsq.x, &the.x, &thi.x, &rr.x, &vv.x, acc, tp, (unsigned)tile, flagword);
+            if (tested) step_cells_f32<MODE, Fetch, DIAG, CM, NSUB1, kF32CellsPerThread, true, WF, FLM>(X, F, &rho.x, &bsq.x, &the.x, &thi.x, &rr.x, &vv.x, acc, tp, (unsigned)tile, flagword);
+            else step_cells_f32<MODE, Fetch, DIAG, CM, NSUB1, kF32CellsPerThread, false, WF, FLM>(X, F, &rho.x, &bsq.x, &the.x, &thi.x, &rr.x, &vv.x, acc, tp, (unsigned)tile, flagword);
         }
         if constexpr (DIAG) {
 #pragma unroll
@@ -911,12 +928,12 @@ inline size_t f32_smem_layout(F32Const &S, int threads, int nst, bool table_in_s
     return off;
 }
 
-template <int MODE, class Fetch, bool DIAG, int CM, bool NSUB1, int THREADS, int NST, bool WF>
+template <int MODE, class Fetch, bool DIAG, int CM, bool NSUB1, int THREADS, int NST, bool WF, int FLM>
 static cudaError_t launch_f32_one(const LaunchCtx32 &L)
 {
     F32Const S = L.S;
     const size_t smem = f32_smem_layout(S, THREADS, NST, Fetch::kSmem, coul_quads<Fetch, CM>(), L.t);
-    auto kern = cool_f32_kernel<MODE, Fetch, DIAG, CM, NSUB1, THREADS, NST, WF>;
+    auto kern = cool_f32_kernel<MODE, Fetch, DIAG, CM, NSUB1, THREADS, NST, WF, FLM>;
     if (smem > 48 * 1024) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
@@ -931,13 +948,14 @@ static cudaError_t launch_f32_one(const LaunchCtx32 &L)
         a.fix_warps = warps; a.fix_cap = S.fix.cap;
     }
     CellPtrs C{a.rho, a.bsq, a.the_in, a.thi_in, a.r, a.vol, a.the_out, a.thi_out, a.ncell, a.flags};
-    note_kernel("cool_f32_kernel<MODE=%d,%s,DIAG=%d,CM=%d,NSUB1=%d,%dx%d%s>", MODE, Fetch::name(), (int)DIAG, CM, (int)NSUB1, THREADS, NST, WF ? ",flags" : "");
+    note_kernel("cool_f32_kernel<MODE=%d,%s,DIAG=%d,CM=%d,NSUB1=%d,%dx%d%s%s>", MODE, Fetch::name(), (int)DIAG, CM, (int)NSUB1, THREADS, NST, WF ? ",flags" : "",
+                FLM ? "" : ",nofloor");
     kern<<<grid, THREADS, smem, L.st>>>(L.t->dev, S, C, a.partials, a.ticket, a.d_diag);
     return cudaGetLastError();
 }
 
 // dispatch over the table variants for fixed <MODE, DIAG, CM, NSUB1>
-template <int MODE, bool DIAG, int CM, bool NSUB1, bool WF>
+template <int MODE, bool DIAG, int CM, bool NSUB1, bool WF, int FLM = 1>
 static cudaError_t launch_f32_by_variant(const LaunchCtx32 &L, cool_variant v)
 {
     // The single-update 3-D step fits 80 registers: 24 warps per SM hide the gather latency (measured best on B200:
@@ -948,13 +966,13 @@ static cudaError_t launch_f32_by_variant(const LaunchCtx32 &L, cool_variant v)
     switch (v) {
         case COOL_V_GLOBAL:
             if constexpr (MODE == 3) {
-                if (L.t->dev.o3) return launch_f32_one<MODE, F32GlobalO, DIAG, CM, NSUB1, TH, NS, WF>(L);
-                if (L.t->dev.q3) return launch_f32_one<MODE, F32GlobalQ, DIAG, CM, NSUB1, TH, NS, WF>(L);
+                if (L.t->dev.o3) return launch_f32_one<MODE, F32GlobalO, DIAG, CM, NSUB1, TH, NS, WF, FLM>(L);
+                if (L.t->dev.q3) return launch_f32_one<MODE, F32GlobalQ, DIAG, CM, NSUB1, TH, NS, WF, FLM>(L);
             }
-            return launch_f32_one<MODE, F32Global, DIAG, CM, NSUB1, TH, NS, WF>(L);
-        case COOL_V_TEX_POINT: return launch_f32_one<MODE, F32TexPoint, DIAG, CM, NSUB1, TH, NS, WF>(L);
-        case COOL_V_TEX_HWFILTER: return launch_f32_one<MODE, F32TexHw, DIAG, CM, NSUB1, TH, NS, WF>(L);
-        case COOL_V_SMEM: return launch_f32_one<MODE, F32Smem, DIAG, CM, NSUB1, kF32SmemThreads, kF32SmemStages, WF>(L);
+            return launch_f32_one<MODE, F32Global, DIAG, CM, NSUB1, TH, NS, WF, FLM>(L);
+        case COOL_V_TEX_POINT: return launch_f32_one<MODE, F32TexPoint, DIAG, CM, NSUB1, TH, NS, WF, FLM>(L);
+        case COOL_V_TEX_HWFILTER: return launch_f32_one<MODE, F32TexHw, DIAG, CM, NSUB1, TH, NS, WF, FLM>(L);
+        case COOL_V_SMEM: return launch_f32_one<MODE, F32Smem, DIAG, CM, NSUB1, kF32SmemThreads, kF32SmemStages, WF, FLM>(L);
         default: return cudaErrorInvalidValue;
     }
 }
