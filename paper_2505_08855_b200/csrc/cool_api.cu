@@ -261,7 +261,7 @@ static cool_status check_args(const cool_table *t, const cool_cells *c, const co
 using namespace cool;
 
 extern "C" const char *cool_last_error(void) { return g_err; }
-extern "C" const char *cool_version(void) { return "cool_b200 0.1 (sm_100a)"; }
+extern "C" const char *cool_version(void) { return "cool_b200 0.2 (sm_100a)"; }
 extern "C" int cool_last_launch_count(void) { return g_launches; }
 extern "C" const char *cool_last_kernel_name(void) { return g_kernel; }
 
