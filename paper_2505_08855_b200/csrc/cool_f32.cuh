@@ -845,9 +845,6 @@ cool_f32_kernel(const DevTable T, const F32Const S, const CellPtrs C, double *pa
                 const bool inb = ((__float_as_uint(the.x) - S.band_lo_bits) < S.band_w) | ((__float_as_uint(the.y) - S.band_lo_bits) < S.band_w) |
                                  ((__float_as_uint(the.z) - S.band_lo_bits) < S.band_w) | ((__float_as_uint(the.w) - S.band_lo_bits) < S.band_w);
                 tested = __any_sync(0xffffffffu, inb);
-#ifdef COOL_EXP_NOPRE
-                tested = false;
-#endif
             }
             if (tested) step_cells_f32<MODE, Fetch, DIAG, CM, NSUB1, kF32CellsPerThread, true, WF, FLM>(X, F, &rho.x, &bsq.x, &the.x, &thi.x, &rr.x, &vv.x, acc, tp, (unsigned)tile, flagword);
             else step_cells_f32<MODE, Fetch, DIAG, CM, NSUB1, kF32CellsPerThread, false, WF, FLM>(X, F, &rho.x, &bsq.x, &the.x, &thi.x, &rr.x, &vv.x, acc, tp, (unsigned)tile, flagword);

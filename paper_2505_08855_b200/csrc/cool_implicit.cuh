@@ -539,14 +539,10 @@ __device__ void implicit_cell_f32(const DevTable &T, const StepConst &S, const F
     if (flags) flags[cell] = (unsigned char)((floored << 1) | (clamped ? 4 : 0));
 }
 
-#ifndef COOL_IMP_MINB3
-#define COOL_IMP_MINB3 3
-#endif
-#ifndef COOL_IMP_MINB4
-#define COOL_IMP_MINB4 2
-#endif
+// Resident blocks per SM: the solve is bound by the latency of its dependent chains, so warps count.  3-D tables fit 80 registers
+// (three blocks of 256 threads: 24 warps, 20 % faster than two); the 4-D solve needs 128 (two blocks; three measured no gain).
 template <int MODE, class Fetch, int THREADS>
-__global__ void __launch_bounds__(THREADS, MODE == 3 ? COOL_IMP_MINB3 : COOL_IMP_MINB4)
+__global__ void __launch_bounds__(THREADS, MODE == 3 ? 3 : 2)
 cool_implicit_f32_kernel(const DevTable T, const StepConst S, const F32Const S32, const CellPtrs C, double *partials, unsigned *ticket, cool_diag *d_diag)
 {
     extern __shared__ __align__(16) unsigned char smem_imp32[];
