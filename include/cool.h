@@ -193,7 +193,11 @@ cool_status cool_table_create(const cool_table_desc *desc, int device, cool_tabl
  * table edge, rho <= 0 leaves the cell unchanged, NaN inputs give NaN outputs for that
  * cell only.  Errors: COOL_EINVAL (NULL/negative sizes/params out of range),
  * COOL_EUNSUPPORTED (variant impossible for this table, e.g. SMEM with a table that does not
- * fit; COOL_V_AUTO never fails this way), COOL_ECUDA. */
+ * fit; COOL_V_AUTO never fails this way), COOL_ECUDA.
+ * Launches: one kernel; two for fp32 cells in a sub-stepped or 4-D step on a table with a steep Theta_e interval (the K2 -> 2 theta^2
+ * switch of PAPER.md L87): the fp32 kernel passes the few cells that visit it through and a small second kernel recomputes them
+ * in fp64, which is what holds 1e-5 on every cell; one more when cells->lum_shell is set.  The library keeps a small per-stream
+ * workspace for this (allocated on the first call on a stream; cool_apply_noalloc below never allocates). */
 cool_status cool_apply(const cool_table *table, const cool_cells *cells, const cool_params *params,
                        cool_diag *d_diag, void *cuda_stream);
 
