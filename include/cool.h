@@ -63,7 +63,9 @@ typedef enum { COOL_COULOMB_AUTO = 0, /* coefficient table if the cool_table has
  * C-18): Theta_e' solves  th - Theta_e + h th Lambda(th_c)/u_e(th_c) - q (Theta_i - th) = 0  with th_c = th clamped to
  * the table's Theta_e range, q = a/(1 + a g), a = h K C(Theta_e, Theta_i) (Coulomb coefficient at the start state,
  * driving difference at the end state), Theta_i' = Theta_i - g q (Theta_i - Theta_e').  No limiter (f_limit is
- * ignored); always positive.  fp64 cells are solved in fp64, fp32 cells by an fp32 search on the library's log2 tables plus an fp64 polish of the root (1e-5).  Variants: GLOBAL, SMEM, TEX_POINT (AUTO picks);
+ * ignored); always positive.  fp64 cells are solved in fp64; fp32 cells by an fp32 search on the library's log2 tables, with
+ * the rate's exponent summed in fp64 inside the bracketing interval where the cell radiates more than 3 % of its energy
+ * (which is what holds 1e-5).  Variants: GLOBAL, SMEM, TEX_POINT (AUTO picks);
  * TEX_HWFILTER and ANALYTIC return COOL_EUNSUPPORTED. */
 typedef enum { COOL_SCHEME_EXPLICIT = 0, COOL_SCHEME_IMPLICIT = 1 } cool_scheme;
 
